@@ -1,0 +1,177 @@
+"""CPU oracle for MicSA (arxiv/paper_2506_16240) -- TEST INFRASTRUCTURE ONLY.
+
+Thin ctypes/numpy wrapper around ``micsa_oracle.c`` (the paper's algorithm
+written out with serial loops) and ``metropolis_oracle.c`` (an independent
+textbook Metropolis used only as a pin).  Only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It shares no code with
+``paper_2506_16240_b200`` and neither imports the other.
+
+Array conventions (the canonical unpacked layout of the C-ABI boundary):
+  s  int8  [n_samples, n_replicas, N]   spins, values -1/+1
+  m  uint8 [n_samples, n_replicas, N]   demon level, n = 4 m
+  J  int8  [n_samples, 3, N]            bond site i -> i + d
+  site i = x + L*(y + L*z)
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_BUILD = _HERE / "_build"
+_LIB = None
+
+_c_i8p = ctypes.POINTER(ctypes.c_int8)
+_c_u8p = ctypes.POINTER(ctypes.c_uint8)
+_c_i64p = ctypes.POINTER(ctypes.c_int64)
+_c_u32p = ctypes.POINTER(ctypes.c_uint32)
+_c_u64p = ctypes.POINTER(ctypes.c_uint64)
+_c_f64p = ctypes.POINTER(ctypes.c_double)
+
+
+def build(force: bool = False) -> Path:
+    """Compile the oracle's C sources with gcc into oracle/_build/liboracle.so."""
+    _BUILD.mkdir(exist_ok=True)
+    so = _BUILD / "liboracle.so"
+    srcs = [_HERE / "micsa_oracle.c", _HERE / "metropolis_oracle.c"]
+    if (not force and so.exists()
+            and all(so.stat().st_mtime >= p.stat().st_mtime for p in srcs)):
+        return so
+    tmp = _BUILD / f"liboracle.{os.getpid()}.tmp.so"
+    cmd = ["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", str(tmp)] + \
+          [str(p) for p in srcs] + ["-lm"]
+    subprocess.run(cmd, check=True)
+    os.replace(tmp, so)
+    return so
+
+
+def lib() -> ctypes.CDLL:
+    global _LIB
+    if _LIB is None:
+        _LIB = ctypes.CDLL(str(build()))
+        _LIB.oracle_thresholds.argtypes = [ctypes.c_double, _c_u64p]
+        _LIB.oracle_thresholds.restype = ctypes.c_int
+        _LIB.oracle_refresh.restype = ctypes.c_int
+        _LIB.oracle_num_threads.restype = ctypes.c_int
+    return _LIB
+
+
+def _p(a, typ):
+    return a.ctypes.data_as(typ)
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().oracle_set_num_threads(ctypes.c_int(n))
+
+
+def philox4x32_10(ctr, key) -> np.ndarray:
+    """One Philox4x32-10 block: ctr = 4 uint32, key = 2 uint32 -> 4 uint32."""
+    c = np.asarray(ctr, dtype=np.uint32).copy()
+    k = np.asarray(key, dtype=np.uint32).copy()
+    o = np.zeros(4, dtype=np.uint32)
+    lib().oracle_philox4x32_10(_p(c, _c_u32p), _p(k, _c_u32p), _p(o, _c_u32p))
+    return o
+
+
+def init_spins(L, n_samples, n_replicas, seed, sample_offset=0) -> np.ndarray:
+    N = L ** 3
+    s = np.empty((n_samples, n_replicas, N), dtype=np.int8)
+    lib().oracle_init_spins(ctypes.c_int(L), ctypes.c_int(n_samples),
+                            ctypes.c_int(n_replicas), ctypes.c_uint64(seed),
+                            ctypes.c_int(sample_offset), _p(s, _c_i8p))
+    return s
+
+
+def init_bonds(L, n_samples, seed, sample_offset=0) -> np.ndarray:
+    N = L ** 3
+    J = np.empty((n_samples, 3, N), dtype=np.int8)
+    lib().oracle_init_bonds(ctypes.c_int(L), ctypes.c_int(n_samples),
+                            ctypes.c_uint64(seed), ctypes.c_int(sample_offset),
+                            _p(J, _c_i8p))
+    return J
+
+
+def _check(L, s, m, J):
+    ns, nr, N = s.shape
+    assert N == L ** 3 and s.dtype == np.int8 and s.flags.c_contiguous
+    if m is not None:
+        assert m.shape == s.shape and m.dtype == np.uint8 and m.flags.c_contiguous
+    if J is not None:
+        assert J.shape == (ns, 3, N) and J.dtype == np.int8 and J.flags.c_contiguous
+    return ns, nr, N
+
+
+def half_sweep(L, s, m, J, parity):
+    """In-place half-sweep on sites of the given parity.
+    Returns (accepted[n_sys], dE[n_sys]) as int64 arrays."""
+    ns, nr, _ = _check(L, s, m, J)
+    acc = np.zeros(ns * nr, dtype=np.int64)
+    dE = np.zeros(ns * nr, dtype=np.int64)
+    lib().oracle_half_sweep(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr),
+                            ctypes.c_int(parity), _p(s, _c_i8p), _p(m, _c_u8p),
+                            _p(J, _c_i8p), _p(acc, _c_i64p), _p(dE, _c_i64p))
+    return acc, dE
+
+
+def sweep(L, s, m, J, n_sweeps=1) -> None:
+    """n full sweeps, each = even half-sweep then odd half-sweep, in place."""
+    ns, nr, _ = _check(L, s, m, J)
+    lib().oracle_sweep(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr),
+                       ctypes.c_int(n_sweeps), _p(s, _c_i8p), _p(m, _c_u8p),
+                       _p(J, _c_i8p))
+
+
+def thresholds(T: float) -> np.ndarray:
+    """Integer thresholds of the cumulative Eq. (11) (R7)."""
+    thr = np.zeros(3, dtype=np.uint64)
+    rc = lib().oracle_thresholds(ctypes.c_double(T), _p(thr, _c_u64p))
+    if rc != 0:
+        raise ValueError(f"invalid temperature {T!r}")
+    return thr
+
+
+def refresh(L, m, seed, T, step, sample_offset=0) -> None:
+    """Overwrite every demon with a draw from Eq. (11) at temperature T."""
+    ns, nr, N = m.shape
+    assert N == L ** 3 and m.dtype == np.uint8 and m.flags.c_contiguous
+    rc = lib().oracle_refresh(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr),
+                              ctypes.c_uint64(seed), ctypes.c_int(sample_offset),
+                              ctypes.c_double(T), ctypes.c_uint32(step),
+                              _p(m, _c_u8p))
+    if rc != 0:
+        raise ValueError(f"invalid temperature {T!r}")
+
+
+def measure(L, s, m, J):
+    """Exact integer sums: E[n_sys], Edem[n_sys], Q[n_samples*nr(nr-1)/2]."""
+    ns, nr, _ = _check(L, s, m, J)
+    E = np.zeros(ns * nr, dtype=np.int64)
+    Ed = np.zeros(ns * nr, dtype=np.int64)
+    Q = np.zeros(ns * nr * (nr - 1) // 2, dtype=np.int64)
+    lib().oracle_measure(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr),
+                         _p(s, _c_i8p), _p(m, _c_u8p), _p(J, _c_i8p),
+                         _p(E, _c_i64p), _p(Ed, _c_i64p),
+                         _p(Q, _c_i64p) if Q.size else None)
+    return E, Ed, Q
+
+
+def metropolis(L, s, J, T, n_sweeps, seed):
+    """Independent textbook Metropolis (metropolis_oracle.c); s updated in
+    place; returns the energy per spin after each sweep, float64
+    [n_sweeps, n_sys]."""
+    ns, nr, N = _check(L, s, None, J)
+    e = np.zeros((n_sweeps, ns * nr), dtype=np.float64)
+    lib().metropolis_run(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr),
+                         ctypes.c_double(T), ctypes.c_int(n_sweeps),
+                         ctypes.c_uint64(seed), _p(s, _c_i8p), _p(J, _c_i8p),
+                         _p(e, _c_f64p))
+    return e

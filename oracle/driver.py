@@ -1,0 +1,43 @@
+"""MicSA driver loop of the oracle -- TEST INFRASTRUCTURE ONLY.
+
+Follows the procedure of PAPER.md:208-217 (Sec. 2.8.1) with gamma = 1 daemon
+per spin and an explicit list of (T, n_sweeps) steps instead of the 2^s
+schedule (PAPER.md:190-192 allows any refresh times; readings R3,
+R12):
+
+    for k, (T_k, n_k, every_k) in enumerate(schedule):
+        refresh all demons from Eq. (11) at T_k, Philox step index step0 + k
+        for j in 1..n_k:
+            sweep (even sites, then odd sites)
+            if every_k > 0 and j % every_k == 0: measure
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import measure, refresh, sweep
+
+
+def anneal(L, s, m, J, seed, schedule, step0=0, sample_offset=0):
+    """Run the schedule in place on (s, m).  Returns a dict with the exact
+    integer sums of every measurement row and the running minimum of E/N."""
+    ns, nr, N = s.shape
+    rows = {"sweep": [], "T": [], "E": [], "Edem": [], "Q": []}
+    min_e = np.full(ns * nr, np.inf)
+    t = 0
+    for k, (T, n_sweeps, every) in enumerate(schedule):
+        refresh(L, m, seed, T, step0 + k, sample_offset)
+        for j in range(1, n_sweeps + 1):
+            sweep(L, s, m, J, 1)
+            t += 1
+            if every > 0 and j % every == 0:
+                E, Ed, Q = measure(L, s, m, J)
+                rows["sweep"].append(t)
+                rows["T"].append(T)
+                rows["E"].append(E)
+                rows["Edem"].append(Ed)
+                rows["Q"].append(Q)
+                min_e = np.minimum(min_e, E / float(N))
+    out = {k: np.array(v) for k, v in rows.items()}
+    out["min_energy"] = min_e
+    return out

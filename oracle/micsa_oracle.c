@@ -1,0 +1,314 @@
+/*
+ * micsa_oracle.c — CPU ORACLE for microcanonical simulated annealing (MicSA).
+ *
+ * THIS FILE IS TEST INFRASTRUCTURE.  It is a plain, slow, obviously-correct
+ * restatement of arxiv/paper_2506_16240 for the 3D +-J
+ * Edwards-Anderson spin glass with one capped demon per site.  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may build, load or call it.  It shares no code with the CUDA library in
+ * paper_2506_16240_b200/csrc/ and neither includes the other.
+ *
+ * State, in the canonical unpacked layout used at the C-ABI boundary:
+ *   s[(sample*R + replica)*N + i]  in {-1,+1}   spins
+ *   m[(sample*R + replica)*N + i]  in {0,1,2,3} demon level, n = 4m
+ *
+ *   J[(sample*3 + d)*N + i]        in {-1,+1}   bond from site i to its +d
+ *                                               neighbour, d = 0,1,2 = x,y,z;
+ *                                               replicas share it
+ *   site i = x + L*(y + L*z), 0-based, periodic boundaries,
+ *   parity (x+y+z) mod 2, parity 0 = "even".
+ *
+ * No blocking, packing or reordering: every function is the paper's
+ * definition written out with serial loops.  The OpenMP pragma only spreads
+ * *independent systems* (sample, replica) over host threads; inside a system
+ * everything is serial.
+ *
+ * Pins (tests/test_oracle_*.py, all -m "not gpu"):
+ *   philox4x32_10      vs cuRAND's host PHILOX4_32_10 generator (library)
+ *   half_sweep         exact conservation of H_EA + H_aux,
+ *                      involution, incremental == from-scratch
+ *                      energy, all 28 (U, m) cases of Eq. (8)+(10),
+ *                      brute-force Boltzmann average on the 2x2x2 lattice,
+ *                      agreement with the independent Metropolis oracle
+ *   measure            vs an independent numpy (np.roll) evaluation of Eq. (1)
+ *   thresholds/refresh histogram vs Eq. (11), mean vs Eq. (12) closed forms
+ * Unpinned by the paper: low-temperature quench curves (configs 3, 4) and the
+ * final annealed energies (config 5) -- see DESIGN.md "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* ------------------------------------------------------------------ */
+/* Philox4x32-10 (Salmon, Moraes, Dror, Shaw 2011; public algorithm).   */
+/* DESIGN.md reading R8.  ctr = 128-bit counter, key = 64-bit key.       */
+/* ------------------------------------------------------------------ */
+void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2],
+                          uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+        uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        uint32_t n0 = hi1 ^ c1 ^ k0;
+        uint32_t n1 = lo1;
+        uint32_t n2 = hi0 ^ c3 ^ k1;
+        uint32_t n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;              /* key schedule: bumped after each round */
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* Domain tags of the counter word c2 (R8). */
+enum { TAG_REFRESH = 0, TAG_SPIN_INIT = 1, TAG_BOND_INIT = 2 };
+
+static inline void seed_key(uint64_t seed, uint32_t key[2])
+{
+    key[0] = (uint32_t)(seed & 0xFFFFFFFFu);
+    key[1] = (uint32_t)(seed >> 32);
+}
+
+static inline int wrap(int a, int L) { return (a + L) % L; }
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void oracle_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* ------------------------------------------------------------------ */
+/* a0  Initial state (PAPER.md:73 couplings +-1 w.p. 1/2; PAPER.md:223  */
+/* "fully disordered" start).  One random bit per spin / bond:          */
+/*   spin : ctr = (i, gsample>>7, (1<<24)|replica, 0)                    */
+/*   bond : ctr = (i, gsample>>7, (2<<24)|d,       0)                    */
+/*   bit (gsample & 31) of output word (gsample>>5)&3; bit 1 <=> -1.     */
+/* gsample = sample_offset + sample is the *global* sample index so that */
+/* a run sharded by sample over several GPUs reproduces the unsharded    */
+/* run (multi-GPU).                                           */
+/* ------------------------------------------------------------------ */
+void oracle_init_spins(int L, int n_samples, int n_replicas, uint64_t seed,
+                       int sample_offset, int8_t *s)
+{
+    const int64_t N = (int64_t)L * L * L;
+    uint32_t key[2]; seed_key(seed, key);
+    for (int sample = 0; sample < n_samples; ++sample)
+        for (int rep = 0; rep < n_replicas; ++rep)
+            for (int64_t i = 0; i < N; ++i) {
+                uint32_t g = (uint32_t)(sample_offset + sample);
+                uint32_t ctr[4] = { (uint32_t)i, g >> 7,
+                                    ((uint32_t)TAG_SPIN_INIT << 24) | (uint32_t)rep, 0u };
+                uint32_t out[4];
+                oracle_philox4x32_10(ctr, key, out);
+                uint32_t bit = (out[(g >> 5) & 3] >> (g & 31)) & 1u;
+                s[((int64_t)sample * n_replicas + rep) * N + i] = bit ? -1 : +1;
+            }
+}
+
+void oracle_init_bonds(int L, int n_samples, uint64_t seed, int sample_offset,
+                       int8_t *J)
+{
+    const int64_t N = (int64_t)L * L * L;
+    uint32_t key[2]; seed_key(seed, key);
+    for (int sample = 0; sample < n_samples; ++sample)
+        for (int d = 0; d < 3; ++d)
+            for (int64_t i = 0; i < N; ++i) {
+                uint32_t g = (uint32_t)(sample_offset + sample);
+                uint32_t ctr[4] = { (uint32_t)i, g >> 7,
+                                    ((uint32_t)TAG_BOND_INIT << 24) | (uint32_t)d, 0u };
+                uint32_t out[4];
+                oracle_philox4x32_10(ctr, key, out);
+                uint32_t bit = (out[(g >> 5) & 3] >> (g & 31)) & 1u;
+                J[((int64_t)sample * 3 + d) * N + i] = bit ? -1 : +1;
+            }
+}
+
+/* ------------------------------------------------------------------ */
+/* a1/a2  Half-sweep on one lattice parity.     */
+/* For every site x of the given parity, in any order:    */
+/*   h      = sum over the 6 neighbours y of J_xy s_y       (Eq. 1)       */
+/*   dH     = H_EA(after flip) - H_EA(before) = 2 s_x h                   */
+/*   n_new  = n_x - dH                                      (Eq. 8)       */
+/*   flip s_x and set n_x = n_new iff 0 <= n_new <= 12      (Eq. 10)      */
+/* Returns, per system, the number of accepted flips and the sum of dH   */
+/* over accepted flips (the incremental energy, pin P4).                 */
+/* ------------------------------------------------------------------ */
+void oracle_half_sweep(int L, int n_samples, int n_replicas, int parity,
+                       int8_t *s, uint8_t *m, const int8_t *J,
+                       int64_t *accepted /* [n_sys] or NULL */,
+                       int64_t *dE       /* [n_sys] or NULL */)
+{
+    const int64_t N = (int64_t)L * L * L;
+    const int n_sys = n_samples * n_replicas;
+#pragma omp parallel for schedule(static)
+    for (int sys = 0; sys < n_sys; ++sys) {
+        const int sample = sys / n_replicas;
+        int8_t  *ss = s + (int64_t)sys * N;
+        uint8_t *mm = m + (int64_t)sys * N;
+        const int8_t *Jx = J + ((int64_t)sample * 3 + 0) * N;
+        const int8_t *Jy = J + ((int64_t)sample * 3 + 1) * N;
+        const int8_t *Jz = J + ((int64_t)sample * 3 + 2) * N;
+        int64_t acc = 0, de = 0;
+        for (int z = 0; z < L; ++z)
+            for (int y = 0; y < L; ++y)
+                for (int x = 0; x < L; ++x) {
+                    if (((x + y + z) & 1) != parity) continue;
+                    const int64_t i   = x + (int64_t)L * (y + (int64_t)L * z);
+                    const int64_t ixp = wrap(x + 1, L) + (int64_t)L * (y + (int64_t)L * z);
+                    const int64_t ixm = wrap(x - 1, L) + (int64_t)L * (y + (int64_t)L * z);
+                    const int64_t iyp = x + (int64_t)L * (wrap(y + 1, L) + (int64_t)L * z);
+                    const int64_t iym = x + (int64_t)L * (wrap(y - 1, L) + (int64_t)L * z);
+                    const int64_t izp = x + (int64_t)L * (y + (int64_t)L * wrap(z + 1, L));
+                    const int64_t izm = x + (int64_t)L * (y + (int64_t)L * wrap(z - 1, L));
+                    /* the bond to the -d neighbour is that neighbour's +d bond */
+                    const int h = Jx[i]   * ss[ixp] + Jx[ixm] * ss[ixm]
+                                + Jy[i]   * ss[iyp] + Jy[iym] * ss[iym]
+                                + Jz[i]   * ss[izp] + Jz[izm] * ss[izm];
+                    const int dH = 2 * ss[i] * h;              /* in {0,+-4,+-8,+-12} */
+                    const int n_new = 4 * (int)mm[i] - dH;     /* Eq. (8) */
+                    if (0 <= n_new && n_new <= 12) {           /* Eq. (10) */
+                        ss[i] = (int8_t)(-ss[i]);
+                        mm[i] = (uint8_t)(n_new / 4);
+                        ++acc; de += dH;
+                    }
+                }
+        if (accepted) accepted[sys] = acc;
+        if (dE) dE[sys] = de;
+    }
+}
+
+/* Sweep = even half-sweep, then odd half-sweep. gamma = 1. */
+void oracle_sweep(int L, int n_samples, int n_replicas, int n_sweeps,
+                  int8_t *s, uint8_t *m, const int8_t *J)
+{
+    for (int t = 0; t < n_sweeps; ++t) {
+        oracle_half_sweep(L, n_samples, n_replicas, 0, s, m, J, NULL, NULL);
+        oracle_half_sweep(L, n_samples, n_replicas, 1, s, m, J, NULL, NULL);
+    }
+}
+
+/* ------------------------------------------------------------------ */
+/* a3  Demon refresh (PAPER.md:154-157 Eq. 11, :190).                    */
+/* Thresholds (R7), float64, this exact operation order:       */
+/*   x = exp(-4/T); x2 = x*x; x3 = x2*x; Z = ((1 + x) + x2) + x3          */
+/*   c0 = 1/Z; c1 = (1 + x)/Z; c2 = ((1 + x) + x2)/Z   (cumulative p)     */
+/*   thr[k] = floor(c_k * 2^32) as uint64 in [0, 2^32]                    */
+/* Draw: u = one 32-bit Philox word; m = #{k : u >= thr[k]}.             */
+/* ------------------------------------------------------------------ */
+int oracle_thresholds(double T, uint64_t thr[3])
+{
+    if (!(T > 0.0) || !isfinite(T)) return -1;
+    const double x  = exp(-4.0 / T);
+    const double x2 = x * x;
+    const double x3 = x2 * x;
+    const double Z  = ((1.0 + x) + x2) + x3;
+    const double c[3] = { 1.0 / Z, (1.0 + x) / Z, ((1.0 + x) + x2) / Z };
+    for (int k = 0; k < 3; ++k) {
+        double t = floor(ldexp(c[k], 32));
+        if (t > 4294967296.0) t = 4294967296.0;
+        thr[k] = (uint64_t)t;
+    }
+    return 0;
+}
+
+/* Refresh counter (R8): ctr = (i, gsample>>2, (0<<24)|replica, step),
+ * key = (seed lo, seed hi); demon of global sample g uses output word g&3.   */
+int oracle_refresh(int L, int n_samples, int n_replicas, uint64_t seed,
+                   int sample_offset, double T, uint32_t step, uint8_t *m)
+{
+    const int64_t N = (int64_t)L * L * L;
+    uint64_t thr[3];
+    if (oracle_thresholds(T, thr) != 0) return -1;
+    uint32_t key[2]; seed_key(seed, key);
+    const int n_sys = n_samples * n_replicas;
+#pragma omp parallel for schedule(static)
+    for (int sys = 0; sys < n_sys; ++sys) {
+        const int sample = sys / n_replicas, rep = sys % n_replicas;
+        const uint32_t g = (uint32_t)(sample_offset + sample);
+        uint8_t *mm = m + (int64_t)sys * N;
+        for (int64_t i = 0; i < N; ++i) {
+            uint32_t ctr[4] = { (uint32_t)i, g >> 2,
+                                ((uint32_t)TAG_REFRESH << 24) | (uint32_t)rep, step };
+            uint32_t out[4];
+            oracle_philox4x32_10(ctr, key, out);
+            const uint64_t u = (uint64_t)out[g & 3];
+            mm[i] = (uint8_t)((u >= thr[0]) + (u >= thr[1]) + (u >= thr[2]));
+        }
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* a4-a6  Measurements, exact integer sums.                              */
+/*   E[sys]    = -sum_i sum_d J[d][i] s[i] s[i+d]      (Eq. 1)            */
+/*   Edem[sys] = sum_i 4 m[i]                          (Eq. 4, n = 4m)    */
+/*   Q[sample][pair(a<b)] = sum_i s^a[i] s^b[i]        (Eq. C.1 times N)  */
+/* Pairs ordered (0,1),(0,2),...,(1,2),... lexicographically.            */
+/* ------------------------------------------------------------------ */
+void oracle_measure(int L, int n_samples, int n_replicas,
+                    const int8_t *s, const uint8_t *m, const int8_t *J,
+                    int64_t *E, int64_t *Edem, int64_t *Q)
+{
+    const int64_t N = (int64_t)L * L * L;
+    const int n_sys = n_samples * n_replicas;
+    if (E) {
+#pragma omp parallel for schedule(static)
+        for (int sys = 0; sys < n_sys; ++sys) {
+            const int sample = sys / n_replicas;
+            const int8_t *ss = s + (int64_t)sys * N;
+            int64_t e = 0;
+            for (int z = 0; z < L; ++z)
+                for (int y = 0; y < L; ++y)
+                    for (int x = 0; x < L; ++x) {
+                        const int64_t i = x + (int64_t)L * (y + (int64_t)L * z);
+                        const int64_t nb[3] = {
+                            wrap(x + 1, L) + (int64_t)L * (y + (int64_t)L * z),
+                            x + (int64_t)L * (wrap(y + 1, L) + (int64_t)L * z),
+                            x + (int64_t)L * (y + (int64_t)L * wrap(z + 1, L)) };
+                        for (int d = 0; d < 3; ++d)
+                            e -= (int64_t)J[((int64_t)sample * 3 + d) * N + i] * ss[i] * ss[nb[d]];
+                    }
+            E[sys] = e;
+        }
+    }
+    if (Edem) {
+        for (int sys = 0; sys < n_sys; ++sys) {
+            const uint8_t *mm = m + (int64_t)sys * N;
+            int64_t a = 0;
+            for (int64_t i = 0; i < N; ++i) a += 4 * (int64_t)mm[i];
+            Edem[sys] = a;
+        }
+    }
+    if (Q) {
+        int64_t k = 0;
+        for (int sample = 0; sample < n_samples; ++sample)
+            for (int a = 0; a < n_replicas; ++a)
+                for (int b = a + 1; b < n_replicas; ++b) {
+                    const int8_t *sa = s + ((int64_t)sample * n_replicas + a) * N;
+                    const int8_t *sb = s + ((int64_t)sample * n_replicas + b) * N;
+                    int64_t q = 0;
+                    for (int64_t i = 0; i < N; ++i) q += (int64_t)sa[i] * sb[i];
+                    Q[k++] = q;
+                }
+    }
+}

@@ -1,0 +1,203 @@
+"""Statistical / closed-form pins for the CPU oracle (-m "not gpu").
+
+  P5  refresh histogram vs Eq. (11), mean vs Eq. (12)
+  R7  integer thresholds: monotone, no 2^32 wrap, = Eq. (11) to 2^-32
+  P7  2x2x2 lattice: long-run <e> == brute-force Boltzmann average (3 sigma)
+  P8  high-T equilibrium <e> == independent Metropolis (3 sigma)
+  P10 equilibrium demon energy before a refresh ~ Eq. (12)
+"""
+import itertools
+import math
+
+import numpy as np
+import pytest
+
+from micsa_workloads import random_pm1
+from oracle import driver
+
+
+def eq11(T):
+    """p(n = 4m), m = 0..3, exactly as printed in PAPER.md:156 (Eq. 11)."""
+    b = 1.0 / T
+    return np.array([math.exp(-4 * m * b) * (1 - math.exp(-4 * b)) / (1 - math.exp(-16 * b))
+                     for m in range(4)])
+
+
+def eq12(T):
+    """<H_aux>/(gamma N) exactly as printed in PAPER.md:186 (Eq. 12)."""
+    b = 1.0 / T
+    return (4 * math.exp(-4 * b) / (1 - math.exp(-4 * b))
+            - 16 * math.exp(-16 * b) / (1 - math.exp(-16 * b)))
+
+
+@pytest.mark.parametrize("T", [3.0, 2.0, 1.5, 0.9, 0.7, 0.2, 50.0])
+def test_thresholds_match_eq11(oracle, T):
+    thr = oracle.thresholds(T).astype(object)
+    assert 0 < thr[0] <= thr[1] <= thr[2] <= 2 ** 32
+    p = eq11(T)
+    assert abs(p.sum() - 1) < 1e-14
+    cdf = np.cumsum(p)[:3]
+    for k in range(3):
+        assert abs(int(thr[k]) / 2.0 ** 32 - cdf[k]) <= 2.0 ** -32 + 1e-15
+    if T == 0.2:   # e^{-20} ~ 2e-9: levels 2, 3 have probability < 2^-32
+        assert int(thr[1]) == 2 ** 32 and int(thr[2]) == 2 ** 32
+
+
+@pytest.mark.parametrize("T", [-1.0, 0.0, float("nan"), float("inf")])
+def test_thresholds_reject_bad_temperature(oracle, T):
+    with pytest.raises(ValueError):
+        oracle.thresholds(T)
+
+
+@pytest.mark.parametrize("T", [3.0, 2.0, 1.5, 0.9])
+def test_refresh_histogram_and_mean(oracle, T):
+    L, ns, nr = 16, 5, 2
+    N = L ** 3
+    m = np.full((ns, nr, N), 7, dtype=np.uint8)
+    oracle.refresh(L, m, seed=2024, T=T, step=3)
+    assert m.max() <= 3
+    n_tot = m.size
+    counts = np.bincount(m.reshape(-1), minlength=4).astype(float)
+    p = eq11(T)
+    # every bin within 4.5 sigma of its binomial expectation
+    for k in range(4):
+        sig = math.sqrt(n_tot * p[k] * (1 - p[k]))
+        assert abs(counts[k] - n_tot * p[k]) < 4.5 * sig + 1, (T, k)
+    mean_n = 4.0 * m.astype(np.float64).mean()
+    var_n = 16.0 * (np.arange(4) ** 2 * p).sum() - eq12(T) ** 2
+    assert abs(mean_n - eq12(T)) < 4.5 * math.sqrt(var_n / n_tot)
+    # per-system streams look independent: system means scatter like 1/sqrt(N)
+    sys_means = 4.0 * m.reshape(ns * nr, N).mean(axis=1)
+    assert np.all(np.abs(sys_means - eq12(T)) < 5 * math.sqrt(var_n / N))
+    flat = m.reshape(ns * nr, N)
+    assert len({flat[k].tobytes() for k in range(ns * nr)}) == ns * nr
+
+
+def test_refresh_is_a_pure_function_of_its_counters(oracle):
+    L, ns, nr = 4, 6, 2
+    N = L ** 3
+    a = np.zeros((ns, nr, N), dtype=np.uint8)
+    b = np.full((ns, nr, N), 3, dtype=np.uint8)
+    oracle.refresh(L, a, 9, 2.0, 5)
+    oracle.refresh(L, b, 9, 2.0, 5)
+    np.testing.assert_array_equal(a, b)             # old demons are thrown away
+    c = np.zeros_like(a)
+    oracle.refresh(L, c, 9, 2.0, 6)
+    assert not np.array_equal(a, c)                 # step enters the counter
+    d = np.zeros_like(a)
+    oracle.refresh(L, d, 10, 2.0, 5)
+    assert not np.array_equal(a, d)                 # seed is the key
+    # sharding by sample: samples [4, 6) generated with sample_offset 4
+    e = np.zeros((2, nr, N), dtype=np.uint8)
+    oracle.refresh(L, e, 9, 2.0, 5, sample_offset=4)
+    np.testing.assert_array_equal(e, a[4:6])
+    # monotone coupling in T: same uniforms, higher T -> level never lower
+    hot = np.zeros_like(a)
+    oracle.refresh(L, hot, 9, 3.0, 5)
+    assert np.all(hot >= a) and np.any(hot > a)
+
+
+def test_init_is_fair_and_shardable(oracle):
+    L, ns, nr = 8, 40, 2
+    s = oracle.init_spins(L, ns, nr, seed=7)
+    J = oracle.init_bonds(L, ns, seed=7)
+    assert set(np.unique(s)) == {-1, 1} and set(np.unique(J)) == {-1, 1}
+    for a in (s, J):
+        n = a.size
+        assert abs(a.astype(np.float64).sum()) < 4.5 * math.sqrt(n)
+    # replicas, samples and directions are distinct streams
+    flat = np.concatenate([s.reshape(ns * nr, -1), J.reshape(ns * 3, -1)])
+    c = np.abs(flat.astype(np.float64) @ flat.T.astype(np.float64)) / flat.shape[1]
+    np.fill_diagonal(c, 0)
+    assert c.max() < 6 / math.sqrt(flat.shape[1])
+    np.testing.assert_array_equal(oracle.init_spins(L, 8, nr, 7, sample_offset=32), s[32:40])
+    np.testing.assert_array_equal(oracle.init_bonds(L, 8, 7, sample_offset=32), J[32:40])
+
+
+# ---------------------------------------------------------------- P7 brute force
+def _boltzmann_2x2x2(J, T):
+    """Exact <e> of the 8-spin periodic cube with its 24 distinct bonds
+    (R10), by enumeration of all 2^8 states; no oracle code."""
+    L, N = 2, 8
+    idx = lambda x, y, z: (x % L) + L * ((y % L) + L * (z % L))
+    bonds = []
+    for z, y, x in itertools.product(range(2), repeat=3):
+        i = idx(x, y, z)
+        bonds += [(i, idx(x + 1, y, z), J[0][i]), (i, idx(x, y + 1, z), J[1][i]),
+                  (i, idx(x, y, z + 1), J[2][i])]
+    assert len(bonds) == 24
+    Z = 0.0
+    Esum = 0.0
+    for bits in range(256):
+        s = [1 - 2 * ((bits >> k) & 1) for k in range(N)]
+        E = -sum(j * s[a] * s[b] for a, b, j in bonds)
+        w = math.exp(-E / T)
+        Z += w
+        Esum += E * w
+    return Esum / Z / N
+
+
+@pytest.mark.parametrize("T,seed", [(2.0, 11), (3.0, 12)])
+def test_2x2x2_matches_exact_boltzmann(oracle, T, seed):
+    L, N, nr = 2, 8, 64
+    J = random_pm1((1, 3, N), seed)
+    exact = _boltzmann_2x2x2(J[0].tolist(), T)
+    s = oracle.init_spins(L, 1, nr, seed)
+    m = np.zeros((1, nr, N), dtype=np.uint8)
+    n_sweeps, therm = 6000, 200
+    sched = [(T, 10, 1)] * (n_sweeps // 10)
+    out = driver.anneal(L, s, m, J, seed, sched)
+    e = out["E"][therm:] / float(N)                       # [t, replica]
+    per_rep = e.mean(axis=0)                              # independent replicas
+    mean, err = per_rep.mean(), per_rep.std(ddof=1) / math.sqrt(nr)
+    assert err < 0.01
+    assert abs(mean - exact) < 3 * err, (mean, exact, err)
+    # and the demons sit at Eq. (12) just after... and on average before a refresh (P10)
+    ed = out["Edem"][therm:][9::10] / float(N)            # last sweep before each refresh
+    per_rep_d = ed.mean(axis=0)
+    derr = per_rep_d.std(ddof=1) / math.sqrt(nr)
+    assert abs(per_rep_d.mean() - eq12(T)) < 3 * derr + 1e-12, (per_rep_d.mean(), eq12(T), derr)
+
+
+def test_2x2x2_wrong_physics_would_fail():
+    """Sanity of the pin itself: the exact average separates T=2 from T=3 and a
+    24-bond from a 12-bond cube by many sigma of the test above."""
+    J = random_pm1((1, 3, 8), 11)[0].tolist()
+    assert abs(_boltzmann_2x2x2(J, 2.0) - _boltzmann_2x2x2(J, 3.0)) > 0.1
+
+
+# ---------------------------------------------------------------- P8 Metropolis
+@pytest.mark.parametrize("T", [3.0, 2.0])
+def test_equilibrium_energy_matches_metropolis(oracle, T):
+    L, ns, nr = 6, 4, 8
+    N = L ** 3
+    J = oracle.init_bonds(L, ns, seed=21)
+    s_mic = oracle.init_spins(L, ns, nr, seed=21)
+    s_met = s_mic.copy()
+    m = np.zeros((ns, nr, N), dtype=np.uint8)
+    n_sweeps, therm = 3000, 500
+    out = driver.anneal(L, s_mic, m, J, 21, [(T, 10, 1)] * (n_sweeps // 10))
+    e_mic = (out["E"][therm:] / float(N)).mean(axis=0).reshape(ns, nr)
+    e_met = oracle.metropolis(L, s_met, J, T, n_sweeps, seed=5)[therm:].mean(axis=0).reshape(ns, nr)
+    # compare sample by sample (same couplings), error from replica scatter
+    for k in range(ns):
+        d = e_mic[k].mean() - e_met[k].mean()
+        err = math.sqrt(e_mic[k].var(ddof=1) / nr + e_met[k].var(ddof=1) / nr)
+        assert abs(d) < 3 * err + 1e-9, (T, k, d, err)
+    d_all = e_mic.mean() - e_met.mean()
+    err_all = math.sqrt(e_mic.var(ddof=1) / e_mic.size + e_met.var(ddof=1) / e_met.size)
+    assert abs(d_all) < 3 * err_all
+    # coarse textbook scale: e ~ -3 tanh(beta) to leading order at high T
+    assert abs(e_mic.mean() / (-3 * math.tanh(1 / T)) - 1) < 0.12
+
+
+def test_metropolis_oracle_itself_on_2x2x2(oracle):
+    """The comparator is pinned too: Metropolis on the 8-spin cube == exact."""
+    T, N, nr = 2.0, 8, 64
+    J = random_pm1((1, 3, N), 33)
+    exact = _boltzmann_2x2x2(J[0].tolist(), T)
+    s = oracle.init_spins(2, 1, nr, 33)
+    e = oracle.metropolis(2, s, J, T, 6000, seed=8)[200:]
+    per_rep = e.mean(axis=0)
+    err = per_rep.std(ddof=1) / math.sqrt(nr)
+    assert abs(per_rep.mean() - exact) < 3 * err
