@@ -1,0 +1,182 @@
+/*
+ * micsa.h -- C ABI of the B200-native MicSA library (libmicsa.so).
+ *
+ * Microcanonical simulated annealing for the 3D +-J Edwards-Anderson spin
+ * glass, arxiv/paper_2506_16240 (citations are PAPER.md:<line>).  One capped
+ * daemon per spin (gamma = 1, n in {0,4,8,12}); checkerboard sweeps without
+ * random numbers; sporadic Philox-driven daemon refresh; E / E_daemon / q
+ * reductions.  Every step runs in hand-written CUDA kernels for sm_100a; there
+ * is no CPU fallback: every call fails with MICSA_ERR_CUDA when no device is
+ * usable.
+ *
+ * Conventions
+ *   N = L^3 sites, site i = x + L*(y + L*z), 0-based, periodic.
+ *   parity(i) = (x+y+z) mod 2; parity 0 = "even" sublattice.
+ *   system  = (sample, replica); sys = sample*n_replicas + replica;
+ *             n_sys = n_samples*n_replicas.  Replicas of a sample share its
+ *             couplings.
+ *   Canonical (unpacked) host layouts -- the byte-for-byte parity surface:
+ *     spins   int8   [n_samples][n_replicas][N]   values -1 / +1
+ *     daemons uint8  [n_samples][n_replicas][N]   level m in 0..3, n = 4m
+ *
+ *     bonds   int8   [n_samples][3][N]            J[s][d][i] = coupling between
+ *                                                 site i and its +d neighbour,
+ *                                                 d = 0,1,2 = x,y,z
+ *   On the device the state is bit-sliced across systems (1 bit per spin,
+ *   2 bit-planes per daemon); that layout is private.
+ *
+ * Pointers: "host" = ordinary (pageable or pinned) host memory owned by the
+ * caller; the library copies in/out and never keeps the pointer.  "device" =
+ * CUDA device memory.  All calls on one context must come from one thread at
+ * a time.  Work is queued on the context's stream; calls documented as
+ * "synchronous" wait for it.
+ *
+ * Errors: every int-returning call gives MICSA_OK (0) or a negative code and
+ * leaves the state unchanged on MICSA_ERR_INVALID.  CUDA errors are sticky on
+ * the context.  Nothing is printed, nothing aborts.
+ */
+#ifndef MICSA_H
+#define MICSA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MICSA_OK            0
+#define MICSA_ERR_INVALID  (-1)   /* bad argument */
+#define MICSA_ERR_NOMEM    (-2)   /* host or device allocation failed */
+#define MICSA_ERR_CUDA     (-3)   /* CUDA runtime error (sticky) */
+
+typedef struct micsa_ctx micsa_ctx;
+
+/* One step of an annealing schedule (Sec. 2.8.1, with an
+ * explicit list of steps instead of the 2^s rule):
+ * refresh all daemons at temperature T, then n_sweeps sweeps; after every
+ * measure_every-th sweep of the step (0 = never) one measurement row is taken. */
+typedef struct micsa_step {
+    double  T;
+    int32_t n_sweeps;
+    int32_t measure_every;
+} micsa_step;
+
+/* Caller-owned host arrays receiving the measurement rows of micsa_anneal.
+ * Row r holds the exact integer sums after global sweep number sweep[r]
+ * (counted from 1 within the call).  Any array pointer may be NULL. */
+typedef struct micsa_trace {
+    int64_t  capacity;     /* in: rows the arrays can hold                      */
+    int64_t  n_rows;       /* out: rows the schedule produced (may exceed
+                              capacity; only the first `capacity` are stored)   */
+    int64_t *sweep;        /* [capacity]                                        */
+    double  *T;            /* [capacity]                                        */
+    int64_t *E;            /* [capacity][n_sys]      H_EA, Eq. (1)              */
+    int64_t *E_daemon;     /* [capacity][n_sys]      H_aux = sum of n, Eq. (4)  */
+    int64_t *Q;            /* [capacity][n_pairs]    N*q, Eq. (C.1)             */
+} micsa_trace;
+
+/* Static description of the last error on this thread ("" if none). */
+const char *micsa_last_error(void);
+
+/* ---- life cycle ---------------------------------------------------------
+ * micsa_create: allocates device state on the current CUDA device and the
+ * default stream, then initialises it with Philox4x32-10 keyed by `seed`
+ * (R8): spins i.i.d. +-1 ("fully disordered" start),
+ * bonds i.i.d. +-1 with p = 1/2, daemons 0.
+ * Errors (NULL returned, see micsa_last_error): L < 2 or L odd (checkerboard
+ * with periodic boundaries needs even L), n_samples < 1,
+ * n_replicas < 1, N*n_sys overflow, no device, out of memory.
+ *
+ * micsa_create_ex: same, with
+ *   sample_offset  global index of this context's first sample; Philox
+ *                  counters use sample_offset + sample, so a run sharded by
+ *                  sample over several GPUs reproduces the unsharded run.
+ *                  Must be a multiple of 4 and >= 0.
+ *   dev_workspace  device memory of at least micsa_workspace_bytes(...) bytes,
+ *                  256-byte aligned, owned by the caller (e.g. a torch tensor)
+ *                  and kept alive until micsa_destroy; NULL = the library
+ *                  allocates with cudaMalloc.
+ *   cuda_stream    a cudaStream_t passed as void*; NULL = default stream.     */
+micsa_ctx *micsa_create(int L, int n_samples, int n_replicas, uint64_t seed);
+micsa_ctx *micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
+                           int sample_offset, void *dev_workspace,
+                           size_t workspace_bytes, void *cuda_stream);
+size_t     micsa_workspace_bytes(int L, int n_samples, int n_replicas);
+int        micsa_destroy(micsa_ctx *ctx);            /* NULL is a no-op */
+int        micsa_synchronize(micsa_ctx *ctx);        /* waits for the stream */
+
+/* ---- state in / out (canonical layouts above; host pointers; synchronous) -
+ * micsa_set_couplings: J = +-1 with replicas sharing the sample's bonds; any
+ * other value -> MICSA_ERR_INVALID and the stored bonds are unchanged.
+ * micsa_set_spins / micsa_set_daemons: same rule (values +-1 / 0..3).
+ * micsa_get_state: any of s, m, J may be NULL.                               */
+int micsa_set_couplings(micsa_ctx *ctx, const int8_t *J);
+int micsa_set_spins(micsa_ctx *ctx, const int8_t *s);
+int micsa_set_daemons(micsa_ctx *ctx, const uint8_t *m);
+int micsa_get_state(micsa_ctx *ctx, int8_t *s, uint8_t *m, int8_t *J);
+
+/* ---- the hot path ------------------------------------------------------
+ * micsa_sweep: n full sweeps; one sweep = elementary move on all even sites,
+ * then on all odd sites.  Elementary move on site x
+ * (PAPER.md:119-124 Eq. 8, :150 Eq. 10): dH = change of H_EA if s_x flips;
+ * if 0 <= n_x - dH <= 12 then s_x <- -s_x, n_x <- n_x - dH; else nothing.
+ * No random numbers.  Asynchronous.  n < 0 -> MICSA_ERR_INVALID; n = 0 no-op.
+ * micsa_half_sweep: the move on one parity only (0 even, 1 odd); applying it
+ * twice restores the state.                                   */
+int micsa_sweep(micsa_ctx *ctx, int n);
+int micsa_half_sweep(micsa_ctx *ctx, int parity);
+
+/* micsa_refresh_demons: every daemon <- independent draw from Eq. (11),
+ * p(n=4m) ~ exp(-4m/T), m = 0..3; spins untouched
+ * (PAPER.md:190).  One 32-bit Philox4x32-10 output per daemon, counter =
+ * (site i, global_sample/4, replica, step), key = seed, output word
+ * global_sample%4, compared with integer thresholds floor(cdf_k * 2^32)
+ * computed on the host (R7, R8).  Same (seed, step, T) => same
+ * daemons whatever happened before.  Asynchronous.  T must be finite and > 0. */
+int micsa_refresh_demons(micsa_ctx *ctx, double T, uint32_t step);
+
+/* The thresholds micsa_refresh_demons uses: thr[k] = floor(cdf_k * 2^32),
+ * k = 0,1,2, each in [0, 2^32]; level m = #{k : u >= thr[k]}.               */
+int micsa_debug_thresholds(double T, uint64_t thr[3]);
+
+/* micsa_measure_i64 (synchronous): exact integer sums into host arrays, any
+ * may be NULL:
+ *   E[n_sys]        H_EA = -sum_<xy> J s s                 (Eq. 1)
+ *   E_daemon[n_sys] H_aux = sum_x n_x = 4 sum_x m_x        (Eq. 4)
+ *   Q[n_samples * n_replicas(n_replicas-1)/2]  sum_x s^a_x s^b_x for replica
+ *                   pairs a < b of each sample, pairs in lexicographic order
+ *                                                          (PAPER.md:441 C.1)
+ * micsa_measure: the same divided by N as float64 (e of Eq. 15, PAPER.md:255;
+ * q of Eq. C.1).  Q != NULL with n_replicas < 2 -> MICSA_ERR_INVALID.        */
+int micsa_measure_i64(micsa_ctx *ctx, int64_t *E, int64_t *E_daemon, int64_t *Q);
+int micsa_measure(micsa_ctx *ctx, double *energy, double *demon_energy,
+                  double *q_overlap);
+
+/* micsa_anneal: for k = 0..n_steps-1: refresh(T_k, step0 + k); n_sweeps_k
+ * sweeps with measurement rows as micsa_step says.  The whole schedule is
+ * queued without host synchronisation; rows are kept on the device and copied
+ * once at the end (synchronous on return).
+ *   min_energy  host [n_sys] or NULL: minimum over this call's rows of E/N
+ *               (+inf if there was no row).
+ *   trace       host struct or NULL.                                         */
+int micsa_anneal(micsa_ctx *ctx, const micsa_step *sched, int n_steps,
+                 uint32_t step0, double *min_energy, micsa_trace *trace);
+
+/* Running totals since create: spin-flip attempts, 32-bit random numbers
+ * consumed by refreshes (one per daemon), Philox4x32-10 blocks evaluated by
+ * refreshes.  Initialisation draws are not counted.  Any pointer may be NULL. */
+int micsa_counters(micsa_ctx *ctx, uint64_t *attempts, uint64_t *rns_drawn,
+                   uint64_t *philox_calls);
+
+/* Geometry of the private device layout, for roofline accounting:
+ * info[0] = bytes of packed state (spins + daemons + bonds),
+ * info[1] = bytes one sweep must read+write at least once (compulsory),
+ * info[2] = number of 32-bit spin words per site, info[3] = bits per bond word,
+ * info[4] = kernel launches issued so far on this context.                   */
+int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MICSA_H */

@@ -1,0 +1,258 @@
+"""paper_2506_16240_b200 -- Python binding of libmicsa.so (include/micsa.h).
+
+Argument marshalling only: every step of the MicSA path (sweep, daemon
+refresh, reductions) runs in the CUDA kernels of ``csrc/``.  PyTorch is used
+for device memory (the workspace tensor) and the CUDA stream, nothing else.
+There is no CPU fallback: importing this package raises if ``libmicsa.so`` has
+not been built (``python -m paper_2506_16240_b200.build``), and creating a
+context raises without a CUDA device.
+
+Method names mirror the C ABI: ``micsa_create`` -> ``MicSA(...)``,
+``micsa_sweep`` -> ``.sweep(n)``, ``micsa_refresh_demons`` ->
+``.refresh_demons(T, step)``, ``micsa_measure`` -> ``.measure()``,
+``micsa_anneal`` -> ``.anneal(schedule)`` ...
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libmicsa.so"
+
+MICSA_OK, MICSA_ERR_INVALID, MICSA_ERR_NOMEM, MICSA_ERR_CUDA = 0, -1, -2, -3
+
+EXPORTS = (
+    "micsa_last_error", "micsa_create", "micsa_create_ex", "micsa_workspace_bytes",
+    "micsa_destroy", "micsa_synchronize", "micsa_set_couplings", "micsa_set_spins",
+    "micsa_set_daemons", "micsa_get_state", "micsa_sweep", "micsa_half_sweep",
+    "micsa_refresh_demons", "micsa_debug_thresholds", "micsa_measure_i64",
+    "micsa_measure", "micsa_anneal", "micsa_counters", "micsa_layout_info",
+)
+
+
+class MicsaError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"micsa error {code}: {msg}")
+        self.code = code
+
+
+class _Step(ctypes.Structure):
+    _fields_ = [("T", ctypes.c_double), ("n_sweeps", ctypes.c_int32),
+                ("measure_every", ctypes.c_int32)]
+
+
+class _Trace(ctypes.Structure):
+    _fields_ = [("capacity", ctypes.c_int64), ("n_rows", ctypes.c_int64),
+                ("sweep", ctypes.c_void_p), ("T", ctypes.c_void_p),
+                ("E", ctypes.c_void_p), ("E_daemon", ctypes.c_void_p),
+                ("Q", ctypes.c_void_p)]
+
+
+def _load() -> ctypes.CDLL:
+    if not LIB_PATH.exists():
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2506_16240_b200.build` "
+            "(nvcc, sm_100a). This package has no CPU fallback.")
+    lib = ctypes.CDLL(str(LIB_PATH))
+    vp, i32, u32, u64, f64 = (ctypes.c_void_p, ctypes.c_int, ctypes.c_uint32,
+                              ctypes.c_uint64, ctypes.c_double)
+    lib.micsa_last_error.restype = ctypes.c_char_p
+    lib.micsa_last_error.argtypes = []
+    lib.micsa_create.restype = vp
+    lib.micsa_create.argtypes = [i32, i32, i32, u64]
+    lib.micsa_create_ex.restype = vp
+    lib.micsa_create_ex.argtypes = [i32, i32, i32, u64, i32, vp, ctypes.c_size_t, vp]
+    lib.micsa_workspace_bytes.restype = ctypes.c_size_t
+    lib.micsa_workspace_bytes.argtypes = [i32, i32, i32]
+    for name, args in (
+            ("micsa_destroy", [vp]), ("micsa_synchronize", [vp]),
+            ("micsa_set_couplings", [vp, vp]), ("micsa_set_spins", [vp, vp]),
+            ("micsa_set_daemons", [vp, vp]), ("micsa_get_state", [vp, vp, vp, vp]),
+            ("micsa_sweep", [vp, i32]), ("micsa_half_sweep", [vp, i32]),
+            ("micsa_refresh_demons", [vp, f64, u32]),
+            ("micsa_debug_thresholds", [f64, vp]),
+            ("micsa_measure_i64", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
+            ("micsa_anneal", [vp, vp, i32, u32, vp, vp]),
+            ("micsa_counters", [vp, vp, vp, vp]), ("micsa_layout_info", [vp, vp])):
+        fn = getattr(lib, name)
+        fn.restype = i32
+        fn.argtypes = args
+    return lib
+
+
+_lib = _load()
+
+
+def last_error() -> str:
+    return _lib.micsa_last_error().decode()
+
+
+def _check(rc):
+    if rc != MICSA_OK:
+        raise MicsaError(rc, last_error())
+
+
+def _ptr(a):
+    return None if a is None else ctypes.c_void_p(a.ctypes.data)
+
+
+def debug_thresholds(T: float) -> np.ndarray:
+    """micsa_debug_thresholds: the integer thresholds of Eq. (11) (R7)."""
+    thr = np.zeros(3, dtype=np.uint64)
+    _check(_lib.micsa_debug_thresholds(float(T), _ptr(thr)))
+    return thr
+
+
+def workspace_bytes(L, n_samples, n_replicas) -> int:
+    return int(_lib.micsa_workspace_bytes(L, n_samples, n_replicas))
+
+
+class MicSA:
+    """One MicSA context (micsa_create_ex).  Device memory and stream come from
+    torch when ``use_torch`` (default), else the library allocates itself."""
+
+    def __init__(self, L, n_samples, n_replicas, seed, sample_offset=0, device=0,
+                 use_torch=True, stream=None):
+        self.L, self.n_samples, self.n_replicas = int(L), int(n_samples), int(n_replicas)
+        self.N = self.L ** 3
+        self.n_sys = self.n_samples * self.n_replicas
+        self.n_pairs = self.n_samples * (self.n_replicas * (self.n_replicas - 1) // 2)
+        self.seed = int(seed)
+        self._h = None
+        self._ws = None
+        self._stream = None
+        ws_ptr, ws_bytes, stream_ptr = None, 0, None
+        if use_torch:
+            import torch
+            if not torch.cuda.is_available():
+                raise MicsaError(MICSA_ERR_CUDA, "no CUDA device (this library has no CPU fallback)")
+            torch.cuda.set_device(device)
+            nbytes = workspace_bytes(self.L, self.n_samples, self.n_replicas)
+            if nbytes == 0:
+                raise MicsaError(MICSA_ERR_INVALID, last_error())
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{device}")
+            base = self._ws.data_ptr()
+            ws_ptr = (base + 255) // 256 * 256
+            ws_bytes = nbytes
+            self._stream = stream if stream is not None else torch.cuda.current_stream()
+            stream_ptr = self._stream.cuda_stream
+        h = _lib.micsa_create_ex(self.L, self.n_samples, self.n_replicas, self.seed,
+                                 int(sample_offset), ws_ptr, ws_bytes, stream_ptr)
+        if not h:
+            raise MicsaError(MICSA_ERR_INVALID, last_error())
+        self._h = ctypes.c_void_p(h)
+
+    # -- life cycle
+    def destroy(self):
+        if self._h is not None:
+            _lib.micsa_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def synchronize(self):
+        _check(_lib.micsa_synchronize(self._h))
+
+    # -- state in / out (canonical layouts of micsa.h)
+    def set_couplings(self, J):
+        J = np.ascontiguousarray(J, dtype=np.int8)
+        assert J.shape == (self.n_samples, 3, self.N), J.shape
+        _check(_lib.micsa_set_couplings(self._h, _ptr(J)))
+
+    def set_spins(self, s):
+        s = np.ascontiguousarray(s, dtype=np.int8)
+        assert s.shape == (self.n_samples, self.n_replicas, self.N), s.shape
+        _check(_lib.micsa_set_spins(self._h, _ptr(s)))
+
+    def set_daemons(self, m):
+        m = np.ascontiguousarray(m, dtype=np.uint8)
+        assert m.shape == (self.n_samples, self.n_replicas, self.N), m.shape
+        _check(_lib.micsa_set_daemons(self._h, _ptr(m)))
+
+    def get_state(self, spins=True, daemons=True, couplings=True):
+        s = np.empty((self.n_samples, self.n_replicas, self.N), np.int8) if spins else None
+        m = np.empty((self.n_samples, self.n_replicas, self.N), np.uint8) if daemons else None
+        J = np.empty((self.n_samples, 3, self.N), np.int8) if couplings else None
+        _check(_lib.micsa_get_state(self._h, _ptr(s), _ptr(m), _ptr(J)))
+        return s, m, J
+
+    # -- hot path
+    def sweep(self, n=1):
+        _check(_lib.micsa_sweep(self._h, int(n)))
+
+    def half_sweep(self, parity):
+        _check(_lib.micsa_half_sweep(self._h, int(parity)))
+
+    def refresh_demons(self, T, step):
+        _check(_lib.micsa_refresh_demons(self._h, float(T), int(step)))
+
+    def measure_i64(self):
+        E = np.empty(self.n_sys, np.int64)
+        Ed = np.empty(self.n_sys, np.int64)
+        Q = np.empty(self.n_pairs, np.int64) if self.n_replicas >= 2 else None
+        _check(_lib.micsa_measure_i64(self._h, _ptr(E), _ptr(Ed), _ptr(Q)))
+        return E, Ed, (Q if Q is not None else np.empty(0, np.int64))
+
+    def measure(self):
+        e = np.empty(self.n_sys, np.float64)
+        ed = np.empty(self.n_sys, np.float64)
+        q = np.empty(self.n_pairs, np.float64) if self.n_replicas >= 2 else None
+        _check(_lib.micsa_measure(self._h, _ptr(e), _ptr(ed), _ptr(q)))
+        return e, ed, (q if q is not None else np.empty(0, np.float64))
+
+    def anneal(self, schedule, step0=0, trace=True):
+        """schedule: iterable of (T, n_sweeps, measure_every).  Returns a dict
+        with the measurement rows (exact int64 sums) and min_energy (E/N)."""
+        sched = list(schedule)
+        arr = (_Step * max(len(sched), 1))()
+        rows = 0
+        for k, (T, n, every) in enumerate(sched):
+            arr[k].T, arr[k].n_sweeps, arr[k].measure_every = float(T), int(n), int(every)
+            if every > 0:
+                rows += int(n) // int(every)
+        min_e = np.empty(self.n_sys, np.float64)
+        out = {}
+        tr = None
+        if trace:
+            cap = max(rows, 1)
+            out = {"sweep": np.zeros(cap, np.int64), "T": np.zeros(cap, np.float64),
+                   "E": np.zeros((cap, self.n_sys), np.int64),
+                   "Edem": np.zeros((cap, self.n_sys), np.int64),
+                   "Q": np.zeros((cap, self.n_pairs), np.int64)}
+            tr = _Trace(cap, 0, out["sweep"].ctypes.data, out["T"].ctypes.data,
+                        out["E"].ctypes.data, out["Edem"].ctypes.data,
+                        out["Q"].ctypes.data if self.n_pairs else None)
+        _check(_lib.micsa_anneal(self._h, arr, len(sched), int(step0), _ptr(min_e),
+                                 ctypes.byref(tr) if tr is not None else None))
+        if trace:
+            out = {k: v[:rows] for k, v in out.items()}
+            assert tr.n_rows == rows
+        out["min_energy"] = min_e
+        return out
+
+    # -- accounting
+    def counters(self):
+        a, r, p = ctypes.c_uint64(), ctypes.c_uint64(), ctypes.c_uint64()
+        _check(_lib.micsa_counters(self._h, ctypes.byref(a), ctypes.byref(r), ctypes.byref(p)))
+        return {"attempts": a.value, "rns_drawn": r.value, "philox_calls": p.value}
+
+    def layout_info(self):
+        info = np.zeros(5, np.uint64)
+        _check(_lib.micsa_layout_info(self._h, _ptr(info)))
+        return {"state_bytes": int(info[0]), "compulsory_bytes_per_sweep": int(info[1]),
+                "words_per_site": int(info[2]), "bond_bits": int(info[3]),
+                "launches": int(info[4])}

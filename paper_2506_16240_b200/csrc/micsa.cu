@@ -1,0 +1,581 @@
+// micsa.cu -- context management and the C ABI of include/micsa.h.
+// Every step of the path runs in the kernels of sweep.cuh / refresh.cuh /
+// measure.cuh; this file only validates arguments, sizes grids and queues
+// launches on the context's stream.  There is no CPU fallback.
+#include "../../include/micsa.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <vector>
+
+#include "layout.cuh"
+#include "measure.cuh"
+#include "pack.cuh"
+#include "philox.cuh"
+#include "refresh.cuh"
+#include "sweep.cuh"
+
+using namespace micsa;
+
+namespace {
+
+thread_local char g_err[256] = "";
+
+void set_err(const char* fmt, const char* detail = "") {
+    snprintf(g_err, sizeof g_err, fmt, detail);
+}
+
+constexpr size_t kAlign = 256;
+size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+struct Plan {                 // byte offsets inside the workspace
+    size_t spin, m0, m1, J, cnt, row, minE, bad, total;
+    size_t plane_bytes, J_bytes, cnt_words, row_len;
+};
+
+bool make_geom(int L, int n_samples, int n_replicas, int sample_offset, Geom& g) {
+    if (L < 2 || (L & 1)) { set_err("L must be even and >= 2"); return false; }
+    if (n_samples < 1 || n_replicas < 1) { set_err("n_samples and n_replicas must be >= 1"); return false; }
+    if (sample_offset < 0 || (sample_offset & 3)) { set_err("sample_offset must be a non-negative multiple of 4"); return false; }
+    const long long N = (long long)L * L * L;
+    if (N > 0xFFFFFFFFll) { set_err("L^3 must fit 32 bits (site index is one Philox counter word)"); return false; }
+    if ((long long)n_samples * n_replicas > (1ll << 24) || n_replicas >= (1 << 24)) {
+        set_err("too many systems"); return false;
+    }
+    if ((long long)sample_offset + n_samples > 0x7FFFFFFFll) { set_err("sample index overflow"); return false; }
+    g.L = L; g.Lh = L / 2;
+    g.n_samples = n_samples; g.n_replicas = n_replicas; g.sample_offset = sample_offset;
+    g.rpw = (n_replicas % 2 == 0) ? 2 : 1;
+    g.spw = 32 / g.rpw;
+    g.n_sg = (n_samples + g.spw - 1) / g.spw;
+    g.n_rg = n_replicas / g.rpw;
+    if ((long long)g.n_sg * g.n_rg * 2 > 65535 || (long long)g.n_sg * 6 > 65535) {
+        set_err("too many word lattices for one grid"); return false;
+    }
+    g.n_words = g.n_sg * g.n_rg;
+    g.half = (long long)L * L * g.Lh;
+    g.N = N;
+    g.n_sys = n_samples * n_replicas;
+    g.n_pairs = n_samples * (n_replicas * (n_replicas - 1) / 2);
+    return true;
+}
+
+Plan make_plan(const Geom& g) {
+    Plan p;
+    p.plane_bytes = (size_t)g.n_words * 2 * g.half * sizeof(uint32_t);
+    p.J_bytes = (size_t)g.n_sg * 6 * g.half * (g.rpw == 2 ? 2 : 4);
+    const int pps = g.n_replicas * (g.n_replicas - 1) / 2;
+    p.cnt_words = (size_t)g.n_words * 32 * 2 + (size_t)g.n_sg * pps * 32;
+    p.row_len = (size_t)2 * g.n_sys + g.n_pairs;
+    size_t o = 0;
+    p.spin = o; o += align_up(p.plane_bytes);
+    p.m0 = o;   o += align_up(p.plane_bytes);
+    p.m1 = o;   o += align_up(p.plane_bytes);
+    p.J = o;    o += align_up(p.J_bytes);
+    p.cnt = o;  o += align_up(p.cnt_words * 8);
+    p.row = o;  o += align_up(p.row_len * 8);
+    p.minE = o; o += align_up((size_t)g.n_sys * 8);
+    p.bad = o;  o += align_up(sizeof(int));
+    p.total = o;
+    return p;
+}
+
+int vec_width(int Lh) { return (Lh % 4 == 0) ? 4 : (Lh % 2 == 0) ? 2 : 1; }
+
+}  // namespace
+
+struct micsa_ctx {
+    Geom g;
+    Plan plan;
+    State st;
+    PhiloxKeys ks;
+    uint64_t seed;
+    cudaStream_t stream;
+    char* ws;
+    bool owns_ws;
+    unsigned long long* cnt;
+    long long* row;
+    long long* minE;
+    int* bad;
+    int V;
+    uint64_t attempts, rns, philox_calls, launches;
+    int sticky;
+};
+
+namespace {
+
+#define CK(ctx, call)                                                          \
+    do {                                                                       \
+        cudaError_t e_ = (call);                                               \
+        if (e_ != cudaSuccess) {                                               \
+            set_err("CUDA error: %s", cudaGetErrorString(e_));                 \
+            if (ctx) (ctx)->sticky = MICSA_ERR_CUDA;                           \
+            return MICSA_ERR_CUDA;                                             \
+        }                                                                      \
+    } while (0)
+
+int check_ctx(micsa_ctx* c) {
+    if (!c) { set_err("null context"); return MICSA_ERR_INVALID; }
+    if (c->sticky) { set_err("context is in a sticky CUDA error state"); return c->sticky; }
+    return MICSA_OK;
+}
+
+SiteGrid site_grid(const Geom& g) {
+    SiteGrid s; s.L = g.L; s.Lh = g.Lh; s.n_rg = g.n_rg; s.n_samples = g.n_samples;
+    s.sample_offset = g.sample_offset; s.half = g.half;
+    return s;
+}
+
+dim3 site_blocks(const Geom& g, int nz) {
+    return dim3((unsigned)((g.L * g.Lh + 127) / 128), (unsigned)g.L, (unsigned)nz);
+}
+
+int post_launch(micsa_ctx* c, int n = 1) {
+    c->launches += (uint64_t)n;
+    CK(c, cudaGetLastError());
+    return MICSA_OK;
+}
+
+// ---- launches -----------------------------------------------------------
+template <int V, int RPW>
+void launch_half_sweep_t(micsa_ctx* c, int parity) {
+    SweepArgs a;
+    a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half;
+    const int per_plane = c->g.L * (c->g.Lh / V);
+    dim3 grid((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
+    half_sweep_kernel<V, RPW><<<grid, 128, 0, c->stream>>>(a, parity);
+}
+
+int launch_half_sweep(micsa_ctx* c, int parity) {
+    const int key = c->V * 10 + c->g.rpw;
+    switch (key) {
+        case 41: launch_half_sweep_t<4, 1>(c, parity); break;
+        case 42: launch_half_sweep_t<4, 2>(c, parity); break;
+        case 21: launch_half_sweep_t<2, 1>(c, parity); break;
+        case 22: launch_half_sweep_t<2, 2>(c, parity); break;
+        case 11: launch_half_sweep_t<1, 1>(c, parity); break;
+        default: launch_half_sweep_t<1, 2>(c, parity); break;
+    }
+    c->attempts += (uint64_t)(c->g.N / 2) * (uint64_t)c->g.n_sys;
+    return post_launch(c);
+}
+
+int thresholds_host(double T, uint64_t thr[3]) {
+    if (!(T > 0.0) || !std::isfinite(T)) return MICSA_ERR_INVALID;
+    // DESIGN.md R7: cumulative Eq. (11) in float64, this operation order
+    const double x = std::exp(-4.0 / T);
+    const double x2 = x * x;
+    const double x3 = x2 * x;
+    const double Z = ((1.0 + x) + x2) + x3;
+    const double cdf[3] = { 1.0 / Z, (1.0 + x) / Z, ((1.0 + x) + x2) / Z };
+    for (int k = 0; k < 3; ++k) {
+        double t = std::floor(std::ldexp(cdf[k], 32));
+        if (t > 4294967296.0) t = 4294967296.0;
+        thr[k] = (uint64_t)t;
+    }
+    return MICSA_OK;
+}
+
+int launch_refresh(micsa_ctx* c, double T, uint32_t step) {
+    uint64_t thr[3];
+    if (thresholds_host(T, thr) != MICSA_OK || thr[0] == 0) {
+        set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID;
+    }
+    const uint32_t a0 = (uint32_t)(thr[0] - 1), a1 = (uint32_t)(thr[1] - 1), a2 = (uint32_t)(thr[2] - 1);
+    const SiteGrid sg = site_grid(c->g);
+    const dim3 grid = site_blocks(c->g, c->g.n_words * 2);
+    if (c->g.rpw == 2)
+        refresh_kernel<2><<<grid, 128, 0, c->stream>>>(c->st.m0, c->st.m1, sg, c->ks, step, a0, a1, a2);
+    else
+        refresh_kernel<1><<<grid, 128, 0, c->stream>>>(c->st.m0, c->st.m1, sg, c->ks, step, a0, a1, a2);
+    c->rns += (uint64_t)c->g.N * (uint64_t)c->g.n_sys;
+    c->philox_calls += (uint64_t)c->g.N * (uint64_t)c->g.n_sg * (uint64_t)(c->g.spw / 4) * (uint64_t)c->g.n_replicas;
+    return post_launch(c);
+}
+
+unsigned count_blocks(long long nvec, long long other) {
+    long long nb = (nvec + kCountBlock * 16 - 1) / (kCountBlock * 16);
+    const long long cap = std::max<long long>(1, (148 * 8) / std::max<long long>(1, other));
+    nb = std::min(nb, cap);
+    const long long need = (nvec + (long long)kCountBlock * 4096 - 1) / ((long long)kCountBlock * 4096);
+    nb = std::max<long long>(std::max<long long>(nb, need), 1);
+    return (unsigned)nb;
+}
+
+template <int V, int RPW>
+void launch_counts_t(micsa_ctx* c, const MeasureArgs& a) {
+    const Geom& g = c->g;
+    const long long nvec_p = g.half / V;
+    count_unsat_kernel<V, RPW><<<dim3(count_blocks(nvec_p, 2ll * g.n_words), 2, (unsigned)g.n_words),
+                                 kCountBlock, 0, c->stream>>>(a);
+    count_levels_kernel<V><<<dim3(count_blocks(2 * nvec_p, g.n_words), (unsigned)g.n_words),
+                             kCountBlock, 0, c->stream>>>(a);
+    c->launches += 2;
+    const int pps = g.n_replicas * (g.n_replicas - 1) / 2;
+    if (pps > 0) {
+        count_xor_kernel<V, RPW><<<dim3(count_blocks(2 * nvec_p, (long long)g.n_sg * pps),
+                                        (unsigned)g.n_sg, (unsigned)pps),
+                                   kCountBlock, 0, c->stream>>>(a);
+        c->launches += 1;
+    }
+}
+
+// one measurement: exact sums into the device row `row`, optional min fold
+int launch_measure(micsa_ctx* c, long long* row, bool fold_min) {
+    const Geom& g = c->g;
+    if (g.n_replicas * (g.n_replicas - 1) / 2 > 65535) { set_err("too many replica pairs"); return MICSA_ERR_INVALID; }
+    CK(c, cudaMemsetAsync(c->cnt, 0, c->plan.cnt_words * 8, c->stream));
+    MeasureArgs a;
+    a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
+    a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg; a.n_replicas = g.n_replicas; a.n_samples = g.n_samples;
+    a.half = g.half;
+    a.cntU = c->cnt; a.cntM = c->cnt + (size_t)g.n_words * 32; a.cntX = c->cnt + (size_t)g.n_words * 64;
+    switch (c->V * 10 + g.rpw) {
+        case 41: launch_counts_t<4, 1>(c, a); break;
+        case 42: launch_counts_t<4, 2>(c, a); break;
+        case 21: launch_counts_t<2, 1>(c, a); break;
+        case 22: launch_counts_t<2, 2>(c, a); break;
+        case 11: launch_counts_t<1, 1>(c, a); break;
+        default: launch_counts_t<1, 2>(c, a); break;
+    }
+    FinalizeArgs f;
+    f.cntU = a.cntU; f.cntM = a.cntM; f.cntX = a.cntX;
+    f.row = row; f.min_E = fold_min ? c->minE : nullptr;
+    f.n_samples = g.n_samples; f.n_replicas = g.n_replicas; f.n_rg = g.n_rg;
+    f.rpw = g.rpw; f.spw = g.spw; f.pairs_per_sample = g.n_replicas * (g.n_replicas - 1) / 2;
+    f.N = g.N;
+    const int n = std::max(g.n_sys, g.n_pairs);
+    finalize_measure_kernel<<<(n + 127) / 128, 128, 0, c->stream>>>(f);
+    return post_launch(c);
+}
+
+// host <-> device staging for the canonical layouts
+struct Staging {
+    void* dev = nullptr;
+    ~Staging() { if (dev) cudaFree(dev); }
+};
+
+int set_sys(micsa_ctx* c, const int8_t* src, int kind) {
+    int rc = check_ctx(c); if (rc) return rc;
+    if (!src) { set_err("null pointer"); return MICSA_ERR_INVALID; }
+    const Geom& g = c->g;
+    const size_t bytes = (size_t)g.n_sys * (size_t)g.N;
+    Staging st;
+    if (cudaMalloc(&st.dev, bytes) != cudaSuccess) { cudaGetLastError(); set_err("out of device memory (staging)"); return MICSA_ERR_NOMEM; }
+    CK(c, cudaMemcpyAsync(st.dev, src, bytes, cudaMemcpyHostToDevice, c->stream));
+    CK(c, cudaMemsetAsync(c->bad, 0, sizeof(int), c->stream));
+    validate_kernel<<<148 * 4, 256, 0, c->stream>>>((const int8_t*)st.dev, (long long)bytes, kind, c->bad);
+    rc = post_launch(c); if (rc) return rc;
+    int bad = 0;
+    CK(c, cudaMemcpyAsync(&bad, c->bad, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CK(c, cudaStreamSynchronize(c->stream));
+    if (bad) { set_err(kind == 0 ? "spin values must be -1 or +1" : "daemon levels must be 0..3"); return MICSA_ERR_INVALID; }
+    const SiteGrid sg = site_grid(g);
+    const dim3 grid = site_blocks(g, g.n_words * 2);
+    uint32_t* d0 = kind == 0 ? c->st.spin : c->st.m0;
+    if (g.rpw == 2) pack_sys_kernel<2><<<grid, 128, 0, c->stream>>>((const int8_t*)st.dev, d0, c->st.m1, sg, g.n_replicas, kind);
+    else            pack_sys_kernel<1><<<grid, 128, 0, c->stream>>>((const int8_t*)st.dev, d0, c->st.m1, sg, g.n_replicas, kind);
+    rc = post_launch(c); if (rc) return rc;
+    CK(c, cudaStreamSynchronize(c->stream));
+    return MICSA_OK;
+}
+
+int init_state(micsa_ctx* c) {
+    const Geom& g = c->g;
+    const SiteGrid sg = site_grid(g);
+    CK(c, cudaMemsetAsync(c->st.m0, 0, c->plan.plane_bytes, c->stream));
+    CK(c, cudaMemsetAsync(c->st.m1, 0, c->plan.plane_bytes, c->stream));
+    if (g.rpw == 2) {
+        init_spins_kernel<2><<<site_blocks(g, g.n_words * 2), 128, 0, c->stream>>>(c->st.spin, sg, c->ks);
+        init_bonds_kernel<2><<<site_blocks(g, g.n_sg * 6), 128, 0, c->stream>>>((uint16_t*)c->st.J, sg, c->ks);
+    } else {
+        init_spins_kernel<1><<<site_blocks(g, g.n_words * 2), 128, 0, c->stream>>>(c->st.spin, sg, c->ks);
+        init_bonds_kernel<1><<<site_blocks(g, g.n_sg * 6), 128, 0, c->stream>>>((uint32_t*)c->st.J, sg, c->ks);
+    }
+    int rc = post_launch(c, 2); if (rc) return rc;
+    CK(c, cudaStreamSynchronize(c->stream));
+    return MICSA_OK;
+}
+
+}  // namespace
+
+// =========================================================================
+extern "C" {
+
+const char* micsa_last_error(void) { return g_err; }
+
+size_t micsa_workspace_bytes(int L, int n_samples, int n_replicas) {
+    Geom g;
+    if (!make_geom(L, n_samples, n_replicas, 0, g)) return 0;
+    return make_plan(g).total;
+}
+
+micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
+                           int sample_offset, void* dev_workspace, size_t workspace_bytes,
+                           void* cuda_stream)
+{
+    g_err[0] = 0;
+    Geom g;
+    if (!make_geom(L, n_samples, n_replicas, sample_offset, g)) return nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        set_err("no usable CUDA device (this library has no CPU fallback)");
+        return nullptr;
+    }
+    micsa_ctx* c = new (std::nothrow) micsa_ctx();
+    if (!c) { set_err("out of host memory"); return nullptr; }
+    c->g = g;
+    c->plan = make_plan(g);
+    c->seed = seed;
+    c->ks = philox_make_keys(seed);
+    c->stream = (cudaStream_t)cuda_stream;
+    c->V = vec_width(g.Lh);
+    c->attempts = c->rns = c->philox_calls = c->launches = 0;
+    c->sticky = 0;
+    if (dev_workspace) {
+        if (workspace_bytes < c->plan.total || ((uintptr_t)dev_workspace % kAlign)) {
+            set_err("workspace too small or not 256-byte aligned"); delete c; return nullptr;
+        }
+        c->ws = (char*)dev_workspace; c->owns_ws = false;
+    } else {
+        void* p = nullptr;
+        if (cudaMalloc(&p, c->plan.total) != cudaSuccess) {
+            cudaGetLastError(); set_err("out of device memory"); delete c; return nullptr;
+        }
+        c->ws = (char*)p; c->owns_ws = true;
+    }
+    c->st.spin = (uint32_t*)(c->ws + c->plan.spin);
+    c->st.m0 = (uint32_t*)(c->ws + c->plan.m0);
+    c->st.m1 = (uint32_t*)(c->ws + c->plan.m1);
+    c->st.J = (void*)(c->ws + c->plan.J);
+    c->cnt = (unsigned long long*)(c->ws + c->plan.cnt);
+    c->row = (long long*)(c->ws + c->plan.row);
+    c->minE = (long long*)(c->ws + c->plan.minE);
+    c->bad = (int*)(c->ws + c->plan.bad);
+    if (init_state(c) != MICSA_OK) { if (c->owns_ws) cudaFree(c->ws); delete c; return nullptr; }
+    return c;
+}
+
+micsa_ctx* micsa_create(int L, int n_samples, int n_replicas, uint64_t seed) {
+    return micsa_create_ex(L, n_samples, n_replicas, seed, 0, nullptr, 0, nullptr);
+}
+
+int micsa_destroy(micsa_ctx* c) {
+    if (!c) return MICSA_OK;
+    cudaStreamSynchronize(c->stream);
+    if (c->owns_ws) cudaFree(c->ws);
+    delete c;
+    return MICSA_OK;
+}
+
+int micsa_synchronize(micsa_ctx* c) {
+    int rc = check_ctx(c); if (rc) return rc;
+    CK(c, cudaStreamSynchronize(c->stream));
+    return MICSA_OK;
+}
+
+int micsa_set_spins(micsa_ctx* c, const int8_t* s) { return set_sys(c, s, 0); }
+int micsa_set_daemons(micsa_ctx* c, const uint8_t* m) { return set_sys(c, (const int8_t*)m, 1); }
+
+int micsa_set_couplings(micsa_ctx* c, const int8_t* J) {
+    int rc = check_ctx(c); if (rc) return rc;
+    if (!J) { set_err("null pointer"); return MICSA_ERR_INVALID; }
+    const Geom& g = c->g;
+    const size_t bytes = (size_t)g.n_samples * 3 * (size_t)g.N;
+    Staging st;
+    if (cudaMalloc(&st.dev, bytes) != cudaSuccess) { cudaGetLastError(); set_err("out of device memory (staging)"); return MICSA_ERR_NOMEM; }
+    CK(c, cudaMemcpyAsync(st.dev, J, bytes, cudaMemcpyHostToDevice, c->stream));
+    CK(c, cudaMemsetAsync(c->bad, 0, sizeof(int), c->stream));
+    validate_kernel<<<148 * 4, 256, 0, c->stream>>>((const int8_t*)st.dev, (long long)bytes, 0, c->bad);
+    rc = post_launch(c); if (rc) return rc;
+    int bad = 0;
+    CK(c, cudaMemcpyAsync(&bad, c->bad, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CK(c, cudaStreamSynchronize(c->stream));
+    if (bad) { set_err("couplings must be -1 or +1"); return MICSA_ERR_INVALID; }
+    const SiteGrid sg = site_grid(g);
+    const dim3 grid = site_blocks(g, g.n_sg * 6);
+    if (g.rpw == 2) pack_bonds_kernel<2><<<grid, 128, 0, c->stream>>>((const int8_t*)st.dev, (uint16_t*)c->st.J, sg);
+    else            pack_bonds_kernel<1><<<grid, 128, 0, c->stream>>>((const int8_t*)st.dev, (uint32_t*)c->st.J, sg);
+    rc = post_launch(c); if (rc) return rc;
+    CK(c, cudaStreamSynchronize(c->stream));
+    return MICSA_OK;
+}
+
+int micsa_get_state(micsa_ctx* c, int8_t* s, uint8_t* m, int8_t* J) {
+    int rc = check_ctx(c); if (rc) return rc;
+    const Geom& g = c->g;
+    const SiteGrid sg = site_grid(g);
+    const size_t sys_bytes = (size_t)g.n_sys * (size_t)g.N;
+    const size_t J_bytes = (size_t)g.n_samples * 3 * (size_t)g.N;
+    Staging st;
+    if (cudaMalloc(&st.dev, std::max(sys_bytes, J_bytes)) != cudaSuccess) { cudaGetLastError(); set_err("out of device memory (staging)"); return MICSA_ERR_NOMEM; }
+    for (int kind = 0; kind < 2; ++kind) {
+        void* dst = kind == 0 ? (void*)s : (void*)m;
+        if (!dst) continue;
+        const dim3 grid = site_blocks(g, g.n_words * 2);
+        const uint32_t* d0 = kind == 0 ? c->st.spin : c->st.m0;
+        if (g.rpw == 2) unpack_sys_kernel<2><<<grid, 128, 0, c->stream>>>((int8_t*)st.dev, d0, c->st.m1, sg, g.n_replicas, kind);
+        else            unpack_sys_kernel<1><<<grid, 128, 0, c->stream>>>((int8_t*)st.dev, d0, c->st.m1, sg, g.n_replicas, kind);
+        rc = post_launch(c); if (rc) return rc;
+        CK(c, cudaMemcpyAsync(dst, st.dev, sys_bytes, cudaMemcpyDeviceToHost, c->stream));
+        CK(c, cudaStreamSynchronize(c->stream));
+    }
+    if (J) {
+        const dim3 grid = site_blocks(g, g.n_sg * 6);
+        if (g.rpw == 2) unpack_bonds_kernel<2><<<grid, 128, 0, c->stream>>>((int8_t*)st.dev, (const uint16_t*)c->st.J, sg);
+        else            unpack_bonds_kernel<1><<<grid, 128, 0, c->stream>>>((int8_t*)st.dev, (const uint32_t*)c->st.J, sg);
+        rc = post_launch(c); if (rc) return rc;
+        CK(c, cudaMemcpyAsync(J, st.dev, J_bytes, cudaMemcpyDeviceToHost, c->stream));
+        CK(c, cudaStreamSynchronize(c->stream));
+    }
+    return MICSA_OK;
+}
+
+int micsa_half_sweep(micsa_ctx* c, int parity) {
+    int rc = check_ctx(c); if (rc) return rc;
+    if (parity != 0 && parity != 1) { set_err("parity must be 0 or 1"); return MICSA_ERR_INVALID; }
+    return launch_half_sweep(c, parity);
+}
+
+int micsa_sweep(micsa_ctx* c, int n) {
+    int rc = check_ctx(c); if (rc) return rc;
+    if (n < 0) { set_err("n must be >= 0"); return MICSA_ERR_INVALID; }
+    for (int t = 0; t < n; ++t) {
+        rc = launch_half_sweep(c, 0); if (rc) return rc;
+        rc = launch_half_sweep(c, 1); if (rc) return rc;
+    }
+    return MICSA_OK;
+}
+
+int micsa_debug_thresholds(double T, uint64_t thr[3]) {
+    if (!thr) { set_err("null pointer"); return MICSA_ERR_INVALID; }
+    if (thresholds_host(T, thr) != MICSA_OK) { set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID; }
+    return MICSA_OK;
+}
+
+int micsa_refresh_demons(micsa_ctx* c, double T, uint32_t step) {
+    int rc = check_ctx(c); if (rc) return rc;
+    return launch_refresh(c, T, step);
+}
+
+int micsa_measure_i64(micsa_ctx* c, int64_t* E, int64_t* Ed, int64_t* Q) {
+    int rc = check_ctx(c); if (rc) return rc;
+    const Geom& g = c->g;
+    if (Q && g.n_replicas < 2) { set_err("q_overlap needs n_replicas >= 2"); return MICSA_ERR_INVALID; }
+    rc = launch_measure(c, c->row, false); if (rc) return rc;
+    std::vector<long long> host(c->plan.row_len);
+    CK(c, cudaMemcpyAsync(host.data(), c->row, c->plan.row_len * 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(c, cudaStreamSynchronize(c->stream));
+    if (E)  memcpy(E, host.data(), (size_t)g.n_sys * 8);
+    if (Ed) memcpy(Ed, host.data() + g.n_sys, (size_t)g.n_sys * 8);
+    if (Q)  memcpy(Q, host.data() + 2 * g.n_sys, (size_t)g.n_pairs * 8);
+    return MICSA_OK;
+}
+
+int micsa_measure(micsa_ctx* c, double* e, double* ed, double* q) {
+    int rc = check_ctx(c); if (rc) return rc;
+    const Geom& g = c->g;
+    if (q && g.n_replicas < 2) { set_err("q_overlap needs n_replicas >= 2"); return MICSA_ERR_INVALID; }
+    std::vector<int64_t> E(g.n_sys), Ed(g.n_sys), Q(std::max(g.n_pairs, 1));
+    rc = micsa_measure_i64(c, E.data(), Ed.data(), g.n_pairs ? Q.data() : nullptr);
+    if (rc) return rc;
+    const double N = (double)g.N;
+    if (e)  for (int i = 0; i < g.n_sys; ++i) e[i] = (double)E[i] / N;
+    if (ed) for (int i = 0; i < g.n_sys; ++i) ed[i] = (double)Ed[i] / N;
+    if (q)  for (int i = 0; i < g.n_pairs; ++i) q[i] = (double)Q[i] / N;
+    return MICSA_OK;
+}
+
+int micsa_anneal(micsa_ctx* c, const micsa_step* sched, int n_steps, uint32_t step0,
+                 double* min_energy, micsa_trace* trace)
+{
+    int rc = check_ctx(c); if (rc) return rc;
+    if (n_steps < 0 || (n_steps > 0 && !sched)) { set_err("bad schedule"); return MICSA_ERR_INVALID; }
+    const Geom& g = c->g;
+    long long rows = 0;
+    for (int k = 0; k < n_steps; ++k) {
+        uint64_t thr[3];
+        if (thresholds_host(sched[k].T, thr) != MICSA_OK) { set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID; }
+        if (sched[k].n_sweeps < 0 || sched[k].measure_every < 0) { set_err("negative sweep count"); return MICSA_ERR_INVALID; }
+        if (sched[k].measure_every > 0) rows += sched[k].n_sweeps / sched[k].measure_every;
+    }
+    if (trace && trace->capacity < 0) { set_err("negative trace capacity"); return MICSA_ERR_INVALID; }
+    const long long keep = trace ? std::min<long long>(rows, trace->capacity) : 0;
+    const size_t row_len = c->plan.row_len;
+    Staging dev_rows;
+    if (keep > 0) {
+        if (cudaMalloc(&dev_rows.dev, (size_t)keep * row_len * 8) != cudaSuccess) {
+            cudaGetLastError(); set_err("out of device memory (trace)"); return MICSA_ERR_NOMEM;
+        }
+    }
+    fill_i64_kernel<<<(g.n_sys + 127) / 128, 128, 0, c->stream>>>(c->minE, std::numeric_limits<long long>::max(), g.n_sys);
+    rc = post_launch(c); if (rc) return rc;
+
+    std::vector<int64_t> row_sweep;
+    std::vector<double> row_T;
+    long long r = 0, t = 0;
+    for (int k = 0; k < n_steps; ++k) {
+        rc = launch_refresh(c, sched[k].T, step0 + (uint32_t)k); if (rc) return rc;
+        for (int j = 1; j <= sched[k].n_sweeps; ++j) {
+            rc = launch_half_sweep(c, 0); if (rc) return rc;
+            rc = launch_half_sweep(c, 1); if (rc) return rc;
+            ++t;
+            if (sched[k].measure_every > 0 && j % sched[k].measure_every == 0) {
+                long long* dst = (r < keep) ? (long long*)dev_rows.dev + (size_t)r * row_len : c->row;
+                rc = launch_measure(c, dst, true); if (rc) return rc;
+                if (r < keep) { row_sweep.push_back(t); row_T.push_back(sched[k].T); }
+                ++r;
+            }
+        }
+    }
+    std::vector<long long> host((size_t)keep * row_len);
+    std::vector<long long> minE(g.n_sys);
+    if (keep > 0)
+        CK(c, cudaMemcpyAsync(host.data(), dev_rows.dev, host.size() * 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(c, cudaMemcpyAsync(minE.data(), c->minE, (size_t)g.n_sys * 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(c, cudaStreamSynchronize(c->stream));
+    if (min_energy)
+        for (int i = 0; i < g.n_sys; ++i)
+            min_energy[i] = (rows > 0) ? (double)minE[i] / (double)g.N : std::numeric_limits<double>::infinity();
+    if (trace) {
+        trace->n_rows = rows;
+        for (long long i = 0; i < keep; ++i) {
+            const long long* src = host.data() + (size_t)i * row_len;
+            if (trace->sweep) trace->sweep[i] = row_sweep[i];
+            if (trace->T) trace->T[i] = row_T[i];
+            if (trace->E) memcpy(trace->E + (size_t)i * g.n_sys, src, (size_t)g.n_sys * 8);
+            if (trace->E_daemon) memcpy(trace->E_daemon + (size_t)i * g.n_sys, src + g.n_sys, (size_t)g.n_sys * 8);
+            if (trace->Q && g.n_pairs) memcpy(trace->Q + (size_t)i * g.n_pairs, src + 2 * g.n_sys, (size_t)g.n_pairs * 8);
+        }
+    }
+    return MICSA_OK;
+}
+
+int micsa_counters(micsa_ctx* c, uint64_t* attempts, uint64_t* rns, uint64_t* philox_calls) {
+    if (!c) { set_err("null context"); return MICSA_ERR_INVALID; }
+    if (attempts) *attempts = c->attempts;
+    if (rns) *rns = c->rns;
+    if (philox_calls) *philox_calls = c->philox_calls;
+    return MICSA_OK;
+}
+
+int micsa_layout_info(micsa_ctx* c, uint64_t info[5]) {
+    if (!c || !info) { set_err("null pointer"); return MICSA_ERR_INVALID; }
+    const Geom& g = c->g;
+    const uint64_t sites = (uint64_t)g.N;
+    const uint64_t spin_b = sites * g.n_words * 4, dem_b = 2 * spin_b;
+    const uint64_t J_b = 3 * sites * g.n_sg * (g.rpw == 2 ? 2 : 4);
+    info[0] = spin_b + dem_b + J_b;
+    info[1] = 2 * (spin_b + dem_b) + J_b;     // state read once + written once, bonds read once
+    info[2] = (uint64_t)g.n_words;
+    info[3] = (uint64_t)(32 / g.rpw);
+    info[4] = c->launches;
+    return MICSA_OK;
+}
+
+}  // extern "C"

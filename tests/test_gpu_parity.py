@@ -1,0 +1,329 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle (-m gpu).
+
+Bit-exact for spins, daemons, couplings and the integer sums; derived float
+observables within 1e-12 relative (BASELINE.json north_star).  Small cases are
+compared element by element after every sweep; BASELINE's full-size configs are
+compared on sampled systems (systems never interact, so the oracle can run any
+subset of samples on its own) plus exact invariants on all of them.
+"""
+import numpy as np
+import pytest
+
+from micsa_workloads import CONFIGS, random_levels, random_pm1, schedule_for
+from oracle import driver
+
+pytestmark = pytest.mark.gpu
+
+# (L, n_samples, n_replicas): V=4/2/1 vector paths, both bond-word widths,
+# ragged sample groups (lanes left empty), several word lattices
+SHAPES = [(8, 1, 2), (2, 1, 2), (4, 3, 2), (6, 5, 3), (8, 40, 2), (8, 33, 1),
+          (10, 2, 4), (16, 17, 2), (12, 70, 1), (24, 2, 2)]
+
+
+def _assert_state(g, s, m, J=None):
+    gs, gm, gJ = g.get_state(couplings=J is not None)
+    np.testing.assert_array_equal(gs, s)
+    np.testing.assert_array_equal(gm, m)
+    if J is not None:
+        np.testing.assert_array_equal(gJ, J)
+
+
+@pytest.mark.parametrize("L,ns,nr", SHAPES)
+def test_init_matches_oracle(micsa, oracle, L, ns, nr):
+    for seed, off in [(1, 0), (0xDEADBEEF12345678, 32), (7, 124)]:
+        with micsa.MicSA(L, ns, nr, seed, sample_offset=off) as g:
+            _assert_state(g, oracle.init_spins(L, ns, nr, seed, off),
+                          np.zeros((ns, nr, L ** 3), np.uint8),
+                          oracle.init_bonds(L, ns, seed, off))
+
+
+@pytest.mark.parametrize("L,ns,nr", SHAPES)
+def test_set_get_roundtrip(micsa, L, ns, nr):
+    N = L ** 3
+    s, J, m = random_pm1((ns, nr, N), 3), random_pm1((ns, 3, N), 4), random_levels((ns, nr, N), 5)
+    with micsa.MicSA(L, ns, nr, 1) as g:
+        g.set_spins(s); g.set_daemons(m); g.set_couplings(J)
+        _assert_state(g, s, m, J)
+
+
+@pytest.mark.parametrize("L,ns,nr", SHAPES)
+def test_sweeps_bit_exact(micsa, oracle, L, ns, nr):
+    N = L ** 3
+    s, J, m = random_pm1((ns, nr, N), 13), random_pm1((ns, 3, N), 14), random_levels((ns, nr, N), 15)
+    with micsa.MicSA(L, ns, nr, 1) as g:
+        g.set_spins(s); g.set_daemons(m); g.set_couplings(J)
+        for t in range(6):
+            for p in (0, 1):
+                g.half_sweep(p)
+                oracle.half_sweep(L, s, m, J, p)
+                _assert_state(g, s, m)
+        g.sweep(5)
+        oracle.sweep(L, s, m, J, 5)
+        _assert_state(g, s, m, J)
+        assert g.counters()["attempts"] == 11 * N * ns * nr
+
+
+@pytest.mark.parametrize("L,ns,nr", SHAPES)
+def test_refresh_bit_exact(micsa, oracle, L, ns, nr):
+    N = L ** 3
+    m = np.zeros((ns, nr, N), np.uint8)
+    for seed, off, T, step in [(1, 0, 2.0, 0), (99, 8, 0.9, 7), (5, 0, 0.2, 2 ** 32 - 1),
+                               (5, 64, 50.0, 12345)]:
+        with micsa.MicSA(L, ns, nr, seed, sample_offset=off) as g:
+            s0 = g.get_state(daemons=False, couplings=False)[0]
+            g.refresh_demons(T, step)
+            oracle.refresh(L, m, seed, T, step, off)
+            _assert_state(g, s0, m)                       # spins untouched
+            c = g.counters()
+            assert c["rns_drawn"] == N * ns * nr
+            g.refresh_demons(T, step)                     # pure function of its counters
+            _assert_state(g, s0, m)
+
+
+@pytest.mark.parametrize("L,ns,nr", SHAPES)
+def test_measure_exact(micsa, oracle, L, ns, nr):
+    N = L ** 3
+    s, J, m = random_pm1((ns, nr, N), 23), random_pm1((ns, 3, N), 24), random_levels((ns, nr, N), 25)
+    with micsa.MicSA(L, ns, nr, 1) as g:
+        g.set_spins(s); g.set_daemons(m); g.set_couplings(J)
+        E, Ed, Q = g.measure_i64()
+        oE, oEd, oQ = oracle.measure(L, s, m, J)
+        np.testing.assert_array_equal(E, oE)
+        np.testing.assert_array_equal(Ed, oEd)
+        np.testing.assert_array_equal(Q, oQ)
+        e, ed, q = g.measure()
+        np.testing.assert_allclose(e, oE / N, rtol=1e-12, atol=0)
+        np.testing.assert_allclose(ed, oEd / N, rtol=1e-12, atol=0)
+        np.testing.assert_allclose(q, oQ / N, rtol=1e-12, atol=0)
+
+
+def test_measure_extremes(micsa):
+    """Ferromagnetic ground state and its inverse; full daemons."""
+    L, ns, nr = 8, 2, 2
+    N = L ** 3
+    with micsa.MicSA(L, ns, nr, 1) as g:
+        s = np.ones((ns, nr, N), np.int8); s[1, 1] = -1
+        g.set_spins(s)
+        g.set_couplings(np.ones((ns, 3, N), np.int8))
+        g.set_daemons(np.full((ns, nr, N), 3, np.uint8))
+        E, Ed, Q = g.measure_i64()
+        assert E.tolist() == [-3 * N] * 4 and Ed.tolist() == [12 * N] * 4
+        assert Q.tolist() == [N, -N]
+        g.set_couplings(-np.ones((ns, 3, N), np.int8))
+        assert g.measure_i64()[0].tolist() == [3 * N] * 4
+
+
+def test_involution_and_conservation_on_gpu(micsa):
+    L, ns, nr = 16, 20, 2
+    with micsa.MicSA(L, ns, nr, 5) as g:
+        g.refresh_demons(1.5, 0)
+        s0, m0, _ = g.get_state(couplings=False)
+        E0, Ed0, _ = g.measure_i64()
+        for p in (0, 1):
+            g.half_sweep(p)
+            E, Ed, _ = g.measure_i64()
+            np.testing.assert_array_equal(E + Ed, E0 + Ed0)
+            g.half_sweep(p)
+            _assert_state(g, s0, m0)
+        g.sweep(9)
+        E, Ed, _ = g.measure_i64()
+        np.testing.assert_array_equal(E + Ed, E0 + Ed0)
+        assert np.all(E < E0)                        # a quench from a random start relaxes
+        for _ in range(9):
+            g.half_sweep(1); g.half_sweep(0)
+        _assert_state(g, s0, m0)
+
+
+def test_invalid_inputs_leave_state_unchanged(micsa):
+    L, ns, nr = 8, 2, 2
+    N = L ** 3
+    with micsa.MicSA(L, ns, nr, 3) as g:
+        s0, m0, J0 = g.get_state()
+        bad = s0.copy(); bad[1, 0, 17] = 0
+        with pytest.raises(micsa.MicsaError) as ei:
+            g.set_spins(bad)
+        assert ei.value.code == micsa.MICSA_ERR_INVALID
+        badJ = J0.copy(); badJ[0, 2, 5] = 3
+        with pytest.raises(micsa.MicsaError):
+            g.set_couplings(badJ)
+        badm = m0.copy(); badm[0, 1, 9] = 4
+        with pytest.raises(micsa.MicsaError):
+            g.set_daemons(badm)
+        for T in (0.0, -1.0, float("nan"), float("inf")):
+            with pytest.raises(micsa.MicsaError):
+                g.refresh_demons(T, 0)
+        with pytest.raises(micsa.MicsaError):
+            g.sweep(-1)
+        with pytest.raises(micsa.MicsaError):
+            g.half_sweep(2)
+        with pytest.raises(micsa.MicsaError):
+            g.anneal([(1.0, 5, 0), (-2.0, 5, 0)])
+        _assert_state(g, s0, m0, J0)
+        g.sweep(0)
+        _assert_state(g, s0, m0, J0)
+    with micsa.MicSA(L, ns, 1, 3) as g1:          # a single replica has no overlap
+        E, Ed, Q = g1.measure_i64()
+        assert Q.size == 0
+        q = np.empty(4)
+        rc = micsa._lib.micsa_measure(g1._h, None, None, q.ctypes.data)
+        assert rc == micsa.MICSA_ERR_INVALID
+
+
+# ---------------------------------------------------------------- BASELINE configs
+def test_config1_full_run(micsa, oracle):
+    """Config 1 exactly as BASELINE.json states it: L=8, 1x2, seed 1, T=2.0,
+    1000 sweeps, refresh every 10, E / E_daemon / q after every sweep."""
+    cfg = CONFIGS[1]
+    sched = schedule_for(cfg, measure_every=1)
+    s = oracle.init_spins(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed)
+    J = oracle.init_bonds(cfg.L, cfg.n_samples, cfg.seed)
+    m = np.zeros_like(s, dtype=np.uint8)
+    ref = driver.anneal(cfg.L, s, m, J, cfg.seed, sched)
+    with micsa.MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed) as g:
+        out = g.anneal(sched)
+        assert out["E"].shape == (1000, 2)
+        for k in ("sweep", "E", "Edem", "Q"):
+            np.testing.assert_array_equal(out[k], ref[k])
+        np.testing.assert_allclose(out["T"], ref["T"], rtol=0, atol=0)
+        np.testing.assert_allclose(out["min_energy"], ref["min_energy"], rtol=1e-12)
+        _assert_state(g, s, m, J)
+        c = g.counters()
+        assert c["attempts"] == 1000 * cfg.attempts_per_sweep
+        assert c["rns_drawn"] == 100 * cfg.attempts_per_sweep
+        assert c["rns_drawn"] / c["attempts"] == 0.1        # RNs per spin update
+
+
+def test_config1_state_after_every_sweep(micsa, oracle):
+    cfg = CONFIGS[1]
+    s = oracle.init_spins(cfg.L, 1, 2, cfg.seed)
+    J = oracle.init_bonds(cfg.L, 1, cfg.seed)
+    m = np.zeros_like(s, dtype=np.uint8)
+    with micsa.MicSA(cfg.L, 1, 2, cfg.seed) as g:
+        for t in range(200):
+            if t % 10 == 0:
+                g.refresh_demons(2.0, t // 10)
+                oracle.refresh(cfg.L, m, cfg.seed, 2.0, t // 10)
+                _assert_state(g, s, m)
+            g.sweep(1)
+            oracle.sweep(cfg.L, s, m, J, 1)
+            _assert_state(g, s, m)
+
+
+def _sampled_parity(micsa, oracle, cfg, sched, samples, width):
+    """Run `sched` on the full-size config on the GPU; the oracle re-runs only
+    the sample blocks [k, k+width) for k in `samples` (sample_offset = k)."""
+    L, nr = cfg.L, cfg.n_replicas
+    with micsa.MicSA(L, cfg.n_samples, nr, cfg.seed) as g:
+        E0, Ed0, _ = g.measure_i64()
+        out = g.anneal(sched)
+        gs, gm, gJ = g.get_state()
+        E1, Ed1, Q1 = g.measure_i64()
+        info = g.counters()
+    for k in samples:
+        s = oracle.init_spins(L, width, nr, cfg.seed, sample_offset=k)
+        J = oracle.init_bonds(L, width, cfg.seed, sample_offset=k)
+        m = np.zeros_like(s, dtype=np.uint8)
+        ref = driver.anneal(L, s, m, J, cfg.seed, sched, sample_offset=k)
+        np.testing.assert_array_equal(gs[k:k + width], s)
+        np.testing.assert_array_equal(gm[k:k + width], m)
+        np.testing.assert_array_equal(gJ[k:k + width], J)
+        sl = slice(k * nr, (k + width) * nr)
+        if len(ref["E"]):
+            np.testing.assert_array_equal(out["E"][:, sl], ref["E"])
+            np.testing.assert_array_equal(out["Edem"][:, sl], ref["Edem"])
+            np.testing.assert_allclose(out["min_energy"][sl], ref["min_energy"], rtol=1e-12)
+            if nr == 2:
+                np.testing.assert_array_equal(out["Q"][:, k:k + width], ref["Q"])
+        oE, oEd, oQ = oracle.measure(L, s, m, J)
+        np.testing.assert_array_equal(E1[sl], oE)
+        np.testing.assert_array_equal(Ed1[sl], oEd)
+    n_sweeps = sum(n for _, n, _ in sched)
+    assert info["attempts"] == n_sweeps * cfg.attempts_per_sweep
+    assert info["rns_drawn"] == len(sched) * cfg.attempts_per_sweep
+    return out
+
+
+def test_config2_truncated_all_temperatures(micsa, oracle):
+    cfg = CONFIGS[2]
+    for T in cfg.temperatures:
+        sched = schedule_for(cfg, T=T, n_sweeps=30, measure_every=10)
+        _sampled_parity(micsa, oracle, cfg, sched, samples=(0, 28, 60), width=4)
+
+
+@pytest.mark.parametrize("interval,n_sweeps,width", [(1, 4, 4), (10, 30, 4), (100, 200, 1)])
+def test_config3_truncated(micsa, oracle, interval, n_sweeps, width):
+    cfg = CONFIGS[3]
+    sched = schedule_for(cfg, interval=interval, n_sweeps=n_sweeps, measure_every=interval)
+    _sampled_parity(micsa, oracle, cfg, sched, samples=(0, 124), width=width)
+
+
+def test_config4_truncated(micsa, oracle):
+    """The headline config at full size, in the launch configuration bench.py
+    times (refresh + 10 sweeps + measure per step)."""
+    cfg = CONFIGS[4]
+    sched = schedule_for(cfg, n_sweeps=30, measure_every=10)
+    _sampled_parity(micsa, oracle, cfg, sched, samples=(0, 14), width=2)
+
+
+def test_config5_truncated(micsa, oracle):
+    cfg = CONFIGS[5]
+    sched = schedule_for(cfg, n_sweeps=30)
+    assert len(sched) == 3 and sched[0][0] == 3.0
+    _sampled_parity(micsa, oracle, cfg, sched, samples=(0, 508, 1020), width=4)
+    # the last ramp steps (lowest T, thresholds saturating at 2^32)
+    full = schedule_for(cfg)
+    assert abs(full[-1][0] - 0.2) < 1e-12
+    with micsa.MicSA(16, 8, 1, 5) as g:
+        s, m, J = g.get_state()
+        tail = full[-3:]
+        out = g.anneal(tail, step0=997)
+        ref = driver.anneal(16, s, m, J, 5, tail, step0=997)
+        _assert_state(g, s, m, J)
+        np.testing.assert_array_equal(out["E"], ref["E"])
+
+
+def test_sharding_by_sample_reproduces_the_unsharded_run(micsa):
+    """two contexts holding samples [0,16) and [16,32) with their
+    global sample offsets give the same bits as one context with 32 samples."""
+    L, nr, seed = 16, 2, 11
+    sched = [(1.2, 5, 5), (0.8, 5, 5)]
+    with micsa.MicSA(L, 32, nr, seed) as g:
+        whole = g.anneal(sched)
+        ws, wm, wJ = g.get_state()
+    for off in (0, 16):
+        with micsa.MicSA(L, 16, nr, seed, sample_offset=off) as g:
+            part = g.anneal(sched)
+            ps, pm, pJ = g.get_state()
+        np.testing.assert_array_equal(ps, ws[off:off + 16])
+        np.testing.assert_array_equal(pm, wm[off:off + 16])
+        np.testing.assert_array_equal(pJ, wJ[off:off + 16])
+        np.testing.assert_array_equal(part["E"], whole["E"][:, off * nr:(off + 16) * nr])
+        np.testing.assert_array_equal(part["Q"], whole["Q"][:, off:off + 16])
+
+
+def test_library_owned_memory_and_default_stream(micsa, oracle):
+    L, ns, nr = 8, 3, 2
+    with micsa.MicSA(L, ns, nr, 2, use_torch=False) as g:
+        s = oracle.init_spins(L, ns, nr, 2); J = oracle.init_bonds(L, ns, 2)
+        m = np.zeros_like(s, dtype=np.uint8)
+        g.refresh_demons(1.0, 0); g.sweep(3)
+        oracle.refresh(L, m, 2, 1.0, 0); oracle.sweep(L, s, m, J, 3)
+        _assert_state(g, s, m, J)
+
+
+def test_paramagnetic_energy_matches_metropolis_on_gpu(micsa, oracle):
+    """Config 2's physics check at reduced length: equilibrium <e> of the CUDA
+    MicSA at T=3.0 and 2.0 vs the independent Metropolis oracle on the same
+    couplings (both far above T_c, equilibration takes tens of sweeps)."""
+    L, ns, nr = 16, 8, 2
+    N = L ** 3
+    for T in (3.0, 2.0):
+        with micsa.MicSA(L, ns, nr, 2) as g:
+            s0, _, J = g.get_state()
+            out = g.anneal(schedule_for(CONFIGS[2], T=T, n_sweeps=1500, measure_every=10))
+        e_gpu = (out["E"][50:] / N).mean(axis=0)
+        e_met = oracle.metropolis(L, s0.copy(), J, T, 600, seed=3)[200:].mean(axis=0)
+        d = e_gpu.mean() - e_met.mean()
+        err = np.sqrt(e_gpu.var(ddof=1) / e_gpu.size + e_met.var(ddof=1) / e_met.size)
+        # per-system time averages scatter by sample-to-sample and thermal noise
+        assert abs(d) < 3 * err + 2e-3, (T, d, err)
