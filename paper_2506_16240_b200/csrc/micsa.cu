@@ -150,11 +150,23 @@ void launch_half_sweep_t(micsa_ctx* c, int parity) {
     half_sweep_kernel<V, RPW><<<grid, 128, 0, c->stream>>>(a, parity);
 }
 
+constexpr int kRowsPerThread = 4;
+
+template <int RPW>
+void launch_half_sweep_rows(micsa_ctx* c, int parity) {
+    SweepArgs a;
+    a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half;
+    const int per_plane = (c->g.L / kRowsPerThread) * (c->g.Lh / 4);
+    dim3 grid((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
+    half_sweep_rows_kernel<RPW, kRowsPerThread><<<grid, 128, 0, c->stream>>>(a, parity);
+}
+
 int launch_half_sweep(micsa_ctx* c, int parity) {
     const int key = c->V * 10 + c->g.rpw;
     switch (key) {
-        case 41: launch_half_sweep_t<4, 1>(c, parity); break;
-        case 42: launch_half_sweep_t<4, 2>(c, parity); break;
+        case 41: launch_half_sweep_rows<1>(c, parity); break;     // L % 8 == 0
+        case 42: launch_half_sweep_rows<2>(c, parity); break;
         case 21: launch_half_sweep_t<2, 1>(c, parity); break;
         case 22: launch_half_sweep_t<2, 2>(c, parity); break;
         case 11: launch_half_sweep_t<1, 1>(c, parity); break;

@@ -113,4 +113,162 @@ half_sweep_kernel(SweepArgs a, int p)
     stg_vec<V>(m1p + h, d1);
 }
 
+
+// ---------------------------------------------------------------------------
+// Row-marching half-sweep for L % 8 == 0 (all BASELINE configs).
+//
+// One thread owns 4 consecutive words (16 B) of a row and marches over YC
+// consecutive rows y0..y0+YC-1 of plane z (grid.y) of word lattice w (grid.z):
+//  * the three opposite-parity rows y-1, y, y+1 slide through registers, so each
+//    step loads one new row instead of three;
+//  * all array bases are block-uniform and the per-thread offsets are 32-bit byte
+//    offsets advanced by a constant, which removes the 64-bit index arithmetic
+//    that dominated the first version (ncu: 104 instructions per site word);
+//  * y0 is even, so the x-shift flag c = (y+z+p)&1 equals (iy&1) ^ f with
+//    f = (z+p)&1 uniform over the block: the block branches once on f and c is
+//    a compile-time constant in the unrolled body -- no per-word selects.
+// Lanes run along (row chunk, x): a warp reads whole 128-byte lines.
+// ---------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ T ld_off(const void* base, uint32_t byte_off) {
+    return *reinterpret_cast<const T*>(static_cast<const char*>(base) + byte_off);
+}
+template <typename T>
+__device__ __forceinline__ void st_off(void* base, uint32_t byte_off, T v) {
+    *reinterpret_cast<T*>(static_cast<char*>(base) + byte_off) = v;
+}
+
+template <int RPW> struct Bond4;                      // 4 consecutive bond words
+template <> struct Bond4<2> {
+    typedef uint2 raw; typedef uint16_t elem;
+    static __device__ __forceinline__ void expand(const raw& r, uint32_t (&o)[4]) {
+        o[0] = __byte_perm(r.x, 0u, 0x1010); o[1] = __byte_perm(r.x, 0u, 0x3232);
+        o[2] = __byte_perm(r.y, 0u, 0x1010); o[3] = __byte_perm(r.y, 0u, 0x3232);
+    }
+    static __device__ __forceinline__ uint32_t expand1(elem e) { return __byte_perm((uint32_t)e, 0u, 0x1010); }
+};
+template <> struct Bond4<1> {
+    typedef uint4 raw; typedef uint32_t elem;
+    static __device__ __forceinline__ void expand(const raw& r, uint32_t (&o)[4]) {
+        o[0] = r.x; o[1] = r.y; o[2] = r.z; o[3] = r.w;
+    }
+    static __device__ __forceinline__ uint32_t expand1(elem e) { return e; }
+};
+
+struct RowPtrs {            // block-uniform bases of plane z (and z+-1) of lattice w
+    uint32_t* sp; uint32_t* m0; uint32_t* m1;          // own parity, plane z
+    const uint32_t* sq; const uint32_t* sq_zp; const uint32_t* sq_zm;   // opposite parity
+    const void* jx; const void* jy; const void* jz;    // own bonds, plane z
+    const void* jxq; const void* jyq; const void* jzq_zm;   // neighbours' bonds
+};
+
+template <int RPW, int YC, int F>
+__device__ __forceinline__ void march_rows(const RowPtrs& P, int L, int Lh, int y0, int xh0)
+{
+    typedef Bond4<RPW> B4;
+    constexpr uint32_t JS = sizeof(typename B4::elem);          // bytes per bond word
+    const uint32_t rowB = (uint32_t)Lh * 4u;                    // bytes per spin row
+    const uint32_t x4 = (uint32_t)xh0 * 4u;
+    const int ym0 = (y0 == 0) ? L - 1 : y0 - 1;
+    // byte offsets inside a plane (spin-word units * 4)
+    uint32_t o = (uint32_t)y0 * rowB + x4;
+    uint32_t o_prev = (uint32_t)ym0 * rowB + x4;
+    const uint32_t xe_up = ((xh0 + 4 == Lh) ? 0u : (uint32_t)(xh0 + 4)) * 4u;     // xh+1 of the last word
+    const uint32_t xe_dn = ((xh0 == 0) ? (uint32_t)(Lh - 1) : (uint32_t)(xh0 - 1)) * 4u;
+
+    uint4 Aprev = ld_off<uint4>(P.sq, o_prev);
+    uint4 Acur  = ld_off<uint4>(P.sq, o);
+#pragma unroll
+    for (int iy = 0; iy < YC; ++iy) {
+        const int c = (iy & 1) ^ F;                    // compile-time after unrolling
+        const int y = y0 + iy;
+        const uint32_t o_next = (y + 1 == L) ? x4 : o + rowB;
+        const uint32_t rowstart = o - x4;
+        const uint4 Anext = ld_off<uint4>(P.sq, o_next);
+        uint4 s  = ld_off<uint4>(P.sp, o);
+        uint4 d0 = ld_off<uint4>(P.m0, o);
+        uint4 d1 = ld_off<uint4>(P.m1, o);
+        const uint4 nzp = ld_off<uint4>(P.sq_zp, o);
+        const uint4 nzm = ld_off<uint4>(P.sq_zm, o);
+        const uint32_t oj = o / 4u * JS, ojm = o_prev / 4u * JS;
+        uint32_t jxo[4], jyo[4], jzo[4], jxm[4], jym[4], jzm[4];
+        B4::expand(ld_off<typename B4::raw>(P.jx, oj), jxo);
+        B4::expand(ld_off<typename B4::raw>(P.jy, oj), jyo);
+        B4::expand(ld_off<typename B4::raw>(P.jz, oj), jzo);
+        B4::expand(ld_off<typename B4::raw>(P.jyq, ojm), jym);
+        B4::expand(ld_off<typename B4::raw>(P.jzq_zm, oj), jzm);
+        uint32_t Bx[4];
+        B4::expand(ld_off<typename B4::raw>(P.jxq, oj), Bx);
+        const uint32_t a[4] = { Acur.x, Acur.y, Acur.z, Acur.w };
+        uint32_t nxp[4], nxm[4];
+        if (c) {        // x = 2xh+1: -x neighbour at xh (bond owned by it), +x neighbour at xh+1
+            const uint32_t e = ld_off<uint32_t>(P.sq, rowstart + xe_up);
+            nxp[0] = a[1]; nxp[1] = a[2]; nxp[2] = a[3]; nxp[3] = e;
+            nxm[0] = a[0]; nxm[1] = a[1]; nxm[2] = a[2]; nxm[3] = a[3];
+            jxm[0] = Bx[0]; jxm[1] = Bx[1]; jxm[2] = Bx[2]; jxm[3] = Bx[3];
+        } else {        // x = 2xh: +x neighbour at xh, -x neighbour at xh-1 (bond owned by it)
+            const uint32_t e = ld_off<uint32_t>(P.sq, rowstart + xe_dn);
+            const uint32_t eJ = B4::expand1(ld_off<typename B4::elem>(P.jxq, (rowstart + xe_dn) / 4u * JS));
+            nxp[0] = a[0]; nxp[1] = a[1]; nxp[2] = a[2]; nxp[3] = a[3];
+            nxm[0] = e; nxm[1] = a[0]; nxm[2] = a[1]; nxm[3] = a[2];
+            jxm[0] = eJ; jxm[1] = Bx[0]; jxm[2] = Bx[1]; jxm[3] = Bx[2];
+        }
+        uint32_t sv[4] = { s.x, s.y, s.z, s.w };
+        uint32_t v0[4] = { d0.x, d0.y, d0.z, d0.w };
+        uint32_t v1[4] = { d1.x, d1.y, d1.z, d1.w };
+        const uint32_t yp[4] = { Anext.x, Anext.y, Anext.z, Anext.w };
+        const uint32_t ym[4] = { Aprev.x, Aprev.y, Aprev.z, Aprev.w };
+        const uint32_t zp[4] = { nzp.x, nzp.y, nzp.z, nzp.w };
+        const uint32_t zm[4] = { nzm.x, nzm.y, nzm.z, nzm.w };
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const uint32_t g = sv[k];
+            creutz_word(g ^ nxp[k] ^ jxo[k], g ^ nxm[k] ^ jxm[k],
+                        g ^ yp[k] ^ jyo[k],  g ^ ym[k] ^ jym[k],
+                        g ^ zp[k] ^ jzo[k],  g ^ zm[k] ^ jzm[k],
+                        sv[k], v0[k], v1[k]);
+        }
+        st_off<uint4>(P.sp, o, make_uint4(sv[0], sv[1], sv[2], sv[3]));
+        st_off<uint4>(P.m0, o, make_uint4(v0[0], v0[1], v0[2], v0[3]));
+        st_off<uint4>(P.m1, o, make_uint4(v1[0], v1[1], v1[2], v1[3]));
+        Aprev = Acur; Acur = Anext;
+        o_prev = o; o = o_next;
+    }
+}
+
+// grid = (ceil((L/YC)*(Lh/4) / block), L, n_words)
+template <int RPW, int YC>
+__global__ void __launch_bounds__(128)
+half_sweep_rows_kernel(SweepArgs a, int p)
+{
+    typedef typename Bond4<RPW>::elem JT;
+    const int L = a.L, Lh = a.Lh;
+    const int nxv = Lh >> 2;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (L / YC) * nxv) return;
+    const int chunk = t / nxv, xv = t - chunk * nxv;
+    const int z = blockIdx.y, w = blockIdx.z, q = 1 - p;
+    const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+    const long long half = a.half;
+    const long long plane = (long long)L * Lh;
+    const int sg = w / a.n_rg;
+    const JT* Jb = reinterpret_cast<const JT*>(a.J) + (long long)sg * 6 * half;
+
+    RowPtrs P;
+    P.sp = a.spin + ((long long)w * 2 + p) * half + z * plane;
+    P.m0 = a.m0 + ((long long)w * 2 + p) * half + z * plane;
+    P.m1 = a.m1 + ((long long)w * 2 + p) * half + z * plane;
+    const uint32_t* sqb = a.spin + ((long long)w * 2 + q) * half;
+    P.sq = sqb + z * plane; P.sq_zp = sqb + zp * plane; P.sq_zm = sqb + zm * plane;
+    P.jx = Jb + (0 * 2 + p) * half + z * plane;
+    P.jy = Jb + (1 * 2 + p) * half + z * plane;
+    P.jz = Jb + (2 * 2 + p) * half + z * plane;
+    P.jxq = Jb + (0 * 2 + q) * half + z * plane;
+    P.jyq = Jb + (1 * 2 + q) * half + z * plane;
+    P.jzq_zm = Jb + (2 * 2 + q) * half + zm * plane;
+
+    if ((z + p) & 1) march_rows<RPW, YC, 1>(P, L, Lh, chunk * YC, xv * 4);
+    else             march_rows<RPW, YC, 0>(P, L, Lh, chunk * YC, xv * 4);
+}
+
 }  // namespace micsa
