@@ -53,9 +53,15 @@ class _Trace(ctypes.Structure):
 
 def _load() -> ctypes.CDLL:
     if not LIB_PATH.exists():
-        raise ImportError(
-            f"{LIB_PATH} is missing: build it with `python -m paper_2506_16240_b200.build` "
-            "(nvcc, sm_100a). This package has no CPU fallback.")
+        # a fresh checkout has no binary: compile it now (nvcc, sm_100a); there is
+        # nothing to fall back to if that fails
+        from .build import build as _build
+        try:
+            _build()
+        except Exception as exc:
+            raise ImportError(
+                f"{LIB_PATH} is missing and `python -m paper_2506_16240_b200.build` failed "
+                f"({exc}). This package has no CPU fallback.") from exc
     lib = ctypes.CDLL(str(LIB_PATH))
     vp, i32, u32, u64, f64 = (ctypes.c_void_p, ctypes.c_int, ctypes.c_uint32,
                               ctypes.c_uint64, ctypes.c_double)
