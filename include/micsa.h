@@ -176,6 +176,16 @@ int micsa_counters(micsa_ctx *ctx, uint64_t *attempts, uint64_t *rns_drawn,
  * info[4] = kernel launches issued so far on this context.                   */
 int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
 
+/* Tuning / A-B switch, never needed for correctness (every setting gives the
+ * same bits; tests/test_gpu_parity.py runs the parity cases under each).
+ * key MICSA_TUNE_SWEEP_KERNEL: 0 = tiled half-sweep, opposite-parity spins
+ *   staged in shared memory by TMA (default whenever L % 8 == 0), 1 =
+ *   row-marching register kernel.  key MICSA_TUNE_TILE_TZ: lattice planes per
+ *   tile of the tiled kernel, 2, 4 (default) or 8.  L % 8 != 0 always uses the
+ *   generic kernel.  Unknown key or value: MICSA_ERR_INVALID, nothing changes. */
+enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_TILE_TZ = 1 };
+int micsa_set_tuning(micsa_ctx *ctx, int key, int value);
+
 #ifdef __cplusplus
 }
 #endif

@@ -30,6 +30,7 @@ EXPORTS = (
     "micsa_set_daemons", "micsa_get_state", "micsa_sweep", "micsa_half_sweep",
     "micsa_refresh_demons", "micsa_debug_thresholds", "micsa_measure_i64",
     "micsa_measure", "micsa_anneal", "micsa_counters", "micsa_layout_info",
+    "micsa_set_tuning",
 )
 
 
@@ -52,6 +53,16 @@ class _Trace(ctypes.Structure):
 
 
 def _load() -> ctypes.CDLL:
+    try:
+        return _bind()
+    except AttributeError:
+        # a stale binary from an older header: rebuild once, then fail loudly
+        from .build import build as _build
+        _build(force=True)
+        return _bind()
+
+
+def _bind() -> ctypes.CDLL:
     if not LIB_PATH.exists():
         # a fresh checkout has no binary: compile it now (nvcc, sm_100a); there is
         # nothing to fall back to if that fails
@@ -82,7 +93,8 @@ def _load() -> ctypes.CDLL:
             ("micsa_debug_thresholds", [f64, vp]),
             ("micsa_measure_i64", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
             ("micsa_anneal", [vp, vp, i32, u32, vp, vp]),
-            ("micsa_counters", [vp, vp, vp, vp]), ("micsa_layout_info", [vp, vp])):
+            ("micsa_counters", [vp, vp, vp, vp]), ("micsa_layout_info", [vp, vp]),
+            ("micsa_set_tuning", [vp, i32, i32])):
         fn = getattr(lib, name)
         fn.restype = i32
         fn.argtypes = args
@@ -255,6 +267,11 @@ class MicSA:
         a, r, p = ctypes.c_uint64(), ctypes.c_uint64(), ctypes.c_uint64()
         _check(_lib.micsa_counters(self._h, ctypes.byref(a), ctypes.byref(r), ctypes.byref(p)))
         return {"attempts": a.value, "rns_drawn": r.value, "philox_calls": p.value}
+
+    def set_tuning(self, key, value):
+        """micsa_set_tuning: 'sweep_kernel' (0 tiled, 1 row-marching) or 'tile_tz' (2, 4, 8)."""
+        k = {"sweep_kernel": 0, "tile_tz": 1}[key]
+        _check(_lib.micsa_set_tuning(self._h, k, int(value)))
 
     def layout_info(self):
         info = np.zeros(5, np.uint64)

@@ -17,6 +17,7 @@
 #include "philox.cuh"
 #include "refresh.cuh"
 #include "sweep.cuh"
+#include "sweep_tile.cuh"
 
 using namespace micsa;
 
@@ -101,6 +102,8 @@ struct micsa_ctx {
     long long* minE;
     int* bad;
     int V;
+    int sweep_kernel;          // 0 = tiled (TMA-staged) when L % 8 == 0, 1 = row-marching
+    int tile_tz;               // planes per tile of the tiled kernel (2, 4 or 8)
     uint64_t attempts, rns, philox_calls, launches;
     int sticky;
 };
@@ -162,7 +165,41 @@ void launch_half_sweep_rows(micsa_ctx* c, int parity) {
     half_sweep_rows_kernel<RPW, kRowsPerThread><<<grid, 128, 0, c->stream>>>(a, parity);
 }
 
+template <int RPW, int TY, int TZ>
+int launch_half_sweep_tile(micsa_ctx* c, int parity) {
+    SweepArgs a;
+    a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half;
+    const int items = TY * TZ * (c->g.Lh / 4);
+    const int block = std::min((items + 31) / 32 * 32, 640);
+    const size_t smem = TileSmem<RPW, TY, TZ>::bytes(c->g.Lh);
+    if (smem > 48 * 1024) {
+        if (smem > 227 * 1024) { set_err("L too large for the tiled sweep kernel"); return MICSA_ERR_INVALID; }
+        CK(c, cudaFuncSetAttribute(half_sweep_tile_kernel<RPW, TY, TZ>,
+                                   cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    }
+    dim3 grid((unsigned)((c->g.L / TY) * (c->g.L / TZ)), (unsigned)c->g.n_words);
+    half_sweep_tile_kernel<RPW, TY, TZ><<<grid, block, smem, c->stream>>>(a, parity);
+    return MICSA_OK;
+}
+
+template <int RPW>
+int launch_half_sweep_tile_tz(micsa_ctx* c, int parity) {
+    switch (c->tile_tz) {
+        case 2:  return launch_half_sweep_tile<RPW, 8, 2>(c, parity);
+        case 8:  return launch_half_sweep_tile<RPW, 8, 8>(c, parity);
+        default: return launch_half_sweep_tile<RPW, 8, 4>(c, parity);
+    }
+}
+
 int launch_half_sweep(micsa_ctx* c, int parity) {
+    if (c->V == 4 && c->sweep_kernel == 0) {
+        const int rc = (c->g.rpw == 2) ? launch_half_sweep_tile_tz<2>(c, parity)
+                                       : launch_half_sweep_tile_tz<1>(c, parity);
+        if (rc) return rc;
+        c->attempts += (uint64_t)(c->g.N / 2) * (uint64_t)c->g.n_sys;
+        return post_launch(c);
+    }
     const int key = c->V * 10 + c->g.rpw;
     switch (key) {
         case 41: launch_half_sweep_rows<1>(c, parity); break;     // L % 8 == 0
@@ -347,6 +384,8 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->ks = philox_make_keys(seed);
     c->stream = (cudaStream_t)cuda_stream;
     c->V = vec_width(g.Lh);
+    c->sweep_kernel = 0;
+    c->tile_tz = 4;
     c->attempts = c->rns = c->philox_calls = c->launches = 0;
     c->sticky = 0;
     if (dev_workspace) {
@@ -574,6 +613,20 @@ int micsa_counters(micsa_ctx* c, uint64_t* attempts, uint64_t* rns, uint64_t* ph
     if (rns) *rns = c->rns;
     if (philox_calls) *philox_calls = c->philox_calls;
     return MICSA_OK;
+}
+
+int micsa_set_tuning(micsa_ctx* c, int key, int value) {
+    int rc = check_ctx(c); if (rc) return rc;
+    switch (key) {
+        case MICSA_TUNE_SWEEP_KERNEL:
+            if (value != 0 && value != 1) { set_err("sweep kernel must be 0 or 1"); return MICSA_ERR_INVALID; }
+            c->sweep_kernel = value; return MICSA_OK;
+        case MICSA_TUNE_TILE_TZ:
+            if (value != 2 && value != 4 && value != 8) { set_err("tile_tz must be 2, 4 or 8"); return MICSA_ERR_INVALID; }
+            c->tile_tz = value; return MICSA_OK;
+        default:
+            set_err("unknown tuning key"); return MICSA_ERR_INVALID;
+    }
 }
 
 int micsa_layout_info(micsa_ctx* c, uint64_t info[5]) {
