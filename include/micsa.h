@@ -92,7 +92,8 @@ const char *micsa_last_error(void);
  *   sample_offset  global index of this context's first sample; Philox
  *                  counters use sample_offset + sample, so a run sharded by
  *                  sample over several GPUs reproduces the unsharded run.
- *                  Must be a multiple of 4 and >= 0.
+ *                  Must be a multiple of 16 (the sample block of the refresh,
+ *                  DESIGN.md R8) and >= 0.
  *   dev_workspace  device memory of at least micsa_workspace_bytes(...) bytes,
  *                  256-byte aligned, owned by the caller (e.g. a torch tensor)
  *                  and kept alive until micsa_destroy; NULL = the library
@@ -129,11 +130,14 @@ int micsa_half_sweep(micsa_ctx *ctx, int parity);
 
 /* micsa_refresh_demons: every daemon <- independent draw from Eq. (11),
  * p(n=4m) ~ exp(-4m/T), m = 0..3; spins untouched
- * (PAPER.md:190).  One 32-bit Philox4x32-10 output per daemon, counter =
- * (site i, global_sample/4, replica, step), key = seed, output word
- * global_sample%4, compared with integer thresholds floor(cdf_k * 2^32)
- * computed on the host (R7, R8).  Same (seed, step, T) => same
- * daemons whatever happened before.  Asynchronous.  T must be finite and > 0. */
+ * (PAPER.md:190).  One 32-bit uniform u per daemon, compared with integer
+ * thresholds floor(cdf_k * 2^32) computed on the host (R7).  u is
+ * defined bit-sliced (R8): the 16 samples gs of block gs/16 share
+ * four Philox4x32-10 calls c = 0..3, counter = (site i, gs/16 | c<<28,
+ * replica, step), key = seed; bit-plane k = 8c+2j+h is the 16-bit half h of
+ * output word j of call c, sample gs owns bit gs%16 and u = sum_k bit_k <<
+ * (31-k).  Same (seed, step, T) => same daemons whatever happened before.
+ * Asynchronous.  T must be finite and > 0. */
 int micsa_refresh_demons(micsa_ctx *ctx, double T, uint32_t step);
 
 /* The thresholds micsa_refresh_demons uses: thr[k] = floor(cdf_k * 2^32),
@@ -163,9 +167,13 @@ int micsa_measure(micsa_ctx *ctx, double *energy, double *demon_energy,
 int micsa_anneal(micsa_ctx *ctx, const micsa_step *sched, int n_steps,
                  uint32_t step0, double *min_energy, micsa_trace *trace);
 
-/* Running totals since create: spin-flip attempts, 32-bit random numbers
- * consumed by refreshes (one per daemon), Philox4x32-10 blocks evaluated by
- * refreshes.  Initialisation draws are not counted.  Any pointer may be NULL. */
+/* Running totals since create: spin-flip attempts; 32-bit uniforms the
+ * refreshes are defined on (one per daemon, R8); Philox4x32-10
+ * blocks the refresh kernels actually evaluated.  The refresh compares
+ * bit-plane by bit-plane and stops once every lane is decided, so the last is
+ * data dependent (about half of the 1 block per 4 daemons a full evaluation
+ * needs); it is counted on the device and asking for it synchronises the
+ * stream.  Initialisation draws are not counted.  Any pointer may be NULL. */
 int micsa_counters(micsa_ctx *ctx, uint64_t *attempts, uint64_t *rns_drawn,
                    uint64_t *philox_calls);
 
@@ -179,8 +187,8 @@ int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
 /* Tuning / A-B switch, never needed for correctness (every setting gives the
  * same bits; tests/test_gpu_parity.py runs the parity cases under each).
  * key MICSA_TUNE_SWEEP_KERNEL: 0 = tiled half-sweep, opposite-parity spins
- *   staged in shared memory by TMA (default whenever L % 8 == 0), 1 =
- *   row-marching register kernel.  key MICSA_TUNE_TILE_TZ: lattice planes per
+ *   staged in shared memory by TMA, 1 =
+ *   row-marching register kernel (default: it measured faster on B200).  key MICSA_TUNE_TILE_TZ: lattice planes per
  *   tile of the tiled kernel, 2, 4 (default) or 8.  L % 8 != 0 always uses the
  *   generic kernel.  Unknown key or value: MICSA_ERR_INVALID, nothing changes. */
 enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_TILE_TZ = 1 };

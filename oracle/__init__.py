@@ -57,6 +57,7 @@ def lib() -> ctypes.CDLL:
         _LIB.oracle_thresholds.argtypes = [ctypes.c_double, _c_u64p]
         _LIB.oracle_thresholds.restype = ctypes.c_int
         _LIB.oracle_refresh.restype = ctypes.c_int
+        _LIB.oracle_refresh_uniform.restype = ctypes.c_uint32
         _LIB.oracle_num_threads.restype = ctypes.c_int
     return _LIB
 
@@ -149,6 +150,14 @@ def refresh(L, m, seed, T, step, sample_offset=0) -> None:
                               _p(m, _c_u8p))
     if rc != 0:
         raise ValueError(f"invalid temperature {T!r}")
+
+
+def refresh_uniform(i, g, rep, step, seed) -> int:
+    """The 32-bit uniform of the demon at site i of global sample g, replica
+    rep, refresh index step (R8)."""
+    return int(lib().oracle_refresh_uniform(ctypes.c_uint32(i), ctypes.c_uint32(g),
+                                            ctypes.c_uint32(rep), ctypes.c_uint32(step),
+                                            ctypes.c_uint64(seed)))
 
 
 def measure(L, s, m, J):

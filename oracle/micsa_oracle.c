@@ -213,7 +213,7 @@ void oracle_sweep(int L, int n_samples, int n_replicas, int n_sweeps,
 /*   x = exp(-4/T); x2 = x*x; x3 = x2*x; Z = ((1 + x) + x2) + x3          */
 /*   c0 = 1/Z; c1 = (1 + x)/Z; c2 = ((1 + x) + x2)/Z   (cumulative p)     */
 /*   thr[k] = floor(c_k * 2^32) as uint64 in [0, 2^32]                    */
-/* Draw: u = one 32-bit Philox word; m = #{k : u >= thr[k]}.             */
+/* Draw: u = one 32-bit uniform per demon; m = #{k : u >= thr[k]}.        */
 /* ------------------------------------------------------------------ */
 int oracle_thresholds(double T, uint64_t thr[3])
 {
@@ -231,8 +231,46 @@ int oracle_thresholds(double T, uint64_t thr[3])
     return 0;
 }
 
-/* Refresh counter (R8): ctr = (i, gsample>>2, (0<<24)|replica, step),
- * key = (seed lo, seed hi); demon of global sample g uses output word g&3.   */
+/* The 32-bit uniform u of one demon (R8; the paper does not say
+ * how the refresh draws its random numbers, north_star asks for Philox keyed
+ * by seed, sample, site and refresh index).  u is assembled most significant
+ * bit first from 32 random bit-planes; the planes of the 16 global samples
+ * g with the same g>>4 (same site, replica, step) come from four Philox
+ * calls c = 0..3 with
+ *     ctr = (i, (g>>4) | (c<<28), (0<<24) | replica, step),  key = (seed lo, hi)
+ * plane k = 8c + 2j + h is the 16-bit half h (0 = low, 1 = high) of output
+ * word j of call c, and sample g owns bit (g & 15) of it:
+ *     u = sum_k  bit_k * 2^(31-k).
+ * Every bit of every output word is used by exactly one demon, so u is a
+ * uniform 32-bit integer and distinct demons are independent. */
+static uint32_t refresh_uniform(uint32_t i, uint32_t g, uint32_t rep,
+                                uint32_t step, const uint32_t key[2])
+{
+    uint32_t u = 0;
+    for (uint32_t c = 0; c < 4; ++c) {
+        uint32_t ctr[4] = { i, (g >> 4) | (c << 28),
+                            ((uint32_t)TAG_REFRESH << 24) | rep, step };
+        uint32_t out[4];
+        oracle_philox4x32_10(ctr, key, out);
+        for (uint32_t j = 0; j < 4; ++j)
+            for (uint32_t h = 0; h < 2; ++h) {
+                const uint32_t k = 8 * c + 2 * j + h;           /* 0 = most significant */
+                const uint32_t bit = (out[j] >> (16 * h + (g & 15))) & 1u;
+                u |= bit << (31 - k);
+            }
+    }
+    return u;
+}
+
+/* Debug/test hook: the uniform itself (pins: uniformity, bit independence). */
+uint32_t oracle_refresh_uniform(uint32_t i, uint32_t g, uint32_t rep,
+                                uint32_t step, uint64_t seed)
+{
+    uint32_t key[2]; seed_key(seed, key);
+    return refresh_uniform(i, g, rep, step, key);
+}
+
+/* Refresh: every demon <- #{k : u >= thr[k]} with its own u (Eq. 11). */
 int oracle_refresh(int L, int n_samples, int n_replicas, uint64_t seed,
                    int sample_offset, double T, uint32_t step, uint8_t *m)
 {
@@ -247,11 +285,7 @@ int oracle_refresh(int L, int n_samples, int n_replicas, uint64_t seed,
         const uint32_t g = (uint32_t)(sample_offset + sample);
         uint8_t *mm = m + (int64_t)sys * N;
         for (int64_t i = 0; i < N; ++i) {
-            uint32_t ctr[4] = { (uint32_t)i, g >> 2,
-                                ((uint32_t)TAG_REFRESH << 24) | (uint32_t)rep, step };
-            uint32_t out[4];
-            oracle_philox4x32_10(ctr, key, out);
-            const uint64_t u = (uint64_t)out[g & 3];
+            const uint64_t u = (uint64_t)refresh_uniform((uint32_t)i, g, (uint32_t)rep, step, key);
             mm[i] = (uint8_t)((u >= thr[0]) + (u >= thr[1]) + (u >= thr[2]));
         }
     }

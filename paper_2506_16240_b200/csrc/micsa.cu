@@ -33,14 +33,14 @@ constexpr size_t kAlign = 256;
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {                 // byte offsets inside the workspace
-    size_t spin, m0, m1, J, cnt, row, minE, bad, total;
+    size_t spin, m0, m1, J, cnt, row, minE, bad, calls, total;
     size_t plane_bytes, J_bytes, cnt_words, row_len;
 };
 
 bool make_geom(int L, int n_samples, int n_replicas, int sample_offset, Geom& g) {
     if (L < 2 || (L & 1)) { set_err("L must be even and >= 2"); return false; }
     if (n_samples < 1 || n_replicas < 1) { set_err("n_samples and n_replicas must be >= 1"); return false; }
-    if (sample_offset < 0 || (sample_offset & 3)) { set_err("sample_offset must be a non-negative multiple of 4"); return false; }
+    if (sample_offset < 0 || (sample_offset & 15)) { set_err("sample_offset must be a non-negative multiple of 16"); return false; }
     const long long N = (long long)L * L * L;
     if (N > 0xFFFFFFFFll) { set_err("L^3 must fit 32 bits (site index is one Philox counter word)"); return false; }
     if ((long long)n_samples * n_replicas > (1ll << 24) || n_replicas >= (1 << 24)) {
@@ -80,6 +80,7 @@ Plan make_plan(const Geom& g) {
     p.row = o;  o += align_up(p.row_len * 8);
     p.minE = o; o += align_up((size_t)g.n_sys * 8);
     p.bad = o;  o += align_up(sizeof(int));
+    p.calls = o; o += align_up(sizeof(unsigned long long));
     p.total = o;
     return p;
 }
@@ -101,10 +102,11 @@ struct micsa_ctx {
     long long* row;
     long long* minE;
     int* bad;
+    unsigned long long* calls;  // Philox calls made by the refresh kernels (device counter)
     int V;
     int sweep_kernel;          // 0 = tiled (TMA-staged) when L % 8 == 0, 1 = row-marching
     int tile_tz;               // planes per tile of the tiled kernel (2, 4 or 8)
-    uint64_t attempts, rns, philox_calls, launches;
+    uint64_t attempts, rns, launches;
     int sticky;
 };
 
@@ -234,15 +236,18 @@ int launch_refresh(micsa_ctx* c, double T, uint32_t step) {
     if (thresholds_host(T, thr) != MICSA_OK || thr[0] == 0) {
         set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID;
     }
-    const uint32_t a0 = (uint32_t)(thr[0] - 1), a1 = (uint32_t)(thr[1] - 1), a2 = (uint32_t)(thr[2] - 1);
+    RefreshThr rt;
+    for (int k = 0; k < 3; ++k) {
+        rt.never[k] = (thr[k] >> 32) ? 1u : 0u;           // 2^32: level k+1 has probability < 2^-32
+        for (int p = 0; p < 32; ++p) rt.tb[k][p] = ((thr[k] >> (31 - p)) & 1u) ? 0xFFFFFFFFu : 0u;
+    }
     const SiteGrid sg = site_grid(c->g);
     const dim3 grid = site_blocks(c->g, c->g.n_words * 2);
     if (c->g.rpw == 2)
-        refresh_kernel<2><<<grid, 128, 0, c->stream>>>(c->st.m0, c->st.m1, sg, c->ks, step, a0, a1, a2);
+        refresh_kernel<2><<<grid, 128, 0, c->stream>>>(c->st.m0, c->st.m1, sg, c->ks, step, rt, c->calls);
     else
-        refresh_kernel<1><<<grid, 128, 0, c->stream>>>(c->st.m0, c->st.m1, sg, c->ks, step, a0, a1, a2);
+        refresh_kernel<1><<<grid, 128, 0, c->stream>>>(c->st.m0, c->st.m1, sg, c->ks, step, rt, c->calls);
     c->rns += (uint64_t)c->g.N * (uint64_t)c->g.n_sys;
-    c->philox_calls += (uint64_t)c->g.N * (uint64_t)c->g.n_sg * (uint64_t)(c->g.spw / 4) * (uint64_t)c->g.n_replicas;
     return post_launch(c);
 }
 
@@ -336,6 +341,7 @@ int set_sys(micsa_ctx* c, const int8_t* src, int kind) {
 int init_state(micsa_ctx* c) {
     const Geom& g = c->g;
     const SiteGrid sg = site_grid(g);
+    CK(c, cudaMemsetAsync(c->calls, 0, sizeof(unsigned long long), c->stream));
     CK(c, cudaMemsetAsync(c->st.m0, 0, c->plan.plane_bytes, c->stream));
     CK(c, cudaMemsetAsync(c->st.m1, 0, c->plan.plane_bytes, c->stream));
     if (g.rpw == 2) {
@@ -384,9 +390,9 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->ks = philox_make_keys(seed);
     c->stream = (cudaStream_t)cuda_stream;
     c->V = vec_width(g.Lh);
-    c->sweep_kernel = 0;
+    c->sweep_kernel = 1;
     c->tile_tz = 4;
-    c->attempts = c->rns = c->philox_calls = c->launches = 0;
+    c->attempts = c->rns = c->launches = 0;
     c->sticky = 0;
     if (dev_workspace) {
         if (workspace_bytes < c->plan.total || ((uintptr_t)dev_workspace % kAlign)) {
@@ -408,6 +414,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->row = (long long*)(c->ws + c->plan.row);
     c->minE = (long long*)(c->ws + c->plan.minE);
     c->bad = (int*)(c->ws + c->plan.bad);
+    c->calls = (unsigned long long*)(c->ws + c->plan.calls);
     if (init_state(c) != MICSA_OK) { if (c->owns_ws) cudaFree(c->ws); delete c; return nullptr; }
     return c;
 }
@@ -611,7 +618,14 @@ int micsa_counters(micsa_ctx* c, uint64_t* attempts, uint64_t* rns, uint64_t* ph
     if (!c) { set_err("null context"); return MICSA_ERR_INVALID; }
     if (attempts) *attempts = c->attempts;
     if (rns) *rns = c->rns;
-    if (philox_calls) *philox_calls = c->philox_calls;
+    if (philox_calls) {
+        // lazy refresh: the number of calls is data dependent and counted on the device
+        if (c->sticky) { set_err("context is in a sticky CUDA error state"); return c->sticky; }
+        unsigned long long n = 0;
+        CK(c, cudaMemcpyAsync(&n, c->calls, sizeof n, cudaMemcpyDeviceToHost, c->stream));
+        CK(c, cudaStreamSynchronize(c->stream));
+        *philox_calls = (uint64_t)n;
+    }
     return MICSA_OK;
 }
 

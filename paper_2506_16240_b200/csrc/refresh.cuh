@@ -4,12 +4,23 @@
 // Refresh, PAPER.md:154-157 (Eq. 11) and :190: every daemon is replaced by an
 // independent draw with p(n=4m) ~ exp(-4m/T), m = 0..3; spins are untouched.
 // It is the only consumer of random numbers.  DESIGN.md R7/R8:
-// one 32-bit Philox4x32-10 output u per daemon,
-//     counter = (site i, global_sample >> 2, kTagRefresh | replica, step)
-//     u       = output word (global_sample & 3)
-//     m       = [u >= thr0] + [u >= thr1] + [u >= thr2]
-// with thr_k = floor(cdf_k * 2^32) in [1, 2^32] computed on the host; the
-// kernel receives thr_k - 1 (a uint32) and tests u > thr_k - 1.
+// every daemon has its own 32-bit uniform u and
+//     m = [u >= thr0] + [u >= thr1] + [u >= thr2],
+// thr_k = floor(cdf_k * 2^32) in [1, 2^32] computed on the host.  u is defined
+// bit-sliced: for the 16 global samples of block B = gs >> 4 (same site i,
+// replica, step) four Philox4x32-10 calls c = 0..3 with
+//     counter = (i, B | (c << 28), kTagRefresh | replica, step)
+// give 32 random 16-lane bit-planes, plane k = 8c + 2j + h = half h of output
+// word j of call c, and u(gs) = sum_k bit_{gs & 15}(plane k) << (31 - k).
+//
+// This is the layout of the state itself, so the kernel never builds u: it
+// compares all 32 lanes of a word with the three thresholds plane by plane,
+// most significant first (eq = lanes still equal to the threshold prefix,
+// gt = lanes already above it), and STOPS as soon as no lane is undecided --
+// the remaining planes cannot change any level, so they are never generated.
+// After 16 planes a lane is undecided with probability 3 * 2^-16: almost every
+// word needs 2 of the 4 call pairs.  The number of Philox calls actually made
+// is counted on the device (micsa_counters).
 #pragma once
 #include "layout.cuh"
 #include "philox.cuh"
@@ -31,43 +42,87 @@ __device__ __forceinline__ uint32_t valid_lane_mask(int n_samples, int sg) {
     return (RPW == 2) ? (f | (f << 16)) : f;
 }
 
-// grid = (ceil(L*Lh/block), L, n_words*2); one thread = one site word
+// Thresholds as the kernel sees them: tb[k][p] = all-ones if bit (31-p) of
+// thr_k is set, else 0 (plane p, most significant first), so the lane-parallel
+// compare takes its threshold bit straight from the constant bank; never[k] =
+// thr_k is 2^32 (level k+1 has probability < 2^-32 and is never reached).
+struct RefreshThr { uint32_t tb[3][32]; uint32_t never[3]; };
+
+// grid = (ceil(L*Lh/block), L, n_words*2); one thread = one site word.
+// A word holds two 16-lane Philox streams a (lanes 0-15) and b (lanes 16-31):
+// RPW = 2: the same sample block, replicas 2rg and 2rg+1;
+// RPW = 1: sample blocks 2sg and 2sg+1 of one replica.
+// Per chunk c of 8 planes (one call per stream) and threshold k:
+//   ge = (u_chunk >= t_chunk), a borrow chain from the least significant plane,
+//   eq = (u_chunk == t_chunk),
+// one 3-input logic op per plane each; chunks combine most significant first:
+//   gt |= EQ & ge & ~eq;  EQ &= eq        (EQ = lanes equal to thr so far).
 template <int RPW>
 __global__ void __launch_bounds__(128)
 refresh_kernel(uint32_t* __restrict__ m0, uint32_t* __restrict__ m1, SiteGrid g,
-               PhiloxKeys ks, uint32_t step, uint32_t a0, uint32_t a1, uint32_t a2)
+               PhiloxKeys ks, uint32_t step, RefreshThr thr,
+               unsigned long long* __restrict__ n_calls)
 {
     constexpr int SPW = 32 / RPW;
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= g.L * g.Lh) return;
-    const int y = t / g.Lh, xh = t - y * g.Lh;
-    const int z = blockIdx.y;
-    const int w = blockIdx.z >> 1, p = blockIdx.z & 1;
-    const int sg = w / g.n_rg, rg = w - sg * g.n_rg;
-    const uint32_t i = canonical_site(g.L, p, z, y, xh);
-    const uint32_t blk0 = (uint32_t)(g.sample_offset + sg * SPW) >> 2;
+    unsigned int calls = 0;
+    if (t < g.L * g.Lh) {
+        const int y = t / g.Lh, xh = t - y * g.Lh;
+        const int z = blockIdx.y;
+        const int w = blockIdx.z >> 1, p = blockIdx.z & 1;
+        const int sg = w / g.n_rg, rg = w - sg * g.n_rg;
+        const uint32_t i = canonical_site(g.L, p, z, y, xh);
+        const uint32_t blk = (uint32_t)(g.sample_offset + sg * SPW) >> 4;
+        const uint32_t blk_a = blk, blk_b = (RPW == 2) ? blk : blk + 1u;
+        const uint32_t rep_a = kTagRefresh | (uint32_t)(rg * RPW);
+        const uint32_t rep_b = (RPW == 2) ? rep_a + 1u : rep_a;
+        const uint32_t vm = valid_lane_mask<RPW>(g.n_samples, sg);
+        const bool has_b = (vm >> 16) != 0u;          // block-uniform
 
-    uint32_t b0 = 0, b1 = 0;
+        uint32_t EQ[3], gt[3] = { 0u, 0u, 0u };
 #pragma unroll
-    for (int r = 0; r < RPW; ++r) {
-        const uint32_t rep = (uint32_t)(rg * RPW + r);
+        for (int k = 0; k < 3; ++k) EQ[k] = thr.never[k] ? 0u : vm;
 #pragma unroll
-        for (int c = 0; c < SPW / 4; ++c) {
-            const uint4 o = philox4x32_10(i, blk0 + c, kTagRefresh | rep, step, ks);
-            const uint32_t u[4] = { o.x, o.y, o.z, o.w };
+        for (uint32_t c = 0; c < 4; ++c) {
+            const uint4 oa = philox4x32_10(i, blk_a | (c << 28), rep_a, step, ks);
+            uint4 ob = make_uint4(0u, 0u, 0u, 0u);
+            if (has_b) ob = philox4x32_10(i, blk_b | (c << 28), rep_b, step, ks);
+            calls += has_b ? 2u : 1u;
+            const uint32_t wa[4] = { oa.x, oa.y, oa.z, oa.w };
+            const uint32_t wb[4] = { ob.x, ob.y, ob.z, ob.w };
+            uint32_t ge[3] = { ~0u, ~0u, ~0u }, eq[3] = { ~0u, ~0u, ~0u };
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int lane = r * SPW + 4 * c + j;
-                const uint32_t g1 = u[j] > a0, g2 = u[j] > a1, g3 = u[j] > a2;
-                b0 |= (g1 ^ g2 ^ g3) << lane;      // level odd
-                b1 |= g2 << lane;                  // level >= 2
+            for (int q = 7; q >= 0; --q) {            // least significant plane of the chunk first
+                const int j = q >> 1, h = q & 1;
+                const uint32_t r = __byte_perm(wa[j], wb[j], h ? 0x7632 : 0x5410);
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const uint32_t tb = thr.tb[k][8 * c + q];
+                    ge[k] = (r & ~tb) | (~(r ^ tb) & ge[k]);
+                    eq[k] &= ~(r ^ tb);
+                }
             }
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                gt[k] |= EQ[k] & ge[k] & ~eq[k];
+                EQ[k] &= eq[k];
+            }
+            if ((EQ[0] | EQ[1] | EQ[2]) == 0u) break;
         }
+        // lanes equal to a threshold in all 32 bits are >= it
+        const uint32_t ge0 = gt[0] | EQ[0], ge1 = gt[1] | EQ[1], ge2 = gt[2] | EQ[2];
+        const long long hh = ((long long)blockIdx.z) * g.half + ((long long)z * g.L + y) * g.Lh + xh;
+        m0[hh] = (ge0 ^ ge1 ^ ge2) & vm;      // level odd
+        m1[hh] = ge1 & vm;                    // level >= 2
     }
-    const uint32_t vm = valid_lane_mask<RPW>(g.n_samples, sg);
-    const long long h = ((long long)blockIdx.z) * g.half + ((long long)z * g.L + y) * g.Lh + xh;
-    m0[h] = b0 & vm;
-    m1[h] = b1 & vm;
+    // Philox calls made by this block -> one atomic
+    calls = __reduce_add_sync(0xFFFFFFFFu, calls);
+    __shared__ unsigned int s_calls;
+    if (threadIdx.x == 0) s_calls = 0;
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0 && calls) atomicAdd(&s_calls, calls);
+    __syncthreads();
+    if (threadIdx.x == 0 && s_calls) atomicAdd(n_calls, (unsigned long long)s_calls);
 }
 
 // one random bit for global sample gs from the block (c0, gs>>7, c2, 0)

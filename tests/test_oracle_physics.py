@@ -73,6 +73,53 @@ def test_refresh_histogram_and_mean(oracle, T):
     assert len({flat[k].tobytes() for k in range(ns * nr)}) == ns * nr
 
 
+def test_refresh_uniform_is_uniform_and_independent(oracle):
+    """DESIGN.md R8: the bit-plane assembly must give one fair 32-bit integer
+    per demon, independent between demons that share Philox calls (the 16
+    samples of a block) and between sites / replicas / steps."""
+    seed, n_sites = 77, 1500
+    U = np.array([[oracle.refresh_uniform(i, g, 0, 4, seed) for g in range(32, 48)]
+                  for i in range(n_sites)], dtype=np.uint64)          # one 16-sample block
+    flat = U.reshape(-1).astype(np.float64) / 2.0 ** 32
+    n = flat.size
+    # Kolmogorov-Smirnov against U(0,1): D * sqrt(n) < 1.95  (p ~ 1e-3)
+    srt = np.sort(flat)
+    D = max(np.max(np.arange(1, n + 1) / n - srt), np.max(srt - np.arange(n) / n))
+    assert D * math.sqrt(n) < 1.95
+    # every one of the 32 bit positions is fair (5 sigma)
+    for k in range(32):
+        ones = int(((U >> np.uint64(k)) & np.uint64(1)).sum())
+        assert abs(ones - n / 2) < 5 * math.sqrt(n / 4), k
+    # demons sharing a block are uncorrelated and never share bits systematically
+    Z = (U.astype(np.float64) / 2.0 ** 32 - 0.5) * math.sqrt(12.0)
+    C = (Z.T @ Z) / n_sites
+    off = C - np.diag(np.diag(C))
+    assert np.max(np.abs(off)) < 5 / math.sqrt(n_sites)
+    x = U[:, :-1] ^ U[:, 1:]                                         # neighbours differ in ~16 bits
+    pop = np.array([bin(int(v)).count("1") for v in x.reshape(-1)])
+    assert abs(pop.mean() - 16) < 5 * math.sqrt(8.0 / pop.size)
+    assert len(set(U.reshape(-1).tolist())) > n - 4                  # no systematic collisions
+    # replica, step and sample block all enter
+    base = oracle.refresh_uniform(5, 33, 0, 4, seed)
+    assert len({base, oracle.refresh_uniform(5, 33, 1, 4, seed), oracle.refresh_uniform(5, 33, 0, 5, seed),
+                oracle.refresh_uniform(5, 49, 0, 4, seed), oracle.refresh_uniform(6, 33, 0, 4, seed),
+                oracle.refresh_uniform(5, 33, 0, 4, seed + 1)}) == 6
+
+
+def test_refresh_uniform_uses_every_philox_bit_once(oracle):
+    """The 16 uniforms of a block are a bit-matrix transpose of the four Philox
+    blocks (R8): same multiset of bits, plane k = 8c + 2j + h is the
+    h-th 16-bit half of output word j of call c, most significant plane first."""
+    seed, i, B, rep, step = 0xABCDEF12345, 1234, 7, 3, 99
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    words = np.concatenate([oracle.philox4x32_10([i, B | (c << 28), rep, step], key) for c in range(4)])
+    halves = words.view(np.uint16)                                   # little endian: low half first
+    planes = np.unpackbits(halves.view(np.uint8).reshape(32, 2), axis=1, bitorder="little")   # [plane, lane]
+    for lane in range(16):
+        u = int("".join(str(b) for b in planes[:, lane]), 2)
+        assert u == oracle.refresh_uniform(i, 16 * B + lane, rep, step, seed)
+
+
 def test_refresh_is_a_pure_function_of_its_counters(oracle):
     L, ns, nr = 4, 6, 2
     N = L ** 3
