@@ -140,6 +140,20 @@ int micsa_half_sweep(micsa_ctx *ctx, int parity);
  * Asynchronous.  T must be finite and > 0. */
 int micsa_refresh_demons(micsa_ctx *ctx, double T, uint32_t step);
 
+/* micsa_prefetch_refresh: the refreshed levels depend only on (seed, T, step),
+ * never on the state (PAPER.md:190 -- the old daemons are thrown away), so the
+ * next refresh can be generated while the sweeps run, as the paper's own
+ * implementation does on CPU threads.  This call queues the
+ * generation of refresh (T, step) into a second pair of daemon planes on a
+ * library-owned side stream; it starts when the context's stream reaches this
+ * point.  A later micsa_refresh_demons with exactly the same (T, step) then
+ * only waits for it and swaps plane pointers; any other (T, step) is generated
+ * directly as usual, and the prefetched planes stay valid until consumed or
+ * replaced by another prefetch.  Results are bit-identical either way.
+ * micsa_anneal prefetches step k+1 under the sweeps of step k by itself.
+ * Asynchronous.  T must be finite and > 0. */
+int micsa_prefetch_refresh(micsa_ctx *ctx, double T, uint32_t step);
+
 /* The thresholds micsa_refresh_demons uses: thr[k] = floor(cdf_k * 2^32),
  * k = 0,1,2, each in [0, 2^32]; level m = #{k : u >= thr[k]}.               */
 int micsa_debug_thresholds(double T, uint64_t thr[3]);

@@ -31,6 +31,7 @@ EXPORTS = (
     "micsa_refresh_demons", "micsa_debug_thresholds", "micsa_measure_i64",
     "micsa_measure", "micsa_anneal", "micsa_counters", "micsa_layout_info",
     "micsa_set_tuning",
+    "micsa_prefetch_refresh",
 )
 
 
@@ -90,6 +91,7 @@ def _bind() -> ctypes.CDLL:
             ("micsa_set_daemons", [vp, vp]), ("micsa_get_state", [vp, vp, vp, vp]),
             ("micsa_sweep", [vp, i32]), ("micsa_half_sweep", [vp, i32]),
             ("micsa_refresh_demons", [vp, f64, u32]),
+            ("micsa_prefetch_refresh", [vp, f64, u32]),
             ("micsa_debug_thresholds", [f64, vp]),
             ("micsa_measure_i64", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
             ("micsa_anneal", [vp, vp, i32, u32, vp, vp]),
@@ -217,6 +219,9 @@ class MicSA:
 
     def refresh_demons(self, T, step):
         _check(_lib.micsa_refresh_demons(self._h, float(T), int(step)))
+
+    def prefetch_refresh(self, T, step):
+        _check(_lib.micsa_prefetch_refresh(self._h, float(T), int(step)))
 
     def measure_i64(self):
         E = np.empty(self.n_sys, np.int64)

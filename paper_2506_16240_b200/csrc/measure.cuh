@@ -43,7 +43,8 @@ constexpr int kWarpPlanes   = 21;     // + 5 bits for the 32 threads of a warp
 constexpr int kCountBlock   = 128;
 
 // Adds the per-thread vertical counter over the block and accumulates the 32
-// lane counts into out[0..31] (global, 64-bit).
+// lane counts into out[0..31] (global, 64-bit).  Shuffle version, used by the
+// general replica-pair kernel below.
 __device__ __forceinline__ void block_lane_counts(const VCount<kThreadPlanes>& acc,
                                                   unsigned long long* out)
 {
@@ -77,6 +78,43 @@ __device__ __forceinline__ void block_lane_counts(const VCount<kThreadPlanes>& a
         atomicAdd(&out[threadIdx.x], (unsigned long long)s_cnt[threadIdx.x]);
 }
 
+// Tree version for the one-pass kernel: the block's vertical counters are
+// added pairwise in shared memory (a vertical add costs two logic ops per
+// plane, and whole warps drop out of the upper levels), then 32 threads pick
+// out their lane.  sm holds (P + log2(B)) * B words; P planes per thread.
+template <int P, int B>
+__device__ __forceinline__ void block_tree_lane_counts(const uint32_t (&c)[P], uint32_t* sm,
+                                                       unsigned long long* out)
+{
+    constexpr int LOG = (B == 512) ? 9 : (B == 256) ? 8 : (B == 128) ? 7 : 6;
+    static_assert((1 << LOG) == B, "block size must be 64..512, a power of two");
+    const int tid = threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < P; ++k) sm[k * B + tid] = c[k];
+    for (int k = P; k < P + LOG; ++k) sm[k * B + tid] = 0u;
+    __syncthreads();
+    int np = P;
+    for (int s = B / 2; s >= 1; s >>= 1) {
+        if (tid < s) {
+            uint32_t carry = 0;
+            for (int k = 0; k < np; ++k) {
+                const uint32_t x = sm[k * B + tid], y = sm[k * B + tid + s];
+                sm[k * B + tid] = x ^ y ^ carry;
+                carry = maj3(x, y, carry);
+            }
+            sm[np * B + tid] = carry;
+        }
+        ++np;
+        __syncthreads();
+    }
+    if (tid < 32) {
+        unsigned long long mine = 0;
+        for (int k = 0; k < P + LOG; ++k) mine += (unsigned long long)((sm[k * B] >> tid) & 1u) << k;
+        if (mine) atomicAdd(&out[tid], mine);
+    }
+    __syncthreads();
+}
+
 struct MeasureArgs {
     const uint32_t* spin; const uint32_t* m0; const uint32_t* m1; const void* J;
     int L, Lh, n_rg, n_replicas, n_samples;
@@ -85,82 +123,6 @@ struct MeasureArgs {
     unsigned long long* cntM;    // [n_words][32]  sum of daemon levels
     unsigned long long* cntX;    // [n_sg][pairs_per_sample][32]  sum of sigma^a ^ sigma^b
 };
-
-// Unsatisfied bonds.  grid = (nblk, 2 parities, n_words); grid-stride over the
-// V-word vectors of the parity array; a vector never straddles a row.
-template <int V, int RPW>
-__global__ void __launch_bounds__(kCountBlock)
-count_unsat_kernel(MeasureArgs a)
-{
-    typedef typename BondT<RPW>::type JT;
-    const int p = blockIdx.y, q = 1 - p, w = blockIdx.z;
-    const int L = a.L, Lh = a.Lh, nxv = Lh / V;
-    const long long half = a.half, nvec = half / V;
-    const uint32_t* sp = a.spin + ((long long)w * 2 + p) * half;
-    const uint32_t* sq = a.spin + ((long long)w * 2 + q) * half;
-    const int sg = w / a.n_rg;
-    const JT* Jb = reinterpret_cast<const JT*>(a.J) + (long long)sg * 6 * half;
-    const JT* Jx = Jb + (0 * 2 + p) * half;
-    const JT* Jy = Jb + (1 * 2 + p) * half;
-    const JT* Jz = Jb + (2 * 2 + p) * half;
-
-    VCount<kThreadPlanes> acc; acc.clear();
-    for (long long iv = (long long)blockIdx.x * blockDim.x + threadIdx.x; iv < nvec;
-         iv += (long long)gridDim.x * blockDim.x) {
-        const long long rowi = iv / nxv;
-        const int xv = (int)(iv - rowi * nxv);
-        const int z = (int)(rowi / L), y = (int)(rowi - (long long)z * L);
-        const int yp = (y + 1 == L) ? 0 : y + 1, zp = (z + 1 == L) ? 0 : z + 1;
-        const int xh0 = xv * V;
-        const long long row = rowi * Lh, h = row + xh0;
-        const int c = (y + z + p) & 1;        // c=1: +x neighbour at xh+1, else same xh
-        const Vec<V> s = ldg_vec<V>(sp + h);
-        const Vec<V> A = ldg_vec<V>(sq + h);
-        const uint32_t e = sq[row + ((xh0 + V == Lh) ? 0 : xh0 + V)];
-        const Vec<V> ny = ldg_vec<V>(sq + ((long long)z * L + yp) * Lh + xh0);
-        const Vec<V> nz = ldg_vec<V>(sq + ((long long)zp * L + y) * Lh + xh0);
-        const Vec<V> jx = ldg_bonds<V, RPW>(Jx + h);
-        const Vec<V> jy = ldg_bonds<V, RPW>(Jy + h);
-        const Vec<V> jz = ldg_bonds<V, RPW>(Jz + h);
-        VCount<4> loc; loc.clear();
-#pragma unroll
-        for (int k = 0; k < V; ++k) {
-            const uint32_t up = (k + 1 < V) ? A.v[k + 1] : e;
-            const uint32_t nx = c ? up : A.v[k];
-            const uint32_t ux = s.v[k] ^ nx ^ jx.v[k];
-            const uint32_t uy = s.v[k] ^ ny.v[k] ^ jy.v[k];
-            const uint32_t uz = s.v[k] ^ nz.v[k] ^ jz.v[k];
-            const uint32_t b[2] = { ux ^ uy ^ uz, maj3(ux, uy, uz) };
-            loc.add(b);
-        }
-        acc.add(loc.c);
-    }
-    block_lane_counts(acc, a.cntU + (long long)w * 32);
-}
-
-// Sum of daemon levels.  grid = (nblk, n_words); both parities are contiguous.
-template <int V>
-__global__ void __launch_bounds__(kCountBlock)
-count_levels_kernel(MeasureArgs a)
-{
-    const int w = blockIdx.y;
-    const long long n = 2 * a.half, nvec = n / V;
-    const uint32_t* p0 = a.m0 + (long long)w * n;
-    const uint32_t* p1 = a.m1 + (long long)w * n;
-    VCount<kThreadPlanes> acc; acc.clear();
-    for (long long iv = (long long)blockIdx.x * blockDim.x + threadIdx.x; iv < nvec;
-         iv += (long long)gridDim.x * blockDim.x) {
-        const Vec<V> b0 = ldg_vec<V>(p0 + iv * V), b1 = ldg_vec<V>(p1 + iv * V);
-        VCount<4> loc; loc.clear();
-#pragma unroll
-        for (int k = 0; k < V; ++k) {
-            const uint32_t b[2] = { b0.v[k], b1.v[k] };
-            loc.add(b);
-        }
-        acc.add(loc.c);
-    }
-    block_lane_counts(acc, a.cntM + (long long)w * 32);
-}
 
 // Replica overlap: differing spins of replicas (ra, rb) of every sample of
 // sample group sg.  grid = (nblk, n_sg, pairs_per_sample).
@@ -195,33 +157,137 @@ count_xor_kernel(MeasureArgs a)
 }
 
 struct FinalizeArgs {
-    const unsigned long long* cntU; const unsigned long long* cntM; const unsigned long long* cntX;
+    unsigned long long* cntU; unsigned long long* cntM; unsigned long long* cntX;
+    long long cnt_words;   // length of the counter area starting at cntU (zeroed after use)
+    unsigned int* ticket;  // blocks done so far (last one finalises and resets it)
     long long* row;        // [n_sys E | n_sys E_daemon | n_pairs Q]
     long long* min_E;      // [n_sys] running minimum, or nullptr
     int n_samples, n_replicas, n_rg, rpw, spw, pairs_per_sample;
     long long N;
 };
 
-// counts -> exact sums in canonical system order; one thread per system / pair
-__global__ void finalize_measure_kernel(FinalizeArgs f)
+// counts -> exact sums in canonical system order (run by one block)
+__device__ __forceinline__ void finalize_rows(const FinalizeArgs& f)
 {
     const int n_sys = f.n_samples * f.n_replicas;
     const int n_pairs = f.n_samples * f.pairs_per_sample;
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t < n_sys) {
+    for (int t = threadIdx.x; t < n_sys; t += blockDim.x) {
         const int sample = t / f.n_replicas, rep = t - sample * f.n_replicas;
         const int sg = sample / f.spw, sl = sample - sg * f.spw;
         const int w = sg * f.n_rg + rep / f.rpw, lane = (rep % f.rpw) * f.spw + sl;
-        const long long E = 2 * (long long)f.cntU[(long long)w * 32 + lane] - 3 * f.N;
+        const long long E = 2 * (long long)__ldcg(&f.cntU[(long long)w * 32 + lane]) - 3 * f.N;
         f.row[t] = E;
-        f.row[n_sys + t] = 4 * (long long)f.cntM[(long long)w * 32 + lane];
+        f.row[n_sys + t] = 4 * (long long)__ldcg(&f.cntM[(long long)w * 32 + lane]);
         if (f.min_E && E < f.min_E[t]) f.min_E[t] = E;
     }
-    if (t < n_pairs) {
+    for (int t = threadIdx.x; t < n_pairs; t += blockDim.x) {
         const int sample = t / f.pairs_per_sample, pr = t - sample * f.pairs_per_sample;
         const int sg = sample / f.spw, sl = sample - sg * f.spw;
         f.row[2 * n_sys + t] =
-            f.N - 2 * (long long)f.cntX[((long long)sg * f.pairs_per_sample + pr) * 32 + sl];
+            f.N - 2 * (long long)__ldcg(&f.cntX[((long long)sg * f.pairs_per_sample + pr) * 32 + sl]);
+    }
+    __syncthreads();
+    for (long long k = threadIdx.x; k < f.cnt_words; k += blockDim.x) f.cntU[k] = 0ull;   // ready for the next one
+}
+
+constexpr int kMeasureBlock = 256;
+constexpr int kMeasureBatch = 16;      // items between flushes of the 8-plane counters
+constexpr int kMeasureMaxItems = 320;  // per thread: 320 * 12 < 2^12
+
+// One pass over the state for all three observables.
+// An item = V consecutive words of one row of one parity array; it counts the
+// unsatisfied +x,+y,+z bonds of its sites (every bond once, at its owner), the
+// daemon levels of its sites and -- when PAIR (n_replicas == 2, both replicas
+// in the word) -- the lanes where the two replicas differ.  Other replica
+// pairs are counted by count_xor_kernel before this kernel runs.  The last
+// block to finish turns the counts into the measurement row.
+// grid = (nblk, n_words), block = kMeasureBlock.
+template <int V, int RPW, bool PAIR>
+__global__ void __launch_bounds__(kMeasureBlock)
+measure_kernel(MeasureArgs a, FinalizeArgs f)
+{
+    typedef typename BondT<RPW>::type JT;
+    __shared__ uint32_t sm[(12 + 8) * kMeasureBlock];
+    __shared__ unsigned int s_last;
+    const int w = blockIdx.y;
+    const int L = a.L, Lh = a.Lh, nxv = Lh / V;
+    const long long half = a.half;
+    const long long items_p = half / V, n_items = 2 * items_p;
+    const uint32_t* s0 = a.spin + (long long)w * 2 * half;
+    const uint32_t* d0 = a.m0 + (long long)w * 2 * half;
+    const uint32_t* d1 = a.m1 + (long long)w * 2 * half;
+    const int sg = w / a.n_rg;
+    const JT* Jb = reinterpret_cast<const JT*>(a.J) + (long long)sg * 6 * half;
+
+    VCount<12> accU, accM, accX; accU.clear(); accM.clear(); accX.clear();
+    const long long stride = (long long)gridDim.x * kMeasureBlock;
+    for (long long base = (long long)blockIdx.x * kMeasureBlock + threadIdx.x; base < n_items;
+         base += stride * kMeasureBatch) {
+        VCount<8> midU, midM, midX; midU.clear(); midM.clear(); midX.clear();
+#pragma unroll 2
+        for (int j = 0; j < kMeasureBatch; ++j) {
+            const long long it = base + j * stride;
+            if (it >= n_items) break;
+            const int p = it >= items_p;
+            const long long iv = it - (p ? items_p : 0);
+            const long long rowi = iv / nxv;
+            const int xv = (int)(iv - rowi * nxv);
+            const int z = (int)(rowi / L), y = (int)(rowi - (long long)z * L);
+            const int yp = (y + 1 == L) ? 0 : y + 1, zp = (z + 1 == L) ? 0 : z + 1;
+            const int xh0 = xv * V;
+            const long long row = rowi * Lh, h = row + xh0;
+            const int c = (y + z + p) & 1;        // c=1: +x neighbour at xh+1, else same xh
+            const uint32_t* sp = s0 + (p ? half : 0);
+            const uint32_t* sq = s0 + (p ? 0 : half);
+            const Vec<V> s = ldg_vec<V>(sp + h);
+            const Vec<V> A = ldg_vec<V>(sq + h);
+            const uint32_t e = sq[row + ((xh0 + V == Lh) ? 0 : xh0 + V)];
+            const Vec<V> ny = ldg_vec<V>(sq + ((long long)z * L + yp) * Lh + xh0);
+            const Vec<V> nz = ldg_vec<V>(sq + ((long long)zp * L + y) * Lh + xh0);
+            const Vec<V> jx = ldg_bonds<V, RPW>(Jb + (0 * 2 + p) * half + h);
+            const Vec<V> jy = ldg_bonds<V, RPW>(Jb + (1 * 2 + p) * half + h);
+            const Vec<V> jz = ldg_bonds<V, RPW>(Jb + (2 * 2 + p) * half + h);
+            const Vec<V> b0 = ldg_vec<V>(d0 + (p ? half : 0) + h);
+            const Vec<V> b1 = ldg_vec<V>(d1 + (p ? half : 0) + h);
+            VCount<4> locU, locM; locU.clear(); locM.clear();
+            VCount<3> locX; locX.clear();
+#pragma unroll
+            for (int k = 0; k < V; ++k) {
+                const uint32_t up = (k + 1 < V) ? A.v[k + 1] : e;
+                const uint32_t nx = c ? up : A.v[k];
+                const uint32_t ux = s.v[k] ^ nx ^ jx.v[k];
+                const uint32_t uy = s.v[k] ^ ny.v[k] ^ jy.v[k];
+                const uint32_t uz = s.v[k] ^ nz.v[k] ^ jz.v[k];
+                const uint32_t bu[2] = { ux ^ uy ^ uz, maj3(ux, uy, uz) };
+                locU.add(bu);
+                const uint32_t bm[2] = { b0.v[k], b1.v[k] };
+                locM.add(bm);
+                if (PAIR) {
+                    const uint32_t bx[1] = { (s.v[k] ^ (s.v[k] >> 16)) & 0xFFFFu };
+                    locX.add(bx);
+                }
+            }
+            midU.add(locU.c); midM.add(locM.c);
+            if (PAIR) midX.add(locX.c);
+        }
+        accU.add(midU.c); accM.add(midM.c);
+        if (PAIR) accX.add(midX.c);
+    }
+    block_tree_lane_counts<12, kMeasureBlock>(accU.c, sm, a.cntU + (long long)w * 32);
+    block_tree_lane_counts<12, kMeasureBlock>(accM.c, sm, a.cntM + (long long)w * 32);
+    if (PAIR) block_tree_lane_counts<12, kMeasureBlock>(accX.c, sm, a.cntX + (long long)sg * 32);
+
+    // the last block to arrive finalises (its reads see every block's atomics)
+    __threadfence();
+    if (threadIdx.x == 0) {
+        const unsigned int total = gridDim.x * gridDim.y;
+        s_last = (atomicAdd(f.ticket, 1u) == total - 1u);
+    }
+    __syncthreads();
+    if (s_last) {
+        __threadfence();
+        finalize_rows(f);
+        if (threadIdx.x == 0) *f.ticket = 0u;
     }
 }
 

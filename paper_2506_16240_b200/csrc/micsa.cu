@@ -33,7 +33,7 @@ constexpr size_t kAlign = 256;
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {                 // byte offsets inside the workspace
-    size_t spin, m0, m1, J, cnt, row, minE, bad, calls, total;
+    size_t spin, m0, m1, m0s, m1s, J, cnt, ticket, row, minE, bad, calls, total;
     size_t plane_bytes, J_bytes, cnt_words, row_len;
 };
 
@@ -75,8 +75,11 @@ Plan make_plan(const Geom& g) {
     p.spin = o; o += align_up(p.plane_bytes);
     p.m0 = o;   o += align_up(p.plane_bytes);
     p.m1 = o;   o += align_up(p.plane_bytes);
+    p.m0s = o;  o += align_up(p.plane_bytes);      // staging planes of a prefetched refresh
+    p.m1s = o;  o += align_up(p.plane_bytes);
     p.J = o;    o += align_up(p.J_bytes);
     p.cnt = o;  o += align_up(p.cnt_words * 8);
+    p.ticket = o; o += align_up(sizeof(unsigned int));
     p.row = o;  o += align_up(p.row_len * 8);
     p.minE = o; o += align_up((size_t)g.n_sys * 8);
     p.bad = o;  o += align_up(sizeof(int));
@@ -99,9 +102,15 @@ struct micsa_ctx {
     char* ws;
     bool owns_ws;
     unsigned long long* cnt;
+    unsigned int* ticket;
     long long* row;
     long long* minE;
     int* bad;
+    uint32_t* m0s; uint32_t* m1s;             // staging planes (swapped with st.m0/m1 when consumed)
+    cudaStream_t side;                        // generates prefetched refreshes under the sweeps
+    cudaEvent_t ev_main, ev_side;
+    bool pending; double pending_T; uint32_t pending_step;
+    long long* host_row;        // pinned host staging for one measurement row
     unsigned long long* calls;  // Philox calls made by the refresh kernels (device counter)
     int V;
     int sweep_kernel;          // 0 = tiled (TMA-staged) when L % 8 == 0, 1 = row-marching
@@ -231,7 +240,8 @@ int thresholds_host(double T, uint64_t thr[3]) {
     return MICSA_OK;
 }
 
-int launch_refresh(micsa_ctx* c, double T, uint32_t step) {
+int launch_refresh_into(micsa_ctx* c, double T, uint32_t step, uint32_t* m0, uint32_t* m1,
+                        cudaStream_t stream) {
     uint64_t thr[3];
     if (thresholds_host(T, thr) != MICSA_OK || thr[0] == 0) {
         set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID;
@@ -244,11 +254,45 @@ int launch_refresh(micsa_ctx* c, double T, uint32_t step) {
     const SiteGrid sg = site_grid(c->g);
     const dim3 grid = site_blocks(c->g, c->g.n_words * 2);
     if (c->g.rpw == 2)
-        refresh_kernel<2><<<grid, 128, 0, c->stream>>>(c->st.m0, c->st.m1, sg, c->ks, step, rt, c->calls);
+        refresh_kernel<2><<<grid, 128, 0, stream>>>(m0, m1, sg, c->ks, step, rt, c->calls);
     else
-        refresh_kernel<1><<<grid, 128, 0, c->stream>>>(c->st.m0, c->st.m1, sg, c->ks, step, rt, c->calls);
-    c->rns += (uint64_t)c->g.N * (uint64_t)c->g.n_sys;
+        refresh_kernel<1><<<grid, 128, 0, stream>>>(m0, m1, sg, c->ks, step, rt, c->calls);
     return post_launch(c);
+}
+
+// Refresh (T, step) on the context's stream.  If exactly this refresh was
+// prefetched, its planes are already (being) generated on the side stream:
+// wait for them and swap the plane pointers -- the old levels are thrown away
+// anyway.
+int launch_refresh(micsa_ctx* c, double T, uint32_t step) {
+    if (c->pending && c->pending_step == step && memcmp(&c->pending_T, &T, sizeof T) == 0) {
+        CK(c, cudaStreamWaitEvent(c->stream, c->ev_side, 0));
+        std::swap(c->st.m0, c->m0s);
+        std::swap(c->st.m1, c->m1s);
+        c->pending = false;
+    } else {
+        const int rc = launch_refresh_into(c, T, step, c->st.m0, c->st.m1, c->stream);
+        if (rc) return rc;
+    }
+    c->rns += (uint64_t)c->g.N * (uint64_t)c->g.n_sys;
+    return MICSA_OK;
+}
+
+// Queue the generation of refresh (T, step) into the staging planes on the side
+// stream; it starts once the main stream has reached this point (everything
+// that still reads the staging planes' previous role has finished).
+int launch_prefetch(micsa_ctx* c, double T, uint32_t step) {
+    uint64_t thr[3];
+    if (thresholds_host(T, thr) != MICSA_OK || thr[0] == 0) {
+        set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID;
+    }
+    CK(c, cudaEventRecord(c->ev_main, c->stream));
+    CK(c, cudaStreamWaitEvent(c->side, c->ev_main, 0));
+    const int rc = launch_refresh_into(c, T, step, c->m0s, c->m1s, c->side);
+    if (rc) return rc;
+    CK(c, cudaEventRecord(c->ev_side, c->side));
+    c->pending = true; c->pending_T = T; c->pending_step = step;
+    return MICSA_OK;
 }
 
 unsigned count_blocks(long long nvec, long long other) {
@@ -261,49 +305,53 @@ unsigned count_blocks(long long nvec, long long other) {
 }
 
 template <int V, int RPW>
-void launch_counts_t(micsa_ctx* c, const MeasureArgs& a) {
+void launch_measure_t(micsa_ctx* c, const MeasureArgs& a, const FinalizeArgs& f) {
     const Geom& g = c->g;
-    const long long nvec_p = g.half / V;
-    count_unsat_kernel<V, RPW><<<dim3(count_blocks(nvec_p, 2ll * g.n_words), 2, (unsigned)g.n_words),
-                                 kCountBlock, 0, c->stream>>>(a);
-    count_levels_kernel<V><<<dim3(count_blocks(2 * nvec_p, g.n_words), (unsigned)g.n_words),
-                             kCountBlock, 0, c->stream>>>(a);
-    c->launches += 2;
     const int pps = g.n_replicas * (g.n_replicas - 1) / 2;
-    if (pps > 0) {
-        count_xor_kernel<V, RPW><<<dim3(count_blocks(2 * nvec_p, (long long)g.n_sg * pps),
+    const bool pair_in_word = (g.n_replicas == 2);          // then RPW == 2
+    if (pps > 0 && !pair_in_word) {
+        count_xor_kernel<V, RPW><<<dim3(count_blocks(2 * g.half / V, (long long)g.n_sg * pps),
                                         (unsigned)g.n_sg, (unsigned)pps),
                                    kCountBlock, 0, c->stream>>>(a);
         c->launches += 1;
     }
+    // two resident blocks per SM over all word lattices, never more than
+    // kMeasureMaxItems items per thread (12-plane per-thread counters)
+    const long long n_items = 2 * g.half / V;
+    long long nb = (n_items + (long long)kMeasureBlock * kMeasureBatch - 1) / ((long long)kMeasureBlock * kMeasureBatch);
+    nb = std::min(nb, std::max<long long>(1, (148 * 2) / g.n_words));
+    const long long need = (n_items + (long long)kMeasureBlock * kMeasureMaxItems - 1) / ((long long)kMeasureBlock * kMeasureMaxItems);
+    nb = std::max<long long>(std::max<long long>(nb, need), 1);
+    const dim3 grid((unsigned)nb, (unsigned)g.n_words);
+    if (RPW == 2 && pair_in_word) measure_kernel<V, RPW, true><<<grid, kMeasureBlock, 0, c->stream>>>(a, f);
+    else                          measure_kernel<V, RPW, false><<<grid, kMeasureBlock, 0, c->stream>>>(a, f);
 }
 
-// one measurement: exact sums into the device row `row`, optional min fold
+// one measurement: exact sums into the device row `row`, optional min fold.
+// The counters are zero on entry (create, and the finalising block re-zeroes).
 int launch_measure(micsa_ctx* c, long long* row, bool fold_min) {
     const Geom& g = c->g;
     if (g.n_replicas * (g.n_replicas - 1) / 2 > 65535) { set_err("too many replica pairs"); return MICSA_ERR_INVALID; }
-    CK(c, cudaMemsetAsync(c->cnt, 0, c->plan.cnt_words * 8, c->stream));
     MeasureArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
     a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg; a.n_replicas = g.n_replicas; a.n_samples = g.n_samples;
     a.half = g.half;
     a.cntU = c->cnt; a.cntM = c->cnt + (size_t)g.n_words * 32; a.cntX = c->cnt + (size_t)g.n_words * 64;
-    switch (c->V * 10 + g.rpw) {
-        case 41: launch_counts_t<4, 1>(c, a); break;
-        case 42: launch_counts_t<4, 2>(c, a); break;
-        case 21: launch_counts_t<2, 1>(c, a); break;
-        case 22: launch_counts_t<2, 2>(c, a); break;
-        case 11: launch_counts_t<1, 1>(c, a); break;
-        default: launch_counts_t<1, 2>(c, a); break;
-    }
     FinalizeArgs f;
     f.cntU = a.cntU; f.cntM = a.cntM; f.cntX = a.cntX;
+    f.cnt_words = (long long)c->plan.cnt_words; f.ticket = c->ticket;
     f.row = row; f.min_E = fold_min ? c->minE : nullptr;
     f.n_samples = g.n_samples; f.n_replicas = g.n_replicas; f.n_rg = g.n_rg;
     f.rpw = g.rpw; f.spw = g.spw; f.pairs_per_sample = g.n_replicas * (g.n_replicas - 1) / 2;
     f.N = g.N;
-    const int n = std::max(g.n_sys, g.n_pairs);
-    finalize_measure_kernel<<<(n + 127) / 128, 128, 0, c->stream>>>(f);
+    switch (c->V * 10 + g.rpw) {
+        case 41: launch_measure_t<4, 1>(c, a, f); break;
+        case 42: launch_measure_t<4, 2>(c, a, f); break;
+        case 21: launch_measure_t<2, 1>(c, a, f); break;
+        case 22: launch_measure_t<2, 2>(c, a, f); break;
+        case 11: launch_measure_t<1, 1>(c, a, f); break;
+        default: launch_measure_t<1, 2>(c, a, f); break;
+    }
     return post_launch(c);
 }
 
@@ -338,10 +386,18 @@ int set_sys(micsa_ctx* c, const int8_t* src, int kind) {
     return MICSA_OK;
 }
 
+void destroy_side(micsa_ctx* c) {
+    if (c->side) { cudaStreamSynchronize(c->side); cudaStreamDestroy(c->side); c->side = nullptr; }
+    if (c->ev_main) { cudaEventDestroy(c->ev_main); c->ev_main = nullptr; }
+    if (c->ev_side) { cudaEventDestroy(c->ev_side); c->ev_side = nullptr; }
+}
+
 int init_state(micsa_ctx* c) {
     const Geom& g = c->g;
     const SiteGrid sg = site_grid(g);
     CK(c, cudaMemsetAsync(c->calls, 0, sizeof(unsigned long long), c->stream));
+    CK(c, cudaMemsetAsync(c->cnt, 0, c->plan.cnt_words * 8, c->stream));
+    CK(c, cudaMemsetAsync(c->ticket, 0, sizeof(unsigned int), c->stream));
     CK(c, cudaMemsetAsync(c->st.m0, 0, c->plan.plane_bytes, c->stream));
     CK(c, cudaMemsetAsync(c->st.m1, 0, c->plan.plane_bytes, c->stream));
     if (g.rpw == 2) {
@@ -410,12 +466,29 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->st.m0 = (uint32_t*)(c->ws + c->plan.m0);
     c->st.m1 = (uint32_t*)(c->ws + c->plan.m1);
     c->st.J = (void*)(c->ws + c->plan.J);
+    c->m0s = (uint32_t*)(c->ws + c->plan.m0s);
+    c->m1s = (uint32_t*)(c->ws + c->plan.m1s);
+    c->pending = false; c->pending_T = 0.0; c->pending_step = 0;
     c->cnt = (unsigned long long*)(c->ws + c->plan.cnt);
+    c->ticket = (unsigned int*)(c->ws + c->plan.ticket);
     c->row = (long long*)(c->ws + c->plan.row);
     c->minE = (long long*)(c->ws + c->plan.minE);
     c->bad = (int*)(c->ws + c->plan.bad);
     c->calls = (unsigned long long*)(c->ws + c->plan.calls);
-    if (init_state(c) != MICSA_OK) { if (c->owns_ws) cudaFree(c->ws); delete c; return nullptr; }
+    c->host_row = nullptr; c->side = nullptr; c->ev_main = nullptr; c->ev_side = nullptr;
+    if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_main, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_side, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError(); set_err("could not create the side stream");
+        destroy_side(c); if (c->owns_ws) cudaFree(c->ws); delete c; return nullptr;
+    }
+    if (cudaHostAlloc((void**)&c->host_row, c->plan.row_len * 8, cudaHostAllocDefault) != cudaSuccess) {
+        cudaGetLastError(); set_err("out of pinned host memory");
+        destroy_side(c); if (c->owns_ws) cudaFree(c->ws); delete c; return nullptr;
+    }
+    if (init_state(c) != MICSA_OK) {
+        cudaFreeHost(c->host_row); destroy_side(c); if (c->owns_ws) cudaFree(c->ws); delete c; return nullptr;
+    }
     return c;
 }
 
@@ -426,7 +499,9 @@ micsa_ctx* micsa_create(int L, int n_samples, int n_replicas, uint64_t seed) {
 int micsa_destroy(micsa_ctx* c) {
     if (!c) return MICSA_OK;
     cudaStreamSynchronize(c->stream);
+    destroy_side(c);
     if (c->owns_ws) cudaFree(c->ws);
+    cudaFreeHost(c->host_row);
     delete c;
     return MICSA_OK;
 }
@@ -434,6 +509,7 @@ int micsa_destroy(micsa_ctx* c) {
 int micsa_synchronize(micsa_ctx* c) {
     int rc = check_ctx(c); if (rc) return rc;
     CK(c, cudaStreamSynchronize(c->stream));
+    CK(c, cudaStreamSynchronize(c->side));
     return MICSA_OK;
 }
 
@@ -521,17 +597,21 @@ int micsa_refresh_demons(micsa_ctx* c, double T, uint32_t step) {
     return launch_refresh(c, T, step);
 }
 
+int micsa_prefetch_refresh(micsa_ctx* c, double T, uint32_t step) {
+    int rc = check_ctx(c); if (rc) return rc;
+    return launch_prefetch(c, T, step);
+}
+
 int micsa_measure_i64(micsa_ctx* c, int64_t* E, int64_t* Ed, int64_t* Q) {
     int rc = check_ctx(c); if (rc) return rc;
     const Geom& g = c->g;
     if (Q && g.n_replicas < 2) { set_err("q_overlap needs n_replicas >= 2"); return MICSA_ERR_INVALID; }
     rc = launch_measure(c, c->row, false); if (rc) return rc;
-    std::vector<long long> host(c->plan.row_len);
-    CK(c, cudaMemcpyAsync(host.data(), c->row, c->plan.row_len * 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(c, cudaMemcpyAsync(c->host_row, c->row, c->plan.row_len * 8, cudaMemcpyDeviceToHost, c->stream));
     CK(c, cudaStreamSynchronize(c->stream));
-    if (E)  memcpy(E, host.data(), (size_t)g.n_sys * 8);
-    if (Ed) memcpy(Ed, host.data() + g.n_sys, (size_t)g.n_sys * 8);
-    if (Q)  memcpy(Q, host.data() + 2 * g.n_sys, (size_t)g.n_pairs * 8);
+    if (E)  memcpy(E, c->host_row, (size_t)g.n_sys * 8);
+    if (Ed) memcpy(Ed, c->host_row + g.n_sys, (size_t)g.n_sys * 8);
+    if (Q)  memcpy(Q, c->host_row + 2 * g.n_sys, (size_t)g.n_pairs * 8);
     return MICSA_OK;
 }
 
@@ -579,6 +659,9 @@ int micsa_anneal(micsa_ctx* c, const micsa_step* sched, int n_steps, uint32_t st
     long long r = 0, t = 0;
     for (int k = 0; k < n_steps; ++k) {
         rc = launch_refresh(c, sched[k].T, step0 + (uint32_t)k); if (rc) return rc;
+        if (k + 1 < n_steps && sched[k].n_sweeps > 0) {       // generated under this step's sweeps
+            rc = launch_prefetch(c, sched[k + 1].T, step0 + (uint32_t)k + 1u); if (rc) return rc;
+        }
         for (int j = 1; j <= sched[k].n_sweeps; ++j) {
             rc = launch_half_sweep(c, 0); if (rc) return rc;
             rc = launch_half_sweep(c, 1); if (rc) return rc;
@@ -622,6 +705,7 @@ int micsa_counters(micsa_ctx* c, uint64_t* attempts, uint64_t* rns, uint64_t* ph
         // lazy refresh: the number of calls is data dependent and counted on the device
         if (c->sticky) { set_err("context is in a sticky CUDA error state"); return c->sticky; }
         unsigned long long n = 0;
+        CK(c, cudaStreamSynchronize(c->side));
         CK(c, cudaMemcpyAsync(&n, c->calls, sizeof n, cudaMemcpyDeviceToHost, c->stream));
         CK(c, cudaStreamSynchronize(c->stream));
         *philox_calls = (uint64_t)n;

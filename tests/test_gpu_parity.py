@@ -327,3 +327,33 @@ def test_paramagnetic_energy_matches_metropolis_on_gpu(micsa, oracle):
         err = np.sqrt(e_gpu.var(ddof=1) / e_gpu.size + e_met.var(ddof=1) / e_met.size)
         # per-system time averages scatter by sample-to-sample and thermal noise
         assert abs(d) < 3 * err + 2e-3, (T, d, err)
+
+
+def test_prefetched_refresh_is_bit_identical(micsa, oracle):
+    """micsa_prefetch_refresh: the levels generated on the side stream under the
+    sweeps equal a direct refresh; a non-matching refresh is generated directly
+    and leaves the prefetched planes valid for later."""
+    L, ns, nr, seed = 16, 20, 2, 21
+    s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+    m = np.zeros_like(s, dtype=np.uint8)
+    with micsa.MicSA(L, ns, nr, seed) as g:
+        g.refresh_demons(1.3, 0); oracle.refresh(L, m, seed, 1.3, 0)
+        for k in range(1, 6):
+            g.prefetch_refresh(1.3 - 0.1 * k, k)          # generated while the sweeps run
+            g.sweep(3); oracle.sweep(L, s, m, J, 3)
+            _assert_state(g, s, m)
+            if k == 3:                                    # an unrelated refresh in between
+                g.refresh_demons(2.5, 77); oracle.refresh(L, m, seed, 2.5, 77)
+                _assert_state(g, s, m)
+                g.sweep(1); oracle.sweep(L, s, m, J, 1)
+            g.refresh_demons(1.3 - 0.1 * k, k); oracle.refresh(L, m, seed, 1.3 - 0.1 * k, k)
+            _assert_state(g, s, m)
+        # same step, other temperature: must not consume the prefetched planes
+        g.prefetch_refresh(0.9, 9)
+        g.refresh_demons(0.8, 9); oracle.refresh(L, m, seed, 0.8, 9)
+        _assert_state(g, s, m)
+        g.refresh_demons(0.9, 9); oracle.refresh(L, m, seed, 0.9, 9)
+        _assert_state(g, s, m)
+        c = g.counters()
+        assert c["rns_drawn"] == 9 * L ** 3 * ns * nr
+        assert 0 < c["philox_calls"] <= 10 * L ** 3 * ns * nr // 4 + 10 * L ** 3 * 4

@@ -59,9 +59,9 @@ def test_thresholds_reject_bad_T(micsa, T):
 
 
 def test_workspace_bytes(micsa):
-    # config 4: 4.096M sites x (1 spin + 2 daemon words) x 4 B + 3 bond planes x 2 B
+    # config 4: 4.096M sites x (1 spin + 2 daemon + 2 staged daemon words) x 4 B + 3 bond planes x 2 B
     N = 160 ** 3
-    packed = N * 4 * 3 + N * 3 * 2
+    packed = N * 4 * 5 + N * 3 * 2
     ws = micsa.workspace_bytes(160, 16, 2)
     assert packed <= ws <= packed + 65536
     assert micsa.workspace_bytes(64, 1024, 1) >= 64 ** 3 * 32 * 4 * 6
