@@ -8,6 +8,8 @@ config 4 (L=160, 16 samples x 2 replicas, T=0.9): daemon refresh at T, then
 10 checkerboard sweeps, then the E / E_daemon / q reductions.  Prints ONE JSON
 line (rank 0).  `value` = spin-flip attempts per ns with the state resident in
 HBM, timed with CUDA events on the library's stream, L2 flushed between steps;
+the refresh of step k+1 is generated on the library's side stream during step
+k (micsa_prefetch_refresh), so every timed step contains one generation;
 `e2e` = the same step through the C ABI with HOST buffers (couplings + spins
 uploaded from pinned host memory, observables read back) inside the timed
 region.  N > 1: one process per GPU (torchrun), samples sharded by rank with
@@ -170,25 +172,35 @@ def main():
         return float(t.item())
 
     L, ns, nr = CFG.L, CFG.n_samples, CFG.n_replicas
-    g = micsa.MicSA(L, ns, nr, CFG.seed, sample_offset=rank * ns, device=local_rank)
+    # a high-priority stream for the path, so that the refresh prefetched on the
+    # library's side stream only fills what the sweeps leave idle
+    stream = torch.cuda.Stream(device=dev, priority=-1)
+    torch.cuda.set_stream(stream)
+    from paper_2506_16240_b200.sharding import sample_offset
+    g = micsa.MicSA(L, ns, nr, CFG.seed, sample_offset=sample_offset(rank, ns), device=local_rank,
+                    stream=stream)
     info = g.layout_info()
     attempts_step = CFG.attempts_per_sweep * SWEEPS_PER_STEP
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
-    stream = torch.cuda.current_stream()
 
     def step(k, ev=None):
-        g.refresh_demons(T_RUN, k)
+        g.refresh_demons(T_RUN, k)              # consumes the planes prefetched during step k-1
+        g.prefetch_refresh(T_RUN, k + 1)        # generated on the side stream under this step's sweeps
         if ev:
             ev[1].record(stream)
         g.sweep(SWEEPS_PER_STEP)
         if ev:
             ev[2].record(stream)
-        return g.measure_i64()
+        g.measure_begin()                       # reduction kernel + D2H of the row, queued
+        if ev:
+            ev[3].record(stream)
+        return g.measure_end()                  # host waits for the row (after the timed region)
 
     for k in range(args.warmup):
         step(k)
     barrier()
     launches0 = g.layout_info()["launches"]
+    calls0 = g.counters()["philox_calls"]
     sampler = ClockSampler(local_rank)
     sampler.start()
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
@@ -199,11 +211,11 @@ def main():
         ev = evs[k]
         ev[0].record(stream)
         step(args.warmup + k, ev)
-        ev[3].record(stream)
     barrier()
     wall = time.perf_counter() - wall0
     clocks = sampler.stop()
     launches = g.layout_info()["launches"] - launches0
+    philox_words = 4.0 * (g.counters()["philox_calls"] - calls0)
     t_step_ms = sum(e[0].elapsed_time(e[3]) for e in evs)
     t_sweep_ms = sum(e[1].elapsed_time(e[2]) for e in evs)
     t_step_ms = max_over_ranks(t_step_ms)
@@ -225,7 +237,7 @@ def main():
     achieved = alg_bytes / t_launch_s / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
-                "kernel": "half_sweep_kernel<4,2>", "peak_source": peak_src,
+                "kernel": "half_sweep_rows_kernel<2,4>", "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "us_per_launch": t_launch_s * 1e6,
                 "convention": "compulsory one-pass traffic: 7.5 bits/attempt (spin 1r+1w, daemon 2r+2w, "
@@ -273,6 +285,7 @@ def main():
                        "l2": "flushed between timed steps (256 MiB write); state 73.7 MB < 126 MB L2",
                        "sharding": "samples by rank, global sample offsets, no collective"},
             "rns_per_attempt": 1.0 / SWEEPS_PER_STEP,
+            "philox_words_generated_per_attempt": philox_words / (attempts_step * args.steps),
             "sweep_only_attempts_per_ns": sweep_only,
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
             "roofline": roofline, "cpu_baseline": cpu, "wall_s": wall,

@@ -168,6 +168,16 @@ int micsa_debug_thresholds(double T, uint64_t thr[3]);
  * micsa_measure: the same divided by N as float64 (e of Eq. 15, PAPER.md:255;
  * q of Eq. C.1).  Q != NULL with n_replicas < 2 -> MICSA_ERR_INVALID.        */
 int micsa_measure_i64(micsa_ctx *ctx, int64_t *E, int64_t *E_daemon, int64_t *Q);
+
+/* The same measurement split in two, so that the caller can queue more work
+ * (or stop a timer on the stream) before waiting: micsa_measure_begin queues
+ * the reduction kernel and the device->host copy of the row into pinned memory
+ * owned by the context and returns at once; micsa_measure_end waits for the
+ * stream and copies the sums out (same arrays and rules as micsa_measure_i64;
+ * MICSA_ERR_INVALID without a preceding _begin).  The row is the state at the
+ * point of _begin in stream order. */
+int micsa_measure_begin(micsa_ctx *ctx);
+int micsa_measure_end(micsa_ctx *ctx, int64_t *E, int64_t *E_daemon, int64_t *Q);
 int micsa_measure(micsa_ctx *ctx, double *energy, double *demon_energy,
                   double *q_overlap);
 

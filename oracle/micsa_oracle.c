@@ -160,7 +160,7 @@ void oracle_half_sweep(int L, int n_samples, int n_replicas, int parity,
 {
     const int64_t N = (int64_t)L * L * L;
     const int n_sys = n_samples * n_replicas;
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if (N * n_sys > 65536)
     for (int sys = 0; sys < n_sys; ++sys) {
         const int sample = sys / n_replicas;
         int8_t  *ss = s + (int64_t)sys * N;
@@ -279,7 +279,7 @@ int oracle_refresh(int L, int n_samples, int n_replicas, uint64_t seed,
     if (oracle_thresholds(T, thr) != 0) return -1;
     uint32_t key[2]; seed_key(seed, key);
     const int n_sys = n_samples * n_replicas;
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if (N * n_sys > 65536)
     for (int sys = 0; sys < n_sys; ++sys) {
         const int sample = sys / n_replicas, rep = sys % n_replicas;
         const uint32_t g = (uint32_t)(sample_offset + sample);
@@ -306,7 +306,7 @@ void oracle_measure(int L, int n_samples, int n_replicas,
     const int64_t N = (int64_t)L * L * L;
     const int n_sys = n_samples * n_replicas;
     if (E) {
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if (N * n_sys > 65536)
         for (int sys = 0; sys < n_sys; ++sys) {
             const int sample = sys / n_replicas;
             const int8_t *ss = s + (int64_t)sys * N;

@@ -31,7 +31,7 @@ EXPORTS = (
     "micsa_refresh_demons", "micsa_debug_thresholds", "micsa_measure_i64",
     "micsa_measure", "micsa_anneal", "micsa_counters", "micsa_layout_info",
     "micsa_set_tuning",
-    "micsa_prefetch_refresh",
+    "micsa_prefetch_refresh", "micsa_measure_begin", "micsa_measure_end",
 )
 
 
@@ -93,7 +93,8 @@ def _bind() -> ctypes.CDLL:
             ("micsa_refresh_demons", [vp, f64, u32]),
             ("micsa_prefetch_refresh", [vp, f64, u32]),
             ("micsa_debug_thresholds", [f64, vp]),
-            ("micsa_measure_i64", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
+            ("micsa_measure_i64", [vp, vp, vp, vp]),
+            ("micsa_measure_begin", [vp]), ("micsa_measure_end", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
             ("micsa_anneal", [vp, vp, i32, u32, vp, vp]),
             ("micsa_counters", [vp, vp, vp, vp]), ("micsa_layout_info", [vp, vp]),
             ("micsa_set_tuning", [vp, i32, i32])):
@@ -228,6 +229,16 @@ class MicSA:
         Ed = np.empty(self.n_sys, np.int64)
         Q = np.empty(self.n_pairs, np.int64) if self.n_replicas >= 2 else None
         _check(_lib.micsa_measure_i64(self._h, _ptr(E), _ptr(Ed), _ptr(Q)))
+        return E, Ed, (Q if Q is not None else np.empty(0, np.int64))
+
+    def measure_begin(self):
+        _check(_lib.micsa_measure_begin(self._h))
+
+    def measure_end(self):
+        E = np.empty(self.n_sys, np.int64)
+        Ed = np.empty(self.n_sys, np.int64)
+        Q = np.empty(self.n_pairs, np.int64) if self.n_replicas >= 2 else None
+        _check(_lib.micsa_measure_end(self._h, _ptr(E), _ptr(Ed), _ptr(Q)))
         return E, Ed, (Q if Q is not None else np.empty(0, np.int64))
 
     def measure(self):

@@ -78,40 +78,40 @@ __device__ __forceinline__ void block_lane_counts(const VCount<kThreadPlanes>& a
         atomicAdd(&out[threadIdx.x], (unsigned long long)s_cnt[threadIdx.x]);
 }
 
-// Tree version for the one-pass kernel: the block's vertical counters are
-// added pairwise in shared memory (a vertical add costs two logic ops per
-// plane, and whole warps drop out of the upper levels), then 32 threads pick
-// out their lane.  sm holds (P + log2(B)) * B words; P planes per thread.
+// Version for the one-pass kernel: P planes per thread, B threads.  The warp
+// adds its 32 vertical counters with a shuffle butterfly (level l works on
+// P + l planes only), every lane picks out its own count, the warps meet in
+// shared-memory atomics and 32 threads issue the global ones.
 template <int P, int B>
-__device__ __forceinline__ void block_tree_lane_counts(const uint32_t (&c)[P], uint32_t* sm,
+__device__ __forceinline__ void block_warp_lane_counts(const uint32_t (&acc)[P], unsigned int* s_cnt,
                                                        unsigned long long* out)
 {
-    constexpr int LOG = (B == 512) ? 9 : (B == 256) ? 8 : (B == 128) ? 7 : 6;
-    static_assert((1 << LOG) == B, "block size must be 64..512, a power of two");
-    const int tid = threadIdx.x;
+    uint32_t c[P + 5];
 #pragma unroll
-    for (int k = 0; k < P; ++k) sm[k * B + tid] = c[k];
-    for (int k = P; k < P + LOG; ++k) sm[k * B + tid] = 0u;
-    __syncthreads();
-    int np = P;
-    for (int s = B / 2; s >= 1; s >>= 1) {
-        if (tid < s) {
-            uint32_t carry = 0;
-            for (int k = 0; k < np; ++k) {
-                const uint32_t x = sm[k * B + tid], y = sm[k * B + tid + s];
-                sm[k * B + tid] = x ^ y ^ carry;
-                carry = maj3(x, y, carry);
+    for (int k = 0; k < P + 5; ++k) c[k] = (k < P) ? acc[k] : 0u;
+#pragma unroll
+    for (int l = 0; l < 5; ++l) {
+        uint32_t carry = 0;
+#pragma unroll
+        for (int k = 0; k < P + 5; ++k) {
+            if (k <= P + l) {                       // planes above P + l are still zero
+                const uint32_t x = __shfl_xor_sync(0xFFFFFFFFu, c[k], 1 << l);
+                const uint32_t s = c[k] ^ x ^ carry;
+                carry = maj3(c[k], x, carry);
+                c[k] = s;
             }
-            sm[np * B + tid] = carry;
         }
-        ++np;
-        __syncthreads();
     }
-    if (tid < 32) {
-        unsigned long long mine = 0;
-        for (int k = 0; k < P + LOG; ++k) mine += (unsigned long long)((sm[k * B] >> tid) & 1u) << k;
-        if (mine) atomicAdd(&out[tid], mine);
-    }
+    const int lane = threadIdx.x & 31;
+    unsigned int mine = 0;
+#pragma unroll
+    for (int k = 0; k < P + 5; ++k) mine += ((c[k] >> lane) & 1u) << k;
+    if (threadIdx.x < 32) s_cnt[threadIdx.x] = 0;
+    __syncthreads();
+    if (mine) atomicAdd(&s_cnt[lane], mine);
+    __syncthreads();
+    if (threadIdx.x < 32 && s_cnt[threadIdx.x])
+        atomicAdd(&out[threadIdx.x], (unsigned long long)s_cnt[threadIdx.x]);
     __syncthreads();
 }
 
@@ -191,8 +191,8 @@ __device__ __forceinline__ void finalize_rows(const FinalizeArgs& f)
 }
 
 constexpr int kMeasureBlock = 256;
-constexpr int kMeasureBatch = 16;      // items between flushes of the 8-plane counters
-constexpr int kMeasureMaxItems = 320;  // per thread: 320 * 12 < 2^12
+constexpr int kMeasurePlanes = 10;     // per-thread vertical counters
+constexpr int kMeasureMaxItems = 85;   // per thread: 85 * 12 < 2^10
 
 // One pass over the state for all three observables.
 // An item = V consecutive words of one row of one parity array; it counts the
@@ -201,81 +201,73 @@ constexpr int kMeasureMaxItems = 320;  // per thread: 320 * 12 < 2^12
 // in the word) -- the lanes where the two replicas differ.  Other replica
 // pairs are counted by count_xor_kernel before this kernel runs.  The last
 // block to finish turns the counts into the measurement row.
-// grid = (nblk, n_words), block = kMeasureBlock.
+// grid = (nblk, n_words), block = kMeasureBlock; 32-bit item indices
+// (half / V < 2^31 because L^3 < 2^32).
 template <int V, int RPW, bool PAIR>
-__global__ void __launch_bounds__(kMeasureBlock)
+__global__ void __launch_bounds__(kMeasureBlock, 3)
 measure_kernel(MeasureArgs a, FinalizeArgs f)
 {
     typedef typename BondT<RPW>::type JT;
-    __shared__ uint32_t sm[(12 + 8) * kMeasureBlock];
+    __shared__ unsigned int sm[32];
     __shared__ unsigned int s_last;
     const int w = blockIdx.y;
-    const int L = a.L, Lh = a.Lh, nxv = Lh / V;
+    const uint32_t L = (uint32_t)a.L, Lh = (uint32_t)a.Lh, nxv = Lh / V;
     const long long half = a.half;
-    const long long items_p = half / V, n_items = 2 * items_p;
+    const uint32_t items_p = (uint32_t)(half / V), n_items = 2u * items_p;
     const uint32_t* s0 = a.spin + (long long)w * 2 * half;
     const uint32_t* d0 = a.m0 + (long long)w * 2 * half;
     const uint32_t* d1 = a.m1 + (long long)w * 2 * half;
     const int sg = w / a.n_rg;
     const JT* Jb = reinterpret_cast<const JT*>(a.J) + (long long)sg * 6 * half;
 
-    VCount<12> accU, accM, accX; accU.clear(); accM.clear(); accX.clear();
-    const long long stride = (long long)gridDim.x * kMeasureBlock;
-    for (long long base = (long long)blockIdx.x * kMeasureBlock + threadIdx.x; base < n_items;
-         base += stride * kMeasureBatch) {
-        VCount<8> midU, midM, midX; midU.clear(); midM.clear(); midX.clear();
+    VCount<kMeasurePlanes> accU, accM, accX; accU.clear(); accM.clear(); accX.clear();
+    const uint32_t stride = gridDim.x * kMeasureBlock;
 #pragma unroll 2
-        for (int j = 0; j < kMeasureBatch; ++j) {
-            const long long it = base + j * stride;
-            if (it >= n_items) break;
-            const int p = it >= items_p;
-            const long long iv = it - (p ? items_p : 0);
-            const long long rowi = iv / nxv;
-            const int xv = (int)(iv - rowi * nxv);
-            const int z = (int)(rowi / L), y = (int)(rowi - (long long)z * L);
-            const int yp = (y + 1 == L) ? 0 : y + 1, zp = (z + 1 == L) ? 0 : z + 1;
-            const int xh0 = xv * V;
-            const long long row = rowi * Lh, h = row + xh0;
-            const int c = (y + z + p) & 1;        // c=1: +x neighbour at xh+1, else same xh
-            const uint32_t* sp = s0 + (p ? half : 0);
-            const uint32_t* sq = s0 + (p ? 0 : half);
-            const Vec<V> s = ldg_vec<V>(sp + h);
-            const Vec<V> A = ldg_vec<V>(sq + h);
-            const uint32_t e = sq[row + ((xh0 + V == Lh) ? 0 : xh0 + V)];
-            const Vec<V> ny = ldg_vec<V>(sq + ((long long)z * L + yp) * Lh + xh0);
-            const Vec<V> nz = ldg_vec<V>(sq + ((long long)zp * L + y) * Lh + xh0);
-            const Vec<V> jx = ldg_bonds<V, RPW>(Jb + (0 * 2 + p) * half + h);
-            const Vec<V> jy = ldg_bonds<V, RPW>(Jb + (1 * 2 + p) * half + h);
-            const Vec<V> jz = ldg_bonds<V, RPW>(Jb + (2 * 2 + p) * half + h);
-            const Vec<V> b0 = ldg_vec<V>(d0 + (p ? half : 0) + h);
-            const Vec<V> b1 = ldg_vec<V>(d1 + (p ? half : 0) + h);
-            VCount<4> locU, locM; locU.clear(); locM.clear();
-            VCount<3> locX; locX.clear();
+    for (uint32_t it = blockIdx.x * kMeasureBlock + threadIdx.x; it < n_items; it += stride) {
+        const uint32_t p = it >= items_p;
+        const uint32_t iv = it - (p ? items_p : 0u);
+        const uint32_t rowi = iv / nxv, xv = iv - rowi * nxv;
+        const uint32_t z = rowi / L, y = rowi - z * L;
+        const uint32_t yp = (y + 1 == L) ? 0 : y + 1, zp = (z + 1 == L) ? 0 : z + 1;
+        const uint32_t xh0 = xv * V;
+        const uint32_t row = rowi * Lh, h = row + xh0;       // < half < 2^31
+        const uint32_t c = (y + z + p) & 1u;      // c=1: +x neighbour at xh+1, else same xh
+        const uint32_t* sp = s0 + (p ? half : 0);
+        const uint32_t* sq = s0 + (p ? 0 : half);
+        const Vec<V> s = ldg_vec<V>(sp + h);
+        const Vec<V> A = ldg_vec<V>(sq + h);
+        const uint32_t e = sq[row + ((xh0 + V == Lh) ? 0 : xh0 + V)];
+        const Vec<V> ny = ldg_vec<V>(sq + (z * L + yp) * Lh + xh0);
+        const Vec<V> nz = ldg_vec<V>(sq + (zp * L + y) * Lh + xh0);
+        const Vec<V> jx = ldg_bonds<V, RPW>(Jb + (0 * 2 + p) * half + h);
+        const Vec<V> jy = ldg_bonds<V, RPW>(Jb + (1 * 2 + p) * half + h);
+        const Vec<V> jz = ldg_bonds<V, RPW>(Jb + (2 * 2 + p) * half + h);
+        const Vec<V> b0 = ldg_vec<V>(d0 + (p ? half : 0) + h);
+        const Vec<V> b1 = ldg_vec<V>(d1 + (p ? half : 0) + h);
+        VCount<4> locU, locM; locU.clear(); locM.clear();
+        VCount<3> locX; locX.clear();
 #pragma unroll
-            for (int k = 0; k < V; ++k) {
-                const uint32_t up = (k + 1 < V) ? A.v[k + 1] : e;
-                const uint32_t nx = c ? up : A.v[k];
-                const uint32_t ux = s.v[k] ^ nx ^ jx.v[k];
-                const uint32_t uy = s.v[k] ^ ny.v[k] ^ jy.v[k];
-                const uint32_t uz = s.v[k] ^ nz.v[k] ^ jz.v[k];
-                const uint32_t bu[2] = { ux ^ uy ^ uz, maj3(ux, uy, uz) };
-                locU.add(bu);
-                const uint32_t bm[2] = { b0.v[k], b1.v[k] };
-                locM.add(bm);
-                if (PAIR) {
-                    const uint32_t bx[1] = { (s.v[k] ^ (s.v[k] >> 16)) & 0xFFFFu };
-                    locX.add(bx);
-                }
+        for (int k = 0; k < V; ++k) {
+            const uint32_t up = (k + 1 < V) ? A.v[k + 1] : e;
+            const uint32_t nx = c ? up : A.v[k];
+            const uint32_t ux = s.v[k] ^ nx ^ jx.v[k];
+            const uint32_t uy = s.v[k] ^ ny.v[k] ^ jy.v[k];
+            const uint32_t uz = s.v[k] ^ nz.v[k] ^ jz.v[k];
+            const uint32_t bu[2] = { ux ^ uy ^ uz, maj3(ux, uy, uz) };
+            locU.add(bu);
+            const uint32_t bm[2] = { b0.v[k], b1.v[k] };
+            locM.add(bm);
+            if (PAIR) {
+                const uint32_t bx[1] = { (s.v[k] ^ (s.v[k] >> 16)) & 0xFFFFu };
+                locX.add(bx);
             }
-            midU.add(locU.c); midM.add(locM.c);
-            if (PAIR) midX.add(locX.c);
         }
-        accU.add(midU.c); accM.add(midM.c);
-        if (PAIR) accX.add(midX.c);
+        accU.add(locU.c); accM.add(locM.c);
+        if (PAIR) accX.add(locX.c);
     }
-    block_tree_lane_counts<12, kMeasureBlock>(accU.c, sm, a.cntU + (long long)w * 32);
-    block_tree_lane_counts<12, kMeasureBlock>(accM.c, sm, a.cntM + (long long)w * 32);
-    if (PAIR) block_tree_lane_counts<12, kMeasureBlock>(accX.c, sm, a.cntX + (long long)sg * 32);
+    block_warp_lane_counts<kMeasurePlanes, kMeasureBlock>(accU.c, sm, a.cntU + (long long)w * 32);
+    block_warp_lane_counts<kMeasurePlanes, kMeasureBlock>(accM.c, sm, a.cntM + (long long)w * 32);
+    if (PAIR) block_warp_lane_counts<kMeasurePlanes, kMeasureBlock>(accX.c, sm, a.cntX + (long long)sg * 32);
 
     // the last block to arrive finalises (its reads see every block's atomics)
     __threadfence();

@@ -110,6 +110,7 @@ struct micsa_ctx {
     cudaStream_t side;                        // generates prefetched refreshes under the sweeps
     cudaEvent_t ev_main, ev_side;
     bool pending; double pending_T; uint32_t pending_step;
+    bool measure_queued;                      // micsa_measure_begin without its _end yet
     long long* host_row;        // pinned host staging for one measurement row
     unsigned long long* calls;  // Philox calls made by the refresh kernels (device counter)
     int V;
@@ -315,11 +316,11 @@ void launch_measure_t(micsa_ctx* c, const MeasureArgs& a, const FinalizeArgs& f)
                                    kCountBlock, 0, c->stream>>>(a);
         c->launches += 1;
     }
-    // two resident blocks per SM over all word lattices, never more than
-    // kMeasureMaxItems items per thread (12-plane per-thread counters)
+    // three resident blocks per SM over all word lattices, never more than
+    // kMeasureMaxItems items per thread (10-plane per-thread counters)
     const long long n_items = 2 * g.half / V;
-    long long nb = (n_items + (long long)kMeasureBlock * kMeasureBatch - 1) / ((long long)kMeasureBlock * kMeasureBatch);
-    nb = std::min(nb, std::max<long long>(1, (148 * 2) / g.n_words));
+    long long nb = (n_items + (long long)kMeasureBlock * 4 - 1) / ((long long)kMeasureBlock * 4);
+    nb = std::min(nb, std::max<long long>(1, (148 * 3) / g.n_words));
     const long long need = (n_items + (long long)kMeasureBlock * kMeasureMaxItems - 1) / ((long long)kMeasureBlock * kMeasureMaxItems);
     nb = std::max<long long>(std::max<long long>(nb, need), 1);
     const dim3 grid((unsigned)nb, (unsigned)g.n_words);
@@ -469,6 +470,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->m0s = (uint32_t*)(c->ws + c->plan.m0s);
     c->m1s = (uint32_t*)(c->ws + c->plan.m1s);
     c->pending = false; c->pending_T = 0.0; c->pending_step = 0;
+    c->measure_queued = false;
     c->cnt = (unsigned long long*)(c->ws + c->plan.cnt);
     c->ticket = (unsigned int*)(c->ws + c->plan.ticket);
     c->row = (long long*)(c->ws + c->plan.row);
@@ -602,17 +604,32 @@ int micsa_prefetch_refresh(micsa_ctx* c, double T, uint32_t step) {
     return launch_prefetch(c, T, step);
 }
 
-int micsa_measure_i64(micsa_ctx* c, int64_t* E, int64_t* Ed, int64_t* Q) {
+int micsa_measure_begin(micsa_ctx* c) {
+    int rc = check_ctx(c); if (rc) return rc;
+    rc = launch_measure(c, c->row, false); if (rc) return rc;
+    CK(c, cudaMemcpyAsync(c->host_row, c->row, c->plan.row_len * 8, cudaMemcpyDeviceToHost, c->stream));
+    c->measure_queued = true;
+    return MICSA_OK;
+}
+
+int micsa_measure_end(micsa_ctx* c, int64_t* E, int64_t* Ed, int64_t* Q) {
     int rc = check_ctx(c); if (rc) return rc;
     const Geom& g = c->g;
     if (Q && g.n_replicas < 2) { set_err("q_overlap needs n_replicas >= 2"); return MICSA_ERR_INVALID; }
-    rc = launch_measure(c, c->row, false); if (rc) return rc;
-    CK(c, cudaMemcpyAsync(c->host_row, c->row, c->plan.row_len * 8, cudaMemcpyDeviceToHost, c->stream));
+    if (!c->measure_queued) { set_err("micsa_measure_end without micsa_measure_begin"); return MICSA_ERR_INVALID; }
     CK(c, cudaStreamSynchronize(c->stream));
+    c->measure_queued = false;
     if (E)  memcpy(E, c->host_row, (size_t)g.n_sys * 8);
     if (Ed) memcpy(Ed, c->host_row + g.n_sys, (size_t)g.n_sys * 8);
     if (Q)  memcpy(Q, c->host_row + 2 * g.n_sys, (size_t)g.n_pairs * 8);
     return MICSA_OK;
+}
+
+int micsa_measure_i64(micsa_ctx* c, int64_t* E, int64_t* Ed, int64_t* Q) {
+    int rc = check_ctx(c); if (rc) return rc;
+    if (Q && c->g.n_replicas < 2) { set_err("q_overlap needs n_replicas >= 2"); return MICSA_ERR_INVALID; }
+    rc = micsa_measure_begin(c); if (rc) return rc;
+    return micsa_measure_end(c, E, Ed, Q);
 }
 
 int micsa_measure(micsa_ctx* c, double* e, double* ed, double* q) {

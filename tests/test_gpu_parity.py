@@ -357,3 +357,26 @@ def test_prefetched_refresh_is_bit_identical(micsa, oracle):
         c = g.counters()
         assert c["rns_drawn"] == 9 * L ** 3 * ns * nr
         assert 0 < c["philox_calls"] <= 10 * L ** 3 * ns * nr // 4 + 10 * L ** 3 * 4
+
+
+def test_measure_begin_end(micsa, oracle):
+    """The split measurement returns the state at the point of _begin."""
+    L, ns, nr = 8, 5, 2
+    N = L ** 3
+    s, J, m = random_pm1((ns, nr, N), 31), random_pm1((ns, 3, N), 32), random_levels((ns, nr, N), 33)
+    with micsa.MicSA(L, ns, nr, 1) as g:
+        g.set_spins(s); g.set_daemons(m); g.set_couplings(J)
+        with pytest.raises(micsa.MicsaError):
+            g.measure_end()
+        g.measure_begin()
+        g.sweep(2)                               # queued behind the measurement
+        E, Ed, Q = g.measure_end()
+        oE, oEd, oQ = oracle.measure(L, s, m, J)
+        np.testing.assert_array_equal(E, oE)
+        np.testing.assert_array_equal(Ed, oEd)
+        np.testing.assert_array_equal(Q, oQ)
+        oracle.sweep(L, s, m, J, 2)
+        E, Ed, Q = g.measure_i64()
+        oE, oEd, oQ = oracle.measure(L, s, m, J)
+        np.testing.assert_array_equal(E, oE)
+        np.testing.assert_array_equal(Ed, oEd)
