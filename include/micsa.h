@@ -209,13 +209,18 @@ int micsa_counters(micsa_ctx *ctx, uint64_t *attempts, uint64_t *rns_drawn,
 int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
 
 /* Tuning / A-B switch, never needed for correctness (every setting gives the
- * same bits; tests/test_gpu_parity.py runs the parity cases under each).
+ * same bits; tests/test_gpu_parity.py runs parity cases under each).  They
+ * only matter when L % 8 == 0; other L always use the generic kernel.
  * key MICSA_TUNE_SWEEP_KERNEL: 0 = tiled half-sweep, opposite-parity spins
- *   staged in shared memory by TMA, 1 =
- *   row-marching register kernel (default: it measured faster on B200).  key MICSA_TUNE_TILE_TZ: lattice planes per
- *   tile of the tiled kernel, 2, 4 (default) or 8.  L % 8 != 0 always uses the
- *   generic kernel.  Unknown key or value: MICSA_ERR_INVALID, nothing changes. */
-enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_TILE_TZ = 1 };
+ *   staged in shared memory by TMA; 1 = row-marching register kernel; 2 =
+ *   software-pipelined row-marching kernel (default); 3 = persistent
+ *   kernel: all the half-sweeps of one micsa_sweep / anneal group in ONE launch,
+ *   slab-wise dependences through device-side flags instead of kernel
+ *   boundaries.
+ * key MICSA_TUNE_TILE_TZ: lattice planes per tile of kernel 0: 2, 4 (default), 8.
+ * key MICSA_TUNE_PIPE_ROWS: rows per thread of kernel 2: 4 (default) or 8.
+ * Unknown key or value: MICSA_ERR_INVALID, nothing changes. */
+enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_TILE_TZ = 1, MICSA_TUNE_PIPE_ROWS = 2 };
 int micsa_set_tuning(micsa_ctx *ctx, int key, int value);
 
 #ifdef __cplusplus

@@ -285,8 +285,9 @@ class MicSA:
         return {"attempts": a.value, "rns_drawn": r.value, "philox_calls": p.value}
 
     def set_tuning(self, key, value):
-        """micsa_set_tuning: 'sweep_kernel' (0 tiled, 1 row-marching) or 'tile_tz' (2, 4, 8)."""
-        k = {"sweep_kernel": 0, "tile_tz": 1}[key]
+        """micsa_set_tuning: 'sweep_kernel' (0 tiled, 1 row-marching, 2 pipelined
+        row-marching, 3 persistent), 'tile_tz' (2, 4, 8) or 'pipe_rows' (4, 8)."""
+        k = {"sweep_kernel": 0, "tile_tz": 1, "pipe_rows": 2}[key]
         _check(_lib.micsa_set_tuning(self._h, k, int(value)))
 
     def layout_info(self):

@@ -17,6 +17,7 @@
 #include "philox.cuh"
 #include "refresh.cuh"
 #include "sweep.cuh"
+#include "sweep_persistent.cuh"
 #include "sweep_tile.cuh"
 
 using namespace micsa;
@@ -33,7 +34,7 @@ constexpr size_t kAlign = 256;
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {                 // byte offsets inside the workspace
-    size_t spin, m0, m1, m0s, m1s, J, cnt, ticket, row, minE, bad, calls, total;
+    size_t spin, m0, m1, m0s, m1s, J, cnt, ticket, row, minE, bad, calls, progress, task_ticket, total;
     size_t plane_bytes, J_bytes, cnt_words, row_len;
 };
 
@@ -84,6 +85,8 @@ Plan make_plan(const Geom& g) {
     p.minE = o; o += align_up((size_t)g.n_sys * 8);
     p.bad = o;  o += align_up(sizeof(int));
     p.calls = o; o += align_up(sizeof(unsigned long long));
+    p.progress = o; o += align_up((size_t)g.n_words * g.L * sizeof(int));
+    p.task_ticket = o; o += align_up(sizeof(unsigned long long));
     p.total = o;
     return p;
 }
@@ -114,7 +117,13 @@ struct micsa_ctx {
     long long* host_row;        // pinned host staging for one measurement row
     unsigned long long* calls;  // Philox calls made by the refresh kernels (device counter)
     int V;
-    int sweep_kernel;          // 0 = tiled (TMA-staged) when L % 8 == 0, 1 = row-marching
+    int sweep_kernel;          // L % 8 == 0: 0 = tiled (TMA-staged), 1 = row-marching, 2 = pipelined row-marching
+    int* progress;             // persistent sweep: half-sweeps done per (word lattice, slab)
+    unsigned long long* task_ticket;
+    unsigned long long ticket0;   // value of *task_ticket when the next launch starts
+    int progress_base;         // value of every progress entry between launches
+    int persist_grid;          // CTAs of the persistent kernel (0 = not computed yet)
+    int pipe_rows;             // rows per thread of the pipelined kernel (4 or 8)
     int tile_tz;               // planes per tile of the tiled kernel (2, 4 or 8)
     uint64_t attempts, rns, launches;
     int sticky;
@@ -177,6 +186,18 @@ void launch_half_sweep_rows(micsa_ctx* c, int parity) {
     half_sweep_rows_kernel<RPW, kRowsPerThread><<<grid, 128, 0, c->stream>>>(a, parity);
 }
 
+template <int RPW>
+void launch_half_sweep_pipe(micsa_ctx* c, int parity) {
+    SweepArgs a;
+    a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half;
+    const int yc = c->pipe_rows;
+    const int per_plane = (c->g.L / yc) * (c->g.Lh / 4);
+    dim3 grid((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
+    if (yc == 8) half_sweep_pipe_kernel<RPW, 8><<<grid, 128, 0, c->stream>>>(a, parity);
+    else         half_sweep_pipe_kernel<RPW, 4><<<grid, 128, 0, c->stream>>>(a, parity);
+}
+
 template <int RPW, int TY, int TZ>
 int launch_half_sweep_tile(micsa_ctx* c, int parity) {
     SweepArgs a;
@@ -204,7 +225,70 @@ int launch_half_sweep_tile_tz(micsa_ctx* c, int parity) {
     }
 }
 
+// n_hs half-sweeps, parities p_first, p_first^1, ... in one persistent launch
+template <int RPW>
+int launch_persistent(micsa_ctx* c, int n_hs, int p_first) {
+    const Geom& g = c->g;
+    constexpr int YC = 4;
+    const int items_per_plane = (g.L / YC) * (g.Lh / 4);
+    // task size: about 200 thread items, and (where the lattice allows) more
+    // than ~2.2 tasks per resident CTA in every half-sweep (sweep_persistent.cuh)
+    int ZT = 1, n_sub = 1;
+    if (items_per_plane > 256) {
+        n_sub = (items_per_plane + 199) / 200;
+    } else {
+        for (int d = 2; d <= g.L; ++d) {
+            if (g.L % d) continue;
+            if (d * items_per_plane > 256 || (long long)g.n_words * (g.L / d) < 650) break;
+            ZT = d;
+        }
+    }
+    const int items = ZT * items_per_plane;
+    const int sub_items = (items + n_sub - 1) / n_sub;
+    const int block = std::min(kPersistBlock, (sub_items + 31) / 32 * 32);
+    const long long tasks_per_hs = (long long)g.n_words * (g.L / ZT) * n_sub;
+    if (c->persist_grid == 0) {
+        int per_sm = 0, dev = 0, sms = 0;
+        CK(c, cudaGetDevice(&dev));
+        CK(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sweep_persistent_kernel<RPW, YC>, block, 0));
+        long long grid = (long long)std::max(1, per_sm) * sms;
+        // small lattices: fewer CTAs than half the tasks of a half-sweep, so that nobody spins
+        grid = std::min(grid, std::max<long long>(1, tasks_per_hs / 2));
+        c->persist_grid = (int)grid;
+    }
+    while (n_hs > 0) {
+        if ((long long)(c->progress_base + std::min(n_hs, 1 << 20)) * n_sub > (1ll << 30)) {   // keep the counters far from overflow
+            CK(c, cudaMemsetAsync(c->progress, 0, (size_t)g.n_words * g.L * sizeof(int), c->stream));
+            c->progress_base = 0;
+        }
+        const int n = std::min(n_hs, 1 << 20);
+        PersistArgs A;
+        A.a.spin = c->st.spin; A.a.m0 = c->st.m0; A.a.m1 = c->st.m1; A.a.J = c->st.J;
+        A.a.L = g.L; A.a.Lh = g.Lh; A.a.n_rg = g.n_rg; A.a.half = g.half;
+        A.n_hs = n; A.p_first = p_first; A.ZT = ZT; A.n_slabs = g.L / ZT; A.n_words = g.n_words;
+        A.n_sub = n_sub; A.sub_items = sub_items;
+        A.base = c->progress_base; A.progress = c->progress;
+        A.ticket = c->task_ticket; A.ticket0 = c->ticket0;
+        const unsigned long long total = (unsigned long long)tasks_per_hs * n;
+        const int grid = (int)std::min<unsigned long long>((unsigned long long)c->persist_grid, total);
+        sweep_persistent_kernel<RPW, YC><<<grid, block, 0, c->stream>>>(A);
+        // every CTA draws one ticket past the end before it leaves
+        c->ticket0 += total + (unsigned long long)grid;
+        c->progress_base += n;
+        c->attempts += (uint64_t)n * (uint64_t)(g.N / 2) * (uint64_t)g.n_sys;
+        const int rc = post_launch(c); if (rc) return rc;
+        p_first ^= (n & 1);
+        n_hs -= n;
+    }
+    return MICSA_OK;
+}
+
+bool use_persistent(const micsa_ctx* c) { return c->V == 4 && c->sweep_kernel == 3; }
+
 int launch_half_sweep(micsa_ctx* c, int parity) {
+    if (use_persistent(c))
+        return (c->g.rpw == 2) ? launch_persistent<2>(c, 1, parity) : launch_persistent<1>(c, 1, parity);
     if (c->V == 4 && c->sweep_kernel == 0) {
         const int rc = (c->g.rpw == 2) ? launch_half_sweep_tile_tz<2>(c, parity)
                                        : launch_half_sweep_tile_tz<1>(c, parity);
@@ -214,8 +298,12 @@ int launch_half_sweep(micsa_ctx* c, int parity) {
     }
     const int key = c->V * 10 + c->g.rpw;
     switch (key) {
-        case 41: launch_half_sweep_rows<1>(c, parity); break;     // L % 8 == 0
-        case 42: launch_half_sweep_rows<2>(c, parity); break;
+        case 41: if (c->sweep_kernel == 2) launch_half_sweep_pipe<1>(c, parity);      // L % 8 == 0
+                 else launch_half_sweep_rows<1>(c, parity);
+                 break;
+        case 42: if (c->sweep_kernel == 2) launch_half_sweep_pipe<2>(c, parity);
+                 else launch_half_sweep_rows<2>(c, parity);
+                 break;
         case 21: launch_half_sweep_t<2, 1>(c, parity); break;
         case 22: launch_half_sweep_t<2, 2>(c, parity); break;
         case 11: launch_half_sweep_t<1, 1>(c, parity); break;
@@ -223,6 +311,18 @@ int launch_half_sweep(micsa_ctx* c, int parity) {
     }
     c->attempts += (uint64_t)(c->g.N / 2) * (uint64_t)c->g.n_sys;
     return post_launch(c);
+}
+
+// n full sweeps (even, odd, even, ...): one persistent launch or 2n launches
+int launch_sweeps(micsa_ctx* c, int n) {
+    if (n <= 0) return MICSA_OK;
+    if (use_persistent(c))
+        return (c->g.rpw == 2) ? launch_persistent<2>(c, 2 * n, 0) : launch_persistent<1>(c, 2 * n, 0);
+    for (int t = 0; t < n; ++t) {
+        int rc = launch_half_sweep(c, 0); if (rc) return rc;
+        rc = launch_half_sweep(c, 1); if (rc) return rc;
+    }
+    return MICSA_OK;
 }
 
 int thresholds_host(double T, uint64_t thr[3]) {
@@ -397,6 +497,8 @@ int init_state(micsa_ctx* c) {
     const Geom& g = c->g;
     const SiteGrid sg = site_grid(g);
     CK(c, cudaMemsetAsync(c->calls, 0, sizeof(unsigned long long), c->stream));
+    CK(c, cudaMemsetAsync(c->progress, 0, (size_t)c->g.n_words * c->g.L * sizeof(int), c->stream));
+    CK(c, cudaMemsetAsync(c->task_ticket, 0, sizeof(unsigned long long), c->stream));
     CK(c, cudaMemsetAsync(c->cnt, 0, c->plan.cnt_words * 8, c->stream));
     CK(c, cudaMemsetAsync(c->ticket, 0, sizeof(unsigned int), c->stream));
     CK(c, cudaMemsetAsync(c->st.m0, 0, c->plan.plane_bytes, c->stream));
@@ -447,8 +549,9 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->ks = philox_make_keys(seed);
     c->stream = (cudaStream_t)cuda_stream;
     c->V = vec_width(g.Lh);
-    c->sweep_kernel = 1;
+    c->sweep_kernel = 2;
     c->tile_tz = 4;
+    c->pipe_rows = 4;
     c->attempts = c->rns = c->launches = 0;
     c->sticky = 0;
     if (dev_workspace) {
@@ -477,6 +580,9 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->minE = (long long*)(c->ws + c->plan.minE);
     c->bad = (int*)(c->ws + c->plan.bad);
     c->calls = (unsigned long long*)(c->ws + c->plan.calls);
+    c->progress = (int*)(c->ws + c->plan.progress);
+    c->task_ticket = (unsigned long long*)(c->ws + c->plan.task_ticket);
+    c->ticket0 = 0; c->progress_base = 0; c->persist_grid = 0;
     c->host_row = nullptr; c->side = nullptr; c->ev_main = nullptr; c->ev_side = nullptr;
     if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_main, cudaEventDisableTiming) != cudaSuccess ||
@@ -581,11 +687,7 @@ int micsa_half_sweep(micsa_ctx* c, int parity) {
 int micsa_sweep(micsa_ctx* c, int n) {
     int rc = check_ctx(c); if (rc) return rc;
     if (n < 0) { set_err("n must be >= 0"); return MICSA_ERR_INVALID; }
-    for (int t = 0; t < n; ++t) {
-        rc = launch_half_sweep(c, 0); if (rc) return rc;
-        rc = launch_half_sweep(c, 1); if (rc) return rc;
-    }
-    return MICSA_OK;
+    return launch_sweeps(c, n);
 }
 
 int micsa_debug_thresholds(double T, uint64_t thr[3]) {
@@ -679,11 +781,13 @@ int micsa_anneal(micsa_ctx* c, const micsa_step* sched, int n_steps, uint32_t st
         if (k + 1 < n_steps && sched[k].n_sweeps > 0) {       // generated under this step's sweeps
             rc = launch_prefetch(c, sched[k + 1].T, step0 + (uint32_t)k + 1u); if (rc) return rc;
         }
-        for (int j = 1; j <= sched[k].n_sweeps; ++j) {
-            rc = launch_half_sweep(c, 0); if (rc) return rc;
-            rc = launch_half_sweep(c, 1); if (rc) return rc;
-            ++t;
-            if (sched[k].measure_every > 0 && j % sched[k].measure_every == 0) {
+        // sweeps in groups that end at a measurement (or at the end of the step)
+        const int me = sched[k].measure_every;
+        for (int j = 0; j < sched[k].n_sweeps; ) {
+            const int group = (me > 0) ? std::min(me - j % me, sched[k].n_sweeps - j) : sched[k].n_sweeps - j;
+            rc = launch_sweeps(c, group); if (rc) return rc;
+            j += group; t += group;
+            if (me > 0 && j % me == 0) {
                 long long* dst = (r < keep) ? (long long*)dev_rows.dev + (size_t)r * row_len : c->row;
                 rc = launch_measure(c, dst, true); if (rc) return rc;
                 if (r < keep) { row_sweep.push_back(t); row_T.push_back(sched[k].T); }
@@ -734,11 +838,14 @@ int micsa_set_tuning(micsa_ctx* c, int key, int value) {
     int rc = check_ctx(c); if (rc) return rc;
     switch (key) {
         case MICSA_TUNE_SWEEP_KERNEL:
-            if (value != 0 && value != 1) { set_err("sweep kernel must be 0 or 1"); return MICSA_ERR_INVALID; }
+            if (value < 0 || value > 3) { set_err("sweep kernel must be 0..3"); return MICSA_ERR_INVALID; }
             c->sweep_kernel = value; return MICSA_OK;
         case MICSA_TUNE_TILE_TZ:
             if (value != 2 && value != 4 && value != 8) { set_err("tile_tz must be 2, 4 or 8"); return MICSA_ERR_INVALID; }
             c->tile_tz = value; return MICSA_OK;
+        case MICSA_TUNE_PIPE_ROWS:
+            if (value != 4 && value != 8) { set_err("pipe_rows must be 4 or 8"); return MICSA_ERR_INVALID; }
+            c->pipe_rows = value; return MICSA_OK;
         default:
             set_err("unknown tuning key"); return MICSA_ERR_INVALID;
     }

@@ -271,4 +271,184 @@ half_sweep_rows_kernel(SweepArgs a, int p)
     else             march_rows<RPW, YC, 0>(P, L, Lh, chunk * YC, xv * 4);
 }
 
+
+// ---------------------------------------------------------------------------
+// Pipelined row-marching half-sweep (L % 8 == 0): the same thread -> data map
+// as half_sweep_rows_kernel, with
+//  * the loads of row iy+1 issued BEFORE the update of row iy (explicit
+//    software pipeline; stores and loads go through different pointers, which
+//    the compiler cannot prove apart, so it never hoists them by itself).  All
+//    warps of the single resident wave start together; without the pipeline
+//    they alternate between "everybody waits for loads" and "everybody
+//    computes" and neither the memory system nor the integer pipe is kept busy;
+//  * a shorter Boolean update (creutz_word20): the daemon's low bit and the
+//    constant +1 join the population count as the 7th and 8th input, so that
+//    V = m + U + 1 has "accept" in bit 2 alone and the new level in bits 1:0.
+// ---------------------------------------------------------------------------
+
+// V = m + U + 1 in [1, 10]; accept iff 3 <= m + U <= 6 iff 4 <= V <= 7 iff bit 2
+// of V is set and bit 3 is not -- and bit 3 set implies bit 2 clear here, so
+// accept = V2; new level m + U - 3 = V - 4 = bits 1:0 of V.
+__device__ __forceinline__ void creutz_word20(uint32_t u1, uint32_t u2, uint32_t u3,
+                                              uint32_t u4, uint32_t u5, uint32_t u6,
+                                              uint32_t& sigma, uint32_t& m0, uint32_t& m1) {
+    const uint32_t sa = u1 ^ u2 ^ u3, ca = (u1 & u2) | (u3 & (u1 ^ u2));
+    const uint32_t sb = u4 ^ u5 ^ u6, cb = (u4 & u5) | (u6 & (u4 ^ u5));
+    const uint32_t t0 = sa ^ sb ^ m0, cd = (sa & sb) | (m0 & (sa ^ sb));    // weight 1 without the +1
+    // + 1: V0 = ~t0 and a carry t0 into weight 2
+    const uint32_t s1 = ca ^ cb ^ cd, c1a = (ca & cb) | (cd & (ca ^ cb));
+    const uint32_t V1 = s1 ^ t0 ^ m1, c1b = (s1 & t0) | (m1 & (s1 ^ t0));
+    const uint32_t acc = c1a ^ c1b;                                         // V2 (V3 = c1a & c1b excludes it)
+    sigma ^= acc;
+    m0 = (acc & ~t0) | (~acc & m0);
+    m1 = (acc & V1) | (~acc & m1);
+}
+
+template <int RPW>
+struct RowRegs {                 // everything one row step reads
+    typedef Bond4<RPW> B4;
+    uint4 An, s, d0, d1, zp, zm;
+    typename B4::raw jx, jy, jz, jyq, jzq, jxq;
+    uint32_t e;
+    typename B4::elem eJ;
+};
+
+template <int RPW, int C>
+__device__ __forceinline__ void load_row(RowRegs<RPW>& r, const RowPtrs& P, uint32_t o, uint32_t o_prev,
+                                         uint32_t o_next, uint32_t x4, uint32_t xe_up, uint32_t xe_dn)
+{
+    typedef Bond4<RPW> B4;
+    constexpr uint32_t JS = sizeof(typename B4::elem);
+    const uint32_t rowstart = o - x4;
+    const uint32_t oj = o / 4u * JS, ojm = o_prev / 4u * JS;
+    r.An = ld_off<uint4>(P.sq, o_next);
+    r.s  = ld_off<uint4>(P.sp, o);
+    r.d0 = ld_off<uint4>(P.m0, o);
+    r.d1 = ld_off<uint4>(P.m1, o);
+    r.zp = ld_off<uint4>(P.sq_zp, o);
+    r.zm = ld_off<uint4>(P.sq_zm, o);
+    r.jx = ld_off<typename B4::raw>(P.jx, oj);
+    r.jy = ld_off<typename B4::raw>(P.jy, oj);
+    r.jz = ld_off<typename B4::raw>(P.jz, oj);
+    r.jyq = ld_off<typename B4::raw>(P.jyq, ojm);
+    r.jzq = ld_off<typename B4::raw>(P.jzq_zm, oj);
+    r.jxq = ld_off<typename B4::raw>(P.jxq, oj);
+    if (C) {
+        r.e = ld_off<uint32_t>(P.sq, rowstart + xe_up);
+        r.eJ = 0;
+    } else {
+        r.e = ld_off<uint32_t>(P.sq, rowstart + xe_dn);
+        r.eJ = ld_off<typename B4::elem>(P.jxq, (rowstart + xe_dn) / 4u * JS);
+    }
+}
+
+template <int RPW, int C>
+__device__ __forceinline__ void update_row(const RowRegs<RPW>& r, const uint4& Aprev, const uint4& Acur,
+                                           const RowPtrs& P, uint32_t o)
+{
+    typedef Bond4<RPW> B4;
+    uint32_t jxo[4], jyo[4], jzo[4], jxm[4], jym[4], jzm[4], Bx[4];
+    B4::expand(r.jx, jxo); B4::expand(r.jy, jyo); B4::expand(r.jz, jzo);
+    B4::expand(r.jyq, jym); B4::expand(r.jzq, jzm); B4::expand(r.jxq, Bx);
+    const uint32_t a[4] = { Acur.x, Acur.y, Acur.z, Acur.w };
+    uint32_t nxp[4], nxm[4];
+    if (C) {        // x = 2xh+1: -x neighbour at xh (bond owned by it), +x neighbour at xh+1
+        nxp[0] = a[1]; nxp[1] = a[2]; nxp[2] = a[3]; nxp[3] = r.e;
+        nxm[0] = a[0]; nxm[1] = a[1]; nxm[2] = a[2]; nxm[3] = a[3];
+        jxm[0] = Bx[0]; jxm[1] = Bx[1]; jxm[2] = Bx[2]; jxm[3] = Bx[3];
+    } else {        // x = 2xh: +x neighbour at xh, -x neighbour at xh-1 (bond owned by it)
+        nxp[0] = a[0]; nxp[1] = a[1]; nxp[2] = a[2]; nxp[3] = a[3];
+        nxm[0] = r.e; nxm[1] = a[0]; nxm[2] = a[1]; nxm[3] = a[2];
+        jxm[0] = B4::expand1(r.eJ); jxm[1] = Bx[0]; jxm[2] = Bx[1]; jxm[3] = Bx[2];
+    }
+    uint32_t sv[4] = { r.s.x, r.s.y, r.s.z, r.s.w };
+    uint32_t v0[4] = { r.d0.x, r.d0.y, r.d0.z, r.d0.w };
+    uint32_t v1[4] = { r.d1.x, r.d1.y, r.d1.z, r.d1.w };
+    const uint32_t yp[4] = { r.An.x, r.An.y, r.An.z, r.An.w };
+    const uint32_t ym[4] = { Aprev.x, Aprev.y, Aprev.z, Aprev.w };
+    const uint32_t zp[4] = { r.zp.x, r.zp.y, r.zp.z, r.zp.w };
+    const uint32_t zm[4] = { r.zm.x, r.zm.y, r.zm.z, r.zm.w };
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const uint32_t g = sv[k];
+        creutz_word20(g ^ nxp[k] ^ jxo[k], g ^ nxm[k] ^ jxm[k],
+                      g ^ yp[k] ^ jyo[k],  g ^ ym[k] ^ jym[k],
+                      g ^ zp[k] ^ jzo[k],  g ^ zm[k] ^ jzm[k],
+                      sv[k], v0[k], v1[k]);
+    }
+    st_off<uint4>(P.sp, o, make_uint4(sv[0], sv[1], sv[2], sv[3]));
+    st_off<uint4>(P.m0, o, make_uint4(v0[0], v0[1], v0[2], v0[3]));
+    st_off<uint4>(P.m1, o, make_uint4(v1[0], v1[1], v1[2], v1[3]));
+}
+
+template <int RPW, int YC, int F>
+__device__ __forceinline__ void march_rows_pipe(const RowPtrs& P, int L, int Lh, int y0, int xh0)
+{
+    const uint32_t rowB = (uint32_t)Lh * 4u;
+    const uint32_t x4 = (uint32_t)xh0 * 4u;
+    const int ym0 = (y0 == 0) ? L - 1 : y0 - 1;
+    const uint32_t xe_up = ((xh0 + 4 == Lh) ? 0u : (uint32_t)(xh0 + 4)) * 4u;
+    const uint32_t xe_dn = ((xh0 == 0) ? (uint32_t)(Lh - 1) : (uint32_t)(xh0 - 1)) * 4u;
+    uint32_t o = (uint32_t)y0 * rowB + x4;
+    uint32_t o_prev = (uint32_t)ym0 * rowB + x4;
+
+    uint4 Aprev = ld_off<uint4>(P.sq, o_prev);
+    uint4 Acur  = ld_off<uint4>(P.sq, o);
+    RowRegs<RPW> cur, nxt;
+    {
+        const uint32_t o_next = (y0 + 1 == L) ? x4 : o + rowB;
+        load_row<RPW, F>(cur, P, o, o_prev, o_next, x4, xe_up, xe_dn);
+    }
+#pragma unroll
+    for (int iy = 0; iy < YC; ++iy) {
+        const int y = y0 + iy;
+        const uint32_t o_next = (y + 1 == L) ? x4 : o + rowB;
+        if (iy + 1 < YC) {                          // y + 1 < L inside a chunk
+            const uint32_t o_next2 = (y + 2 == L) ? x4 : o_next + rowB;
+            if ((iy & 1) ^ F) load_row<RPW, 0>(nxt, P, o_next, o, o_next2, x4, xe_up, xe_dn);
+            else              load_row<RPW, 1>(nxt, P, o_next, o, o_next2, x4, xe_up, xe_dn);
+        }
+        if ((iy & 1) ^ F) update_row<RPW, 1>(cur, Aprev, Acur, P, o);
+        else              update_row<RPW, 0>(cur, Aprev, Acur, P, o);
+        Aprev = Acur; Acur = cur.An;
+        if (iy + 1 < YC) cur = nxt;
+        o_prev = o; o = o_next;
+    }
+}
+
+// grid = (ceil((L/YC)*(Lh/4) / block), L, n_words)
+template <int RPW, int YC>
+__global__ void __launch_bounds__(128)
+half_sweep_pipe_kernel(SweepArgs a, int p)
+{
+    typedef typename Bond4<RPW>::elem JT;
+    const int L = a.L, Lh = a.Lh;
+    const int nxv = Lh >> 2;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (L / YC) * nxv) return;
+    const int chunk = t / nxv, xv = t - chunk * nxv;
+    const int z = blockIdx.y, w = blockIdx.z, q = 1 - p;
+    const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+    const long long half = a.half;
+    const long long plane = (long long)L * Lh;
+    const int sg = w / a.n_rg;
+    const JT* Jb = reinterpret_cast<const JT*>(a.J) + (long long)sg * 6 * half;
+
+    RowPtrs P;
+    P.sp = a.spin + ((long long)w * 2 + p) * half + z * plane;
+    P.m0 = a.m0 + ((long long)w * 2 + p) * half + z * plane;
+    P.m1 = a.m1 + ((long long)w * 2 + p) * half + z * plane;
+    const uint32_t* sqb = a.spin + ((long long)w * 2 + q) * half;
+    P.sq = sqb + z * plane; P.sq_zp = sqb + zp * plane; P.sq_zm = sqb + zm * plane;
+    P.jx = Jb + (0 * 2 + p) * half + z * plane;
+    P.jy = Jb + (1 * 2 + p) * half + z * plane;
+    P.jz = Jb + (2 * 2 + p) * half + z * plane;
+    P.jxq = Jb + (0 * 2 + q) * half + z * plane;
+    P.jyq = Jb + (1 * 2 + q) * half + z * plane;
+    P.jzq_zm = Jb + (2 * 2 + q) * half + zm * plane;
+
+    if ((z + p) & 1) march_rows_pipe<RPW, YC, 1>(P, L, Lh, chunk * YC, xv * 4);
+    else             march_rows_pipe<RPW, YC, 0>(P, L, Lh, chunk * YC, xv * 4);
+}
+
 }  // namespace micsa

@@ -380,3 +380,38 @@ def test_measure_begin_end(micsa, oracle):
         oE, oEd, oQ = oracle.measure(L, s, m, J)
         np.testing.assert_array_equal(E, oE)
         np.testing.assert_array_equal(Ed, oEd)
+
+
+TUNINGS = [{"sweep_kernel": 0, "tile_tz": 2}, {"sweep_kernel": 0, "tile_tz": 4}, {"sweep_kernel": 0, "tile_tz": 8},
+           {"sweep_kernel": 1}, {"sweep_kernel": 2, "pipe_rows": 4}, {"sweep_kernel": 2, "pipe_rows": 8}, {"sweep_kernel": 3}]
+
+
+@pytest.mark.parametrize("L,ns,nr", [(8, 40, 2), (8, 33, 1), (16, 17, 2), (24, 2, 2), (32, 3, 3)])
+def test_every_sweep_kernel_gives_the_same_bits(micsa, oracle, L, ns, nr):
+    """micsa_set_tuning never changes results: every half-sweep kernel variant
+    against the oracle, half-sweep by half-sweep, on lattices with L % 8 == 0."""
+    N = L ** 3
+    s0, J, m0 = random_pm1((ns, nr, N), 41), random_pm1((ns, 3, N), 42), random_levels((ns, nr, N), 43)
+    ref = []
+    s, m = s0.copy(), m0.copy()
+    for t in range(3):
+        for p in (0, 1):
+            oracle.half_sweep(L, s, m, J, p)
+            ref.append((s.copy(), m.copy()))
+    with micsa.MicSA(L, ns, nr, 1) as g:
+        g.set_couplings(J)
+        for tune in TUNINGS:
+            for k, v in tune.items():
+                g.set_tuning(k, v)
+            g.set_spins(s0); g.set_daemons(m0)
+            i = 0
+            for t in range(3):
+                for p in (0, 1):
+                    g.half_sweep(p)
+                    _assert_state(g, *ref[i]); i += 1
+            g.sweep(2)
+            s2, m2 = ref[-1][0].copy(), ref[-1][1].copy()
+            oracle.sweep(L, s2, m2, J, 2)
+            _assert_state(g, s2, m2)
+        with pytest.raises(micsa.MicsaError):
+            g.set_tuning("pipe_rows", 5)
