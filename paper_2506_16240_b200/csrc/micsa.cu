@@ -43,7 +43,7 @@ bool make_geom(int L, int n_samples, int n_replicas, int sample_offset, Geom& g)
     if (n_samples < 1 || n_replicas < 1) { set_err("n_samples and n_replicas must be >= 1"); return false; }
     if (sample_offset < 0 || (sample_offset & 15)) { set_err("sample_offset must be a non-negative multiple of 16"); return false; }
     const long long N = (long long)L * L * L;
-    if (N > 0xFFFFFFFFll) { set_err("L^3 must fit 32 bits (site index is one Philox counter word)"); return false; }
+    if (N > 0x7FFFFFFFll) { set_err("L^3 must be below 2^31 (32-bit site index and byte offsets inside a parity array)"); return false; }
     if ((long long)n_samples * n_replicas > (1ll << 24) || n_replicas >= (1 << 24)) {
         set_err("too many systems"); return false;
     }
@@ -86,7 +86,7 @@ Plan make_plan(const Geom& g) {
     p.bad = o;  o += align_up(sizeof(int));
     p.calls = o; o += align_up(sizeof(unsigned long long));
     p.progress = o; o += align_up((size_t)g.n_words * g.L * sizeof(int));
-    p.task_ticket = o; o += align_up(sizeof(unsigned long long));
+    p.task_ticket = o; o += align_up((size_t)g.n_words * sizeof(unsigned long long));
     p.total = o;
     return p;
 }
@@ -94,6 +94,12 @@ Plan make_plan(const Geom& g) {
 int vec_width(int Lh) { return (Lh % 4 == 0) ? 4 : (Lh % 2 == 0) ? 2 : 1; }
 
 }  // namespace
+
+struct PersistPlan {          // launch shape of the persistent sweep kernel
+    bool valid = false;
+    int ZT, n_sub, sub_items, block, n_groups, grid;
+    long long tasks_per_hs;   // per word lattice
+};
 
 struct micsa_ctx {
     Geom g;
@@ -122,7 +128,8 @@ struct micsa_ctx {
     unsigned long long* task_ticket;
     unsigned long long ticket0;   // value of *task_ticket when the next launch starts
     int progress_base;         // value of every progress entry between launches
-    int persist_grid;          // CTAs of the persistent kernel (0 = not computed yet)
+    PersistPlan pp;
+    int use_pdl;               // programmatic dependent launch for the pipelined kernel
     int pipe_rows;             // rows per thread of the pipelined kernel (4 or 8)
     int tile_tz;               // planes per tile of the tiled kernel (2, 4 or 8)
     uint64_t attempts, rns, launches;
@@ -194,8 +201,16 @@ void launch_half_sweep_pipe(micsa_ctx* c, int parity) {
     const int yc = c->pipe_rows;
     const int per_plane = (c->g.L / yc) * (c->g.Lh / 4);
     dim3 grid((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
-    if (yc == 8) half_sweep_pipe_kernel<RPW, 8><<<grid, 128, 0, c->stream>>>(a, parity);
-    else         half_sweep_pipe_kernel<RPW, 4><<<grid, 128, 0, c->stream>>>(a, parity);
+    // programmatic dependent launch (the kernel waits with griddepcontrol.wait before
+    // its first load): launch latency and ramp overlap the previous grid's tail
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = c->use_pdl ? 1 : 0;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (yc == 8) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8>, a, parity);
+    else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4>, a, parity);
 }
 
 template <int RPW, int TY, int TZ>
@@ -225,56 +240,70 @@ int launch_half_sweep_tile_tz(micsa_ctx* c, int parity) {
     }
 }
 
+// Shape of the persistent launch (sweep_persistent.cuh), computed once.
+template <int RPW>
+int plan_persistent(micsa_ctx* c) {
+    const Geom& g = c->g;
+    constexpr int YC = 4;
+    PersistPlan& pp = c->pp;
+    const int items_per_plane = (g.L / YC) * (g.Lh / 4);
+    int per_sm = 0, dev = 0, sms = 0;
+    CK(c, cudaGetDevice(&dev));
+    CK(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sweep_persistent_kernel<RPW, YC>, kPersistBlock, 0));
+    const long long grid_max = (long long)std::max(1, per_sm) * sms;
+    // lattices worked on together: as many as keep their state (12 B of spins and daemons +
+    // the bond words per site) inside ~96 MB of L2, a divisor of n_words so that groups stay balanced
+    const double bytes_per_lattice = (double)g.N * (12.0 + 3.0 * (g.rpw == 2 ? 2 : 4) / g.n_rg);
+    const long long n_fit = std::max<long long>(1, (long long)(96e6 / bytes_per_lattice));
+    int n_groups = 1;
+    for (int d = 1; d <= g.n_words && d <= n_fit && d <= grid_max; ++d)
+        if (g.n_words % d == 0) n_groups = d;
+    long long cpg = std::max<long long>(1, grid_max / n_groups);      // CTAs per lattice
+    // task size: <= 256 thread items, and (where the lattice allows) > 2.2 tasks per CTA per half-sweep
+    int ZT = 1, n_sub = 1;
+    if (items_per_plane > 256) n_sub = (items_per_plane + 255) / 256;
+    while ((long long)g.L * n_sub * 10 < 22 * cpg && (items_per_plane + n_sub) / (n_sub + 1) >= 64) ++n_sub;
+    if (n_sub == 1)
+        for (int d = 2; d <= g.L; ++d) {
+            if (g.L % d) continue;
+            if (d * items_per_plane > 256 || (long long)(g.L / d) * 10 < 22 * cpg) break;
+            ZT = d;
+        }
+    const int items = ZT * items_per_plane;
+    const long long tasks_per_hs = (long long)(g.L / ZT) * n_sub;
+    cpg = std::min(cpg, std::max<long long>(1, tasks_per_hs / 2));   // small lattices: nobody should spin
+    pp.ZT = ZT; pp.n_sub = n_sub; pp.sub_items = (items + n_sub - 1) / n_sub;
+    pp.block = std::min(kPersistBlock, (pp.sub_items + 31) / 32 * 32);
+    pp.n_groups = n_groups; pp.grid = (int)(cpg * n_groups);
+    pp.tasks_per_hs = tasks_per_hs;
+    pp.valid = true;
+    return MICSA_OK;
+}
+
 // n_hs half-sweeps, parities p_first, p_first^1, ... in one persistent launch
 template <int RPW>
 int launch_persistent(micsa_ctx* c, int n_hs, int p_first) {
     const Geom& g = c->g;
     constexpr int YC = 4;
-    const int items_per_plane = (g.L / YC) * (g.Lh / 4);
-    // task size: about 200 thread items, and (where the lattice allows) more
-    // than ~2.2 tasks per resident CTA in every half-sweep (sweep_persistent.cuh)
-    int ZT = 1, n_sub = 1;
-    if (items_per_plane > 256) {
-        n_sub = (items_per_plane + 199) / 200;
-    } else {
-        for (int d = 2; d <= g.L; ++d) {
-            if (g.L % d) continue;
-            if (d * items_per_plane > 256 || (long long)g.n_words * (g.L / d) < 650) break;
-            ZT = d;
-        }
-    }
-    const int items = ZT * items_per_plane;
-    const int sub_items = (items + n_sub - 1) / n_sub;
-    const int block = std::min(kPersistBlock, (sub_items + 31) / 32 * 32);
-    const long long tasks_per_hs = (long long)g.n_words * (g.L / ZT) * n_sub;
-    if (c->persist_grid == 0) {
-        int per_sm = 0, dev = 0, sms = 0;
-        CK(c, cudaGetDevice(&dev));
-        CK(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sweep_persistent_kernel<RPW, YC>, block, 0));
-        long long grid = (long long)std::max(1, per_sm) * sms;
-        // small lattices: fewer CTAs than half the tasks of a half-sweep, so that nobody spins
-        grid = std::min(grid, std::max<long long>(1, tasks_per_hs / 2));
-        c->persist_grid = (int)grid;
-    }
+    if (!c->pp.valid) { const int rc = plan_persistent<RPW>(c); if (rc) return rc; }
+    const PersistPlan& pp = c->pp;
     while (n_hs > 0) {
-        if ((long long)(c->progress_base + std::min(n_hs, 1 << 20)) * n_sub > (1ll << 30)) {   // keep the counters far from overflow
+        const int n = std::min(n_hs, 1 << 20);
+        if ((long long)(c->progress_base + n) * pp.n_sub > (1ll << 30)) {   // keep the counters far from overflow
             CK(c, cudaMemsetAsync(c->progress, 0, (size_t)g.n_words * g.L * sizeof(int), c->stream));
             c->progress_base = 0;
         }
-        const int n = std::min(n_hs, 1 << 20);
         PersistArgs A;
         A.a.spin = c->st.spin; A.a.m0 = c->st.m0; A.a.m1 = c->st.m1; A.a.J = c->st.J;
         A.a.L = g.L; A.a.Lh = g.Lh; A.a.n_rg = g.n_rg; A.a.half = g.half;
-        A.n_hs = n; A.p_first = p_first; A.ZT = ZT; A.n_slabs = g.L / ZT; A.n_words = g.n_words;
-        A.n_sub = n_sub; A.sub_items = sub_items;
+        A.n_hs = n; A.p_first = p_first; A.ZT = pp.ZT; A.n_slabs = g.L / pp.ZT; A.n_words = g.n_words;
+        A.n_sub = pp.n_sub; A.sub_items = pp.sub_items; A.n_groups = pp.n_groups;
         A.base = c->progress_base; A.progress = c->progress;
         A.ticket = c->task_ticket; A.ticket0 = c->ticket0;
-        const unsigned long long total = (unsigned long long)tasks_per_hs * n;
-        const int grid = (int)std::min<unsigned long long>((unsigned long long)c->persist_grid, total);
-        sweep_persistent_kernel<RPW, YC><<<grid, block, 0, c->stream>>>(A);
-        // every CTA draws one ticket past the end before it leaves
-        c->ticket0 += total + (unsigned long long)grid;
+        sweep_persistent_kernel<RPW, YC><<<pp.grid, pp.block, 0, c->stream>>>(A);
+        // per lattice: its tasks, plus one ticket past the end drawn by each CTA of its group
+        c->ticket0 += (unsigned long long)pp.tasks_per_hs * n + (unsigned long long)(pp.grid / pp.n_groups);
         c->progress_base += n;
         c->attempts += (uint64_t)n * (uint64_t)(g.N / 2) * (uint64_t)g.n_sys;
         const int rc = post_launch(c); if (rc) return rc;
@@ -498,7 +527,7 @@ int init_state(micsa_ctx* c) {
     const SiteGrid sg = site_grid(g);
     CK(c, cudaMemsetAsync(c->calls, 0, sizeof(unsigned long long), c->stream));
     CK(c, cudaMemsetAsync(c->progress, 0, (size_t)c->g.n_words * c->g.L * sizeof(int), c->stream));
-    CK(c, cudaMemsetAsync(c->task_ticket, 0, sizeof(unsigned long long), c->stream));
+    CK(c, cudaMemsetAsync(c->task_ticket, 0, (size_t)c->g.n_words * sizeof(unsigned long long), c->stream));
     CK(c, cudaMemsetAsync(c->cnt, 0, c->plan.cnt_words * 8, c->stream));
     CK(c, cudaMemsetAsync(c->ticket, 0, sizeof(unsigned int), c->stream));
     CK(c, cudaMemsetAsync(c->st.m0, 0, c->plan.plane_bytes, c->stream));
@@ -552,6 +581,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->sweep_kernel = 2;
     c->tile_tz = 4;
     c->pipe_rows = 4;
+    c->use_pdl = 1;
     c->attempts = c->rns = c->launches = 0;
     c->sticky = 0;
     if (dev_workspace) {
@@ -582,7 +612,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->calls = (unsigned long long*)(c->ws + c->plan.calls);
     c->progress = (int*)(c->ws + c->plan.progress);
     c->task_ticket = (unsigned long long*)(c->ws + c->plan.task_ticket);
-    c->ticket0 = 0; c->progress_base = 0; c->persist_grid = 0;
+    c->ticket0 = 0; c->progress_base = 0;
     c->host_row = nullptr; c->side = nullptr; c->ev_main = nullptr; c->ev_side = nullptr;
     if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_main, cudaEventDisableTiming) != cudaSuccess ||
@@ -843,6 +873,9 @@ int micsa_set_tuning(micsa_ctx* c, int key, int value) {
         case MICSA_TUNE_TILE_TZ:
             if (value != 2 && value != 4 && value != 8) { set_err("tile_tz must be 2, 4 or 8"); return MICSA_ERR_INVALID; }
             c->tile_tz = value; return MICSA_OK;
+        case MICSA_TUNE_PDL:
+            if (value != 0 && value != 1) { set_err("pdl must be 0 or 1"); return MICSA_ERR_INVALID; }
+            c->use_pdl = value; return MICSA_OK;
         case MICSA_TUNE_PIPE_ROWS:
             if (value != 4 && value != 8) { set_err("pipe_rows must be 4 or 8"); return MICSA_ERR_INVALID; }
             c->pipe_rows = value; return MICSA_OK;

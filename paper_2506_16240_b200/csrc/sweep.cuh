@@ -304,6 +304,13 @@ __device__ __forceinline__ void creutz_word20(uint32_t u1, uint32_t u2, uint32_t
     m1 = (acc & V1) | (~acc & m1);
 }
 
+struct PipeBase {           // block-uniform bases of lattice w: plane 0 of each parity array
+    uint32_t* sp; uint32_t* m0; uint32_t* m1;          // own parity
+    const uint32_t* sq;                                // opposite parity
+    const void* jx; const void* jy; const void* jz;    // own bonds
+    const void* jxq; const void* jyq; const void* jzq; // the -d neighbours' bonds (opposite parity arrays)
+};
+
 template <int RPW>
 struct RowRegs {                 // everything one row step reads
     typedef Bond4<RPW> B4;
@@ -313,9 +320,24 @@ struct RowRegs {                 // everything one row step reads
     typename B4::elem eJ;
 };
 
+// o, o_prev, o_next: byte offsets (inside a parity array of spin words) of
+// the thread's 4 words in rows y, y-1, y+1 of plane z; dzp, dzm: byte distance
+// to the same row of planes z+1, z-1 (mod 2^32, periodic); rowstart = o - x4.
+// Where the x-neighbour words just outside a thread's 4 words come from: the
+// lane that owns the adjacent quad of the same row holds them in registers, so
+// they are fetched with a shuffle; only lanes whose neighbour sits in another
+// warp (or is not running) load them.  A lone 4-byte load costs a whole 32-byte
+// sector of L2 bandwidth, which is what bounds this kernel.
+struct XNb {
+    unsigned mask;          // lanes taking part (all of them run the same row step)
+    int lane_up, lane_dn;   // lanes owning quads xv+1 and xv-1 (periodic) of the same row
+    bool in_up, in_dn;      // ... and whether they can be reached by a shuffle
+};
+
 template <int RPW, int C>
-__device__ __forceinline__ void load_row(RowRegs<RPW>& r, const RowPtrs& P, uint32_t o, uint32_t o_prev,
-                                         uint32_t o_next, uint32_t x4, uint32_t xe_up, uint32_t xe_dn)
+__device__ __forceinline__ void load_row(RowRegs<RPW>& r, const PipeBase& P, uint32_t o, uint32_t o_prev,
+                                         uint32_t o_next, uint32_t x4, uint32_t xe_up, uint32_t xe_dn,
+                                         uint32_t dzp, uint32_t dzm, const XNb& nb)
 {
     typedef Bond4<RPW> B4;
     constexpr uint32_t JS = sizeof(typename B4::elem);
@@ -325,26 +347,30 @@ __device__ __forceinline__ void load_row(RowRegs<RPW>& r, const RowPtrs& P, uint
     r.s  = ld_off<uint4>(P.sp, o);
     r.d0 = ld_off<uint4>(P.m0, o);
     r.d1 = ld_off<uint4>(P.m1, o);
-    r.zp = ld_off<uint4>(P.sq_zp, o);
-    r.zm = ld_off<uint4>(P.sq_zm, o);
+    r.zp = ld_off<uint4>(P.sq, o + dzp);
+    r.zm = ld_off<uint4>(P.sq, o + dzm);
     r.jx = ld_off<typename B4::raw>(P.jx, oj);
     r.jy = ld_off<typename B4::raw>(P.jy, oj);
     r.jz = ld_off<typename B4::raw>(P.jz, oj);
     r.jyq = ld_off<typename B4::raw>(P.jyq, ojm);
-    r.jzq = ld_off<typename B4::raw>(P.jzq_zm, oj);
+    r.jzq = ld_off<typename B4::raw>(P.jzq, (o + dzm) / 4u * JS);
     r.jxq = ld_off<typename B4::raw>(P.jxq, oj);
+    r.e = 0; r.eJ = 0;
     if (C) {
-        r.e = ld_off<uint32_t>(P.sq, rowstart + xe_up);
-        r.eJ = 0;
-    } else {
+        if (!nb.in_up) r.e = ld_off<uint32_t>(P.sq, rowstart + xe_up);
+    } else if (!nb.in_dn) {
         r.e = ld_off<uint32_t>(P.sq, rowstart + xe_dn);
         r.eJ = ld_off<typename B4::elem>(P.jxq, (rowstart + xe_dn) / 4u * JS);
     }
 }
 
+template <int RPW> __device__ __forceinline__ uint32_t last_bond_word(const typename Bond4<RPW>::raw& j);
+template <> __device__ __forceinline__ uint32_t last_bond_word<2>(const uint2& j) { return j.y >> 16; }
+template <> __device__ __forceinline__ uint32_t last_bond_word<1>(const uint4& j) { return j.w; }
+
 template <int RPW, int C>
 __device__ __forceinline__ void update_row(const RowRegs<RPW>& r, const uint4& Aprev, const uint4& Acur,
-                                           const RowPtrs& P, uint32_t o)
+                                           const PipeBase& P, uint32_t o, const XNb& nb)
 {
     typedef Bond4<RPW> B4;
     uint32_t jxo[4], jyo[4], jzo[4], jxm[4], jym[4], jzm[4], Bx[4];
@@ -353,13 +379,18 @@ __device__ __forceinline__ void update_row(const RowRegs<RPW>& r, const uint4& A
     const uint32_t a[4] = { Acur.x, Acur.y, Acur.z, Acur.w };
     uint32_t nxp[4], nxm[4];
     if (C) {        // x = 2xh+1: -x neighbour at xh (bond owned by it), +x neighbour at xh+1
-        nxp[0] = a[1]; nxp[1] = a[2]; nxp[2] = a[3]; nxp[3] = r.e;
+        uint32_t e = __shfl_sync(nb.mask, Acur.x, nb.lane_up);
+        if (!nb.in_up) e = r.e;
+        nxp[0] = a[1]; nxp[1] = a[2]; nxp[2] = a[3]; nxp[3] = e;
         nxm[0] = a[0]; nxm[1] = a[1]; nxm[2] = a[2]; nxm[3] = a[3];
         jxm[0] = Bx[0]; jxm[1] = Bx[1]; jxm[2] = Bx[2]; jxm[3] = Bx[3];
     } else {        // x = 2xh: +x neighbour at xh, -x neighbour at xh-1 (bond owned by it)
+        uint32_t e = __shfl_sync(nb.mask, Acur.w, nb.lane_dn);
+        uint32_t eJ = __shfl_sync(nb.mask, last_bond_word<RPW>(r.jxq), nb.lane_dn);
+        if (!nb.in_dn) { e = r.e; eJ = (uint32_t)r.eJ; }
         nxp[0] = a[0]; nxp[1] = a[1]; nxp[2] = a[2]; nxp[3] = a[3];
-        nxm[0] = r.e; nxm[1] = a[0]; nxm[2] = a[1]; nxm[3] = a[2];
-        jxm[0] = B4::expand1(r.eJ); jxm[1] = Bx[0]; jxm[2] = Bx[1]; jxm[3] = Bx[2];
+        nxm[0] = e; nxm[1] = a[0]; nxm[2] = a[1]; nxm[3] = a[2];
+        jxm[0] = B4::expand1((typename B4::elem)eJ); jxm[1] = Bx[0]; jxm[2] = Bx[1]; jxm[3] = Bx[2];
     }
     uint32_t sv[4] = { r.s.x, r.s.y, r.s.z, r.s.w };
     uint32_t v0[4] = { r.d0.x, r.d0.y, r.d0.z, r.d0.w };
@@ -381,39 +412,79 @@ __device__ __forceinline__ void update_row(const RowRegs<RPW>& r, const uint4& A
     st_off<uint4>(P.m1, o, make_uint4(v1[0], v1[1], v1[2], v1[3]));
 }
 
+// rows y0 .. y0+YC-1 of plane z (y0 % YC == 0, YC even, L % YC == 0), words xh0 .. xh0+3
 template <int RPW, int YC, int F>
-__device__ __forceinline__ void march_rows_pipe(const RowPtrs& P, int L, int Lh, int y0, int xh0)
+__device__ __forceinline__ void march_rows_pipe(const PipeBase& P, int L, int Lh, int z, int y0, int xh0,
+                                                const XNb& nb)
 {
     const uint32_t rowB = (uint32_t)Lh * 4u;
+    const uint32_t planeB = (uint32_t)L * rowB;
     const uint32_t x4 = (uint32_t)xh0 * 4u;
+    const uint32_t zB = (uint32_t)z * planeB;
+    const uint32_t dzp = (z + 1 == L) ? 0u - zB : planeB;
+    const uint32_t dzm = (z == 0) ? (uint32_t)(L - 1) * planeB : 0u - planeB;
     const int ym0 = (y0 == 0) ? L - 1 : y0 - 1;
     const uint32_t xe_up = ((xh0 + 4 == Lh) ? 0u : (uint32_t)(xh0 + 4)) * 4u;
     const uint32_t xe_dn = ((xh0 == 0) ? (uint32_t)(Lh - 1) : (uint32_t)(xh0 - 1)) * 4u;
-    uint32_t o = (uint32_t)y0 * rowB + x4;
-    uint32_t o_prev = (uint32_t)ym0 * rowB + x4;
+    const uint32_t row0 = zB + x4;                       // row 0 of the plane, this thread's words
+    uint32_t o = row0 + (uint32_t)y0 * rowB;
+    uint32_t o_prev = row0 + (uint32_t)ym0 * rowB;
 
     uint4 Aprev = ld_off<uint4>(P.sq, o_prev);
     uint4 Acur  = ld_off<uint4>(P.sq, o);
     RowRegs<RPW> cur, nxt;
     {
-        const uint32_t o_next = (y0 + 1 == L) ? x4 : o + rowB;
-        load_row<RPW, F>(cur, P, o, o_prev, o_next, x4, xe_up, xe_dn);
+        const uint32_t o_next = (y0 + 1 == L) ? row0 : o + rowB;
+        load_row<RPW, F>(cur, P, o, o_prev, o_next, x4, xe_up, xe_dn, dzp, dzm, nb);
     }
 #pragma unroll
     for (int iy = 0; iy < YC; ++iy) {
         const int y = y0 + iy;
-        const uint32_t o_next = (y + 1 == L) ? x4 : o + rowB;
+        const uint32_t o_next = (y + 1 == L) ? row0 : o + rowB;
         if (iy + 1 < YC) {                          // y + 1 < L inside a chunk
-            const uint32_t o_next2 = (y + 2 == L) ? x4 : o_next + rowB;
-            if ((iy & 1) ^ F) load_row<RPW, 0>(nxt, P, o_next, o, o_next2, x4, xe_up, xe_dn);
-            else              load_row<RPW, 1>(nxt, P, o_next, o, o_next2, x4, xe_up, xe_dn);
+            const uint32_t o_next2 = (y + 2 == L) ? row0 : o_next + rowB;
+            if ((iy & 1) ^ F) load_row<RPW, 0>(nxt, P, o_next, o, o_next2, x4, xe_up, xe_dn, dzp, dzm, nb);
+            else              load_row<RPW, 1>(nxt, P, o_next, o, o_next2, x4, xe_up, xe_dn, dzp, dzm, nb);
         }
-        if ((iy & 1) ^ F) update_row<RPW, 1>(cur, Aprev, Acur, P, o);
-        else              update_row<RPW, 0>(cur, Aprev, Acur, P, o);
+        if ((iy & 1) ^ F) update_row<RPW, 1>(cur, Aprev, Acur, P, o, nb);
+        else              update_row<RPW, 0>(cur, Aprev, Acur, P, o, nb);
         Aprev = Acur; Acur = cur.An;
         if (iy + 1 < YC) cur = nxt;
         o_prev = o; o = o_next;
     }
+}
+
+// x-neighbour lanes of the thread whose item index inside its warp-aligned
+// index space is `idx` (consecutive idx = consecutive quads of a row, rows of
+// nxv quads one after the other); mask = lanes running this step.
+__device__ __forceinline__ XNb x_neighbours(int idx, int xv, int nxv, unsigned mask, bool use_shuffle)
+{
+    XNb nb;
+    nb.mask = mask;
+    const int up = (xv == nxv - 1) ? idx - (nxv - 1) : idx + 1;
+    const int dn = (xv == 0) ? idx + (nxv - 1) : idx - 1;
+    nb.lane_up = up & 31; nb.lane_dn = dn & 31;
+    nb.in_up = use_shuffle && (up >> 5) == (idx >> 5) && ((mask >> nb.lane_up) & 1u);
+    nb.in_dn = use_shuffle && (dn >> 5) == (idx >> 5) && ((mask >> nb.lane_dn) & 1u);
+    return nb;
+}
+
+template <int RPW>
+__device__ __forceinline__ PipeBase pipe_base(const SweepArgs& a, int w, int p)
+{
+    typedef typename Bond4<RPW>::elem JT;
+    const int q = 1 - p;
+    const long long half = a.half;
+    const int sg = w / a.n_rg;
+    const JT* Jb = reinterpret_cast<const JT*>(a.J) + (long long)sg * 6 * half;
+    PipeBase P;
+    P.sp = a.spin + ((long long)w * 2 + p) * half;
+    P.m0 = a.m0 + ((long long)w * 2 + p) * half;
+    P.m1 = a.m1 + ((long long)w * 2 + p) * half;
+    P.sq = a.spin + ((long long)w * 2 + q) * half;
+    P.jx = Jb + (0 * 2 + p) * half; P.jy = Jb + (1 * 2 + p) * half; P.jz = Jb + (2 * 2 + p) * half;
+    P.jxq = Jb + (0 * 2 + q) * half; P.jyq = Jb + (1 * 2 + q) * half; P.jzq = Jb + (2 * 2 + q) * half;
+    return P;
 }
 
 // grid = (ceil((L/YC)*(Lh/4) / block), L, n_words)
@@ -421,34 +492,23 @@ template <int RPW, int YC>
 __global__ void __launch_bounds__(128)
 half_sweep_pipe_kernel(SweepArgs a, int p)
 {
-    typedef typename Bond4<RPW>::elem JT;
     const int L = a.L, Lh = a.Lh;
     const int nxv = Lh >> 2;
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= (L / YC) * nxv) return;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;          // blockDim.x % 32 == 0: idx = t
+    const bool active = t < (L / YC) * nxv;
+    const unsigned mask = __ballot_sync(0xFFFFFFFFu, active);
+    if (!active) return;
     const int chunk = t / nxv, xv = t - chunk * nxv;
-    const int z = blockIdx.y, w = blockIdx.z, q = 1 - p;
-    const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
-    const long long half = a.half;
-    const long long plane = (long long)L * Lh;
-    const int sg = w / a.n_rg;
-    const JT* Jb = reinterpret_cast<const JT*>(a.J) + (long long)sg * 6 * half;
-
-    RowPtrs P;
-    P.sp = a.spin + ((long long)w * 2 + p) * half + z * plane;
-    P.m0 = a.m0 + ((long long)w * 2 + p) * half + z * plane;
-    P.m1 = a.m1 + ((long long)w * 2 + p) * half + z * plane;
-    const uint32_t* sqb = a.spin + ((long long)w * 2 + q) * half;
-    P.sq = sqb + z * plane; P.sq_zp = sqb + zp * plane; P.sq_zm = sqb + zm * plane;
-    P.jx = Jb + (0 * 2 + p) * half + z * plane;
-    P.jy = Jb + (1 * 2 + p) * half + z * plane;
-    P.jz = Jb + (2 * 2 + p) * half + z * plane;
-    P.jxq = Jb + (0 * 2 + q) * half + z * plane;
-    P.jyq = Jb + (1 * 2 + q) * half + z * plane;
-    P.jzq_zm = Jb + (2 * 2 + q) * half + zm * plane;
-
-    if ((z + p) & 1) march_rows_pipe<RPW, YC, 1>(P, L, Lh, chunk * YC, xv * 4);
-    else             march_rows_pipe<RPW, YC, 0>(P, L, Lh, chunk * YC, xv * 4);
+    const int z = blockIdx.y, w = blockIdx.z;                     // z is block-uniform: one code path per warp
+    const PipeBase P = pipe_base<RPW>(a, w, p);
+    const XNb nb = x_neighbours(t, xv, nxv, mask, true);
+    // programmatic dependent launch: this grid may have been scheduled while the
+    // previous half-sweep was still draining; its results are needed from here on,
+    // and the next grid may be scheduled as soon as every CTA of this one got here
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if ((z + p) & 1) march_rows_pipe<RPW, YC, 1>(P, L, Lh, z, chunk * YC, xv * 4, nb);
+    else             march_rows_pipe<RPW, YC, 0>(P, L, Lh, z, chunk * YC, xv * 4, nb);
 }
 
 }  // namespace micsa

@@ -16,8 +16,8 @@
 // than twice as many tasks as there are resident CTAs: then the tasks a CTA
 // draws depend on tasks that finished long ago and nobody waits.
 //
-// CTAs are persistent and take tasks from a global ticket counter in
-// lexicographic (hs, w, slab) order.  Every dependence of a ticket is a lower
+// CTAs are persistent and take the tasks of a lattice from its ticket counter
+// in lexicographic (hs, slab, sub) order.  Every dependence of a ticket is a lower
 // ticket, already claimed by a CTA that is running or done, so the lowest
 // unfinished ticket can always proceed: no co-residency assumption, no
 // deadlock.  Completion is published per slab as a monotone counter
@@ -37,10 +37,11 @@ struct PersistArgs {
     int ZT, n_slabs;             // planes per slab, slabs per word lattice (L = ZT * n_slabs)
     int n_sub, sub_items;        // parts per slab, thread items per part (the last part may be short)
     int n_words;
+    int n_groups;                // word lattices worked on at the same time (gridDim.x % n_groups == 0)
     int base;                    // half-sweeps every slab had done at launch (progress = n_sub * base)
     int* progress;               // [n_words][n_slabs]
-    unsigned long long* ticket;  // global task counter (monotone across launches)
-    unsigned long long ticket0;  // its value at launch
+    unsigned long long* ticket;  // [n_words] task counters (monotone across launches)
+    unsigned long long ticket0;  // their common value at launch
 };
 
 __device__ __forceinline__ int ld_acquire_gpu(const int* p) {
@@ -54,73 +55,72 @@ __device__ __forceinline__ void add_release_gpu(int* p, int v) {
 
 constexpr int kPersistBlock = 256;
 
-template <int RPW, int YC>
-__global__ void __launch_bounds__(kPersistBlock, 2)
-sweep_persistent_kernel(PersistArgs A)
+// one task: items [item0, item1) of slab `slab` of lattice w, parity P (compile time)
+template <int RPW, int YC, int P>
+__device__ __forceinline__ void persistent_task(const PersistArgs& A, int w, int slab, int item0, int item1)
 {
-    typedef typename Bond4<RPW>::elem JT;
-    __shared__ unsigned long long s_ticket;
     const SweepArgs& a = A.a;
     const int L = a.L, Lh = a.Lh;
     const int nxv = Lh >> 2;
     const int items_per_plane = (L / YC) * nxv;
-    const int items = A.ZT * items_per_plane;
-    const long long half = a.half;
-    const long long plane = (long long)L * Lh;
-    const int tasks_per_word = A.n_slabs * A.n_sub;
-    const unsigned long long tasks_per_hs = (unsigned long long)A.n_words * tasks_per_word;
-    const unsigned long long total = tasks_per_hs * (unsigned long long)A.n_hs;
+    const PipeBase B = pipe_base<RPW>(a, w, P);            // w comes from blockIdx: uniform registers
+    // consecutive threads own consecutive items (quads of a row, rows one after the other)
+    for (int item = item0 + (int)threadIdx.x; ; item += (int)blockDim.x) {
+        const bool active = item < item1;
+        const unsigned mask = __ballot_sync(0xFFFFFFFFu, active);
+        if (mask == 0u) break;                              // the whole warp is past the end
+        if (!active) continue;
+        const int lz = item / items_per_plane, it = item - lz * items_per_plane;
+        const int chunk = it / nxv, xv = it - chunk * nxv;
+        const int z = slab * A.ZT + lz;
+        // shuffles need one code path per warp: only when a task lies inside one plane
+        const XNb nb = x_neighbours((int)threadIdx.x, xv, nxv, mask, A.ZT == 1);
+        if ((z + P) & 1) march_rows_pipe<RPW, YC, 1>(B, L, Lh, z, chunk * YC, xv * 4, nb);
+        else             march_rows_pipe<RPW, YC, 0>(B, L, Lh, z, chunk * YC, xv * 4, nb);
+    }
+}
 
-    for (;;) {
-        __syncthreads();                                   // everyone has read the previous ticket
-        if (threadIdx.x == 0) s_ticket = atomicAdd(A.ticket, 1ull) - A.ticket0;
-        __syncthreads();
-        const unsigned long long t = s_ticket;
-        if (t >= total) break;
-        const int hs = (int)(t / tasks_per_hs);
-        const int r = (int)(t - (unsigned long long)hs * tasks_per_hs);
-        const int w = r / tasks_per_word, r2 = r - w * tasks_per_word;
-        const int slab = r2 / A.n_sub, sub = r2 - slab * A.n_sub;
+// CTA b works for the lattices w = b % n_groups, + n_groups, ... one after the
+// other, each for all n_hs half-sweeps (a lattice never interacts with
+// another one, and finishing one before touching the next keeps its state in
+// L2 for the whole launch when the full state does not fit).
+template <int RPW, int YC>
+__global__ void __launch_bounds__(kPersistBlock, 2)
+sweep_persistent_kernel(PersistArgs A)
+{
+    __shared__ unsigned long long s_ticket;
+    const int items = A.ZT * (A.a.L / YC) * (A.a.Lh >> 2);
+    const int tasks_per_hs = A.n_slabs * A.n_sub;
+    const unsigned long long total = (unsigned long long)tasks_per_hs * (unsigned long long)A.n_hs;
+
+    for (int w = (int)blockIdx.x % A.n_groups; w < A.n_words; w += A.n_groups) {
         int* prog = A.progress + (long long)w * A.n_slabs;
+        for (;;) {
+            __syncthreads();                               // everyone has read the previous ticket
+            if (threadIdx.x == 0) s_ticket = atomicAdd(A.ticket + w, 1ull) - A.ticket0;
+            __syncthreads();
+            const unsigned long long t = s_ticket;
+            if (t >= total) break;
+            const int hs = (int)(t / (unsigned)tasks_per_hs);
+            const int r = (int)(t - (unsigned long long)hs * tasks_per_hs);
+            const int slab = r / A.n_sub, sub = r - slab * A.n_sub;
 
-        if (hs > 0 && threadIdx.x < 3) {                   // the three neighbour slabs, previous half-sweep
-            int sn = slab - 1 + (int)threadIdx.x;
-            sn = (sn < 0) ? sn + A.n_slabs : (sn >= A.n_slabs ? sn - A.n_slabs : sn);
-            const int need = (A.base + hs) * A.n_sub;
-            while (ld_acquire_gpu(prog + sn) < need) __nanosleep(32);
+            if (hs > 0 && threadIdx.x < 3) {               // the three neighbour slabs, previous half-sweep
+                int sn = slab - 1 + (int)threadIdx.x;
+                sn = (sn < 0) ? sn + A.n_slabs : (sn >= A.n_slabs ? sn - A.n_slabs : sn);
+                const int need = (A.base + hs) * A.n_sub;
+                while (ld_acquire_gpu(prog + sn) < need) __nanosleep(32);
+            }
+            __syncthreads();
+
+            const int item0 = sub * A.sub_items, item1 = min(items, item0 + A.sub_items);
+            if ((A.p_first ^ hs) & 1) persistent_task<RPW, YC, 1>(A, w, slab, item0, item1);
+            else                      persistent_task<RPW, YC, 0>(A, w, slab, item0, item1);
+
+            __threadfence();                               // every writer: results visible device-wide ...
+            __syncthreads();
+            if (threadIdx.x == 0) add_release_gpu(prog + slab, 1);   // ... before the part is published
         }
-        __syncthreads();
-
-        const int p = A.p_first ^ (hs & 1), q = 1 - p;
-        const int sg = w / a.n_rg;
-        const JT* Jb = reinterpret_cast<const JT*>(a.J) + (long long)sg * 6 * half;
-        uint32_t* spb = a.spin + ((long long)w * 2 + p) * half;
-        uint32_t* m0b = a.m0 + ((long long)w * 2 + p) * half;
-        uint32_t* m1b = a.m1 + ((long long)w * 2 + p) * half;
-        const uint32_t* sqb = a.spin + ((long long)w * 2 + q) * half;
-
-        const int item_end = min(items, (sub + 1) * A.sub_items);
-        for (int item = sub * A.sub_items + threadIdx.x; item < item_end; item += blockDim.x) {
-            const int lz = item / items_per_plane, it = item - lz * items_per_plane;
-            const int chunk = it / nxv, xv = it - chunk * nxv;
-            const int z = slab * A.ZT + lz;
-            const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
-            RowPtrs P;
-            P.sp = spb + z * plane; P.m0 = m0b + z * plane; P.m1 = m1b + z * plane;
-            P.sq = sqb + z * plane; P.sq_zp = sqb + zp * plane; P.sq_zm = sqb + zm * plane;
-            P.jx = Jb + (0 * 2 + p) * half + z * plane;
-            P.jy = Jb + (1 * 2 + p) * half + z * plane;
-            P.jz = Jb + (2 * 2 + p) * half + z * plane;
-            P.jxq = Jb + (0 * 2 + q) * half + z * plane;
-            P.jyq = Jb + (1 * 2 + q) * half + z * plane;
-            P.jzq_zm = Jb + (2 * 2 + q) * half + zm * plane;
-            if ((z + p) & 1) march_rows_pipe<RPW, YC, 1>(P, L, Lh, chunk * YC, xv * 4);
-            else             march_rows_pipe<RPW, YC, 0>(P, L, Lh, chunk * YC, xv * 4);
-        }
-
-        __threadfence();                                   // every writer: results visible device-wide ...
-        __syncthreads();
-        if (threadIdx.x == 0) add_release_gpu(prog + slab, 1);               // ... before the part is published
     }
 }
 

@@ -382,8 +382,8 @@ def test_measure_begin_end(micsa, oracle):
         np.testing.assert_array_equal(Ed, oEd)
 
 
-TUNINGS = [{"sweep_kernel": 0, "tile_tz": 2}, {"sweep_kernel": 0, "tile_tz": 4}, {"sweep_kernel": 0, "tile_tz": 8},
-           {"sweep_kernel": 1}, {"sweep_kernel": 2, "pipe_rows": 4}, {"sweep_kernel": 2, "pipe_rows": 8}, {"sweep_kernel": 3}]
+TUNINGS = [{"sweep_kernel": 2, "pipe_rows": 4, "pdl": 1}, {"sweep_kernel": 0, "tile_tz": 2}, {"sweep_kernel": 0, "tile_tz": 4}, {"sweep_kernel": 0, "tile_tz": 8},
+           {"sweep_kernel": 1}, {"sweep_kernel": 2, "pipe_rows": 4}, {"sweep_kernel": 2, "pipe_rows": 8}, {"sweep_kernel": 2, "pipe_rows": 4, "pdl": 0}, {"sweep_kernel": 3}]
 
 
 @pytest.mark.parametrize("L,ns,nr", [(8, 40, 2), (8, 33, 1), (16, 17, 2), (24, 2, 2), (32, 3, 3)])
