@@ -39,8 +39,10 @@ T_RUN = CFG.temperatures[0]
 METRIC = "spin-flip attempts/ns (refresh + 10 sweeps + measure per step)"
 UNIT = "attempts/ns"
 # dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch from the
-# ncu --set full capture summarised in profiles/ (None until captured)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+# ncu --set full capture summarised in profiles/r1b_half_sweep_pipe_full.md
+# (cold L2: ncu flushes caches before every replay; in a real step the 73.7 MB
+# state stays in the 126 MB L2 after the first sweep)
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 57_378_560 + 282_112
 
 
 def measured_peaks():
@@ -237,7 +239,7 @@ def main():
     achieved = alg_bytes / t_launch_s / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
-                "kernel": "half_sweep_rows_kernel<2,4>", "peak_source": peak_src,
+                "kernel": "half_sweep_pipe_kernel<2,4>", "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "us_per_launch": t_launch_s * 1e6,
                 "convention": "compulsory one-pass traffic: 7.5 bits/attempt (spin 1r+1w, daemon 2r+2w, "
