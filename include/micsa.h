@@ -219,11 +219,14 @@ int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
  *   boundaries.
  * key MICSA_TUNE_TILE_TZ: lattice planes per tile of kernel 0: 2, 4 (default), 8.
  * key MICSA_TUNE_PIPE_ROWS: rows per thread of kernel 2: 4 (default) or 8.
+ * key MICSA_TUNE_PIPE_PLANES: lattice planes per CTA of kernel 2 (one warp
+ *   each): 4 (default) or 1.
  * key MICSA_TUNE_PDL: 1 (default) = kernel 2 is launched with programmatic
  *   stream serialization (the next half-sweep's grid is scheduled while this
  *   one drains and waits on the device for its completion), 0 = plain launches.
  * Unknown key or value: MICSA_ERR_INVALID, nothing changes. */
-enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_TILE_TZ = 1, MICSA_TUNE_PIPE_ROWS = 2, MICSA_TUNE_PDL = 3 };
+enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_TILE_TZ = 1, MICSA_TUNE_PIPE_ROWS = 2, MICSA_TUNE_PDL = 3,
+       MICSA_TUNE_PIPE_PLANES = 4 };
 int micsa_set_tuning(micsa_ctx *ctx, int key, int value);
 
 #ifdef __cplusplus

@@ -286,8 +286,8 @@ class MicSA:
 
     def set_tuning(self, key, value):
         """micsa_set_tuning: 'sweep_kernel' (0 tiled, 1 row-marching, 2 pipelined
-        row-marching, 3 persistent), 'tile_tz' (2, 4, 8), 'pipe_rows' (4, 8) or 'pdl' (0, 1)."""
-        k = {"sweep_kernel": 0, "tile_tz": 1, "pipe_rows": 2, "pdl": 3}[key]
+        row-marching, 3 persistent), 'tile_tz' (2, 4, 8), 'pipe_rows' (4, 8), 'pdl' (0, 1) or 'pipe_planes' (1, 4)."""
+        k = {"sweep_kernel": 0, "tile_tz": 1, "pipe_rows": 2, "pdl": 3, "pipe_planes": 4}[key]
         _check(_lib.micsa_set_tuning(self._h, k, int(value)))
 
     def layout_info(self):

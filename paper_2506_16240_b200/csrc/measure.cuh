@@ -192,19 +192,111 @@ __device__ __forceinline__ void finalize_rows(const FinalizeArgs& f)
 
 constexpr int kMeasureBlock = 256;
 constexpr int kMeasurePlanes = 10;     // per-thread vertical counters
-constexpr int kMeasureMaxItems = 85;   // per thread: 85 * 12 < 2^10
+constexpr int kMeasureMaxItems = 84;   // per thread (even): 84 * 12 < 2^10
+
+__device__ __forceinline__ void full_add(uint32_t a, uint32_t b, uint32_t c, uint32_t& s, uint32_t& cy) {
+    s = a ^ b ^ c; cy = maj3(a, b, c);
+}
+__device__ __forceinline__ void half_add(uint32_t a, uint32_t b, uint32_t& s, uint32_t& cy) {
+    s = a ^ b; cy = a & b;
+}
+
+// sum of four 1-bit lanes-wise numbers (weight 1) and four more of weight 2 -> 4 planes (<= 12)
+__device__ __forceinline__ void csa_4x1_4x2(const uint32_t (&lo)[4], const uint32_t (&hi)[4], uint32_t (&o)[4]) {
+    uint32_t a, b, b2, d, e4, f, g4, h4;
+    full_add(lo[0], lo[1], lo[2], a, b);
+    half_add(a, lo[3], o[0], b2);
+    full_add(hi[0], hi[1], hi[2], d, e4);
+    full_add(hi[3], b, b2, f, g4);
+    half_add(d, f, o[1], h4);
+    full_add(e4, g4, h4, o[2], o[3]);
+}
+
+// partial sums of one item: unsatisfied own bonds (<= 3V), daemon levels (<= 3V), differing replica lanes (<= V)
+struct ItemSums { uint32_t u[4], m[4], x[3]; };
+
+template <int V, int RPW, bool PAIR>
+__device__ __forceinline__ void measure_item(ItemSums& r, uint32_t it, uint32_t items_p, uint32_t nxv, uint32_t L,
+                                             uint32_t Lh, long long half, const uint32_t* s0, const uint32_t* d0,
+                                             const uint32_t* d1, const typename BondT<RPW>::type* Jb)
+{
+    const uint32_t p = it >= items_p;
+    const uint32_t iv = it - (p ? items_p : 0u);
+    const uint32_t rowi = iv / nxv, xv = iv - rowi * nxv;
+    const uint32_t z = rowi / L, y = rowi - z * L;
+    const uint32_t yp = (y + 1 == L) ? 0 : y + 1, zp = (z + 1 == L) ? 0 : z + 1;
+    const uint32_t xh0 = xv * V;
+    const uint32_t row = rowi * Lh, h = row + xh0;       // < half < 2^31
+    const uint32_t c = (y + z + p) & 1u;      // c=1: +x neighbour at xh+1, else same xh
+    const uint32_t* sp = s0 + (p ? half : 0);
+    const uint32_t* sq = s0 + (p ? 0 : half);
+    const Vec<V> s = ldg_vec<V>(sp + h);
+    const Vec<V> A = ldg_vec<V>(sq + h);
+    const uint32_t e = sq[row + ((xh0 + V == Lh) ? 0 : xh0 + V)];
+    const Vec<V> ny = ldg_vec<V>(sq + (z * L + yp) * Lh + xh0);
+    const Vec<V> nz = ldg_vec<V>(sq + (zp * L + y) * Lh + xh0);
+    const Vec<V> jx = ldg_bonds<V, RPW>(Jb + (0 * 2 + p) * half + h);
+    const Vec<V> jy = ldg_bonds<V, RPW>(Jb + (1 * 2 + p) * half + h);
+    const Vec<V> jz = ldg_bonds<V, RPW>(Jb + (2 * 2 + p) * half + h);
+    const Vec<V> b0 = ldg_vec<V>(d0 + (p ? half : 0) + h);
+    const Vec<V> b1 = ldg_vec<V>(d1 + (p ? half : 0) + h);
+    uint32_t us[V], uc[V], xs[V];
+#pragma unroll
+    for (int k = 0; k < V; ++k) {
+        const uint32_t up = (k + 1 < V) ? A.v[k + 1] : e;
+        const uint32_t nx = c ? up : A.v[k];
+        full_add(s.v[k] ^ nx ^ jx.v[k], s.v[k] ^ ny.v[k] ^ jy.v[k], s.v[k] ^ nz.v[k] ^ jz.v[k], us[k], uc[k]);
+        xs[k] = PAIR ? ((s.v[k] ^ (s.v[k] >> 16)) & 0xFFFFu) : 0u;
+    }
+    if (V == 4) {                             // carry-save adder trees
+        const uint32_t u_lo[4] = { us[0], us[1], us[2], us[3] }, u_hi[4] = { uc[0], uc[1], uc[2], uc[3] };
+        csa_4x1_4x2(u_lo, u_hi, r.u);
+        const uint32_t m_lo[4] = { b0.v[0], b0.v[1], b0.v[2], b0.v[3] }, m_hi[4] = { b1.v[0], b1.v[1], b1.v[2], b1.v[3] };
+        csa_4x1_4x2(m_lo, m_hi, r.m);
+        if (PAIR) {
+            uint32_t a2, b2, b3;
+            full_add(xs[0], xs[1], xs[2], a2, b2);
+            half_add(a2, xs[3], r.x[0], b3);
+            r.x[1] = b2 ^ b3; r.x[2] = b2 & b3;
+        } else { r.x[0] = r.x[1] = r.x[2] = 0u; }
+    } else {                                  // small odd-sized lattices: plain ripple adds
+        VCount<4> locU, locM; locU.clear(); locM.clear();
+        VCount<3> locX; locX.clear();
+#pragma unroll
+        for (int k = 0; k < V; ++k) {
+            const uint32_t bu[2] = { us[k], uc[k] }; locU.add(bu);
+            const uint32_t bm[2] = { b0.v[k], b1.v[k] }; locM.add(bm);
+            const uint32_t bx[1] = { xs[k] }; locX.add(bx);
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { r.u[k] = locU.c[k]; r.m[k] = locM.c[k]; }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) r.x[k] = locX.c[k];
+    }
+}
+
+// a + b for K-plane numbers -> K+1 planes
+template <int K>
+__device__ __forceinline__ void add_planes(const uint32_t (&a)[K], const uint32_t (&b)[K], uint32_t (&o)[K + 1]) {
+    uint32_t carry = 0;
+#pragma unroll
+    for (int k = 0; k < K; ++k) { o[k] = a[k] ^ b[k] ^ carry; carry = maj3(a[k], b[k], carry); }
+    o[K] = carry;
+}
 
 // One pass over the state for all three observables.
 // An item = V consecutive words of one row of one parity array; it counts the
 // unsatisfied +x,+y,+z bonds of its sites (every bond once, at its owner), the
 // daemon levels of its sites and -- when PAIR (n_replicas == 2, both replicas
 // in the word) -- the lanes where the two replicas differ.  Other replica
-// pairs are counted by count_xor_kernel before this kernel runs.  The last
-// block to finish turns the counts into the measurement row.
+// pairs are counted by count_xor_kernel before this kernel runs.  Per item the
+// bits are compressed by carry-save adder trees; two items' sums are added
+// before they enter the thread's 10-plane vertical counters.  The last block
+// to finish turns the counts into the measurement row.
 // grid = (nblk, n_words), block = kMeasureBlock; 32-bit item indices
-// (half / V < 2^31 because L^3 < 2^32).
+// (half / V < 2^31 because L^3 < 2^31).
 template <int V, int RPW, bool PAIR>
-__global__ void __launch_bounds__(kMeasureBlock, 3)
+__global__ void __launch_bounds__(kMeasureBlock, 2)
 measure_kernel(MeasureArgs a, FinalizeArgs f)
 {
     typedef typename BondT<RPW>::type JT;
@@ -222,48 +314,21 @@ measure_kernel(MeasureArgs a, FinalizeArgs f)
 
     VCount<kMeasurePlanes> accU, accM, accX; accU.clear(); accM.clear(); accX.clear();
     const uint32_t stride = gridDim.x * kMeasureBlock;
-#pragma unroll 2
-    for (uint32_t it = blockIdx.x * kMeasureBlock + threadIdx.x; it < n_items; it += stride) {
-        const uint32_t p = it >= items_p;
-        const uint32_t iv = it - (p ? items_p : 0u);
-        const uint32_t rowi = iv / nxv, xv = iv - rowi * nxv;
-        const uint32_t z = rowi / L, y = rowi - z * L;
-        const uint32_t yp = (y + 1 == L) ? 0 : y + 1, zp = (z + 1 == L) ? 0 : z + 1;
-        const uint32_t xh0 = xv * V;
-        const uint32_t row = rowi * Lh, h = row + xh0;       // < half < 2^31
-        const uint32_t c = (y + z + p) & 1u;      // c=1: +x neighbour at xh+1, else same xh
-        const uint32_t* sp = s0 + (p ? half : 0);
-        const uint32_t* sq = s0 + (p ? 0 : half);
-        const Vec<V> s = ldg_vec<V>(sp + h);
-        const Vec<V> A = ldg_vec<V>(sq + h);
-        const uint32_t e = sq[row + ((xh0 + V == Lh) ? 0 : xh0 + V)];
-        const Vec<V> ny = ldg_vec<V>(sq + (z * L + yp) * Lh + xh0);
-        const Vec<V> nz = ldg_vec<V>(sq + (zp * L + y) * Lh + xh0);
-        const Vec<V> jx = ldg_bonds<V, RPW>(Jb + (0 * 2 + p) * half + h);
-        const Vec<V> jy = ldg_bonds<V, RPW>(Jb + (1 * 2 + p) * half + h);
-        const Vec<V> jz = ldg_bonds<V, RPW>(Jb + (2 * 2 + p) * half + h);
-        const Vec<V> b0 = ldg_vec<V>(d0 + (p ? half : 0) + h);
-        const Vec<V> b1 = ldg_vec<V>(d1 + (p ? half : 0) + h);
-        VCount<4> locU, locM; locU.clear(); locM.clear();
-        VCount<3> locX; locX.clear();
+    for (uint32_t it = blockIdx.x * kMeasureBlock + threadIdx.x; it < n_items; it += 2u * stride) {
+        ItemSums A0, A1;
+        measure_item<V, RPW, PAIR>(A0, it, items_p, nxv, L, Lh, half, s0, d0, d1, Jb);
+        if (it + stride < n_items) {
+            measure_item<V, RPW, PAIR>(A1, it + stride, items_p, nxv, L, Lh, half, s0, d0, d1, Jb);
+        } else {
 #pragma unroll
-        for (int k = 0; k < V; ++k) {
-            const uint32_t up = (k + 1 < V) ? A.v[k + 1] : e;
-            const uint32_t nx = c ? up : A.v[k];
-            const uint32_t ux = s.v[k] ^ nx ^ jx.v[k];
-            const uint32_t uy = s.v[k] ^ ny.v[k] ^ jy.v[k];
-            const uint32_t uz = s.v[k] ^ nz.v[k] ^ jz.v[k];
-            const uint32_t bu[2] = { ux ^ uy ^ uz, maj3(ux, uy, uz) };
-            locU.add(bu);
-            const uint32_t bm[2] = { b0.v[k], b1.v[k] };
-            locM.add(bm);
-            if (PAIR) {
-                const uint32_t bx[1] = { (s.v[k] ^ (s.v[k] >> 16)) & 0xFFFFu };
-                locX.add(bx);
-            }
+            for (int k = 0; k < 4; ++k) { A1.u[k] = 0u; A1.m[k] = 0u; }
+#pragma unroll
+            for (int k = 0; k < 3; ++k) A1.x[k] = 0u;
         }
-        accU.add(locU.c); accM.add(locM.c);
-        if (PAIR) accX.add(locX.c);
+        uint32_t su[5], sm5[5], sx[4];
+        add_planes<4>(A0.u, A1.u, su);  accU.add(su);
+        add_planes<4>(A0.m, A1.m, sm5); accM.add(sm5);
+        if (PAIR) { add_planes<3>(A0.x, A1.x, sx); accX.add(sx); }
     }
     block_warp_lane_counts<kMeasurePlanes, kMeasureBlock>(accU.c, sm, a.cntU + (long long)w * 32);
     block_warp_lane_counts<kMeasurePlanes, kMeasureBlock>(accM.c, sm, a.cntM + (long long)w * 32);

@@ -129,6 +129,7 @@ struct micsa_ctx {
     unsigned long long ticket0;   // value of *task_ticket when the next launch starts
     int progress_base;         // value of every progress entry between launches
     PersistPlan pp;
+    int pipe_planes;           // planes per CTA of the pipelined kernel (1 or 4)
     int use_pdl;               // programmatic dependent launch for the pipelined kernel
     int pipe_rows;             // rows per thread of the pipelined kernel (4 or 8)
     int tile_tz;               // planes per tile of the tiled kernel (2, 4 or 8)
@@ -200,7 +201,9 @@ void launch_half_sweep_pipe(micsa_ctx* c, int parity) {
     a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half;
     const int yc = c->pipe_rows;
     const int per_plane = (c->g.L / yc) * (c->g.Lh / 4);
-    dim3 grid((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
+    const int zw = c->pipe_planes;
+    dim3 grid = (zw == 4) ? dim3((unsigned)((per_plane + 31) / 32), (unsigned)(c->g.L / 4), (unsigned)c->g.n_words)
+                          : dim3((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
     // programmatic dependent launch (the kernel waits with griddepcontrol.wait before
     // its first load): launch latency and ramp overlap the previous grid's tail
     cudaLaunchConfig_t cfg = {};
@@ -209,8 +212,13 @@ void launch_half_sweep_pipe(micsa_ctx* c, int parity) {
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = c->use_pdl ? 1 : 0;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    if (yc == 8) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8>, a, parity);
-    else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4>, a, parity);
+    if (zw == 4) {
+        if (yc == 8) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8, 4>, a, parity);
+        else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4>, a, parity);
+    } else {
+        if (yc == 8) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8, 1>, a, parity);
+        else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1>, a, parity);
+    }
 }
 
 template <int RPW, int TY, int TZ>
@@ -445,11 +453,11 @@ void launch_measure_t(micsa_ctx* c, const MeasureArgs& a, const FinalizeArgs& f)
                                    kCountBlock, 0, c->stream>>>(a);
         c->launches += 1;
     }
-    // three resident blocks per SM over all word lattices, never more than
+    // two resident blocks per SM over all word lattices, never more than
     // kMeasureMaxItems items per thread (10-plane per-thread counters)
     const long long n_items = 2 * g.half / V;
     long long nb = (n_items + (long long)kMeasureBlock * 4 - 1) / ((long long)kMeasureBlock * 4);
-    nb = std::min(nb, std::max<long long>(1, (148 * 3) / g.n_words));
+    nb = std::min(nb, std::max<long long>(1, (148 * 2) / g.n_words));
     const long long need = (n_items + (long long)kMeasureBlock * kMeasureMaxItems - 1) / ((long long)kMeasureBlock * kMeasureMaxItems);
     nb = std::max<long long>(std::max<long long>(nb, need), 1);
     const dim3 grid((unsigned)nb, (unsigned)g.n_words);
@@ -582,6 +590,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->tile_tz = 4;
     c->pipe_rows = 4;
     c->use_pdl = 1;
+    c->pipe_planes = 4;
     c->attempts = c->rns = c->launches = 0;
     c->sticky = 0;
     if (dev_workspace) {
@@ -873,6 +882,9 @@ int micsa_set_tuning(micsa_ctx* c, int key, int value) {
         case MICSA_TUNE_TILE_TZ:
             if (value != 2 && value != 4 && value != 8) { set_err("tile_tz must be 2, 4 or 8"); return MICSA_ERR_INVALID; }
             c->tile_tz = value; return MICSA_OK;
+        case MICSA_TUNE_PIPE_PLANES:
+            if (value != 1 && value != 4) { set_err("pipe_planes must be 1 or 4"); return MICSA_ERR_INVALID; }
+            c->pipe_planes = value; return MICSA_OK;
         case MICSA_TUNE_PDL:
             if (value != 0 && value != 1) { set_err("pdl must be 0 or 1"); return MICSA_ERR_INVALID; }
             c->use_pdl = value; return MICSA_OK;

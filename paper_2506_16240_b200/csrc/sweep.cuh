@@ -487,21 +487,29 @@ __device__ __forceinline__ PipeBase pipe_base(const SweepArgs& a, int w, int p)
     return P;
 }
 
-// grid = (ceil((L/YC)*(Lh/4) / block), L, n_words)
-template <int RPW, int YC>
+// ZW = 1: grid = (ceil((L/YC)*(Lh/4) / 128), L, n_words), a CTA works inside one plane.
+// ZW = 4: grid = (ceil((L/YC)*(Lh/4) / 32), L/4, n_words), warp k of a CTA works on plane
+//         4*blockIdx.y + k with the same (row chunk, quad) items as its sibling warps: the
+//         +-z neighbour rows of a warp are the own-plane rows of the next / previous warp and
+//         are found in the SM's L1 (hit or hit-on-miss) instead of crossing the L2 -> SM path,
+//         which is what bounds this kernel.
+template <int RPW, int YC, int ZW>
 __global__ void __launch_bounds__(128)
 half_sweep_pipe_kernel(SweepArgs a, int p)
 {
     const int L = a.L, Lh = a.Lh;
     const int nxv = Lh >> 2;
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;          // blockDim.x % 32 == 0: idx = t
+    // idx: item index inside the plane; a warp always holds 32 consecutive items of one plane
+    const int t = (ZW == 1) ? (int)(blockIdx.x * blockDim.x + threadIdx.x)
+                            : (int)(blockIdx.x * 32 + (threadIdx.x & 31));
+    const int z = (ZW == 1) ? (int)blockIdx.y : (int)(blockIdx.y * ZW + (threadIdx.x >> 5));
     const bool active = t < (L / YC) * nxv;
     const unsigned mask = __ballot_sync(0xFFFFFFFFu, active);
     if (!active) return;
     const int chunk = t / nxv, xv = t - chunk * nxv;
-    const int z = blockIdx.y, w = blockIdx.z;                     // z is block-uniform: one code path per warp
+    const int w = blockIdx.z;
     const PipeBase P = pipe_base<RPW>(a, w, p);
-    const XNb nb = x_neighbours(t, xv, nxv, mask, true);
+    const XNb nb = x_neighbours(t, xv, nxv, mask, true);          // z is warp-uniform: one code path per warp
     // programmatic dependent launch: this grid may have been scheduled while the
     // previous half-sweep was still draining; its results are needed from here on,
     // and the next grid may be scheduled as soon as every CTA of this one got here

@@ -382,7 +382,8 @@ def test_measure_begin_end(micsa, oracle):
         np.testing.assert_array_equal(Ed, oEd)
 
 
-TUNINGS = [{"sweep_kernel": 2, "pipe_rows": 4, "pdl": 1}, {"sweep_kernel": 0, "tile_tz": 2}, {"sweep_kernel": 0, "tile_tz": 4}, {"sweep_kernel": 0, "tile_tz": 8},
+TUNINGS = [{"sweep_kernel": 2, "pipe_rows": 4, "pdl": 1, "pipe_planes": 4}, {"sweep_kernel": 2, "pipe_rows": 8, "pipe_planes": 4},
+           {"sweep_kernel": 2, "pipe_rows": 4, "pdl": 1, "pipe_planes": 1}, {"sweep_kernel": 0, "tile_tz": 2}, {"sweep_kernel": 0, "tile_tz": 4}, {"sweep_kernel": 0, "tile_tz": 8},
            {"sweep_kernel": 1}, {"sweep_kernel": 2, "pipe_rows": 4}, {"sweep_kernel": 2, "pipe_rows": 8}, {"sweep_kernel": 2, "pipe_rows": 4, "pdl": 0}, {"sweep_kernel": 3}]
 
 
