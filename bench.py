@@ -136,6 +136,8 @@ def main():
     ap.add_argument("--impl", default="micsa", choices=["micsa", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-fuse-measure", action="store_true",
+                    help="A/B: separate measurement kernel instead of counting inside the last sweep")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "micsa" else args.warmup
 
@@ -181,6 +183,8 @@ def main():
     from paper_2506_16240_b200.sharding import sample_offset
     g = micsa.MicSA(L, ns, nr, CFG.seed, sample_offset=sample_offset(rank, ns), device=local_rank,
                     stream=stream)
+    if args.no_fuse_measure:
+        g.set_tuning("fuse_measure", 0)
     info = g.layout_info()
     attempts_step = CFG.attempts_per_sweep * SWEEPS_PER_STEP
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
@@ -190,11 +194,9 @@ def main():
         g.prefetch_refresh(T_RUN, k + 1)        # generated on the side stream under this step's sweeps
         if ev:
             ev[1].record(stream)
-        g.sweep(SWEEPS_PER_STEP)
+        g.sweep_measure(SWEEPS_PER_STEP)        # the last sweep also counts E, E_daemon, q; row D2H queued
         if ev:
             ev[2].record(stream)
-        g.measure_begin()                       # reduction kernel + D2H of the row, queued
-        if ev:
             ev[3].record(stream)
         return g.measure_end()                  # host waits for the row (after the timed region)
 

@@ -177,6 +177,13 @@ int micsa_measure_i64(micsa_ctx *ctx, int64_t *E, int64_t *E_daemon, int64_t *Q)
  * MICSA_ERR_INVALID without a preceding _begin).  The row is the state at the
  * point of _begin in stream order. */
 int micsa_measure_begin(micsa_ctx *ctx);
+/* micsa_sweep_measure(n) == micsa_sweep(n) followed by micsa_measure_begin(),
+ * with the counting done inside the two launches of the last sweep (after a
+ * sweep every bond has exactly one odd end, whose half-sweep holds all its six
+ * bonds in registers), so the state is not read a second time.  Falls back to
+ * the separate measurement kernel when n == 0, n_replicas > 2, L % 8 != 0 or
+ * another sweep kernel is selected.  Same bits either way. */
+int micsa_sweep_measure(micsa_ctx *ctx, int n);
 int micsa_measure_end(micsa_ctx *ctx, int64_t *E, int64_t *E_daemon, int64_t *Q);
 int micsa_measure(micsa_ctx *ctx, double *energy, double *demon_energy,
                   double *q_overlap);
@@ -221,12 +228,14 @@ int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
  * key MICSA_TUNE_PIPE_ROWS: rows per thread of kernel 2: 4 (default) or 8.
  * key MICSA_TUNE_PIPE_PLANES: lattice planes per CTA of kernel 2 (one warp
  *   each): 4 (default) or 1.
+ * key MICSA_TUNE_FUSE_MEASURE: 1 (default) = micsa_sweep_measure and micsa_anneal count
+ *   the observables inside the last sweep, 0 = separate measurement kernel.
  * key MICSA_TUNE_PDL: 1 (default) = kernel 2 is launched with programmatic
  *   stream serialization (the next half-sweep's grid is scheduled while this
  *   one drains and waits on the device for its completion), 0 = plain launches.
  * Unknown key or value: MICSA_ERR_INVALID, nothing changes. */
 enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_TILE_TZ = 1, MICSA_TUNE_PIPE_ROWS = 2, MICSA_TUNE_PDL = 3,
-       MICSA_TUNE_PIPE_PLANES = 4 };
+       MICSA_TUNE_PIPE_PLANES = 4, MICSA_TUNE_FUSE_MEASURE = 5 };
 int micsa_set_tuning(micsa_ctx *ctx, int key, int value);
 
 #ifdef __cplusplus

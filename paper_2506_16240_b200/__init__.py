@@ -31,7 +31,7 @@ EXPORTS = (
     "micsa_refresh_demons", "micsa_debug_thresholds", "micsa_measure_i64",
     "micsa_measure", "micsa_anneal", "micsa_counters", "micsa_layout_info",
     "micsa_set_tuning",
-    "micsa_prefetch_refresh", "micsa_measure_begin", "micsa_measure_end",
+    "micsa_prefetch_refresh", "micsa_measure_begin", "micsa_measure_end", "micsa_sweep_measure",
 )
 
 
@@ -89,7 +89,7 @@ def _bind() -> ctypes.CDLL:
             ("micsa_destroy", [vp]), ("micsa_synchronize", [vp]),
             ("micsa_set_couplings", [vp, vp]), ("micsa_set_spins", [vp, vp]),
             ("micsa_set_daemons", [vp, vp]), ("micsa_get_state", [vp, vp, vp, vp]),
-            ("micsa_sweep", [vp, i32]), ("micsa_half_sweep", [vp, i32]),
+            ("micsa_sweep", [vp, i32]), ("micsa_sweep_measure", [vp, i32]), ("micsa_half_sweep", [vp, i32]),
             ("micsa_refresh_demons", [vp, f64, u32]),
             ("micsa_prefetch_refresh", [vp, f64, u32]),
             ("micsa_debug_thresholds", [f64, vp]),
@@ -215,6 +215,10 @@ class MicSA:
     def sweep(self, n=1):
         _check(_lib.micsa_sweep(self._h, int(n)))
 
+    def sweep_measure(self, n=1):
+        """n sweeps, then the measurement queued (fetch it with measure_end)."""
+        _check(_lib.micsa_sweep_measure(self._h, int(n)))
+
     def half_sweep(self, parity):
         _check(_lib.micsa_half_sweep(self._h, int(parity)))
 
@@ -286,8 +290,8 @@ class MicSA:
 
     def set_tuning(self, key, value):
         """micsa_set_tuning: 'sweep_kernel' (0 tiled, 1 row-marching, 2 pipelined
-        row-marching, 3 persistent), 'tile_tz' (2, 4, 8), 'pipe_rows' (4, 8), 'pdl' (0, 1) or 'pipe_planes' (1, 4)."""
-        k = {"sweep_kernel": 0, "tile_tz": 1, "pipe_rows": 2, "pdl": 3, "pipe_planes": 4}[key]
+        row-marching, 3 persistent), 'tile_tz' (2, 4, 8), 'pipe_rows' (4, 8), 'pdl' (0, 1), 'pipe_planes' (1, 4) or 'fuse_measure' (0, 1)."""
+        k = {"sweep_kernel": 0, "tile_tz": 1, "pipe_rows": 2, "pdl": 3, "pipe_planes": 4, "fuse_measure": 5}[key]
         _check(_lib.micsa_set_tuning(self._h, k, int(value)))
 
     def layout_info(self):

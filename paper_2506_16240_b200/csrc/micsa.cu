@@ -129,6 +129,7 @@ struct micsa_ctx {
     unsigned long long ticket0;   // value of *task_ticket when the next launch starts
     int progress_base;         // value of every progress entry between launches
     PersistPlan pp;
+    int fuse_measure;          // count the observables inside the last sweep of a measured group
     int pipe_planes;           // planes per CTA of the pipelined kernel (1 or 4)
     int use_pdl;               // programmatic dependent launch for the pipelined kernel
     int pipe_rows;             // rows per thread of the pipelined kernel (4 or 8)
@@ -467,21 +468,25 @@ void launch_measure_t(micsa_ctx* c, const MeasureArgs& a, const FinalizeArgs& f)
 
 // one measurement: exact sums into the device row `row`, optional min fold.
 // The counters are zero on entry (create, and the finalising block re-zeroes).
-int launch_measure(micsa_ctx* c, long long* row, bool fold_min) {
+void make_measure_args(micsa_ctx* c, long long* row, bool fold_min, MeasureArgs& a, FinalizeArgs& f) {
     const Geom& g = c->g;
-    if (g.n_replicas * (g.n_replicas - 1) / 2 > 65535) { set_err("too many replica pairs"); return MICSA_ERR_INVALID; }
-    MeasureArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
     a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg; a.n_replicas = g.n_replicas; a.n_samples = g.n_samples;
     a.half = g.half;
     a.cntU = c->cnt; a.cntM = c->cnt + (size_t)g.n_words * 32; a.cntX = c->cnt + (size_t)g.n_words * 64;
-    FinalizeArgs f;
     f.cntU = a.cntU; f.cntM = a.cntM; f.cntX = a.cntX;
     f.cnt_words = (long long)c->plan.cnt_words; f.ticket = c->ticket;
     f.row = row; f.min_E = fold_min ? c->minE : nullptr;
     f.n_samples = g.n_samples; f.n_replicas = g.n_replicas; f.n_rg = g.n_rg;
     f.rpw = g.rpw; f.spw = g.spw; f.pairs_per_sample = g.n_replicas * (g.n_replicas - 1) / 2;
     f.N = g.N;
+}
+
+int launch_measure(micsa_ctx* c, long long* row, bool fold_min) {
+    const Geom& g = c->g;
+    if (g.n_replicas * (g.n_replicas - 1) / 2 > 65535) { set_err("too many replica pairs"); return MICSA_ERR_INVALID; }
+    MeasureArgs a; FinalizeArgs f;
+    make_measure_args(c, row, fold_min, a, f);
     switch (c->V * 10 + g.rpw) {
         case 41: launch_measure_t<4, 1>(c, a, f); break;
         case 42: launch_measure_t<4, 2>(c, a, f); break;
@@ -491,6 +496,49 @@ int launch_measure(micsa_ctx* c, long long* row, bool fold_min) {
         default: launch_measure_t<1, 2>(c, a, f); break;
     }
     return post_launch(c);
+}
+
+// The last sweep of a measured group with the counting fused into its two launches
+// (sweep.cuh, MeasAcc): the state is not read again for the observables.
+template <int RPW>
+int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min) {
+    const Geom& g = c->g;
+    SweepArgs a;
+    a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
+    a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg; a.half = g.half;
+    MeasureArgs ma; FinalizeArgs fa;
+    make_measure_args(c, row, fold_min, ma, fa);
+    const int per_plane = (g.L / 4) * (g.Lh / 4);
+    const int zw = c->pipe_planes;
+    dim3 grid = (zw == 4) ? dim3((unsigned)((per_plane + 31) / 32), (unsigned)(g.L / 4), (unsigned)g.n_words)
+                          : dim3((unsigned)((per_plane + 127) / 128), (unsigned)g.L, (unsigned)g.n_words);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = c->use_pdl ? 1 : 0;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (zw == 4) {
+        cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 1>, a, 0, ma, fa);
+        cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2>, a, 1, ma, fa);
+    } else {
+        cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 1>, a, 0, ma, fa);
+        cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2>, a, 1, ma, fa);
+    }
+    c->attempts += (uint64_t)g.N * (uint64_t)g.n_sys;
+    return post_launch(c, 2);
+}
+
+// n sweeps, then one measurement into `row`
+int launch_sweeps_measured(micsa_ctx* c, int n, long long* row, bool fold_min) {
+    const Geom& g = c->g;
+    const bool fused = n >= 1 && c->fuse_measure && c->V == 4 && c->sweep_kernel == 2 && g.n_replicas <= 2;
+    if (!fused) {
+        const int rc = launch_sweeps(c, n); if (rc) return rc;
+        return launch_measure(c, row, fold_min);
+    }
+    const int rc = launch_sweeps(c, n - 1); if (rc) return rc;
+    return (g.rpw == 2) ? launch_measuring_sweep<2>(c, row, fold_min) : launch_measuring_sweep<1>(c, row, fold_min);
 }
 
 // host <-> device staging for the canonical layouts
@@ -591,6 +639,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->pipe_rows = 4;
     c->use_pdl = 1;
     c->pipe_planes = 4;
+    c->fuse_measure = 1;
     c->attempts = c->rns = c->launches = 0;
     c->sticky = 0;
     if (dev_workspace) {
@@ -753,6 +802,15 @@ int micsa_measure_begin(micsa_ctx* c) {
     return MICSA_OK;
 }
 
+int micsa_sweep_measure(micsa_ctx* c, int n) {
+    int rc = check_ctx(c); if (rc) return rc;
+    if (n < 0) { set_err("n must be >= 0"); return MICSA_ERR_INVALID; }
+    rc = launch_sweeps_measured(c, n, c->row, false); if (rc) return rc;
+    CK(c, cudaMemcpyAsync(c->host_row, c->row, c->plan.row_len * 8, cudaMemcpyDeviceToHost, c->stream));
+    c->measure_queued = true;
+    return MICSA_OK;
+}
+
 int micsa_measure_end(micsa_ctx* c, int64_t* E, int64_t* Ed, int64_t* Q) {
     int rc = check_ctx(c); if (rc) return rc;
     const Geom& g = c->g;
@@ -824,13 +882,14 @@ int micsa_anneal(micsa_ctx* c, const micsa_step* sched, int n_steps, uint32_t st
         const int me = sched[k].measure_every;
         for (int j = 0; j < sched[k].n_sweeps; ) {
             const int group = (me > 0) ? std::min(me - j % me, sched[k].n_sweeps - j) : sched[k].n_sweeps - j;
-            rc = launch_sweeps(c, group); if (rc) return rc;
             j += group; t += group;
             if (me > 0 && j % me == 0) {
                 long long* dst = (r < keep) ? (long long*)dev_rows.dev + (size_t)r * row_len : c->row;
-                rc = launch_measure(c, dst, true); if (rc) return rc;
+                rc = launch_sweeps_measured(c, group, dst, true); if (rc) return rc;
                 if (r < keep) { row_sweep.push_back(t); row_T.push_back(sched[k].T); }
                 ++r;
+            } else {
+                rc = launch_sweeps(c, group); if (rc) return rc;
             }
         }
     }
@@ -885,6 +944,9 @@ int micsa_set_tuning(micsa_ctx* c, int key, int value) {
         case MICSA_TUNE_PIPE_PLANES:
             if (value != 1 && value != 4) { set_err("pipe_planes must be 1 or 4"); return MICSA_ERR_INVALID; }
             c->pipe_planes = value; return MICSA_OK;
+        case MICSA_TUNE_FUSE_MEASURE:
+            if (value != 0 && value != 1) { set_err("fuse_measure must be 0 or 1"); return MICSA_ERR_INVALID; }
+            c->fuse_measure = value; return MICSA_OK;
         case MICSA_TUNE_PDL:
             if (value != 0 && value != 1) { set_err("pdl must be 0 or 1"); return MICSA_ERR_INVALID; }
             c->use_pdl = value; return MICSA_OK;

@@ -7,6 +7,7 @@
 // iff 3 <= m + U <= 6 and then m <- m + U - 3.
 #pragma once
 #include "layout.cuh"
+#include "measure.cuh"
 
 namespace micsa {
 
@@ -368,9 +369,54 @@ template <int RPW> __device__ __forceinline__ uint32_t last_bond_word(const type
 template <> __device__ __forceinline__ uint32_t last_bond_word<2>(const uint2& j) { return j.y >> 16; }
 template <> __device__ __forceinline__ uint32_t last_bond_word<1>(const uint4& j) { return j.w; }
 
-template <int RPW, int C>
+// ---- measurement fused into the last sweep of a group ----
+// After a sweep every bond has exactly one odd end, and the odd half-sweep has
+// all six bonds of each odd site in registers: the unsatisfied bonds after its
+// update, summed over the odd sites, are U_tot of Eq. (1).  Daemon levels and
+// replica differences of a site are final once its own half-sweep of the last
+// sweep has passed.  So the even launch of the last sweep adds the levels and
+// differences of the even sites (MEAS = 1), the odd launch those of the odd
+// sites plus all unsatisfied bonds (MEAS = 2) and its last CTA writes the row;
+// the state is not read again.
+template <int YC> struct MeasAcc {            // per-thread vertical counters over YC rows x 4 words
+    static constexpr int PU = (YC <= 4) ? 7 : 8;     // <= 24 * YC unsatisfied bonds per lane
+    static constexpr int PM = (YC <= 4) ? 6 : 7;     // <= 12 * YC level units
+    static constexpr int PX = (YC <= 4) ? 5 : 6;     // <=  4 * YC differing sites
+    VCount<PU> u; VCount<PM> m; VCount<PX> x;
+    __device__ __forceinline__ void clear() { u.clear(); m.clear(); x.clear(); }
+};
+
+// lane-wise sum of 6 flags for each of 4 words -> 5 planes (<= 24)
+__device__ __forceinline__ void count6x4(const uint32_t (&f)[6][4], uint32_t (&o)[5]) {
+    uint32_t sa[4], ca[4], sb[4], cb[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        full_add(f[0][k], f[1][k], f[2][k], sa[k], ca[k]);
+        full_add(f[3][k], f[4][k], f[5][k], sb[k], cb[k]);
+    }
+    uint32_t p0, p1, p2, q0, q1, q2, q3;                     // weight 1: sa, sb
+    full_add(sa[0], sa[1], sa[2], p0, q0);
+    full_add(sa[3], sb[0], sb[1], p1, q1);
+    full_add(sb[2], sb[3], p0, p2, q2);
+    half_add(p1, p2, o[0], q3);
+    uint32_t r0, r1, r2, r3, r4, t0, t1, t2, t3, t4, t5;     // weight 2: ca, cb, q
+    full_add(ca[0], ca[1], ca[2], r0, t0);
+    full_add(ca[3], cb[0], cb[1], r1, t1);
+    full_add(cb[2], cb[3], q0, r2, t2);
+    full_add(q1, q2, q3, r3, t3);
+    full_add(r0, r1, r2, r4, t4);
+    half_add(r4, r3, o[1], t5);
+    uint32_t v0, v1, x0, x1, x2;                             // weight 4: t
+    full_add(t0, t1, t2, v0, x0);
+    full_add(t3, t4, t5, v1, x1);
+    half_add(v0, v1, o[2], x2);
+    full_add(x0, x1, x2, o[3], o[4]);                        // weight 8, 16
+}
+
+template <int RPW, int C, int MEAS, int YC>
 __device__ __forceinline__ void update_row(const RowRegs<RPW>& r, const uint4& Aprev, const uint4& Acur,
-                                           const PipeBase& P, uint32_t o, const XNb& nb)
+                                           const PipeBase& P, uint32_t o, const XNb& nb,
+                                           MeasAcc<YC>* acc, bool pair)
 {
     typedef Bond4<RPW> B4;
     uint32_t jxo[4], jyo[4], jzo[4], jxm[4], jym[4], jzm[4], Bx[4];
@@ -410,12 +456,38 @@ __device__ __forceinline__ void update_row(const RowRegs<RPW>& r, const uint4& A
     st_off<uint4>(P.sp, o, make_uint4(sv[0], sv[1], sv[2], sv[3]));
     st_off<uint4>(P.m0, o, make_uint4(v0[0], v0[1], v0[2], v0[3]));
     st_off<uint4>(P.m1, o, make_uint4(v1[0], v1[1], v1[2], v1[3]));
+    if (MEAS) {
+        uint32_t pm[4];
+        csa_4x1_4x2(v0, v1, pm);                              // levels after the update
+        acc->m.add(pm);
+        if (RPW == 2 && pair) {                               // lanes where the two replicas of a sample differ
+            uint32_t xs[4], a2, b2, b3, px[3];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) xs[k] = (sv[k] ^ (sv[k] >> 16)) & 0xFFFFu;
+            full_add(xs[0], xs[1], xs[2], a2, b2);
+            half_add(a2, xs[3], px[0], b3);
+            px[1] = b2 ^ b3; px[2] = b2 & b3;
+            acc->x.add(px);
+        }
+        if (MEAS == 2) {                                      // bonds of these sites that are unsatisfied NOW
+            uint32_t f[6][4], pu[5];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const uint32_t g = sv[k];
+                f[0][k] = g ^ nxp[k] ^ jxo[k]; f[1][k] = g ^ nxm[k] ^ jxm[k];
+                f[2][k] = g ^ yp[k] ^ jyo[k];  f[3][k] = g ^ ym[k] ^ jym[k];
+                f[4][k] = g ^ zp[k] ^ jzo[k];  f[5][k] = g ^ zm[k] ^ jzm[k];
+            }
+            count6x4(f, pu);
+            acc->u.add(pu);
+        }
+    }
 }
 
 // rows y0 .. y0+YC-1 of plane z (y0 % YC == 0, YC even, L % YC == 0), words xh0 .. xh0+3
-template <int RPW, int YC, int F>
+template <int RPW, int YC, int F, int MEAS = 0>
 __device__ __forceinline__ void march_rows_pipe(const PipeBase& P, int L, int Lh, int z, int y0, int xh0,
-                                                const XNb& nb)
+                                                const XNb& nb, MeasAcc<YC>* acc = nullptr, bool pair = false)
 {
     const uint32_t rowB = (uint32_t)Lh * 4u;
     const uint32_t planeB = (uint32_t)L * rowB;
@@ -446,8 +518,8 @@ __device__ __forceinline__ void march_rows_pipe(const PipeBase& P, int L, int Lh
             if ((iy & 1) ^ F) load_row<RPW, 0>(nxt, P, o_next, o, o_next2, x4, xe_up, xe_dn, dzp, dzm, nb);
             else              load_row<RPW, 1>(nxt, P, o_next, o, o_next2, x4, xe_up, xe_dn, dzp, dzm, nb);
         }
-        if ((iy & 1) ^ F) update_row<RPW, 1>(cur, Aprev, Acur, P, o, nb);
-        else              update_row<RPW, 0>(cur, Aprev, Acur, P, o, nb);
+        if ((iy & 1) ^ F) update_row<RPW, 1, MEAS, YC>(cur, Aprev, Acur, P, o, nb, acc, pair);
+        else              update_row<RPW, 0, MEAS, YC>(cur, Aprev, Acur, P, o, nb, acc, pair);
         Aprev = Acur; Acur = cur.An;
         if (iy + 1 < YC) cur = nxt;
         o_prev = o; o = o_next;
@@ -517,6 +589,57 @@ half_sweep_pipe_kernel(SweepArgs a, int p)
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if ((z + p) & 1) march_rows_pipe<RPW, YC, 1>(P, L, Lh, z, chunk * YC, xv * 4, nb);
     else             march_rows_pipe<RPW, YC, 0>(P, L, Lh, z, chunk * YC, xv * 4, nb);
+}
+
+// The two launches of the LAST sweep of a measured group: same update, plus the
+// counting described above MeasAcc.  MEAS = 1: even launch (levels, replica
+// differences); MEAS = 2: odd launch (also unsatisfied bonds) whose last CTA turns
+// the counts into the measurement row (finalize_rows) and re-zeroes them.
+// Same grids as half_sweep_pipe_kernel<RPW, 4, ZW>; every thread stays for the
+// block-wide reduction.
+template <int RPW, int ZW, int MEAS>
+__global__ void __launch_bounds__(128, 4)
+half_sweep_pipe_meas_kernel(SweepArgs a, int p, MeasureArgs ma, FinalizeArgs fa)
+{
+    constexpr int YC = 4;
+    __shared__ unsigned int s_cnt[32];
+    __shared__ unsigned int s_last;
+    const int L = a.L, Lh = a.Lh;
+    const int nxv = Lh >> 2;
+    const int t = (ZW == 1) ? (int)(blockIdx.x * blockDim.x + threadIdx.x)
+                            : (int)(blockIdx.x * 32 + (threadIdx.x & 31));
+    const int z = (ZW == 1) ? (int)blockIdx.y : (int)(blockIdx.y * ZW + (threadIdx.x >> 5));
+    const bool active = t < (L / YC) * nxv;
+    const unsigned mask = __ballot_sync(0xFFFFFFFFu, active);
+    const int w = blockIdx.z;
+    const bool pair = (RPW == 2) && ma.n_replicas == 2;
+    MeasAcc<YC> acc; acc.clear();
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (active) {
+        const int chunk = t / nxv, xv = t - chunk * nxv;
+        const PipeBase P = pipe_base<RPW>(a, w, p);
+        const XNb nb = x_neighbours(t, xv, nxv, mask, true);
+        if ((z + p) & 1) march_rows_pipe<RPW, YC, 1, MEAS>(P, L, Lh, z, chunk * YC, xv * 4, nb, &acc, pair);
+        else             march_rows_pipe<RPW, YC, 0, MEAS>(P, L, Lh, z, chunk * YC, xv * 4, nb, &acc, pair);
+    }
+    if (MEAS == 2) block_warp_lane_counts<MeasAcc<YC>::PU, 128>(acc.u.c, s_cnt, ma.cntU + (long long)w * 32);
+    block_warp_lane_counts<MeasAcc<YC>::PM, 128>(acc.m.c, s_cnt, ma.cntM + (long long)w * 32);
+    if (pair) block_warp_lane_counts<MeasAcc<YC>::PX, 128>(acc.x.c, s_cnt, ma.cntX + (long long)(w / a.n_rg) * 32);
+    if (MEAS == 2) {
+        // the last block to arrive finalises (its reads see every block's atomics)
+        __threadfence();
+        if (threadIdx.x == 0) {
+            const unsigned int total = gridDim.x * gridDim.y * gridDim.z;
+            s_last = (atomicAdd(fa.ticket, 1u) == total - 1u);
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            finalize_rows(fa);
+            if (threadIdx.x == 0) *fa.ticket = 0u;
+        }
+    }
 }
 
 }  // namespace micsa

@@ -416,3 +416,30 @@ def test_every_sweep_kernel_gives_the_same_bits(micsa, oracle, L, ns, nr):
             _assert_state(g, s2, m2)
         with pytest.raises(micsa.MicsaError):
             g.set_tuning("pipe_rows", 5)
+
+
+@pytest.mark.parametrize("L,ns,nr", [(8, 40, 2), (8, 33, 1), (16, 17, 2), (24, 2, 2), (32, 3, 3), (6, 5, 2), (32, 20, 2)])
+def test_sweep_measure_fused_equals_separate(micsa, oracle, L, ns, nr):
+    """micsa_sweep_measure: the observables counted inside the last sweep equal
+    the oracle's on the swept state, under every kernel mapping, and the
+    separate kernel gives the same row (fuse_measure 0, fallbacks)."""
+    N = L ** 3
+    s, J, m = random_pm1((ns, nr, N), 51), random_pm1((ns, 3, N), 52), random_levels((ns, nr, N), 53)
+    with micsa.MicSA(L, ns, nr, 1) as g:
+        g.set_spins(s); g.set_daemons(m); g.set_couplings(J)
+        for n, tune in [(1, {}), (3, {"pipe_planes": 1}), (2, {"pipe_planes": 4, "pdl": 0}), (2, {"fuse_measure": 0}),
+                        (0, {"fuse_measure": 1}), (2, {"sweep_kernel": 1}), (1, {"sweep_kernel": 2, "pipe_rows": 8})]:
+            for k, v in tune.items():
+                g.set_tuning(k, v)
+            g.sweep_measure(n)
+            E, Ed, Q = g.measure_end()
+            oracle.sweep(L, s, m, J, n)
+            oE, oEd, oQ = oracle.measure(L, s, m, J)
+            np.testing.assert_array_equal(E, oE)
+            np.testing.assert_array_equal(Ed, oEd)
+            np.testing.assert_array_equal(Q, oQ)
+            _assert_state(g, s, m)
+            E2, Ed2, Q2 = g.measure_i64()            # the separate kernel on the same state
+            np.testing.assert_array_equal(E2, oE)
+            np.testing.assert_array_equal(Ed2, oEd)
+            np.testing.assert_array_equal(Q2, oQ)
