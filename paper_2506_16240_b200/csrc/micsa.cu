@@ -638,7 +638,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->tile_tz = 4;
     c->pipe_rows = 4;
     c->use_pdl = 1;
-    c->pipe_planes = 4;
+    c->pipe_planes = (g.n_words == 1 && (g.L / 4) * (g.Lh / 4) >= 512) ? 4 : 1;   // measured: DESIGN.md 6.1
     c->fuse_measure = 1;
     c->attempts = c->rns = c->launches = 0;
     c->sticky = 0;
