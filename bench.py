@@ -39,10 +39,10 @@ T_RUN = CFG.temperatures[0]
 METRIC = "spin-flip attempts/ns (refresh + 10 sweeps + measure per step)"
 UNIT = "attempts/ns"
 # dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch from the
-# ncu --set full capture summarised in profiles/r1b_half_sweep_pipe_full.md
+# ncu --set full capture summarised in profiles/r1c_final_launches_and_sweep.md
 # (cold L2: ncu flushes caches before every replay; in a real step the 73.7 MB
 # state stays in the 126 MB L2 after the first sweep)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 57_378_560 + 282_112
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 57_401_600 + 172_288
 
 
 def measured_peaks():
@@ -54,7 +54,10 @@ def measured_peaks():
 
 
 class ClockSampler(threading.Thread):
-    """nvidia-smi clocks / throttle reasons during the timed region."""
+    """SM clock and throttle reasons during the timed region, sampled through
+    NVML in-process every 2 ms (spawning nvidia-smi from a thread steals the
+    launching thread's CPU and shows up as GPU idle time in a 0.3 ms step);
+    falls back to nvidia-smi when the NVML binding is missing."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -62,19 +65,44 @@ class ClockSampler(threading.Thread):
     def __init__(self, index):
         super().__init__(daemon=True)
         self.index, self.rows, self._stop_evt = index, [], threading.Event()
+        self.nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            # NVML indices follow the PCI order; honour CUDA_VISIBLE_DEVICES when it is a plain list
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+            ids = [int(x) for x in vis.split(",")] if vis and all(x.strip().isdigit() for x in vis.split(",")) else None
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(ids[index] if ids else index)
+            self.nvml = pynvml
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nvml = None
+
+    def _sample_nvml(self):
+        n = self.nvml
+        sm = float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM))
+        r = int(n.nvmlDeviceGetCurrentClocksEventReasons(self.handle)) \
+            if hasattr(n, "nvmlDeviceGetCurrentClocksEventReasons") \
+            else int(n.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle))
+        flags = [("hw_slowdown", 0x8), ("hw_thermal_slowdown", 0x40), ("sw_thermal_slowdown", 0x20),
+                 ("sw_power_cap", 0x4)]
+        self.rows.append([str(sm), str(self.sm_max)] + ["Active" if r & bit else "Not Active" for _, bit in flags])
 
     def run(self):
-        while not self._stop_evt.is_set():
+        while not self._stop_evt.is_set() and not os.environ.get('MICSA_NO_SAMPLER'):
             try:
-                out = subprocess.run(
-                    ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                     "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
-                f = [x.strip() for x in out.strip().split(",")]
-                if len(f) >= 6:
-                    self.rows.append(f)
+                if self.nvml is not None:
+                    self._sample_nvml()
+                else:
+                    out = subprocess.run(
+                        ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                         "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                    f = [x.strip() for x in out.strip().split(",")]
+                    if len(f) >= 6:
+                        self.rows.append(f)
             except Exception:
                 pass
-            self._stop_evt.wait(0.2)
+            self._stop_evt.wait(0.002 if self.nvml is not None else 0.2)
 
     def stop(self):
         self._stop_evt.set()
@@ -84,7 +112,8 @@ class ClockSampler(threading.Thread):
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         reasons = sorted({names[i] for r in self.rows for i in range(4) if r[2 + i].lower() == "active"})
         return {"sm_mhz": float(np.median(sm)) if sm else None,
-                "sm_max_mhz": max(mx) if mx else None, "reasons": reasons, "samples": len(self.rows)}
+                "sm_max_mhz": max(mx) if mx else None, "reasons": reasons, "samples": len(self.rows),
+                "source": "nvml" if self.nvml is not None else "nvidia-smi"}
 
 
 def oracle_step_rate(n_samples, steps, warmup):
@@ -131,7 +160,7 @@ def run_reference(args, rank):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="micsa", choices=["micsa", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -194,9 +223,11 @@ def main():
         g.prefetch_refresh(T_RUN, k + 1)        # generated on the side stream under this step's sweeps
         if ev:
             ev[1].record(stream)
-        g.sweep_measure(SWEEPS_PER_STEP)        # the last sweep also counts E, E_daemon, q; row D2H queued
+        g.sweep(SWEEPS_PER_STEP - 1)            # 18 plain half-sweep launches: the roofline kernel
         if ev:
             ev[2].record(stream)
+        g.sweep_measure(1)                      # the last sweep also counts E, E_daemon, q; row D2H queued
+        if ev:
             ev[3].record(stream)
         return g.measure_end()                  # host waits for the row (after the timed region)
 
@@ -235,18 +266,20 @@ def main():
 
     # roofline of the dominant kernel (half-sweep), live from the timed region
     peak, peak_src = measured_peaks()
-    n_launch = 2 * SWEEPS_PER_STEP * args.steps
+    n_launch = 2 * (SWEEPS_PER_STEP - 1) * args.steps        # the plain launches between events 1 and 2
     t_launch_s = t_sweep_ms * 1e-3 / n_launch
     alg_bytes = info["compulsory_bytes_per_sweep"] / 2          # per half-sweep launch
     achieved = alg_bytes / t_launch_s / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
-                "kernel": "half_sweep_pipe_kernel<2,4>", "peak_source": peak_src,
+                "kernel": "half_sweep_pipe_kernel<2,4,4>", "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "us_per_launch": t_launch_s * 1e6,
                 "convention": "compulsory one-pass traffic: 7.5 bits/attempt (spin 1r+1w, daemon 2r+2w, "
                               "bonds 1.5r shared by the replica pair)",
-                "sweep_share_of_step": t_sweep_ms_max / t_step_ms}
+                "sweep_share_of_step": t_sweep_ms_max / t_step_ms,
+                "note": "share = the 18 plain half-sweep launches of a step; the 2 launches of the last sweep "
+                        "also do the measurement and are timed with the rest of the step"}
 
     # end to end through the C ABI with host buffers
     e2e = None
