@@ -131,6 +131,25 @@ def sweep(L, s, m, J, n_sweeps=1) -> None:
                        _p(J, _c_i8p))
 
 
+def wander(L, m, axis=0, sign=+1, parity=0) -> None:
+    """One half of the wandering cycle: walkers on sites of
+    `parity` exchange with their neighbour along sign * axis, in place."""
+    ns, nr, N = m.shape
+    assert N == L ** 3 and m.dtype == np.uint8 and m.flags.c_contiguous
+    assert axis in (0, 1, 2) and sign in (-1, 1) and parity in (0, 1)
+    lib().oracle_wander(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr), ctypes.c_int(axis),
+                        ctypes.c_int(sign), ctypes.c_int(parity), _p(m, _c_u8p))
+
+
+def timesteps_walkers(L, s, m, J, n_steps=1, t0=0) -> None:
+    """n timesteps with one forward-X walker per spin:
+    sweep, then the wandering half-cycle of parity t mod 2, t = t0, t0+1, ..."""
+    ns, nr, _ = _check(L, s, m, J)
+    lib().oracle_timesteps_walkers(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr),
+                                   ctypes.c_int(n_steps), ctypes.c_int64(t0),
+                                   _p(s, _c_i8p), _p(m, _c_u8p), _p(J, _c_i8p))
+
+
 def thresholds(T: float) -> np.ndarray:
     """Integer thresholds of the cumulative Eq. (11) (R7)."""
     thr = np.zeros(3, dtype=np.uint64)

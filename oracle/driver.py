@@ -15,12 +15,15 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import measure, refresh, sweep
+from . import measure, refresh, sweep, timesteps_walkers
 
 
-def anneal(L, s, m, J, seed, schedule, step0=0, sample_offset=0):
+def anneal(L, s, m, J, seed, schedule, step0=0, sample_offset=0, walkers=False, t0=0):
     """Run the schedule in place on (s, m).  Returns a dict with the exact
-    integer sums of every measurement row and the running minimum of E/N."""
+    integer sums of every measurement row and the running minimum of E/N.
+    walkers=True: one forward-X walker per spin instead of a daemon -- after
+    every sweep the wandering half-cycle of parity t mod 2 (PAPER.md:200,
+    :215), t = t0 + sweeps done; a refresh does not reset t."""
     ns, nr, N = s.shape
     rows = {"sweep": [], "T": [], "E": [], "Edem": [], "Q": []}
     min_e = np.full(ns * nr, np.inf)
@@ -28,7 +31,10 @@ def anneal(L, s, m, J, seed, schedule, step0=0, sample_offset=0):
     for k, (T, n_sweeps, every) in enumerate(schedule):
         refresh(L, m, seed, T, step0 + k, sample_offset)
         for j in range(1, n_sweeps + 1):
-            sweep(L, s, m, J, 1)
+            if walkers:
+                timesteps_walkers(L, s, m, J, 1, t0 + t)
+            else:
+                sweep(L, s, m, J, 1)
             t += 1
             if every > 0 and j % every == 0:
                 E, Ed, Q = measure(L, s, m, J)

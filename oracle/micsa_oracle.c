@@ -32,6 +32,8 @@
  *                      agreement with the independent Metropolis oracle
  *   measure            vs an independent numpy (np.roll) evaluation of Eq. (1)
  *   thresholds/refresh histogram vs Eq. (11), mean vs Eq. (12) closed forms
+ *   wander             period L, involution, conservation, 2x2x2
+ *                      Boltzmann average with walkers
  * Unpinned by the paper: low-temperature quench curves (configs 3, 4) and the
  * final annealed energies (config 5) -- see DESIGN.md "parity unpinned".
  */
@@ -204,6 +206,51 @@ void oracle_sweep(int L, int n_samples, int n_replicas, int n_sweeps,
     for (int t = 0; t < n_sweeps; ++t) {
         oracle_half_sweep(L, n_samples, n_replicas, 0, s, m, J, NULL, NULL);
         oracle_half_sweep(L, n_samples, n_replicas, 1, s, m, J, NULL, NULL);
+    }
+}
+
+/* ------------------------------------------------------------------ */
+/* NEXT-1  Walkers (Sec. 2.6).  One half of the        */
+/* two-timestep wandering cycle along axis d (0,1,2 = X,Y,Z), direction  */
+/* sign (+1 forward, -1 backward): every walker sitting on a site of the */
+/* given lattice parity exchanges its value with the walker on that      */
+/* site's nearest neighbour along sign*d (periodic; the neighbour has    */
+/* the other parity, L even).  PAPER.md:172-174: even sites exchange at  */
+/* the first timestep of a cycle, odd sites at the second.  Spins are    */
+/* not touched.                                                          */
+/* ------------------------------------------------------------------ */
+void oracle_wander(int L, int n_samples, int n_replicas, int axis, int sign,
+                   int parity, uint8_t *m)
+{
+    const int64_t N = (int64_t)L * L * L;
+    const int n_sys = n_samples * n_replicas;
+    for (int sys = 0; sys < n_sys; ++sys) {
+        uint8_t *mm = m + (int64_t)sys * N;
+        for (int z = 0; z < L; ++z)
+            for (int y = 0; y < L; ++y)
+                for (int x = 0; x < L; ++x) {
+                    if (((x + y + z) & 1) != parity) continue;
+                    const int xn = (axis == 0) ? wrap(x + sign, L) : x;
+                    const int yn = (axis == 1) ? wrap(y + sign, L) : y;
+                    const int zn = (axis == 2) ? wrap(z + sign, L) : z;
+                    const int64_t i = x + (int64_t)L * (y + (int64_t)L * z);
+                    const int64_t j = xn + (int64_t)L * (yn + (int64_t)L * zn);
+                    const uint8_t tmp = mm[i]; mm[i] = mm[j]; mm[j] = tmp;
+                }
+    }
+}
+
+/* Timesteps with gamma = 1 walker per spin, forward-X wandering          */
+/* (Sec. 2.8.1 step 3): each step = one sweep,     */
+/* then the half of the wandering cycle dictated by the parity of the     */
+/* time index t (even t: walkers on even sites exchange), then t += 1.    */
+void oracle_timesteps_walkers(int L, int n_samples, int n_replicas, int n_steps,
+                              int64_t t0, int8_t *s, uint8_t *m, const int8_t *J)
+{
+    for (int64_t t = t0; t < t0 + n_steps; ++t) {
+        oracle_half_sweep(L, n_samples, n_replicas, 0, s, m, J, NULL, NULL);
+        oracle_half_sweep(L, n_samples, n_replicas, 1, s, m, J, NULL, NULL);
+        oracle_wander(L, n_samples, n_replicas, 0, +1, (int)(t & 1), m);
     }
 }
 

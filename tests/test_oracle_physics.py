@@ -248,3 +248,77 @@ def test_metropolis_oracle_itself_on_2x2x2(oracle):
     per_rep = e.mean(axis=0)
     err = per_rep.std(ddof=1) / math.sqrt(nr)
     assert abs(per_rep.mean() - exact) < 3 * err
+
+
+# ---------------------------------------------------------------- walkers (Sec. 2.6, 2.8)
+@pytest.mark.parametrize("L", [2, 4, 6])
+@pytest.mark.parametrize("axis,sign", [(0, 1), (1, 1), (2, 1), (0, -1), (1, -1), (2, -1)])
+def test_wandering_is_a_permutation_with_period_L(oracle, L, axis, sign):
+    """after L/2 cycles (L timesteps) every walker is back where it
+    started; each half-cycle is an exchange, hence its own inverse and a
+    permutation; walkers starting on even sites travel one site per timestep
+    in the wandering direction, the others against it."""
+    ns, nr, N = 2, 2, L ** 3
+    m0 = (np.arange(ns * nr * N, dtype=np.int64) % 251).astype(np.uint8).reshape(ns, nr, N)   # labels, not levels
+    m = m0.copy()
+    oracle.wander(L, m, axis, sign, 0); oracle.wander(L, m, axis, sign, 0)
+    np.testing.assert_array_equal(m, m0)                                   # exchange twice = identity
+    for t in range(L):
+        oracle.wander(L, m, axis, sign, t & 1)
+        assert sorted(m[1, 1].tolist()) == sorted(m0[1, 1].tolist())      # permutation
+        if 0 < t + 1 < L and L > 2:
+            assert not np.array_equal(m, m0)
+    np.testing.assert_array_equal(m, m0)                                   # period L
+    # direction: follow the walker that starts at the origin (an even site)
+    if L >= 4:
+        tag = np.zeros((1, 1, N), np.uint8); tag[0, 0, 0] = 1
+        for t in range(L // 2):
+            oracle.wander(L, tag, axis, sign, t & 1)
+        pos = int(np.flatnonzero(tag[0, 0])[0])
+        xyz = [pos % L, (pos // L) % L, pos // (L * L)]
+        want = [0, 0, 0]; want[axis] = (sign * (L // 2)) % L
+        assert xyz == want
+
+
+def test_walkers_conserve_total_energy_and_do_not_touch_spins(oracle):
+    L, ns, nr = 6, 3, 2
+    N = L ** 3
+    s, J = random_pm1((ns, nr, N), 61), random_pm1((ns, 3, N), 62)
+    m = np.zeros((ns, nr, N), np.uint8)
+    oracle.refresh(L, m, 5, 1.5, 0)
+    E0, Ed0, _ = oracle.measure(L, s, m, J)
+    s_before = s.copy()
+    mw = m.copy()
+    oracle.wander(L, mw, 0, +1, 0)
+    assert not np.array_equal(mw, m)
+    assert np.array_equal(oracle.measure(L, s, mw, J)[1], Ed0)             # walker energy only moves around
+    for t in range(9):
+        oracle.timesteps_walkers(L, s, m, J, 1, t0=t)
+        E, Ed, _ = oracle.measure(L, s, m, J)
+        np.testing.assert_array_equal(E + Ed, E0 + Ed0)                    # PAPER.md:124
+    # same thing in one call
+    s2, m2 = s_before.copy(), np.zeros_like(m); oracle.refresh(L, m2, 5, 1.5, 0)
+    oracle.timesteps_walkers(L, s2, m2, J, 9, t0=0)
+    np.testing.assert_array_equal(s2, s); np.testing.assert_array_equal(m2, m)
+    # and it differs from fixed daemons
+    s3, m3 = s_before.copy(), np.zeros_like(m); oracle.refresh(L, m3, 5, 1.5, 0)
+    oracle.sweep(L, s3, m3, J, 9)
+    assert not np.array_equal(s3, s)
+
+
+@pytest.mark.parametrize("T,seed", [(2.0, 21), (3.0, 22)])
+def test_2x2x2_walkers_match_exact_boltzmann(oracle, T, seed):
+    """Same pin as P7 with walkers: wandering must not spoil stationarity."""
+    L, N, nr = 2, 8, 64
+    J = random_pm1((1, 3, N), seed)
+    exact = _boltzmann_2x2x2(J[0].tolist(), T)
+    s = oracle.init_spins(L, 1, nr, seed)
+    m = np.zeros((1, nr, N), dtype=np.uint8)
+    n_sweeps, therm = 6000, 200
+    sched = [(T, 10, 1)] * (n_sweeps // 10)
+    out = driver.anneal(L, s, m, J, seed, sched, walkers=True)
+    e = out["E"][therm:] / float(N)
+    per_rep = e.mean(axis=0)
+    mean, err = per_rep.mean(), per_rep.std(ddof=1) / math.sqrt(nr)
+    assert err < 0.01
+    assert abs(mean - exact) < 3 * err, (mean, exact, err)
