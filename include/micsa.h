@@ -128,6 +128,27 @@ int micsa_get_state(micsa_ctx *ctx, int8_t *s, uint8_t *m, int8_t *J);
 int micsa_sweep(micsa_ctx *ctx, int n);
 int micsa_half_sweep(micsa_ctx *ctx, int parity);
 
+/* ---- walkers (PAPER.md:163-178 Sec. 2.6, :196-217 Sec. 2.8) ---------------
+ * micsa_wander: one half of the two-timestep wandering cycle along axis
+ * (0,1,2 = X,Y,Z) in direction sign (+1 forward, -1 backward): every walker
+ * (auxiliary variable) on a site of lattice parity `parity` exchanges its
+ * value with the walker on that site's neighbour along sign*axis, periodic.
+ * Even sites exchange at the first timestep of a cycle, odd sites at the
+ * second.  Spins untouched.  Asynchronous.
+ *
+ * micsa_set_walkers(mode): 0 (default) = the auxiliary variables are daemons
+ * bound to their site; 1 = one forward-X walker per spin (the paper's gamma = 1
+ * walker variant): micsa_sweep, micsa_sweep_measure and
+ * micsa_anneal then run TIMESTEPS -- a sweep, then micsa_wander(0, +1, t & 1),
+ * then t += 1.  t is the context's time index: sweeps done
+ * through those calls since create, settable with micsa_set_time (a refresh
+ * does not reset it; micsa_half_sweep does not advance it).  gamma > 1 and the
+ * other five directions of Eq. (13) are not wired into the timestep yet. */
+int micsa_wander(micsa_ctx *ctx, int axis, int sign, int parity);
+int micsa_set_walkers(micsa_ctx *ctx, int mode);
+int micsa_set_time(micsa_ctx *ctx, int64_t t);
+int micsa_get_time(micsa_ctx *ctx, int64_t *t);
+
 /* micsa_refresh_demons: every daemon <- independent draw from Eq. (11),
  * p(n=4m) ~ exp(-4m/T), m = 0..3; spins untouched
  * (PAPER.md:190).  One 32-bit uniform u per daemon, compared with integer

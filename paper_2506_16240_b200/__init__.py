@@ -32,6 +32,7 @@ EXPORTS = (
     "micsa_measure", "micsa_anneal", "micsa_counters", "micsa_layout_info",
     "micsa_set_tuning",
     "micsa_prefetch_refresh", "micsa_measure_begin", "micsa_measure_end", "micsa_sweep_measure",
+    "micsa_wander", "micsa_set_walkers", "micsa_set_time", "micsa_get_time",
 )
 
 
@@ -89,7 +90,9 @@ def _bind() -> ctypes.CDLL:
             ("micsa_destroy", [vp]), ("micsa_synchronize", [vp]),
             ("micsa_set_couplings", [vp, vp]), ("micsa_set_spins", [vp, vp]),
             ("micsa_set_daemons", [vp, vp]), ("micsa_get_state", [vp, vp, vp, vp]),
-            ("micsa_sweep", [vp, i32]), ("micsa_sweep_measure", [vp, i32]), ("micsa_half_sweep", [vp, i32]),
+            ("micsa_sweep", [vp, i32]), ("micsa_sweep_measure", [vp, i32]),
+            ("micsa_wander", [vp, i32, i32, i32]), ("micsa_set_walkers", [vp, i32]),
+            ("micsa_set_time", [vp, ctypes.c_int64]), ("micsa_get_time", [vp, vp]), ("micsa_half_sweep", [vp, i32]),
             ("micsa_refresh_demons", [vp, f64, u32]),
             ("micsa_prefetch_refresh", [vp, f64, u32]),
             ("micsa_debug_thresholds", [f64, vp]),
@@ -218,6 +221,20 @@ class MicSA:
     def sweep_measure(self, n=1):
         """n sweeps, then the measurement queued (fetch it with measure_end)."""
         _check(_lib.micsa_sweep_measure(self._h, int(n)))
+
+    def wander(self, axis=0, sign=+1, parity=0):
+        _check(_lib.micsa_wander(self._h, int(axis), int(sign), int(parity)))
+
+    def set_walkers(self, mode):
+        _check(_lib.micsa_set_walkers(self._h, int(mode)))
+
+    def set_time(self, t):
+        _check(_lib.micsa_set_time(self._h, int(t)))
+
+    def get_time(self) -> int:
+        t = ctypes.c_int64(0)
+        _check(_lib.micsa_get_time(self._h, ctypes.byref(t)))
+        return int(t.value)
 
     def half_sweep(self, parity):
         _check(_lib.micsa_half_sweep(self._h, int(parity)))

@@ -19,6 +19,7 @@
 #include "sweep.cuh"
 #include "sweep_persistent.cuh"
 #include "sweep_tile.cuh"
+#include "wander.cuh"
 
 using namespace micsa;
 
@@ -129,6 +130,8 @@ struct micsa_ctx {
     unsigned long long ticket0;   // value of *task_ticket when the next launch starts
     int progress_base;         // value of every progress entry between launches
     PersistPlan pp;
+    int walkers;               // 0 = daemons stay on their site, 1 = one forward-X walker per spin
+    long long t;               // time index (timesteps = sweeps done since create / micsa_set_time)
     int fuse_measure;          // count the observables inside the last sweep of a measured group
     int pipe_planes;           // planes per CTA of the pipelined kernel (1 or 4)
     int use_pdl;               // programmatic dependent launch for the pipelined kernel
@@ -351,8 +354,31 @@ int launch_half_sweep(micsa_ctx* c, int parity) {
     return post_launch(c);
 }
 
-// n full sweeps (even, odd, even, ...): one persistent launch or 2n launches
+int launch_wander(micsa_ctx* c, int axis, int sign, int parity) {
+    WanderArgs a;
+    a.m0 = c->st.m0; a.m1 = c->st.m1; a.L = c->g.L; a.Lh = c->g.Lh; a.half = c->g.half;
+    wander_kernel<<<site_blocks(c->g, c->g.n_words), 128, 0, c->stream>>>(a, axis, sign, parity);
+    return post_launch(c);
+}
+
+int launch_plain_sweeps(micsa_ctx* c, int n);
+
+// n timesteps (PAPER.md:208-217 step 3 with gamma = 1): a sweep, then -- for
+// walkers -- the half of the wandering cycle given by the parity of the time
+// index, then t += 1.  Without walkers: n sweeps back to back.
 int launch_sweeps(micsa_ctx* c, int n) {
+    if (n <= 0) return MICSA_OK;
+    if (!c->walkers) { c->t += n; return launch_plain_sweeps(c, n); }
+    for (int k = 0; k < n; ++k) {
+        int rc = launch_plain_sweeps(c, 1); if (rc) return rc;
+        rc = launch_wander(c, 0, +1, (int)(c->t & 1)); if (rc) return rc;
+        c->t += 1;
+    }
+    return MICSA_OK;
+}
+
+// n full sweeps (even, odd, even, ...): one persistent launch or 2n launches
+int launch_plain_sweeps(micsa_ctx* c, int n) {
     if (n <= 0) return MICSA_OK;
     if (use_persistent(c))
         return (c->g.rpw == 2) ? launch_persistent<2>(c, 2 * n, 0) : launch_persistent<1>(c, 2 * n, 0);
@@ -537,8 +563,13 @@ int launch_sweeps_measured(micsa_ctx* c, int n, long long* row, bool fold_min) {
         const int rc = launch_sweeps(c, n); if (rc) return rc;
         return launch_measure(c, row, fold_min);
     }
-    const int rc = launch_sweeps(c, n - 1); if (rc) return rc;
-    return (g.rpw == 2) ? launch_measuring_sweep<2>(c, row, fold_min) : launch_measuring_sweep<1>(c, row, fold_min);
+    int rc = launch_sweeps(c, n - 1); if (rc) return rc;
+    rc = (g.rpw == 2) ? launch_measuring_sweep<2>(c, row, fold_min) : launch_measuring_sweep<1>(c, row, fold_min);
+    if (rc) return rc;
+    // the wandering only permutes the walkers: E, E_daemon and q of the timestep are already counted
+    if (c->walkers) { rc = launch_wander(c, 0, +1, (int)(c->t & 1)); if (rc) return rc; }
+    c->t += 1;
+    return MICSA_OK;
 }
 
 // host <-> device staging for the canonical layouts
@@ -640,6 +671,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->use_pdl = 1;
     c->pipe_planes = (g.n_words == 1 && (g.L / 4) * (g.Lh / 4) >= 512) ? 4 : 1;   // measured: DESIGN.md 6.1
     c->fuse_measure = 1;
+    c->walkers = 0; c->t = 0;
     c->attempts = c->rns = c->launches = 0;
     c->sticky = 0;
     if (dev_workspace) {
@@ -776,6 +808,34 @@ int micsa_sweep(micsa_ctx* c, int n) {
     int rc = check_ctx(c); if (rc) return rc;
     if (n < 0) { set_err("n must be >= 0"); return MICSA_ERR_INVALID; }
     return launch_sweeps(c, n);
+}
+
+int micsa_wander(micsa_ctx* c, int axis, int sign, int parity) {
+    int rc = check_ctx(c); if (rc) return rc;
+    if (axis < 0 || axis > 2 || (sign != 1 && sign != -1) || (parity != 0 && parity != 1)) {
+        set_err("axis must be 0..2, sign +1 or -1, parity 0 or 1"); return MICSA_ERR_INVALID;
+    }
+    return launch_wander(c, axis, sign, parity);
+}
+
+int micsa_set_walkers(micsa_ctx* c, int mode) {
+    int rc = check_ctx(c); if (rc) return rc;
+    if (mode != 0 && mode != 1) { set_err("walkers mode must be 0 (daemons) or 1 (one forward-X walker per spin)"); return MICSA_ERR_INVALID; }
+    c->walkers = mode;
+    return MICSA_OK;
+}
+
+int micsa_set_time(micsa_ctx* c, int64_t t) {
+    int rc = check_ctx(c); if (rc) return rc;
+    if (t < 0) { set_err("t must be >= 0"); return MICSA_ERR_INVALID; }
+    c->t = t;
+    return MICSA_OK;
+}
+
+int micsa_get_time(micsa_ctx* c, int64_t* t) {
+    if (!c || !t) { set_err("null pointer"); return MICSA_ERR_INVALID; }
+    *t = c->t;
+    return MICSA_OK;
 }
 
 int micsa_debug_thresholds(double T, uint64_t thr[3]) {

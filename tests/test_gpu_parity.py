@@ -443,3 +443,72 @@ def test_sweep_measure_fused_equals_separate(micsa, oracle, L, ns, nr):
             np.testing.assert_array_equal(E2, oE)
             np.testing.assert_array_equal(Ed2, oEd)
             np.testing.assert_array_equal(Q2, oQ)
+
+
+# ---------------------------------------------------------------- walkers
+@pytest.mark.parametrize("L,ns,nr", SHAPES)
+def test_wander_bit_exact(micsa, oracle, L, ns, nr):
+    """Every half-cycle of the wandering (3 axes x 2 directions x 2 parities)
+    against the oracle's literal exchange; spins untouched."""
+    N = L ** 3
+    s, m = random_pm1((ns, nr, N), 71), random_levels((ns, nr, N), 72)
+    with micsa.MicSA(L, ns, nr, 1) as g:
+        g.set_spins(s); g.set_daemons(m)
+        for axis in (0, 1, 2):
+            for sign in (1, -1):
+                for parity in (0, 1):
+                    g.wander(axis, sign, parity)
+                    oracle.wander(L, m, axis, sign, parity)
+                    _assert_state(g, s, m)
+        with pytest.raises(micsa.MicsaError):
+            g.wander(3, 1, 0)
+        with pytest.raises(micsa.MicsaError):
+            g.wander(0, 0, 0)
+
+
+@pytest.mark.parametrize("L,ns,nr", [(8, 40, 2), (6, 5, 3), (16, 17, 2), (24, 2, 2), (4, 3, 2)])
+def test_walker_timesteps_bit_exact(micsa, oracle, L, ns, nr):
+    """gamma = 1 forward-X walkers: timesteps (sweep + wandering half-cycle of
+    parity t mod 2) against the oracle, with refreshes in between, through
+    sweep, sweep_measure and anneal; period L with the sweeps switched off."""
+    N = L ** 3
+    seed = 9
+    s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+    m = np.zeros_like(s, dtype=np.uint8)
+    with micsa.MicSA(L, ns, nr, seed) as g:
+        g.set_walkers(1)
+        g.refresh_demons(1.2, 0); oracle.refresh(L, m, seed, 1.2, 0)
+        t = 0
+        for n in (1, 2, 3):
+            g.sweep(n); oracle.timesteps_walkers(L, s, m, J, n, t0=t); t += n
+            _assert_state(g, s, m)
+        assert g.get_time() == t
+        g.sweep_measure(3); E, Ed, Q = g.measure_end()
+        oracle.timesteps_walkers(L, s, m, J, 3, t0=t); t += 3
+        _assert_state(g, s, m)
+        oE, oEd, oQ = oracle.measure(L, s, m, J)
+        np.testing.assert_array_equal(E, oE); np.testing.assert_array_equal(Ed, oEd)
+        if nr == 2:
+            np.testing.assert_array_equal(Q, oQ)
+        sched = [(1.0, 5, 5), (0.8, 4, 2)]
+        out = g.anneal(sched, step0=1)
+        ref = driver.anneal(L, s, m, J, seed, sched, step0=1, walkers=True, t0=t); t += 9
+        _assert_state(g, s, m)
+        np.testing.assert_array_equal(out["E"], ref["E"])
+        np.testing.assert_array_equal(out["Edem"], ref["Edem"])
+        assert g.get_time() == t
+        # an odd starting time: the odd sites exchange first
+        g.set_time(7)
+        g.sweep(2); oracle.timesteps_walkers(L, s, m, J, 2, t0=7)
+        _assert_state(g, s, m)
+        # daemons again
+        g.set_walkers(0)
+        g.sweep(2); oracle.sweep(L, s, m, J, 2)
+        _assert_state(g, s, m)
+    # PAPER.md:176: L half-cycles bring every walker home
+    lab = random_levels((ns, nr, N), 5)
+    with micsa.MicSA(L, ns, nr, 1) as g:
+        g.set_daemons(lab)
+        for tt in range(L):
+            g.wander(1, -1, tt & 1)
+        np.testing.assert_array_equal(g.get_state(spins=False, couplings=False)[1], lab)
