@@ -165,6 +165,9 @@ def main():
     ap.add_argument("--impl", default="micsa", choices=["micsa", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--walkers", action="store_true",
+                    help="one forward-X walker per spin instead of a daemon (PAPER.md Sec. 2.6): every sweep is "
+                         "followed by a wandering half-cycle; reported under its own metric name")
     ap.add_argument("--no-fuse-measure", action="store_true",
                     help="A/B: separate measurement kernel instead of counting inside the last sweep")
     args = ap.parse_args()
@@ -214,6 +217,8 @@ def main():
                     stream=stream)
     if args.no_fuse_measure:
         g.set_tuning("fuse_measure", 0)
+    if args.walkers:
+        g.set_walkers(1)
     info = g.layout_info()
     attempts_step = CFG.attempts_per_sweep * SWEEPS_PER_STEP
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
@@ -314,7 +319,8 @@ def main():
 
     if rank == 0:
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "metric": METRIC + (" [gamma=1 forward-X walkers]" if args.walkers else ""),
+            "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": t_step_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u32-bitsliced", "data": "synthetic",
             "config": {"workload": CFG.name, "L": L, "n_samples": ns, "n_replicas": nr, "T": T_RUN,

@@ -130,6 +130,7 @@ struct micsa_ctx {
     unsigned long long ticket0;   // value of *task_ticket when the next launch starts
     int progress_base;         // value of every progress entry between launches
     PersistPlan pp;
+    int fuse_walk;             // walkers: exchange inside the odd half-sweep instead of a separate kernel
     int walkers;               // 0 = daemons stay on their site, 1 = one forward-X walker per spin
     long long t;               // time index (timesteps = sweeps done since create / micsa_set_time)
     int fuse_measure;          // count the observables inside the last sweep of a measured group
@@ -198,8 +199,9 @@ void launch_half_sweep_rows(micsa_ctx* c, int parity) {
     half_sweep_rows_kernel<RPW, kRowsPerThread><<<grid, 128, 0, c->stream>>>(a, parity);
 }
 
+// dir != 0 (odd launches of walker timesteps): the launch also does the wandering exchange
 template <int RPW>
-void launch_half_sweep_pipe(micsa_ctx* c, int parity) {
+void launch_half_sweep_pipe(micsa_ctx* c, int parity, int dir = 0) {
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
     a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half;
@@ -216,7 +218,18 @@ void launch_half_sweep_pipe(micsa_ctx* c, int parity) {
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = c->use_pdl ? 1 : 0;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    if (zw == 4) {
+    if (dir != 0) {                                  // 4 rows per thread only (grid was sized for yc; redo it)
+        const int pp4 = (c->g.L / 4) * (c->g.Lh / 4);
+        cfg.gridDim = (zw == 4) ? dim3((unsigned)((pp4 + 31) / 32), (unsigned)(c->g.L / 4), (unsigned)c->g.n_words)
+                                : dim3((unsigned)((pp4 + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
+        if (zw == 4) {
+            if (dir > 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, +1>, a, parity);
+            else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, -1>, a, parity);
+        } else {
+            if (dir > 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, +1>, a, parity);
+            else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, -1>, a, parity);
+        }
+    } else if (zw == 4) {
         if (yc == 8) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8, 4>, a, parity);
         else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4>, a, parity);
     } else {
@@ -366,12 +379,25 @@ int launch_plain_sweeps(micsa_ctx* c, int n);
 // n timesteps (PAPER.md:208-217 step 3 with gamma = 1): a sweep, then -- for
 // walkers -- the half of the wandering cycle given by the parity of the time
 // index, then t += 1.  Without walkers: n sweeps back to back.
+// the wandering can ride on the odd half-sweep (sweep.cuh exchange_walkers) with the pipelined kernel
+bool fused_walk(const micsa_ctx* c) { return c->walkers && c->fuse_walk && c->V == 4 && c->sweep_kernel == 2; }
+
 int launch_sweeps(micsa_ctx* c, int n) {
     if (n <= 0) return MICSA_OK;
     if (!c->walkers) { c->t += n; return launch_plain_sweeps(c, n); }
     for (int k = 0; k < n; ++k) {
-        int rc = launch_plain_sweeps(c, 1); if (rc) return rc;
-        rc = launch_wander(c, 0, +1, (int)(c->t & 1)); if (rc) return rc;
+        if (fused_walk(c)) {
+            // sources of parity t & 1 exchange with their +X neighbour: seen from the odd sites the
+            // partner is x+1 when they are the sources (t odd), x-1 when the even sites are (t even)
+            int rc = launch_half_sweep(c, 0); if (rc) return rc;
+            const int dir = (c->t & 1) ? +1 : -1;
+            if (c->g.rpw == 2) launch_half_sweep_pipe<2>(c, 1, dir); else launch_half_sweep_pipe<1>(c, 1, dir);
+            c->attempts += (uint64_t)(c->g.N / 2) * (uint64_t)c->g.n_sys;
+            rc = post_launch(c); if (rc) return rc;
+        } else {
+            int rc = launch_plain_sweeps(c, 1); if (rc) return rc;
+            rc = launch_wander(c, 0, +1, (int)(c->t & 1)); if (rc) return rc;
+        }
         c->t += 1;
     }
     return MICSA_OK;
@@ -527,7 +553,7 @@ int launch_measure(micsa_ctx* c, long long* row, bool fold_min) {
 // The last sweep of a measured group with the counting fused into its two launches
 // (sweep.cuh, MeasAcc): the state is not read again for the observables.
 template <int RPW>
-int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min) {
+int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min, int dir) {
     const Geom& g = c->g;
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
@@ -546,10 +572,14 @@ int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min) {
     cfg.attrs = attr; cfg.numAttrs = 1;
     if (zw == 4) {
         cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 1>, a, 0, ma, fa);
-        cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2>, a, 1, ma, fa);
+        if (dir > 0)      cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2, +1>, a, 1, ma, fa);
+        else if (dir < 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2, -1>, a, 1, ma, fa);
+        else              cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2>, a, 1, ma, fa);
     } else {
         cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 1>, a, 0, ma, fa);
-        cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2>, a, 1, ma, fa);
+        if (dir > 0)      cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2, +1>, a, 1, ma, fa);
+        else if (dir < 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2, -1>, a, 1, ma, fa);
+        else              cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2>, a, 1, ma, fa);
     }
     c->attempts += (uint64_t)g.N * (uint64_t)g.n_sys;
     return post_launch(c, 2);
@@ -564,10 +594,11 @@ int launch_sweeps_measured(micsa_ctx* c, int n, long long* row, bool fold_min) {
         return launch_measure(c, row, fold_min);
     }
     int rc = launch_sweeps(c, n - 1); if (rc) return rc;
-    rc = (g.rpw == 2) ? launch_measuring_sweep<2>(c, row, fold_min) : launch_measuring_sweep<1>(c, row, fold_min);
+    // the wandering only permutes the walkers: E, E_daemon and q of the timestep are counted before it
+    const int dir = fused_walk(c) ? ((c->t & 1) ? +1 : -1) : 0;
+    rc = (g.rpw == 2) ? launch_measuring_sweep<2>(c, row, fold_min, dir) : launch_measuring_sweep<1>(c, row, fold_min, dir);
     if (rc) return rc;
-    // the wandering only permutes the walkers: E, E_daemon and q of the timestep are already counted
-    if (c->walkers) { rc = launch_wander(c, 0, +1, (int)(c->t & 1)); if (rc) return rc; }
+    if (c->walkers && dir == 0) { rc = launch_wander(c, 0, +1, (int)(c->t & 1)); if (rc) return rc; }
     c->t += 1;
     return MICSA_OK;
 }
@@ -671,7 +702,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->use_pdl = 1;
     c->pipe_planes = (g.n_words == 1 && (g.L / 4) * (g.Lh / 4) >= 512) ? 4 : 1;   // measured: DESIGN.md 6.1
     c->fuse_measure = 1;
-    c->walkers = 0; c->t = 0;
+    c->walkers = 0; c->t = 0; c->fuse_walk = 1;
     c->attempts = c->rns = c->launches = 0;
     c->sticky = 0;
     if (dev_workspace) {
@@ -1004,6 +1035,9 @@ int micsa_set_tuning(micsa_ctx* c, int key, int value) {
         case MICSA_TUNE_PIPE_PLANES:
             if (value != 1 && value != 4) { set_err("pipe_planes must be 1 or 4"); return MICSA_ERR_INVALID; }
             c->pipe_planes = value; return MICSA_OK;
+        case MICSA_TUNE_FUSE_WALK:
+            if (value != 0 && value != 1) { set_err("fuse_walk must be 0 or 1"); return MICSA_ERR_INVALID; }
+            c->fuse_walk = value; return MICSA_OK;
         case MICSA_TUNE_FUSE_MEASURE:
             if (value != 0 && value != 1) { set_err("fuse_measure must be 0 or 1"); return MICSA_ERR_INVALID; }
             c->fuse_measure = value; return MICSA_OK;

@@ -308,6 +308,7 @@ __device__ __forceinline__ void creutz_word20(uint32_t u1, uint32_t u2, uint32_t
 struct PipeBase {           // block-uniform bases of lattice w: plane 0 of each parity array
     uint32_t* sp; uint32_t* m0; uint32_t* m1;          // own parity
     const uint32_t* sq;                                // opposite parity
+    uint32_t* m0q; uint32_t* m1q;                      // opposite parity's daemon planes (walkers only)
     const void* jx; const void* jy; const void* jz;    // own bonds
     const void* jxq; const void* jyq; const void* jzq; // the -d neighbours' bonds (opposite parity arrays)
 };
@@ -319,6 +320,8 @@ struct RowRegs {                 // everything one row step reads
     typename B4::raw jx, jy, jz, jyq, jzq, jxq;
     uint32_t e;
     typename B4::elem eJ;
+    uint4 w0, w1;                // walkers: the exchange partners' planes, same quad ...
+    uint32_t we0, we1;           // ... and the word just outside it
 };
 
 // o, o_prev, o_next: byte offsets (inside a parity array of spin words) of
@@ -335,7 +338,7 @@ struct XNb {
     bool in_up, in_dn;      // ... and whether they can be reached by a shuffle
 };
 
-template <int RPW, int C>
+template <int RPW, int C, int DIR = 0>
 __device__ __forceinline__ void load_row(RowRegs<RPW>& r, const PipeBase& P, uint32_t o, uint32_t o_prev,
                                          uint32_t o_next, uint32_t x4, uint32_t xe_up, uint32_t xe_dn,
                                          uint32_t dzp, uint32_t dzm, const XNb& nb)
@@ -356,6 +359,12 @@ __device__ __forceinline__ void load_row(RowRegs<RPW>& r, const PipeBase& P, uin
     r.jyq = ld_off<typename B4::raw>(P.jyq, ojm);
     r.jzq = ld_off<typename B4::raw>(P.jzq, (o + dzm) / 4u * JS);
     r.jxq = ld_off<typename B4::raw>(P.jxq, oj);
+    if (DIR != 0) {              // walkers: the planes of the sites these sites exchange with (see exchange_walkers)
+        r.w0 = ld_off<uint4>(P.m0q, o);
+        r.w1 = ld_off<uint4>(P.m1q, o);
+        if (DIR > 0 && C)  { r.we0 = ld_off<uint32_t>(P.m0q, rowstart + xe_up); r.we1 = ld_off<uint32_t>(P.m1q, rowstart + xe_up); }
+        if (DIR < 0 && !C) { r.we0 = ld_off<uint32_t>(P.m0q, rowstart + xe_dn); r.we1 = ld_off<uint32_t>(P.m1q, rowstart + xe_dn); }
+    }
     r.e = 0; r.eJ = 0;
     if (C) {
         if (!nb.in_up) r.e = ld_off<uint32_t>(P.sq, rowstart + xe_up);
@@ -413,10 +422,55 @@ __device__ __forceinline__ void count6x4(const uint32_t (&f)[6][4], uint32_t (&o
     full_add(x0, x1, x2, o[3], o[4]);                        // weight 8, 16
 }
 
-template <int RPW, int C, int MEAS, int YC>
+// Walkers: the wandering half-cycle that closes a timestep
+// exchanges every walker of the source parity with its +X neighbour's.  It is
+// done by the ODD half-sweep of that timestep, the last one to touch daemon
+// values: an odd site x sends its just-updated level to its partner -- the even
+// site x-1 when the even sites are the sources (t even, DIR = -1), x+1 when the
+// odd sites are (t odd, DIR = +1) -- and takes the partner's level (final since
+// the even half-sweep) in return.  In the x-compressed arrays the partner of
+// word xh is word xh of the other parity's planes, or xh+1 (DIR > 0, rows with
+// C = 1) / xh-1 (DIR < 0, rows with C = 0): the same edge word as the spin
+// neighbour's.  Every word is written by exactly one thread.
+template <int RPW, int C, int DIR>
+__device__ __forceinline__ void exchange_walkers(const RowRegs<RPW>& r, const PipeBase& P, uint32_t o,
+                                                 uint32_t rowstart, uint32_t xe_up, uint32_t xe_dn,
+                                                 uint32_t (&v0)[4], uint32_t (&v1)[4])
+{
+    const uint32_t a0[4] = { r.w0.x, r.w0.y, r.w0.z, r.w0.w }, a1[4] = { r.w1.x, r.w1.y, r.w1.z, r.w1.w };
+    if ((DIR > 0 && !C) || (DIR < 0 && C)) {              // partner words = the same quad
+        st_off<uint4>(P.m0q, o, make_uint4(v0[0], v0[1], v0[2], v0[3]));
+        st_off<uint4>(P.m1q, o, make_uint4(v1[0], v1[1], v1[2], v1[3]));
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { v0[k] = a0[k]; v1[k] = a1[k]; }
+    } else if (DIR > 0) {                                 // partner words xh0+1 .. xh0+4 (periodic)
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            st_off<uint32_t>(P.m0q, o + 4u * (k + 1), v0[k]);
+            st_off<uint32_t>(P.m1q, o + 4u * (k + 1), v1[k]);
+        }
+        st_off<uint32_t>(P.m0q, rowstart + xe_up, v0[3]);
+        st_off<uint32_t>(P.m1q, rowstart + xe_up, v1[3]);
+        v0[0] = a0[1]; v0[1] = a0[2]; v0[2] = a0[3]; v0[3] = r.we0;
+        v1[0] = a1[1]; v1[1] = a1[2]; v1[2] = a1[3]; v1[3] = r.we1;
+    } else {                                              // partner words xh0-1 .. xh0+2 (periodic)
+        st_off<uint32_t>(P.m0q, rowstart + xe_dn, v0[0]);
+        st_off<uint32_t>(P.m1q, rowstart + xe_dn, v1[0]);
+#pragma unroll
+        for (int k = 1; k < 4; ++k) {
+            st_off<uint32_t>(P.m0q, o + 4u * (k - 1), v0[k]);
+            st_off<uint32_t>(P.m1q, o + 4u * (k - 1), v1[k]);
+        }
+        v0[3] = a0[2]; v0[2] = a0[1]; v0[1] = a0[0]; v0[0] = r.we0;
+        v1[3] = a1[2]; v1[2] = a1[1]; v1[1] = a1[0]; v1[0] = r.we1;
+    }
+}
+
+template <int RPW, int C, int MEAS, int YC, int DIR = 0>
 __device__ __forceinline__ void update_row(const RowRegs<RPW>& r, const uint4& Aprev, const uint4& Acur,
                                            const PipeBase& P, uint32_t o, const XNb& nb,
-                                           MeasAcc<YC>* acc, bool pair)
+                                           MeasAcc<YC>* acc, bool pair,
+                                           uint32_t x4 = 0, uint32_t xe_up = 0, uint32_t xe_dn = 0)
 {
     typedef Bond4<RPW> B4;
     uint32_t jxo[4], jyo[4], jzo[4], jxm[4], jym[4], jzm[4], Bx[4];
@@ -454,8 +508,10 @@ __device__ __forceinline__ void update_row(const RowRegs<RPW>& r, const uint4& A
                       sv[k], v0[k], v1[k]);
     }
     st_off<uint4>(P.sp, o, make_uint4(sv[0], sv[1], sv[2], sv[3]));
-    st_off<uint4>(P.m0, o, make_uint4(v0[0], v0[1], v0[2], v0[3]));
-    st_off<uint4>(P.m1, o, make_uint4(v1[0], v1[1], v1[2], v1[3]));
+    if (DIR == 0) {
+        st_off<uint4>(P.m0, o, make_uint4(v0[0], v0[1], v0[2], v0[3]));
+        st_off<uint4>(P.m1, o, make_uint4(v1[0], v1[1], v1[2], v1[3]));
+    }
     if (MEAS) {
         uint32_t pm[4];
         csa_4x1_4x2(v0, v1, pm);                              // levels after the update
@@ -482,10 +538,15 @@ __device__ __forceinline__ void update_row(const RowRegs<RPW>& r, const uint4& A
             acc->u.add(pu);
         }
     }
+    if (DIR != 0) {              // walkers: hand the new levels to the partner sites, keep theirs
+        exchange_walkers<RPW, C, DIR>(r, P, o, o - x4, xe_up, xe_dn, v0, v1);
+        st_off<uint4>(P.m0, o, make_uint4(v0[0], v0[1], v0[2], v0[3]));
+        st_off<uint4>(P.m1, o, make_uint4(v1[0], v1[1], v1[2], v1[3]));
+    }
 }
 
 // rows y0 .. y0+YC-1 of plane z (y0 % YC == 0, YC even, L % YC == 0), words xh0 .. xh0+3
-template <int RPW, int YC, int F, int MEAS = 0>
+template <int RPW, int YC, int F, int MEAS = 0, int DIR = 0>
 __device__ __forceinline__ void march_rows_pipe(const PipeBase& P, int L, int Lh, int z, int y0, int xh0,
                                                 const XNb& nb, MeasAcc<YC>* acc = nullptr, bool pair = false)
 {
@@ -507,7 +568,7 @@ __device__ __forceinline__ void march_rows_pipe(const PipeBase& P, int L, int Lh
     RowRegs<RPW> cur, nxt;
     {
         const uint32_t o_next = (y0 + 1 == L) ? row0 : o + rowB;
-        load_row<RPW, F>(cur, P, o, o_prev, o_next, x4, xe_up, xe_dn, dzp, dzm, nb);
+        load_row<RPW, F, DIR>(cur, P, o, o_prev, o_next, x4, xe_up, xe_dn, dzp, dzm, nb);
     }
 #pragma unroll
     for (int iy = 0; iy < YC; ++iy) {
@@ -515,11 +576,11 @@ __device__ __forceinline__ void march_rows_pipe(const PipeBase& P, int L, int Lh
         const uint32_t o_next = (y + 1 == L) ? row0 : o + rowB;
         if (iy + 1 < YC) {                          // y + 1 < L inside a chunk
             const uint32_t o_next2 = (y + 2 == L) ? row0 : o_next + rowB;
-            if ((iy & 1) ^ F) load_row<RPW, 0>(nxt, P, o_next, o, o_next2, x4, xe_up, xe_dn, dzp, dzm, nb);
-            else              load_row<RPW, 1>(nxt, P, o_next, o, o_next2, x4, xe_up, xe_dn, dzp, dzm, nb);
+            if ((iy & 1) ^ F) load_row<RPW, 0, DIR>(nxt, P, o_next, o, o_next2, x4, xe_up, xe_dn, dzp, dzm, nb);
+            else              load_row<RPW, 1, DIR>(nxt, P, o_next, o, o_next2, x4, xe_up, xe_dn, dzp, dzm, nb);
         }
-        if ((iy & 1) ^ F) update_row<RPW, 1, MEAS, YC>(cur, Aprev, Acur, P, o, nb, acc, pair);
-        else              update_row<RPW, 0, MEAS, YC>(cur, Aprev, Acur, P, o, nb, acc, pair);
+        if ((iy & 1) ^ F) update_row<RPW, 1, MEAS, YC, DIR>(cur, Aprev, Acur, P, o, nb, acc, pair, x4, xe_up, xe_dn);
+        else              update_row<RPW, 0, MEAS, YC, DIR>(cur, Aprev, Acur, P, o, nb, acc, pair, x4, xe_up, xe_dn);
         Aprev = Acur; Acur = cur.An;
         if (iy + 1 < YC) cur = nxt;
         o_prev = o; o = o_next;
@@ -553,6 +614,8 @@ __device__ __forceinline__ PipeBase pipe_base(const SweepArgs& a, int w, int p)
     P.sp = a.spin + ((long long)w * 2 + p) * half;
     P.m0 = a.m0 + ((long long)w * 2 + p) * half;
     P.m1 = a.m1 + ((long long)w * 2 + p) * half;
+    P.m0q = a.m0 + ((long long)w * 2 + q) * half;
+    P.m1q = a.m1 + ((long long)w * 2 + q) * half;
     P.sq = a.spin + ((long long)w * 2 + q) * half;
     P.jx = Jb + (0 * 2 + p) * half; P.jy = Jb + (1 * 2 + p) * half; P.jz = Jb + (2 * 2 + p) * half;
     P.jxq = Jb + (0 * 2 + q) * half; P.jyq = Jb + (1 * 2 + q) * half; P.jzq = Jb + (2 * 2 + q) * half;
@@ -565,7 +628,9 @@ __device__ __forceinline__ PipeBase pipe_base(const SweepArgs& a, int w, int p)
 //         +-z neighbour rows of a warp are the own-plane rows of the next / previous warp and
 //         are found in the SM's L1 (hit or hit-on-miss) instead of crossing the L2 -> SM path,
 //         which is what bounds this kernel.
-template <int RPW, int YC, int ZW>
+// DIR = +-1: this (odd) launch also performs the wandering half-cycle that closes the timestep
+// (exchange_walkers).
+template <int RPW, int YC, int ZW, int DIR = 0>
 __global__ void __launch_bounds__(128)
 half_sweep_pipe_kernel(SweepArgs a, int p)
 {
@@ -587,8 +652,8 @@ half_sweep_pipe_kernel(SweepArgs a, int p)
     // and the next grid may be scheduled as soon as every CTA of this one got here
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    if ((z + p) & 1) march_rows_pipe<RPW, YC, 1>(P, L, Lh, z, chunk * YC, xv * 4, nb);
-    else             march_rows_pipe<RPW, YC, 0>(P, L, Lh, z, chunk * YC, xv * 4, nb);
+    if ((z + p) & 1) march_rows_pipe<RPW, YC, 1, 0, DIR>(P, L, Lh, z, chunk * YC, xv * 4, nb);
+    else             march_rows_pipe<RPW, YC, 0, 0, DIR>(P, L, Lh, z, chunk * YC, xv * 4, nb);
 }
 
 // The two launches of the LAST sweep of a measured group: same update, plus the
@@ -597,7 +662,7 @@ half_sweep_pipe_kernel(SweepArgs a, int p)
 // the counts into the measurement row (finalize_rows) and re-zeroes them.
 // Same grids as half_sweep_pipe_kernel<RPW, 4, ZW>; every thread stays for the
 // block-wide reduction.
-template <int RPW, int ZW, int MEAS>
+template <int RPW, int ZW, int MEAS, int DIR = 0>
 __global__ void __launch_bounds__(128, 4)
 half_sweep_pipe_meas_kernel(SweepArgs a, int p, MeasureArgs ma, FinalizeArgs fa)
 {
@@ -620,8 +685,8 @@ half_sweep_pipe_meas_kernel(SweepArgs a, int p, MeasureArgs ma, FinalizeArgs fa)
         const int chunk = t / nxv, xv = t - chunk * nxv;
         const PipeBase P = pipe_base<RPW>(a, w, p);
         const XNb nb = x_neighbours(t, xv, nxv, mask, true);
-        if ((z + p) & 1) march_rows_pipe<RPW, YC, 1, MEAS>(P, L, Lh, z, chunk * YC, xv * 4, nb, &acc, pair);
-        else             march_rows_pipe<RPW, YC, 0, MEAS>(P, L, Lh, z, chunk * YC, xv * 4, nb, &acc, pair);
+        if ((z + p) & 1) march_rows_pipe<RPW, YC, 1, MEAS, DIR>(P, L, Lh, z, chunk * YC, xv * 4, nb, &acc, pair);
+        else             march_rows_pipe<RPW, YC, 0, MEAS, DIR>(P, L, Lh, z, chunk * YC, xv * 4, nb, &acc, pair);
     }
     if (MEAS == 2) block_warp_lane_counts<MeasAcc<YC>::PU, 128>(acc.u.c, s_cnt, ma.cntU + (long long)w * 32);
     block_warp_lane_counts<MeasAcc<YC>::PM, 128>(acc.m.c, s_cnt, ma.cntM + (long long)w * 32);

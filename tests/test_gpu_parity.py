@@ -466,8 +466,10 @@ def test_wander_bit_exact(micsa, oracle, L, ns, nr):
             g.wander(0, 0, 0)
 
 
-@pytest.mark.parametrize("L,ns,nr", [(8, 40, 2), (6, 5, 3), (16, 17, 2), (24, 2, 2), (4, 3, 2)])
-def test_walker_timesteps_bit_exact(micsa, oracle, L, ns, nr):
+@pytest.mark.parametrize("tune", [{}, {"fuse_walk": 0}, {"pipe_planes": 4}, {"pipe_planes": 1, "fuse_measure": 0},
+                                  {"sweep_kernel": 1}])
+@pytest.mark.parametrize("L,ns,nr", [(8, 40, 2), (6, 5, 3), (16, 17, 2), (24, 2, 2), (4, 3, 2), (8, 33, 1), (32, 3, 2)])
+def test_walker_timesteps_bit_exact(micsa, oracle, L, ns, nr, tune):
     """gamma = 1 forward-X walkers: timesteps (sweep + wandering half-cycle of
     parity t mod 2) against the oracle, with refreshes in between, through
     sweep, sweep_measure and anneal; period L with the sweeps switched off."""
@@ -477,6 +479,8 @@ def test_walker_timesteps_bit_exact(micsa, oracle, L, ns, nr):
     m = np.zeros_like(s, dtype=np.uint8)
     with micsa.MicSA(L, ns, nr, seed) as g:
         g.set_walkers(1)
+        for k, v in tune.items():
+            g.set_tuning(k, v)
         g.refresh_demons(1.2, 0); oracle.refresh(L, m, seed, 1.2, 0)
         t = 0
         for n in (1, 2, 3):
