@@ -57,6 +57,10 @@ def lib() -> ctypes.CDLL:
         _LIB.oracle_thresholds.argtypes = [ctypes.c_double, _c_u64p]
         _LIB.oracle_thresholds.restype = ctypes.c_int
         _LIB.oracle_refresh.restype = ctypes.c_int
+        _LIB.oracle_metropolis_thresholds.argtypes = [ctypes.c_double, _c_u64p]
+        _LIB.oracle_metropolis_thresholds.restype = ctypes.c_int
+        _LIB.oracle_metropolis_sweep.restype = ctypes.c_int
+        _LIB.oracle_metropolis_half_sweep.restype = ctypes.c_int
         _LIB.oracle_refresh_uniform.restype = ctypes.c_uint32
         _LIB.oracle_num_threads.restype = ctypes.c_int
     return _LIB
@@ -148,6 +152,33 @@ def timesteps_walkers(L, s, m, J, n_steps=1, t0=0) -> None:
     lib().oracle_timesteps_walkers(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr),
                                    ctypes.c_int(n_steps), ctypes.c_int64(t0),
                                    _p(s, _c_i8p), _p(m, _c_u8p), _p(J, _c_i8p))
+
+
+def metropolis_thresholds(T: float) -> np.ndarray:
+    """floor(exp(-4(k+1)/T) * 2^32), k = 0, 1, 2: acceptance thresholds for dH = 4, 8, 12."""
+    thr = np.zeros(3, dtype=np.uint64)
+    if lib().oracle_metropolis_thresholds(ctypes.c_double(T), _p(thr, _c_u64p)) != 0:
+        raise ValueError(f"invalid temperature {T!r}")
+    return thr
+
+
+def metropolis_checkerboard(L, s, J, seed, T, tau0=0, n_sweeps=1, sample_offset=0, parity=None) -> None:
+    """Standard Metropolis on the checkerboard with one Philox uniform per
+    attempt, in place.  parity=None: n full sweeps with
+    sweep indices tau0, tau0+1, ...; parity=0/1: one half-sweep with index tau0."""
+    ns, nr, N = s.shape
+    assert N == L ** 3 and s.dtype == np.int8 and s.flags.c_contiguous
+    if parity is None:
+        rc = lib().oracle_metropolis_sweep(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr), ctypes.c_uint64(seed),
+                                           ctypes.c_int(sample_offset), ctypes.c_double(T), ctypes.c_uint32(tau0),
+                                           ctypes.c_int(n_sweeps), _p(s, _c_i8p), _p(J, _c_i8p))
+    else:
+        rc = lib().oracle_metropolis_half_sweep(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr),
+                                                ctypes.c_uint64(seed), ctypes.c_int(sample_offset),
+                                                ctypes.c_double(T), ctypes.c_uint32(tau0), ctypes.c_int(parity),
+                                                _p(s, _c_i8p), _p(J, _c_i8p))
+    if rc != 0:
+        raise ValueError(f"invalid temperature {T!r}")
 
 
 def thresholds(T: float) -> np.ndarray:

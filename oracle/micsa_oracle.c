@@ -71,7 +71,7 @@ void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2],
 }
 
 /* Domain tags of the counter word c2 (R8). */
-enum { TAG_REFRESH = 0, TAG_SPIN_INIT = 1, TAG_BOND_INIT = 2 };
+enum { TAG_REFRESH = 0, TAG_SPIN_INIT = 1, TAG_BOND_INIT = 2, TAG_METROPOLIS = 3 };
 
 static inline void seed_key(uint64_t seed, uint32_t key[2])
 {
@@ -290,13 +290,12 @@ int oracle_thresholds(double T, uint64_t thr[3])
  *     u = sum_k  bit_k * 2^(31-k).
  * Every bit of every output word is used by exactly one demon, so u is a
  * uniform 32-bit integer and distinct demons are independent. */
-static uint32_t refresh_uniform(uint32_t i, uint32_t g, uint32_t rep,
-                                uint32_t step, const uint32_t key[2])
+static uint32_t tagged_uniform(uint32_t tag, uint32_t i, uint32_t g, uint32_t rep,
+                               uint32_t step, const uint32_t key[2])
 {
     uint32_t u = 0;
     for (uint32_t c = 0; c < 4; ++c) {
-        uint32_t ctr[4] = { i, (g >> 4) | (c << 28),
-                            ((uint32_t)TAG_REFRESH << 24) | rep, step };
+        uint32_t ctr[4] = { i, (g >> 4) | (c << 28), (tag << 24) | rep, step };
         uint32_t out[4];
         oracle_philox4x32_10(ctr, key, out);
         for (uint32_t j = 0; j < 4; ++j)
@@ -307,6 +306,12 @@ static uint32_t refresh_uniform(uint32_t i, uint32_t g, uint32_t rep,
             }
     }
     return u;
+}
+
+static uint32_t refresh_uniform(uint32_t i, uint32_t g, uint32_t rep,
+                                uint32_t step, const uint32_t key[2])
+{
+    return tagged_uniform((uint32_t)TAG_REFRESH, i, g, rep, step, key);
 }
 
 /* Debug/test hook: the uniform itself (pins: uniformity, bit independence). */
@@ -336,6 +341,90 @@ int oracle_refresh(int L, int n_samples, int n_replicas, uint64_t seed,
             mm[i] = (uint8_t)((u >= thr[0]) + (u >= thr[1]) + (u >= thr[2]));
         }
     }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* NEXT-3  Canonical comparator: standard Metropolis on the same         */
+/* checkerboard (Table 3; a fresh random   */
+/* number per spin-flip attempt).  Flip s_x with probability             */
+/* min(1, exp(-dH/T)), dH = 2 s_x h in {0,+-4,+-8,+-12}:                  */
+/*   accept iff dH <= 0 or u < thr[dH/4 - 1],                             */
+/*   thr[k] = floor(exp(-4/T)^(k+1) * 2^32), this operation order:        */
+/*   x = exp(-4/T); x2 = x*x; x3 = x2*x; capped at 2^32                   */
+/* u = the attempt's own 32-bit uniform: the bit-sliced map of the        */
+/* refresh (R8) with domain tag 3 and the sweep index tau in    */
+/* the counter word the refresh uses for its step -- every site is        */
+/* attempted once per sweep, so (site, sample, replica, tau) is unique.   */
+/* ------------------------------------------------------------------ */
+int oracle_metropolis_thresholds(double T, uint64_t thr[3])
+{
+    if (!(T > 0.0) || !isfinite(T)) return -1;
+    const double x  = exp(-4.0 / T);
+    const double x2 = x * x;
+    const double x3 = x2 * x;
+    const double p[3] = { x, x2, x3 };
+    for (int k = 0; k < 3; ++k) {
+        double t = floor(ldexp(p[k], 32));
+        if (t > 4294967296.0) t = 4294967296.0;
+        thr[k] = (uint64_t)t;
+    }
+    return 0;
+}
+
+int oracle_metropolis_half_sweep(int L, int n_samples, int n_replicas, uint64_t seed,
+                                 int sample_offset, double T, uint32_t tau, int parity,
+                                 int8_t *s, const int8_t *J)
+{
+    const int64_t N = (int64_t)L * L * L;
+    uint64_t thr[3];
+    if (oracle_metropolis_thresholds(T, thr) != 0) return -1;
+    uint32_t key[2]; seed_key(seed, key);
+    const int n_sys = n_samples * n_replicas;
+#pragma omp parallel for schedule(static) if (N * n_sys > 65536)
+    for (int sys = 0; sys < n_sys; ++sys) {
+        const int sample = sys / n_replicas, rep = sys % n_replicas;
+        const uint32_t g = (uint32_t)(sample_offset + sample);
+        int8_t *ss = s + (int64_t)sys * N;
+        const int8_t *Jx = J + ((int64_t)sample * 3 + 0) * N;
+        const int8_t *Jy = J + ((int64_t)sample * 3 + 1) * N;
+        const int8_t *Jz = J + ((int64_t)sample * 3 + 2) * N;
+        for (int z = 0; z < L; ++z)
+            for (int y = 0; y < L; ++y)
+                for (int x = 0; x < L; ++x) {
+                    if (((x + y + z) & 1) != parity) continue;
+                    const int64_t i   = x + (int64_t)L * (y + (int64_t)L * z);
+                    const int64_t ixp = wrap(x + 1, L) + (int64_t)L * (y + (int64_t)L * z);
+                    const int64_t ixm = wrap(x - 1, L) + (int64_t)L * (y + (int64_t)L * z);
+                    const int64_t iyp = x + (int64_t)L * (wrap(y + 1, L) + (int64_t)L * z);
+                    const int64_t iym = x + (int64_t)L * (wrap(y - 1, L) + (int64_t)L * z);
+                    const int64_t izp = x + (int64_t)L * (y + (int64_t)L * wrap(z + 1, L));
+                    const int64_t izm = x + (int64_t)L * (y + (int64_t)L * wrap(z - 1, L));
+                    const int h = Jx[i]   * ss[ixp] + Jx[ixm] * ss[ixm]
+                                + Jy[i]   * ss[iyp] + Jy[iym] * ss[iym]
+                                + Jz[i]   * ss[izp] + Jz[izm] * ss[izm];
+                    const int dH = 2 * ss[i] * h;
+                    int accept = (dH <= 0);
+                    if (!accept) {
+                        const uint64_t u = (uint64_t)tagged_uniform((uint32_t)TAG_METROPOLIS, (uint32_t)i, g,
+                                                                    (uint32_t)rep, tau, key);
+                        accept = (u < thr[dH / 4 - 1]);
+                    }
+                    if (accept) ss[i] = (int8_t)(-ss[i]);
+                }
+    }
+    return 0;
+}
+
+/* n Metropolis sweeps (even sites, then odd sites) with sweep indices tau0, tau0+1, ... */
+int oracle_metropolis_sweep(int L, int n_samples, int n_replicas, uint64_t seed,
+                            int sample_offset, double T, uint32_t tau0, int n_sweeps,
+                            int8_t *s, const int8_t *J)
+{
+    for (int t = 0; t < n_sweeps; ++t)
+        for (int parity = 0; parity < 2; ++parity)
+            if (oracle_metropolis_half_sweep(L, n_samples, n_replicas, seed, sample_offset, T,
+                                             tau0 + (uint32_t)t, parity, s, J) != 0) return -1;
     return 0;
 }
 

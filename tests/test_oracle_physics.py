@@ -322,3 +322,86 @@ def test_2x2x2_walkers_match_exact_boltzmann(oracle, T, seed):
     mean, err = per_rep.mean(), per_rep.std(ddof=1) / math.sqrt(nr)
     assert err < 0.01
     assert abs(mean - exact) < 3 * err, (mean, exact, err)
+
+
+# ---------------------------------------------------------------- canonical comparator
+def test_checkerboard_metropolis_acceptance_rates(oracle):
+    """Single-attempt pins: dH <= 0 always flips; dH = +12 / +8 / +4 flips with
+    probability exp(-dH/T) (binomial, 4.5 sigma); thresholds = the Boltzmann
+    factors to 2^-32."""
+    T = 6.0
+    thr = oracle.metropolis_thresholds(T).astype(object)
+    for k in range(3):
+        assert abs(int(thr[k]) / 2.0 ** 32 - math.exp(-4.0 * (k + 1) / T)) <= 2.0 ** -32 + 1e-15
+    hot = [int(v) for v in oracle.metropolis_thresholds(1e9)]
+    assert 2 ** 32 - 100 < hot[2] <= hot[1] <= hot[0] <= 2 ** 32
+    with pytest.raises(ValueError):
+        oracle.metropolis_thresholds(0.0)
+    L, ns, nr = 8, 16, 2
+    N = L ** 3
+    even = (np.indices((L, L, L)).sum(axis=0) % 2 == 0).transpose(2, 1, 0).reshape(-1)      # i = x + L(y + Lz)
+    J = np.ones((ns, 3, N), np.int8)
+    # ferromagnetic ground state: every flip costs +12
+    s = np.ones((ns, nr, N), np.int8)
+    oracle.metropolis_checkerboard(L, s, J, seed=3, T=T, tau0=5, parity=0)
+    assert np.all(s[:, :, ~even] == 1)                                 # the odd sites were not attempted
+    n_att = ns * nr * N // 2
+    flipped = int((s[:, :, even] == -1).sum())
+    p = math.exp(-12.0 / T)
+    assert abs(flipped - n_att * p) < 4.5 * math.sqrt(n_att * p * (1 - p))
+    # Neel state in a ferromagnet: every bond unsatisfied, dH = -12, every attempted spin flips
+    s = np.where(even, 1, -1).astype(np.int8)[None, None, :].repeat(ns, 0).repeat(nr, 1).copy()
+    oracle.metropolis_checkerboard(L, s, J, seed=3, T=T, tau0=5, parity=1)
+    assert np.all(s == 1)
+    # one wrong neighbour each: flipping an even spin whose +x neighbour is already flipped costs +8
+    s = np.ones((ns, nr, N), np.int8)
+    xs = np.arange(N) % L
+    s[:, :, (~even) & (xs % 4 == 1)] = -1                              # odd sites with x = 1 mod 4
+    tgt = even & (xs % 4 == 0)                                         # their -x neighbours: exactly one flipped neighbour
+    oracle.metropolis_checkerboard(L, s, J, seed=4, T=T, tau0=9, parity=0)
+    n_att = ns * nr * int(tgt.sum())
+    flipped = int((s[:, :, tgt] == -1).sum())
+    p = math.exp(-8.0 / T)
+    assert abs(flipped - n_att * p) < 4.5 * math.sqrt(n_att * p * (1 - p))
+    # determinism and the role of the sweep index
+    a = np.ones((ns, nr, N), np.int8); b = a.copy(); c = a.copy()
+    oracle.metropolis_checkerboard(L, a, J, 3, T, tau0=5, n_sweeps=2)
+    oracle.metropolis_checkerboard(L, b, J, 3, T, tau0=5, n_sweeps=2)
+    oracle.metropolis_checkerboard(L, c, J, 3, T, tau0=6, n_sweeps=2)
+    assert np.array_equal(a, b) and not np.array_equal(a, c)
+
+
+@pytest.mark.parametrize("T,seed", [(2.0, 31), (3.0, 32)])
+def test_checkerboard_metropolis_2x2x2_exact_boltzmann(oracle, T, seed):
+    L, N, nr = 2, 8, 64
+    J = random_pm1((1, 3, N), seed)
+    exact = _boltzmann_2x2x2(J[0].tolist(), T)
+    s = oracle.init_spins(L, 1, nr, seed)
+    es = []
+    for tau in range(6000):
+        oracle.metropolis_checkerboard(L, s, J, seed, T, tau0=tau, n_sweeps=1)
+        if tau >= 200:
+            es.append(oracle.measure(L, s, np.zeros_like(s, dtype=np.uint8), J)[0] / float(N))
+    per_rep = np.array(es).mean(axis=0)
+    mean, err = per_rep.mean(), per_rep.std(ddof=1) / math.sqrt(nr)
+    assert err < 0.01 and abs(mean - exact) < 3 * err, (mean, exact, err)
+
+
+def test_checkerboard_metropolis_matches_independent_metropolis(oracle):
+    """Equilibrium energy per spin at T = 2.0 on real-sized lattices against the
+    typewriter-order splitmix64 Metropolis of metropolis_oracle.c (3 sigma)."""
+    L, ns, nr, T = 8, 6, 2, 2.0
+    N = L ** 3
+    J = random_pm1((ns, 3, N), 41)
+    s = random_pm1((ns, nr, N), 42)
+    s_ind = s.copy()
+    es = []
+    for tau in range(700):
+        oracle.metropolis_checkerboard(L, s, J, 7, T, tau0=tau, n_sweeps=1)
+        if tau >= 200:
+            es.append(oracle.measure(L, s, np.zeros_like(s, dtype=np.uint8), J)[0] / float(N))
+    e_chk = np.array(es).mean(axis=0)
+    e_ind = oracle.metropolis(L, s_ind, J, T, 700, seed=5)[200:].mean(axis=0)
+    d = e_chk.mean() - e_ind.mean()
+    err = math.sqrt(e_chk.var(ddof=1) / e_chk.size + e_ind.var(ddof=1) / e_ind.size)
+    assert abs(d) < 3 * err + 2e-3, (d, err)
