@@ -149,6 +149,20 @@ int micsa_set_walkers(micsa_ctx *ctx, int mode);
 int micsa_set_time(micsa_ctx *ctx, int64_t t);
 int micsa_get_time(micsa_ctx *ctx, int64_t *t);
 
+/* ---- canonical comparator (PAPER.md:339-350 Table 3, :130) -----------------
+ * micsa_metropolis_sweep: n standard Metropolis sweeps (even sites, then odd
+ * sites) at temperature T on the same spins and couplings: flip with
+ * probability min(1, exp(-dH/T)); daemons are neither read nor written.  One
+ * 32-bit uniform per attempt, defined bit-sliced like the refresh's (DESIGN.md
+ * 2.1) with domain tag 3 and the sweep index tau0 + k where the refresh has its
+ * step; accept iff dH <= 0 or u < floor(exp(-dH/T) * 2^32)
+ * (micsa_debug_metropolis_thresholds gives the three integers for dH = 4, 8,
+ * 12).  The caller chooses tau0 so that sweep indices never repeat.
+ * micsa_metropolis_half_sweep: one parity, index tau.  Asynchronous. */
+int micsa_metropolis_sweep(micsa_ctx *ctx, double T, uint32_t tau0, int n);
+int micsa_metropolis_half_sweep(micsa_ctx *ctx, double T, uint32_t tau, int parity);
+int micsa_debug_metropolis_thresholds(double T, uint64_t thr[3]);
+
 /* micsa_refresh_demons: every daemon <- independent draw from Eq. (11),
  * p(n=4m) ~ exp(-4m/T), m = 0..3; spins untouched
  * (PAPER.md:190).  One 32-bit uniform u per daemon, compared with integer
@@ -220,7 +234,8 @@ int micsa_anneal(micsa_ctx *ctx, const micsa_step *sched, int n_steps,
                  uint32_t step0, double *min_energy, micsa_trace *trace);
 
 /* Running totals since create: spin-flip attempts; 32-bit uniforms the
- * refreshes are defined on (one per daemon, R8); Philox4x32-10
+ * refreshes are defined on (one per daemon, R8) plus one per Metropolis
+ * attempt; Philox4x32-10
  * blocks the refresh kernels actually evaluated.  The refresh compares
  * bit-plane by bit-plane and stops once every lane is decided, so the last is
  * data dependent (about half of the 1 block per 4 daemons a full evaluation

@@ -32,6 +32,7 @@ EXPORTS = (
     "micsa_measure", "micsa_anneal", "micsa_counters", "micsa_layout_info",
     "micsa_set_tuning",
     "micsa_prefetch_refresh", "micsa_measure_begin", "micsa_measure_end", "micsa_sweep_measure",
+    "micsa_metropolis_sweep", "micsa_metropolis_half_sweep", "micsa_debug_metropolis_thresholds",
     "micsa_wander", "micsa_set_walkers", "micsa_set_time", "micsa_get_time",
 )
 
@@ -91,6 +92,8 @@ def _bind() -> ctypes.CDLL:
             ("micsa_set_couplings", [vp, vp]), ("micsa_set_spins", [vp, vp]),
             ("micsa_set_daemons", [vp, vp]), ("micsa_get_state", [vp, vp, vp, vp]),
             ("micsa_sweep", [vp, i32]), ("micsa_sweep_measure", [vp, i32]),
+            ("micsa_metropolis_sweep", [vp, f64, u32, i32]), ("micsa_metropolis_half_sweep", [vp, f64, u32, i32]),
+            ("micsa_debug_metropolis_thresholds", [f64, vp]),
             ("micsa_wander", [vp, i32, i32, i32]), ("micsa_set_walkers", [vp, i32]),
             ("micsa_set_time", [vp, ctypes.c_int64]), ("micsa_get_time", [vp, vp]), ("micsa_half_sweep", [vp, i32]),
             ("micsa_refresh_demons", [vp, f64, u32]),
@@ -127,6 +130,12 @@ def debug_thresholds(T: float) -> np.ndarray:
     """micsa_debug_thresholds: the integer thresholds of Eq. (11) (R7)."""
     thr = np.zeros(3, dtype=np.uint64)
     _check(_lib.micsa_debug_thresholds(float(T), _ptr(thr)))
+    return thr
+
+
+def debug_metropolis_thresholds(T: float) -> np.ndarray:
+    thr = np.zeros(3, dtype=np.uint64)
+    _check(_lib.micsa_debug_metropolis_thresholds(float(T), _ptr(thr)))
     return thr
 
 
@@ -221,6 +230,12 @@ class MicSA:
     def sweep_measure(self, n=1):
         """n sweeps, then the measurement queued (fetch it with measure_end)."""
         _check(_lib.micsa_sweep_measure(self._h, int(n)))
+
+    def metropolis_sweep(self, T, tau0, n=1):
+        _check(_lib.micsa_metropolis_sweep(self._h, float(T), int(tau0), int(n)))
+
+    def metropolis_half_sweep(self, T, tau, parity):
+        _check(_lib.micsa_metropolis_half_sweep(self._h, float(T), int(tau), int(parity)))
 
     def wander(self, axis=0, sign=+1, parity=0):
         _check(_lib.micsa_wander(self._h, int(axis), int(sign), int(parity)))

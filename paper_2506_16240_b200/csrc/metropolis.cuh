@@ -1,0 +1,104 @@
+// metropolis.cuh -- canonical comparator (PAPER.md:339-350
+// Table 3, :130): standard Metropolis on the same checkerboard and the same
+// bit-sliced layout, with a fresh random number per spin-flip attempt.
+//
+// Flip with probability min(1, exp(-dH/T)), dH = 12 - 4U for U unsatisfied
+// bonds: always if U >= 3, else iff u < thr[2-U], thr[k] = floor(exp(-4(k+1)/T)
+// * 2^32) from the host.  u is the attempt's own 32-bit uniform, defined
+// bit-sliced exactly like the refresh's with domain tag 3 and
+// the sweep index tau where the refresh has its step -- so the same
+// lane-parallel, most-significant-plane-first compare applies (refresh_chunk)
+// and planes that cannot change any decision are never generated: a lane only
+// takes part in the compare with the one threshold its U selects, and not at
+// all when dH <= 0.  No daemons are read or written.
+#pragma once
+#include "layout.cuh"
+#include "philox.cuh"
+#include "refresh.cuh"
+
+namespace micsa {
+
+struct MetropolisArgs {
+    uint32_t* spin; const void* J;
+    int L, Lh, n_rg, n_samples, sample_offset;
+    long long half;
+};
+
+// grid = (ceil(L*Lh/128), L, n_words); one thread = one word of the parity-p array
+template <int RPW>
+__global__ void __launch_bounds__(128)
+metropolis_half_sweep_kernel(MetropolisArgs a, int p, PhiloxKeys ks, uint32_t tau, RefreshThr thr,
+                             unsigned long long* __restrict__ n_calls)
+{
+    typedef typename BondT<RPW>::type JT;
+    constexpr int SPW = 32 / RPW;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned int calls = 0;
+    if (t < a.L * a.Lh) {
+        const int L = a.L, Lh = a.Lh, q = 1 - p;
+        const int y = t / Lh, xh = t - y * Lh;
+        const int z = blockIdx.y, w = blockIdx.z;
+        const long long half = a.half;
+        uint32_t* sp = a.spin + ((long long)w * 2 + p) * half;
+        const uint32_t* sq = a.spin + ((long long)w * 2 + q) * half;
+        const int sg = w / a.n_rg, rg = w - sg * a.n_rg;
+        const JT* Jb = reinterpret_cast<const JT*>(a.J) + (long long)sg * 6 * half;
+        const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
+        const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+        const long long row = ((long long)z * L + y) * Lh, h = row + xh;
+        const long long h_yp = ((long long)z * L + yp) * Lh + xh, h_ym = ((long long)z * L + ym) * Lh + xh;
+        const long long h_zp = ((long long)zp * L + y) * Lh + xh, h_zm = ((long long)zm * L + y) * Lh + xh;
+        // c = 1: x = 2xh+1, -x neighbour at xh (it owns the bond), +x neighbour at xh+1
+        // c = 0: x = 2xh,   +x neighbour at xh, -x neighbour at xh-1 (it owns the bond)
+        const int c = (y + z + p) & 1;
+        const int xo = c ? ((xh + 1 == Lh) ? 0 : xh + 1) : ((xh == 0) ? Lh - 1 : xh - 1);
+        const uint32_t s = sp[h];
+        const uint32_t A = sq[h], E = sq[row + xo];
+        const uint32_t n_xp = c ? E : A, n_xm = c ? A : E;
+        const uint32_t j_xp = bond_expand<RPW>(Jb[(0 * 2 + p) * half + h]);
+        const uint32_t j_xm = bond_expand<RPW>(Jb[(0 * 2 + q) * half + (c ? h : row + xo)]);
+        const uint32_t u1 = s ^ n_xp ^ j_xp, u2 = s ^ n_xm ^ j_xm;
+        const uint32_t u3 = s ^ sq[h_yp] ^ bond_expand<RPW>(Jb[(1 * 2 + p) * half + h]);
+        const uint32_t u4 = s ^ sq[h_ym] ^ bond_expand<RPW>(Jb[(1 * 2 + q) * half + h_ym]);
+        const uint32_t u5 = s ^ sq[h_zp] ^ bond_expand<RPW>(Jb[(2 * 2 + p) * half + h]);
+        const uint32_t u6 = s ^ sq[h_zm] ^ bond_expand<RPW>(Jb[(2 * 2 + q) * half + h_zm]);
+        // U = number of unsatisfied bonds, 3 planes
+        const uint32_t sa = u1 ^ u2 ^ u3, ca = (u1 & u2) | (u3 & (u1 ^ u2));
+        const uint32_t sb = u4 ^ u5 ^ u6, cb = (u4 & u5) | (u6 & (u4 ^ u5));
+        const uint32_t U0 = sa ^ sb, cc = sa & sb;
+        const uint32_t U1 = ca ^ cb ^ cc, U2 = (ca & cb) | (cc & (ca ^ cb));
+        const uint32_t vm = valid_lane_mask<RPW>(a.n_samples, sg);
+        const uint32_t always = U2 | (U1 & U0);                     // U >= 3: dH <= 0
+        const uint32_t need[3] = { ~U2 & U1 & ~U0, ~U2 & ~U1 & U0, ~U2 & ~U1 & ~U0 };   // U = 2, 1, 0: dH = 4, 8, 12
+
+        RefreshWord wd;
+        const uint32_t blk = (uint32_t)(a.sample_offset + sg * SPW) >> 4;
+        wd.i = canonical_site(L, p, z, y, xh);
+        wd.blk_a = blk; wd.blk_b = (RPW == 2) ? blk : blk + 1u;
+        wd.rep_a = kTagMetropolis | (uint32_t)(rg * RPW);
+        wd.rep_b = (RPW == 2) ? wd.rep_a + 1u : wd.rep_a;
+        wd.has_b = (vm >> 16) != 0u;
+        uint32_t EQ[3], gt[3] = { 0u, 0u, 0u };
+#pragma unroll
+        for (int k = 0; k < 3; ++k) EQ[k] = thr.never[k] ? 0u : (need[k] & vm);
+#pragma unroll 1
+        for (uint32_t cchunk = 0; cchunk < 4 && (EQ[0] | EQ[1] | EQ[2]) != 0u; ++cchunk) {
+            refresh_chunk<-1>(cchunk, wd, tau, EQ, gt, thr, ks);
+            calls += wd.has_b ? 2u : 1u;
+        }
+        // u >= thr_k where the lane is above or equal in all planes seen; accept iff u < thr
+        uint32_t acc = always;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) acc |= need[k] & ~(gt[k] | EQ[k]);
+        sp[h] = s ^ (acc & vm);
+    }
+    calls = __reduce_add_sync(0xFFFFFFFFu, calls);
+    __shared__ unsigned int s_calls;
+    if (threadIdx.x == 0) s_calls = 0;
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0 && calls) atomicAdd(&s_calls, calls);
+    __syncthreads();
+    if (threadIdx.x == 0 && s_calls) atomicAdd(n_calls, (unsigned long long)s_calls);
+}
+
+}  // namespace micsa

@@ -13,6 +13,7 @@
 
 #include "layout.cuh"
 #include "measure.cuh"
+#include "metropolis.cuh"
 #include "pack.cuh"
 #include "philox.cuh"
 #include "refresh.cuh"
@@ -429,6 +430,43 @@ int thresholds_host(double T, uint64_t thr[3]) {
         thr[k] = (uint64_t)t;
     }
     return MICSA_OK;
+}
+
+int metropolis_thresholds_host(double T, uint64_t thr[3]) {
+    if (!(T > 0.0) || !std::isfinite(T)) return MICSA_ERR_INVALID;
+    // Boltzmann factors of dH = 4, 8, 12 in float64, this operation order (metropolis.cuh)
+    const double x = std::exp(-4.0 / T);
+    const double x2 = x * x;
+    const double x3 = x2 * x;
+    const double p[3] = { x, x2, x3 };
+    for (int k = 0; k < 3; ++k) {
+        double t = std::floor(std::ldexp(p[k], 32));
+        if (t > 4294967296.0) t = 4294967296.0;
+        thr[k] = (uint64_t)t;
+    }
+    return MICSA_OK;
+}
+
+RefreshThr make_thr(const uint64_t thr[3]) {
+    RefreshThr rt;
+    for (int k = 0; k < 3; ++k) {
+        rt.never[k] = (thr[k] >> 32) ? 1u : 0u;
+        for (int p = 0; p < 32; ++p) rt.tb[k][p] = ((thr[k] >> (31 - p)) & 1u) ? 0xFFFFFFFFu : 0u;
+    }
+    return rt;
+}
+
+int launch_metropolis_half_sweep(micsa_ctx* c, const RefreshThr& rt, uint32_t tau, int parity) {
+    const Geom& g = c->g;
+    MetropolisArgs a;
+    a.spin = c->st.spin; a.J = c->st.J; a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg;
+    a.n_samples = g.n_samples; a.sample_offset = g.sample_offset; a.half = g.half;
+    const dim3 grid = site_blocks(g, g.n_words);
+    if (g.rpw == 2) metropolis_half_sweep_kernel<2><<<grid, 128, 0, c->stream>>>(a, parity, c->ks, tau, rt, c->calls);
+    else            metropolis_half_sweep_kernel<1><<<grid, 128, 0, c->stream>>>(a, parity, c->ks, tau, rt, c->calls);
+    c->attempts += (uint64_t)(g.N / 2) * (uint64_t)g.n_sys;
+    c->rns += (uint64_t)(g.N / 2) * (uint64_t)g.n_sys;
+    return post_launch(c);
 }
 
 int launch_refresh_into(micsa_ctx* c, double T, uint32_t step, uint32_t* m0, uint32_t* m1,
@@ -866,6 +904,33 @@ int micsa_set_time(micsa_ctx* c, int64_t t) {
 int micsa_get_time(micsa_ctx* c, int64_t* t) {
     if (!c || !t) { set_err("null pointer"); return MICSA_ERR_INVALID; }
     *t = c->t;
+    return MICSA_OK;
+}
+
+int micsa_metropolis_sweep(micsa_ctx* c, double T, uint32_t tau0, int n) {
+    int rc = check_ctx(c); if (rc) return rc;
+    uint64_t thr[3];
+    if (n < 0 || metropolis_thresholds_host(T, thr) != MICSA_OK) { set_err("n must be >= 0 and T finite and > 0"); return MICSA_ERR_INVALID; }
+    const RefreshThr rt = make_thr(thr);
+    for (int t = 0; t < n; ++t)
+        for (int parity = 0; parity < 2; ++parity) {
+            rc = launch_metropolis_half_sweep(c, rt, tau0 + (uint32_t)t, parity); if (rc) return rc;
+        }
+    return MICSA_OK;
+}
+
+int micsa_metropolis_half_sweep(micsa_ctx* c, double T, uint32_t tau, int parity) {
+    int rc = check_ctx(c); if (rc) return rc;
+    uint64_t thr[3];
+    if ((parity != 0 && parity != 1) || metropolis_thresholds_host(T, thr) != MICSA_OK) {
+        set_err("parity must be 0 or 1 and T finite and > 0"); return MICSA_ERR_INVALID;
+    }
+    return launch_metropolis_half_sweep(c, make_thr(thr), tau, parity);
+}
+
+int micsa_debug_metropolis_thresholds(double T, uint64_t thr[3]) {
+    if (!thr) { set_err("null pointer"); return MICSA_ERR_INVALID; }
+    if (metropolis_thresholds_host(T, thr) != MICSA_OK) { set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID; }
     return MICSA_OK;
 }
 

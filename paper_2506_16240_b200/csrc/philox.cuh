@@ -42,6 +42,6 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
 }
 
 // domain tags carried in the top byte of counter word c2
-enum : uint32_t { kTagRefresh = 0u, kTagSpinInit = 1u << 24, kTagBondInit = 2u << 24 };
+enum : uint32_t { kTagRefresh = 0u, kTagSpinInit = 1u << 24, kTagBondInit = 2u << 24, kTagMetropolis = 3u << 24 };
 
 }  // namespace micsa

@@ -516,3 +516,44 @@ def test_walker_timesteps_bit_exact(micsa, oracle, L, ns, nr, tune):
         for tt in range(L):
             g.wander(1, -1, tt & 1)
         np.testing.assert_array_equal(g.get_state(spins=False, couplings=False)[1], lab)
+
+
+# ---------------------------------------------------------------- canonical comparator
+@pytest.mark.parametrize("L,ns,nr", SHAPES)
+def test_metropolis_bit_exact(micsa, oracle, L, ns, nr):
+    """Standard Metropolis with one Philox uniform per attempt: spins equal the
+    oracle's after every half-sweep and after blocks of sweeps, at a hot, a
+    critical and a cold temperature (thresholds saturate), with a sample offset."""
+    N = L ** 3
+    for T in (50.0, 3.0, 1.1, 0.3):
+        np.testing.assert_array_equal(micsa.debug_metropolis_thresholds(T), oracle.metropolis_thresholds(T))
+    for seed, off, T in [(1, 0, 2.0), (77, 32, 0.9)]:
+        s = oracle.init_spins(L, ns, nr, seed, off); J = oracle.init_bonds(L, ns, seed, off)
+        m = np.zeros_like(s, dtype=np.uint8)
+        with micsa.MicSA(L, ns, nr, seed, sample_offset=off) as g:
+            for tau in range(3):
+                for p in (0, 1):
+                    g.metropolis_half_sweep(T, tau, p)
+                    oracle.metropolis_checkerboard(L, s, J, seed, T, tau0=tau, sample_offset=off, parity=p)
+                    _assert_state(g, s, m, J)
+            g.metropolis_sweep(T, 100, 4)
+            oracle.metropolis_checkerboard(L, s, J, seed, T, tau0=100, n_sweeps=4, sample_offset=off)
+            _assert_state(g, s, m, J)
+            g.metropolis_sweep(0.2, 2 ** 32 - 2, 2)                       # deep quench, index at the top of its range
+            oracle.metropolis_checkerboard(L, s, J, seed, 0.2, tau0=2 ** 32 - 2, n_sweeps=2, sample_offset=off)
+            _assert_state(g, s, m, J)
+            with pytest.raises(micsa.MicsaError):
+                g.metropolis_sweep(0.0, 0, 1)
+
+
+def test_metropolis_config2_sampled(micsa, oracle):
+    """Config 2's shape at full size: 20 Metropolis sweeps, sampled systems against the oracle."""
+    cfg = CONFIGS[2]
+    L, nr, T = cfg.L, cfg.n_replicas, 2.0
+    with micsa.MicSA(L, cfg.n_samples, nr, cfg.seed) as g:
+        g.metropolis_sweep(T, 0, 20)
+        gs = g.get_state(daemons=False, couplings=False)[0]
+    for k in (0, 28, 60):
+        s = oracle.init_spins(L, 4, nr, cfg.seed, sample_offset=k); J = oracle.init_bonds(L, 4, cfg.seed, sample_offset=k)
+        oracle.metropolis_checkerboard(L, s, J, cfg.seed, T, tau0=0, n_sweeps=20, sample_offset=k)
+        np.testing.assert_array_equal(gs[k:k + 4], s)
