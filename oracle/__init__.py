@@ -223,6 +223,16 @@ def measure(L, s, m, J):
     return E, Ed, Q
 
 
+def c4(L, s) -> np.ndarray:
+    """S[pair, axis, r] = sum_x q_x q_{x + r e_axis}, q = s^a s^b, r = 0..L/2 (Eq. 16
+    before normalisation); pairs ordered like Q in measure()."""
+    ns, nr, N = s.shape
+    assert N == L ** 3 and s.dtype == np.int8 and s.flags.c_contiguous
+    S = np.zeros((ns * nr * (nr - 1) // 2, 3, L // 2 + 1), dtype=np.int64)
+    lib().oracle_c4(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr), _p(s, _c_i8p), _p(S, _c_i64p))
+    return S
+
+
 def metropolis(L, s, J, T, n_sweeps, seed):
     """Independent textbook Metropolis (metropolis_oracle.c); s updated in
     place; returns the energy per spin after each sweep, float64

@@ -482,3 +482,40 @@ void oracle_measure(int L, int n_samples, int n_replicas,
                 }
     }
 }
+
+/* ------------------------------------------------------------------ */
+/* NEXT-2  Four-point replica correlation along the axes, Eq. (16)       */
+/* before the normalisation and the average over      */
+/* axes: for the replica pair (a<b) of a sample, axis d and r = 0..L/2,   */
+/*   S[pair][d][r] = sum_x q_x q_{x + r e_d},  q_x = s^a_x s^b_x,          */
+/* periodic.  C4(r) = (S[.][0][r] + S[.][1][r] + S[.][2][r]) / (3N) for    */
+/* one pair.  Pairs ordered like Q in oracle_measure.                     */
+/* ------------------------------------------------------------------ */
+void oracle_c4(int L, int n_samples, int n_replicas, const int8_t *s, int64_t *S)
+{
+    const int64_t N = (int64_t)L * L * L;
+    const int R = L / 2 + 1;
+    int64_t k = 0;
+    for (int sample = 0; sample < n_samples; ++sample)
+        for (int a = 0; a < n_replicas; ++a)
+            for (int b = a + 1; b < n_replicas; ++b, ++k) {
+                const int8_t *sa = s + ((int64_t)sample * n_replicas + a) * N;
+                const int8_t *sb = s + ((int64_t)sample * n_replicas + b) * N;
+                for (int d = 0; d < 3; ++d)
+                    for (int r = 0; r < R; ++r) {
+                        int64_t acc = 0;
+                        for (int z = 0; z < L; ++z)
+                            for (int y = 0; y < L; ++y)
+                                for (int x = 0; x < L; ++x) {
+                                    const int xn = (d == 0) ? wrap(x + r, L) : x;
+                                    const int yn = (d == 1) ? wrap(y + r, L) : y;
+                                    const int zn = (d == 2) ? wrap(z + r, L) : z;
+                                    const int64_t i = x + (int64_t)L * (y + (int64_t)L * z);
+                                    const int64_t j = xn + (int64_t)L * (yn + (int64_t)L * zn);
+                                    acc += (int64_t)(sa[i] * sb[i]) * (sa[j] * sb[j]);
+                                }
+                        S[(k * 3 + d) * R + r] = acc;
+                    }
+            }
+}
+

@@ -258,3 +258,33 @@ def test_paper_table3_consistency():
     assert abs(t["metropolis_rng"] / metro - 0.72) < 0.01
     attempts = 160 ** 3 * 128
     assert abs(mic * 1e3 / attempts - 0.4) < 0.02          # "~0.4 ps"
+
+
+# ---------------------------------------------------------------- C4 (Eq. 16)
+@pytest.mark.parametrize("L,ns,nr", [(4, 2, 2), (6, 1, 3), (8, 2, 2)])
+def test_c4_against_numpy_roll_and_identities(oracle, L, ns, nr):
+    N = L ** 3
+    s = random_pm1((ns, nr, N), 91)
+    S = oracle.c4(L, s)
+    assert S.shape == (ns * nr * (nr - 1) // 2, 3, L // 2 + 1)
+    k = 0
+    for sample in range(ns):
+        for a in range(nr):
+            for b in range(a + 1, nr):
+                q = (s[sample, a].astype(np.int64) * s[sample, b]).reshape(L, L, L)      # [z, y, x]
+                for d, ax in enumerate((2, 1, 0)):                                      # x is the last numpy axis
+                    for r in range(L // 2 + 1):
+                        assert S[k, d, r] == int((q * np.roll(q, -r, axis=ax)).sum())
+                    # sum over all displacements along the axis = sum of squared line sums
+                    full = sum(int((q * np.roll(q, -r, axis=ax)).sum()) for r in range(L))
+                    assert full == int((q.sum(axis=ax) ** 2).sum())
+                    # S(r) = S(L - r): the half range holds everything
+                    assert full == int(S[k, d, 0] + 2 * S[k, d, 1:L // 2].sum() + S[k, d, L // 2])
+                assert np.all(S[k, :, 0] == N)
+                k += 1
+    same = np.repeat(random_pm1((1, 1, N), 92), 2, axis=1)                              # identical replicas
+    assert np.all(oracle.c4(L, same) == N)
+    stag = np.where(np.indices((L, L, L)).sum(axis=0) % 2 == 0, 1, -1).astype(np.int8).reshape(1, 1, N)
+    pair = np.concatenate([stag, np.ones((1, 1, N), np.int8)], axis=1)                  # q = staggered field
+    want = np.array([N * (-1) ** r for r in range(L // 2 + 1)])
+    assert np.all(oracle.c4(L, pair)[0] == want[None, :])
