@@ -204,6 +204,16 @@ int micsa_debug_thresholds(double T, uint64_t thr[3]);
  * q of Eq. C.1).  Q != NULL with n_replicas < 2 -> MICSA_ERR_INVALID.        */
 int micsa_measure_i64(micsa_ctx *ctx, int64_t *E, int64_t *E_daemon, int64_t *Q);
 
+/* micsa_measure_c4 (synchronous): four-point replica correlation along the
+ * lattice axes, Eq. (16), as exact integer sums for the
+ * replica pair of every sample (n_replicas must be 2, else MICSA_ERR_INVALID):
+ *   S[n_samples][3][L/2 + 1],  S[s][d][r] = sum_x q_x q_{x + r e_d},  q = s^a s^b,
+ * periodic; d = 0,1,2 = x,y,z.  C4(r) of Eq. (16) for one pair =
+ * (S[s][0][r] + S[s][1][r] + S[s][2][r]) / (3N).  The integrals I_n and xi_12
+ * (Eq. 17-18) need the cut-off procedure of the paper's refs. [61,46] and are
+ * left to the caller.  Caller-owned host array. */
+int micsa_measure_c4(micsa_ctx *ctx, int64_t *S);
+
 /* The same measurement split in two, so that the caller can queue more work
  * (or stop a timer on the stream) before waiting: micsa_measure_begin queues
  * the reduction kernel and the device->host copy of the row into pinned memory

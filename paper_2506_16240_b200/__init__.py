@@ -32,7 +32,7 @@ EXPORTS = (
     "micsa_measure", "micsa_anneal", "micsa_counters", "micsa_layout_info",
     "micsa_set_tuning",
     "micsa_prefetch_refresh", "micsa_measure_begin", "micsa_measure_end", "micsa_sweep_measure",
-    "micsa_metropolis_sweep", "micsa_metropolis_half_sweep", "micsa_debug_metropolis_thresholds",
+    "micsa_measure_c4", "micsa_metropolis_sweep", "micsa_metropolis_half_sweep", "micsa_debug_metropolis_thresholds",
     "micsa_wander", "micsa_set_walkers", "micsa_set_time", "micsa_get_time",
 )
 
@@ -100,7 +100,7 @@ def _bind() -> ctypes.CDLL:
             ("micsa_prefetch_refresh", [vp, f64, u32]),
             ("micsa_debug_thresholds", [f64, vp]),
             ("micsa_measure_i64", [vp, vp, vp, vp]),
-            ("micsa_measure_begin", [vp]), ("micsa_measure_end", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
+            ("micsa_measure_c4", [vp, vp]), ("micsa_measure_begin", [vp]), ("micsa_measure_end", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
             ("micsa_anneal", [vp, vp, i32, u32, vp, vp]),
             ("micsa_counters", [vp, vp, vp, vp]), ("micsa_layout_info", [vp, vp]),
             ("micsa_set_tuning", [vp, i32, i32])):
@@ -266,6 +266,12 @@ class MicSA:
         Q = np.empty(self.n_pairs, np.int64) if self.n_replicas >= 2 else None
         _check(_lib.micsa_measure_i64(self._h, _ptr(E), _ptr(Ed), _ptr(Q)))
         return E, Ed, (Q if Q is not None else np.empty(0, np.int64))
+
+    def measure_c4(self):
+        """S[sample, axis, r] = sum_x q_x q_{x + r e_axis} (exact int64), r = 0..L/2."""
+        S = np.empty((self.n_samples, 3, self.L // 2 + 1), np.int64)
+        _check(_lib.micsa_measure_c4(self._h, _ptr(S)))
+        return S
 
     def measure_begin(self):
         _check(_lib.micsa_measure_begin(self._h))

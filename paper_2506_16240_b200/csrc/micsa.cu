@@ -13,6 +13,7 @@
 
 #include "layout.cuh"
 #include "measure.cuh"
+#include "c4.cuh"
 #include "metropolis.cuh"
 #include "pack.cuh"
 #include "philox.cuh"
@@ -985,6 +986,39 @@ int micsa_measure_i64(micsa_ctx* c, int64_t* E, int64_t* Ed, int64_t* Q) {
     if (Q && c->g.n_replicas < 2) { set_err("q_overlap needs n_replicas >= 2"); return MICSA_ERR_INVALID; }
     rc = micsa_measure_begin(c); if (rc) return rc;
     return micsa_measure_end(c, E, Ed, Q);
+}
+
+int micsa_measure_c4(micsa_ctx* c, int64_t* S) {
+    int rc = check_ctx(c); if (rc) return rc;
+    const Geom& g = c->g;
+    if (!S) { set_err("null pointer"); return MICSA_ERR_INVALID; }
+    if (g.n_replicas != 2) { set_err("micsa_measure_c4 needs n_replicas == 2"); return MICSA_ERR_INVALID; }
+    const int R = g.L / 2 + 1;
+    const size_t x_bytes = (size_t)g.n_sg * (size_t)g.N * sizeof(uint32_t);
+    const size_t cnt_words = (size_t)g.n_sg * 3 * R * 32;
+    Staging X, cnt;
+    if (cudaMalloc(&X.dev, x_bytes) != cudaSuccess || cudaMalloc(&cnt.dev, cnt_words * 8) != cudaSuccess) {
+        cudaGetLastError(); set_err("out of device memory (c4)"); return MICSA_ERR_NOMEM;
+    }
+    CK(c, cudaMemsetAsync(cnt.dev, 0, cnt_words * 8, c->stream));
+    overlap_field_kernel<<<site_blocks(g, g.n_sg * 2), 128, 0, c->stream>>>(c->st.spin, (uint32_t*)X.dev, g.L, g.Lh, g.half);
+    // every thread counts at most 65535 sites (16-plane counters)
+    long long nb = std::max<long long>(1, std::min<long long>((g.N + kCountBlock * 64 - 1) / (kCountBlock * 64), 64));
+    nb = std::max<long long>(nb, (g.N + (long long)kCountBlock * 60000 - 1) / ((long long)kCountBlock * 60000));
+    c4_count_kernel<<<dim3((unsigned)nb, (unsigned)R, (unsigned)(3 * g.n_sg)), kCountBlock, 0, c->stream>>>(
+        (const uint32_t*)X.dev, (unsigned long long*)cnt.dev, g.L);
+    rc = post_launch(c, 2); if (rc) return rc;
+    std::vector<unsigned long long> host(cnt_words);
+    CK(c, cudaMemcpyAsync(host.data(), cnt.dev, cnt_words * 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(c, cudaStreamSynchronize(c->stream));
+    for (int sample = 0; sample < g.n_samples; ++sample) {
+        const int sg = sample / g.spw, sl = sample - sg * g.spw;
+        for (int d = 0; d < 3; ++d)
+            for (int r = 0; r < R; ++r)
+                S[((size_t)sample * 3 + d) * R + r] =
+                    (int64_t)g.N - 2 * (int64_t)host[(((size_t)sg * 3 + d) * R + r) * 32 + sl];
+    }
+    return MICSA_OK;
 }
 
 int micsa_measure(micsa_ctx* c, double* e, double* ed, double* q) {

@@ -557,3 +557,32 @@ def test_metropolis_config2_sampled(micsa, oracle):
         s = oracle.init_spins(L, 4, nr, cfg.seed, sample_offset=k); J = oracle.init_bonds(L, 4, cfg.seed, sample_offset=k)
         oracle.metropolis_checkerboard(L, s, J, cfg.seed, T, tau0=0, n_sweeps=20, sample_offset=k)
         np.testing.assert_array_equal(gs[k:k + 4], s)
+
+
+# ---------------------------------------------------------------- C4
+@pytest.mark.parametrize("L,ns", [(8, 1), (2, 1), (4, 3), (6, 17), (8, 40), (16, 5), (24, 2)])
+def test_c4_exact(micsa, oracle, L, ns):
+    nr, N = 2, L ** 3
+    s = random_pm1((ns, nr, N), 81)
+    with micsa.MicSA(L, ns, nr, 1) as g:
+        g.set_spins(s)
+        np.testing.assert_array_equal(g.measure_c4(), oracle.c4(L, s))
+        g.refresh_demons(1.0, 0); g.sweep(3)                   # correlated replicas after a short quench
+        gs = g.get_state(daemons=False, couplings=False)[0]
+        S = g.measure_c4()
+        np.testing.assert_array_equal(S, oracle.c4(L, gs))
+        assert np.all(S[:, :, 0] == N)
+    with micsa.MicSA(L, ns, 3, 1) as g3:
+        with pytest.raises(micsa.MicsaError):
+            g3.measure_c4()
+
+
+def test_c4_config3_shape(micsa, oracle):
+    """L = 80, two of the 128 samples of config 3 against the oracle."""
+    cfg = CONFIGS[3]
+    with micsa.MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed) as g:
+        g.refresh_demons(0.7, 0); g.sweep(5)
+        S = g.measure_c4()
+        gs = g.get_state(daemons=False, couplings=False)[0]
+    for k in (0, 127):
+        np.testing.assert_array_equal(S[k], oracle.c4(cfg.L, gs[k:k + 1])[0])
