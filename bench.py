@@ -165,6 +165,8 @@ def main():
     ap.add_argument("--impl", default="micsa", choices=["micsa", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
+                    help="micsa_set_tuning for A/B runs, e.g. --tune pipe_smem_kb=48")
     ap.add_argument("--walkers", action="store_true",
                     help="one forward-X walker per spin instead of a daemon (PAPER.md Sec. 2.6): every sweep is "
                          "followed by a wandering half-cycle; reported under its own metric name")
@@ -219,6 +221,9 @@ def main():
         g.set_tuning("fuse_measure", 0)
     if args.walkers:
         g.set_walkers(1)
+    for kv in args.tune:
+        k, v = kv.split("=")
+        g.set_tuning(k, int(v))
     info = g.layout_info()
     attempts_step = CFG.attempts_per_sweep * SWEEPS_PER_STEP
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2

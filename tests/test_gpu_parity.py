@@ -586,3 +586,32 @@ def test_c4_config3_shape(micsa, oracle):
         gs = g.get_state(daemons=False, couplings=False)[0]
     for k in (0, 127):
         np.testing.assert_array_equal(S[k], oracle.c4(cfg.L, gs[k:k + 1])[0])
+
+
+def test_config4_walkers_and_metropolis_sampled(micsa, oracle):
+    """The headline lattice at full size with the two comparison dynamics: walker
+    timesteps in the launch configuration bench.py --walkers times (refresh +
+    9 timesteps + measuring timestep per step, fused exchange), and Metropolis
+    sweeps; sampled systems against the oracle."""
+    cfg = CONFIGS[4]
+    L, nr = cfg.L, cfg.n_replicas
+    sched = schedule_for(cfg, n_sweeps=20, measure_every=10)
+    with micsa.MicSA(L, cfg.n_samples, nr, cfg.seed) as g:
+        g.set_walkers(1)
+        out = g.anneal(sched)
+        ws, wm, _ = g.get_state(couplings=False)
+        assert g.get_time() == 20
+        g.set_walkers(0)
+        g.metropolis_sweep(0.9, 0, 3)
+        ms = g.get_state(daemons=False, couplings=False)[0]
+    for k in (0, 15):
+        s = oracle.init_spins(L, 1, nr, cfg.seed, sample_offset=k); J = oracle.init_bonds(L, 1, cfg.seed, sample_offset=k)
+        m = np.zeros_like(s, dtype=np.uint8)
+        ref = driver.anneal(L, s, m, J, cfg.seed, sched, sample_offset=k, walkers=True)
+        np.testing.assert_array_equal(ws[k:k + 1], s)
+        np.testing.assert_array_equal(wm[k:k + 1], m)
+        np.testing.assert_array_equal(out["E"][:, k * nr:(k + 1) * nr], ref["E"])
+        np.testing.assert_array_equal(out["Edem"][:, k * nr:(k + 1) * nr], ref["Edem"])
+        np.testing.assert_array_equal(out["Q"][:, k:k + 1], ref["Q"])
+        oracle.metropolis_checkerboard(L, s, J, cfg.seed, 0.9, tau0=0, n_sweeps=3, sample_offset=k)
+        np.testing.assert_array_equal(ms[k:k + 1], s)
