@@ -57,6 +57,7 @@ def lib() -> ctypes.CDLL:
         _LIB.oracle_thresholds.argtypes = [ctypes.c_double, _c_u64p]
         _LIB.oracle_thresholds.restype = ctypes.c_int
         _LIB.oracle_refresh.restype = ctypes.c_int
+        _LIB.oracle_refresh_alpha.restype = ctypes.c_int
         _LIB.oracle_metropolis_thresholds.argtypes = [ctypes.c_double, _c_u64p]
         _LIB.oracle_metropolis_thresholds.restype = ctypes.c_int
         _LIB.oracle_metropolis_sweep.restype = ctypes.c_int
@@ -200,6 +201,18 @@ def refresh(L, m, seed, T, step, sample_offset=0) -> None:
                               _p(m, _c_u8p))
     if rc != 0:
         raise ValueError(f"invalid temperature {T!r}")
+
+
+def refresh_alpha(L, m, seed, T, step, alpha, sample_offset=0) -> None:
+    """Refresh of the alpha-th daemon family (gamma daemons per spin)."""
+    ns, nr, N = m.shape
+    assert N == L ** 3 and m.dtype == np.uint8 and m.flags.c_contiguous
+    rc = lib().oracle_refresh_alpha(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr),
+                                    ctypes.c_uint64(seed), ctypes.c_int(sample_offset),
+                                    ctypes.c_double(T), ctypes.c_uint32(step), ctypes.c_int(alpha),
+                                    _p(m, _c_u8p))
+    if rc != 0:
+        raise ValueError(f"invalid temperature {T!r} or alpha {alpha!r}")
 
 
 def refresh_uniform(i, g, rep, step, seed) -> int:

@@ -15,7 +15,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import measure, refresh, sweep, timesteps_walkers
+from . import measure, refresh, refresh_alpha, sweep, timesteps_walkers
 
 
 def anneal(L, s, m, J, seed, schedule, step0=0, sample_offset=0, walkers=False, t0=0):
@@ -23,21 +23,37 @@ def anneal(L, s, m, J, seed, schedule, step0=0, sample_offset=0, walkers=False, 
     integer sums of every measurement row and the running minimum of E/N.
     walkers=True: one forward-X walker per spin instead of a daemon -- after
     every sweep the wandering half-cycle of parity t mod 2 (PAPER.md:200,
-    :215), t = t0 + sweeps done; a refresh does not reset t."""
+    :215), t = t0 + sweeps done; a refresh does not reset t.
+    gamma daemons per spin: m has shape [gamma, ns, nr, N]; a
+    timestep is gamma sweeps, the alpha-th one uses m[alpha]; n_sweeps and
+    `every` then count timesteps, E_daemon sums over the families."""
     ns, nr, N = s.shape
+    gamma = m.shape[0] if m.ndim == 4 else 1
+    assert not (walkers and gamma > 1), "walkers are wired for gamma = 1 only"
     rows = {"sweep": [], "T": [], "E": [], "Edem": [], "Q": []}
     min_e = np.full(ns * nr, np.inf)
     t = 0
     for k, (T, n_sweeps, every) in enumerate(schedule):
-        refresh(L, m, seed, T, step0 + k, sample_offset)
+        if gamma > 1:
+            for alpha in range(gamma):
+                refresh_alpha(L, m[alpha], seed, T, step0 + k, alpha, sample_offset)
+        else:
+            refresh(L, m, seed, T, step0 + k, sample_offset)
         for j in range(1, n_sweeps + 1):
             if walkers:
                 timesteps_walkers(L, s, m, J, 1, t0 + t)
+            elif gamma > 1:
+                for alpha in range(gamma):
+                    sweep(L, s, m[alpha], J, 1)
             else:
                 sweep(L, s, m, J, 1)
             t += 1
             if every > 0 and j % every == 0:
-                E, Ed, Q = measure(L, s, m, J)
+                if gamma > 1:
+                    E, Ed, Q = measure(L, s, m[0], J)
+                    Ed = sum(measure(L, s, m[alpha], J)[1] for alpha in range(gamma))
+                else:
+                    E, Ed, Q = measure(L, s, m, J)
                 rows["sweep"].append(t)
                 rows["T"].append(T)
                 rows["E"].append(E)

@@ -322,6 +322,32 @@ uint32_t oracle_refresh_uniform(uint32_t i, uint32_t g, uint32_t rep,
     return refresh_uniform(i, g, rep, step, key);
 }
 
+/* Refresh of the alpha-th family of auxiliary variables (PAPER.md:196-198:
+ * gamma daemons n_{x,alpha} per spin): the same draw with alpha in bits 20..23
+ * of the counter word that carries the replica (replica < 2^20), so that the
+ * gamma families are independent and alpha = 0 is the single-daemon refresh. */
+int oracle_refresh_alpha(int L, int n_samples, int n_replicas, uint64_t seed,
+                         int sample_offset, double T, uint32_t step, int alpha, uint8_t *m)
+{
+    const int64_t N = (int64_t)L * L * L;
+    uint64_t thr[3];
+    if (oracle_thresholds(T, thr) != 0 || alpha < 0 || alpha > 15) return -1;
+    uint32_t key[2]; seed_key(seed, key);
+    const int n_sys = n_samples * n_replicas;
+#pragma omp parallel for schedule(static) if (N * n_sys > 65536)
+    for (int sys = 0; sys < n_sys; ++sys) {
+        const int sample = sys / n_replicas, rep = sys % n_replicas;
+        const uint32_t g = (uint32_t)(sample_offset + sample);
+        uint8_t *mm = m + (int64_t)sys * N;
+        for (int64_t i = 0; i < N; ++i) {
+            const uint64_t u = (uint64_t)refresh_uniform((uint32_t)i, g, ((uint32_t)alpha << 20) | (uint32_t)rep,
+                                                         step, key);
+            mm[i] = (uint8_t)((u >= thr[0]) + (u >= thr[1]) + (u >= thr[2]));
+        }
+    }
+    return 0;
+}
+
 /* Refresh: every demon <- #{k : u >= thr[k]} with its own u (Eq. 11). */
 int oracle_refresh(int L, int n_samples, int n_replicas, uint64_t seed,
                    int sample_offset, double T, uint32_t step, uint8_t *m)

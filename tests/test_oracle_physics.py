@@ -405,3 +405,40 @@ def test_checkerboard_metropolis_matches_independent_metropolis(oracle):
     d = e_chk.mean() - e_ind.mean()
     err = math.sqrt(e_chk.var(ddof=1) / e_chk.size + e_ind.var(ddof=1) / e_ind.size)
     assert abs(d) < 3 * err + 2e-3, (d, err)
+
+
+# ---------------------------------------------------------------- gamma daemons per spin
+def test_gamma_families_are_independent_and_alpha0_is_the_single_daemon(oracle):
+    L, ns, nr = 6, 3, 2
+    N = L ** 3
+    a = np.zeros((ns, nr, N), np.uint8); b = np.zeros_like(a); c = np.zeros_like(a)
+    oracle.refresh(L, a, 11, 1.5, 4)
+    oracle.refresh_alpha(L, b, 11, 1.5, 4, 0)
+    oracle.refresh_alpha(L, c, 11, 1.5, 4, 3)
+    np.testing.assert_array_equal(a, b)
+    assert not np.array_equal(a, c)
+    x, y = a.astype(np.float64).ravel() - a.mean(), c.astype(np.float64).ravel() - c.mean()
+    corr = float((x * y).sum() / math.sqrt((x * x).sum() * (y * y).sum()))
+    assert abs(corr) < 5 / math.sqrt(x.size)
+    assert abs(4.0 * c.mean() - eq12(1.5)) < 0.05
+
+
+@pytest.mark.parametrize("gamma", [2, 6])
+def test_gamma_daemons_conserve_energy_and_reach_boltzmann_on_2x2x2(oracle, gamma):
+    """A timestep of gamma sweeps, the alpha-th with its own daemon family: the
+    total H_EA + sum_alpha H_aux,alpha is conserved between refreshes and the
+    long-run energy is the exact Boltzmann average (same pin as P7)."""
+    L, N, nr, T, seed = 2, 8, 64, 2.0, 58        # (sample 57 is non-ergodic on 2x2x2 for every gamma, 1 included)
+    J = random_pm1((1, 3, N), seed)
+    exact = _boltzmann_2x2x2(J[0].tolist(), T)
+    s = oracle.init_spins(L, 1, nr, seed)
+    m = np.zeros((gamma, 1, nr, N), dtype=np.uint8)
+    out = driver.anneal(L, s, m, J, seed, [(T, 10, 1)] * 400)
+    tot = out["E"] + out["Edem"]
+    for k in range(400):                                   # constant inside every refresh interval
+        blk = tot[10 * k:10 * k + 10]
+        assert np.all(blk == blk[0])
+    e = out["E"][200:] / float(N)
+    per_rep = e.mean(axis=0)
+    mean, err = per_rep.mean(), per_rep.std(ddof=1) / math.sqrt(nr)
+    assert err < 0.012 and abs(mean - exact) < 3 * err, (mean, exact, err)
