@@ -144,6 +144,20 @@ int micsa_half_sweep(micsa_ctx *ctx, int parity);
  * through those calls since create, settable with micsa_set_time (a refresh
  * does not reset it; micsa_half_sweep does not advance it).  gamma > 1 and the
  * other five directions of Eq. (13) are not wired into the timestep yet. */
+/* gamma daemons per spin: micsa_set_gamma(gamma), gamma = 1..6
+ * (the paper tests 1, 2, 4, 6), keeps gamma families n_{x,alpha} of auxiliary
+ * variables; a new family starts at level 0.  micsa_sweep / micsa_sweep_measure
+ * / micsa_anneal then run TIMESTEPS of gamma sweeps, the alpha-th sweep of a
+ * timestep using family alpha; micsa_refresh_demons redraws every family (the
+ * family index sits in bits 20..23 of the Philox counter word that carries the
+ * replica, so family 0 is the gamma = 1 refresh and n_replicas < 2^20);
+ * E_daemon sums over the families; refreshes are not prefetched.
+ * micsa_set_daemons / micsa_get_state address the family chosen with
+ * micsa_select_daemon_set(alpha) (default 0).  Walkers are wired for gamma = 1
+ * only: gamma > 1 with walkers on, or walkers with gamma > 1 -> MICSA_ERR_INVALID.
+ * Synchronises the stream. */
+int micsa_set_gamma(micsa_ctx *ctx, int gamma);
+int micsa_select_daemon_set(micsa_ctx *ctx, int alpha);
 int micsa_wander(micsa_ctx *ctx, int axis, int sign, int parity);
 int micsa_set_walkers(micsa_ctx *ctx, int mode);
 int micsa_set_time(micsa_ctx *ctx, int64_t t);

@@ -33,6 +33,7 @@ EXPORTS = (
     "micsa_set_tuning",
     "micsa_prefetch_refresh", "micsa_measure_begin", "micsa_measure_end", "micsa_sweep_measure",
     "micsa_measure_c4", "micsa_metropolis_sweep", "micsa_metropolis_half_sweep", "micsa_debug_metropolis_thresholds",
+    "micsa_set_gamma", "micsa_select_daemon_set",
     "micsa_wander", "micsa_set_walkers", "micsa_set_time", "micsa_get_time",
 )
 
@@ -94,6 +95,7 @@ def _bind() -> ctypes.CDLL:
             ("micsa_sweep", [vp, i32]), ("micsa_sweep_measure", [vp, i32]),
             ("micsa_metropolis_sweep", [vp, f64, u32, i32]), ("micsa_metropolis_half_sweep", [vp, f64, u32, i32]),
             ("micsa_debug_metropolis_thresholds", [f64, vp]),
+            ("micsa_set_gamma", [vp, i32]), ("micsa_select_daemon_set", [vp, i32]),
             ("micsa_wander", [vp, i32, i32, i32]), ("micsa_set_walkers", [vp, i32]),
             ("micsa_set_time", [vp, ctypes.c_int64]), ("micsa_get_time", [vp, vp]), ("micsa_half_sweep", [vp, i32]),
             ("micsa_refresh_demons", [vp, f64, u32]),
@@ -236,6 +238,12 @@ class MicSA:
 
     def metropolis_half_sweep(self, T, tau, parity):
         _check(_lib.micsa_metropolis_half_sweep(self._h, float(T), int(tau), int(parity)))
+
+    def set_gamma(self, gamma):
+        _check(_lib.micsa_set_gamma(self._h, int(gamma)))
+
+    def select_daemon_set(self, alpha):
+        _check(_lib.micsa_select_daemon_set(self._h, int(alpha)))
 
     def wander(self, axis=0, sign=+1, parity=0):
         _check(_lib.micsa_wander(self._h, int(axis), int(sign), int(parity)))

@@ -156,6 +156,23 @@ count_xor_kernel(MeasureArgs a)
     block_lane_counts(acc, a.cntX + ((long long)sg * gridDim.z + blockIdx.z) * 32);
 }
 
+// Sum of the daemon levels of one more family (gamma > 1) into cntM.
+// grid = (nblk, n_words); both parities of a lattice are contiguous (n words).
+__global__ void __launch_bounds__(kCountBlock)
+count_levels_kernel(const uint32_t* __restrict__ m0, const uint32_t* __restrict__ m1, long long n,
+                    unsigned long long* __restrict__ cntM)
+{
+    const int w = blockIdx.y;
+    const uint32_t* p0 = m0 + (long long)w * n;
+    const uint32_t* p1 = m1 + (long long)w * n;
+    VCount<kThreadPlanes> acc; acc.clear();
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const uint32_t b[2] = { p0[i], p1[i] };
+        acc.add(b);
+    }
+    block_lane_counts(acc, cntM + (long long)w * 32);
+}
+
 struct FinalizeArgs {
     unsigned long long* cntU; unsigned long long* cntM; unsigned long long* cntX;
     long long cnt_words;   // length of the counter area starting at cntU (zeroed after use)

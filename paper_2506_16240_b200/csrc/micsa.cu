@@ -47,7 +47,7 @@ bool make_geom(int L, int n_samples, int n_replicas, int sample_offset, Geom& g)
     if (sample_offset < 0 || (sample_offset & 15)) { set_err("sample_offset must be a non-negative multiple of 16"); return false; }
     const long long N = (long long)L * L * L;
     if (N > 0x7FFFFFFFll) { set_err("L^3 must be below 2^31 (32-bit site index and byte offsets inside a parity array)"); return false; }
-    if ((long long)n_samples * n_replicas > (1ll << 24) || n_replicas >= (1 << 24)) {
+    if ((long long)n_samples * n_replicas > (1ll << 24) || n_replicas >= (1 << 20)) {
         set_err("too many systems"); return false;
     }
     if ((long long)sample_offset + n_samples > 0x7FFFFFFFll) { set_err("sample index overflow"); return false; }
@@ -132,6 +132,9 @@ struct micsa_ctx {
     unsigned long long ticket0;   // value of *task_ticket when the next launch starts
     int progress_base;         // value of every progress entry between launches
     PersistPlan pp;
+    int gamma;                 // daemon families per spin; family 0 lives in st.m0/m1
+    int sel;                   // family that set_daemons / get_state address
+    std::vector<uint32_t*> xm0, xm1;   // families 1 .. gamma-1 (library-owned)
     int fuse_walk;             // walkers: exchange inside the odd half-sweep instead of a separate kernel
     int walkers;               // 0 = daemons stay on their site, 1 = one forward-X walker per spin
     long long t;               // time index (timesteps = sweeps done since create / micsa_set_time)
@@ -386,6 +389,20 @@ bool fused_walk(const micsa_ctx* c) { return c->walkers && c->fuse_walk && c->V 
 
 int launch_sweeps(micsa_ctx* c, int n) {
     if (n <= 0) return MICSA_OK;
+    if (c->gamma > 1) {                         // a timestep = gamma sweeps, the alpha-th with family alpha
+        uint32_t* const h0 = c->st.m0; uint32_t* const h1 = c->st.m1;
+        int rc = MICSA_OK;
+        for (int k = 0; k < n && rc == MICSA_OK; ++k) {
+            for (int alpha = 0; alpha < c->gamma && rc == MICSA_OK; ++alpha) {
+                c->st.m0 = alpha == 0 ? h0 : c->xm0[alpha - 1];
+                c->st.m1 = alpha == 0 ? h1 : c->xm1[alpha - 1];
+                rc = launch_plain_sweeps(c, 1);
+            }
+            c->t += 1;
+        }
+        c->st.m0 = h0; c->st.m1 = h1;
+        return rc;
+    }
     if (!c->walkers) { c->t += n; return launch_plain_sweeps(c, n); }
     for (int k = 0; k < n; ++k) {
         if (fused_walk(c)) {
@@ -471,7 +488,7 @@ int launch_metropolis_half_sweep(micsa_ctx* c, const RefreshThr& rt, uint32_t ta
 }
 
 int launch_refresh_into(micsa_ctx* c, double T, uint32_t step, uint32_t* m0, uint32_t* m1,
-                        cudaStream_t stream) {
+                        cudaStream_t stream, int alpha = 0) {
     uint64_t thr[3];
     if (thresholds_host(T, thr) != MICSA_OK || thr[0] == 0) {
         set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID;
@@ -484,9 +501,9 @@ int launch_refresh_into(micsa_ctx* c, double T, uint32_t step, uint32_t* m0, uin
     const SiteGrid sg = site_grid(c->g);
     const dim3 grid = site_blocks(c->g, c->g.n_words * 2);
     if (c->g.rpw == 2)
-        refresh_kernel<2><<<grid, 128, 0, stream>>>(m0, m1, sg, c->ks, step, rt, c->calls);
+        refresh_kernel<2><<<grid, 128, 0, stream>>>(m0, m1, sg, c->ks, step, rt, c->calls, (uint32_t)alpha << 20);
     else
-        refresh_kernel<1><<<grid, 128, 0, stream>>>(m0, m1, sg, c->ks, step, rt, c->calls);
+        refresh_kernel<1><<<grid, 128, 0, stream>>>(m0, m1, sg, c->ks, step, rt, c->calls, (uint32_t)alpha << 20);
     return post_launch(c);
 }
 
@@ -494,7 +511,18 @@ int launch_refresh_into(micsa_ctx* c, double T, uint32_t step, uint32_t* m0, uin
 // prefetched, its planes are already (being) generated on the side stream:
 // wait for them and swap the plane pointers -- the old levels are thrown away
 // anyway.
+uint32_t* family_m0(micsa_ctx* c, int alpha) { return alpha == 0 ? c->st.m0 : c->xm0[alpha - 1]; }
+uint32_t* family_m1(micsa_ctx* c, int alpha) { return alpha == 0 ? c->st.m1 : c->xm1[alpha - 1]; }
+
 int launch_refresh(micsa_ctx* c, double T, uint32_t step) {
+    if (c->gamma > 1) {                         // every family, its index in the counter; no prefetch
+        for (int alpha = 0; alpha < c->gamma; ++alpha) {
+            const int rc = launch_refresh_into(c, T, step, family_m0(c, alpha), family_m1(c, alpha), c->stream, alpha);
+            if (rc) return rc;
+        }
+        c->rns += (uint64_t)c->gamma * (uint64_t)c->g.N * (uint64_t)c->g.n_sys;
+        return MICSA_OK;
+    }
     if (c->pending && c->pending_step == step && memcmp(&c->pending_T, &T, sizeof T) == 0) {
         CK(c, cudaStreamWaitEvent(c->stream, c->ev_side, 0));
         std::swap(c->st.m0, c->m0s);
@@ -512,6 +540,7 @@ int launch_refresh(micsa_ctx* c, double T, uint32_t step) {
 // stream; it starts once the main stream has reached this point (everything
 // that still reads the staging planes' previous role has finished).
 int launch_prefetch(micsa_ctx* c, double T, uint32_t step) {
+    if (c->gamma > 1) return MICSA_OK;          // one staging pair only: gamma > 1 refreshes in place
     uint64_t thr[3];
     if (thresholds_host(T, thr) != MICSA_OK || thr[0] == 0) {
         set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID;
@@ -578,6 +607,12 @@ int launch_measure(micsa_ctx* c, long long* row, bool fold_min) {
     if (g.n_replicas * (g.n_replicas - 1) / 2 > 65535) { set_err("too many replica pairs"); return MICSA_ERR_INVALID; }
     MeasureArgs a; FinalizeArgs f;
     make_measure_args(c, row, fold_min, a, f);
+    for (int alpha = 1; alpha < c->gamma; ++alpha) {        // E_daemon sums over the families
+        const long long n = 2 * g.half;
+        const unsigned nb = (unsigned)std::max<long long>(1, std::min<long long>((n + kCountBlock * 64 - 1) / (kCountBlock * 64), std::max(1, 592 / g.n_words)));
+        count_levels_kernel<<<dim3(nb, (unsigned)g.n_words), kCountBlock, 0, c->stream>>>(c->xm0[alpha - 1], c->xm1[alpha - 1], n, a.cntM);
+        c->launches += 1;
+    }
     switch (c->V * 10 + g.rpw) {
         case 41: launch_measure_t<4, 1>(c, a, f); break;
         case 42: launch_measure_t<4, 2>(c, a, f); break;
@@ -627,7 +662,7 @@ int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min, int dir)
 // n sweeps, then one measurement into `row`
 int launch_sweeps_measured(micsa_ctx* c, int n, long long* row, bool fold_min) {
     const Geom& g = c->g;
-    const bool fused = n >= 1 && c->fuse_measure && c->V == 4 && c->sweep_kernel == 2 && g.n_replicas <= 2;
+    const bool fused = n >= 1 && c->fuse_measure && c->V == 4 && c->sweep_kernel == 2 && g.n_replicas <= 2 && c->gamma == 1;
     if (!fused) {
         const int rc = launch_sweeps(c, n); if (rc) return rc;
         return launch_measure(c, row, fold_min);
@@ -665,9 +700,10 @@ int set_sys(micsa_ctx* c, const int8_t* src, int kind) {
     if (bad) { set_err(kind == 0 ? "spin values must be -1 or +1" : "daemon levels must be 0..3"); return MICSA_ERR_INVALID; }
     const SiteGrid sg = site_grid(g);
     const dim3 grid = site_blocks(g, g.n_words * 2);
-    uint32_t* d0 = kind == 0 ? c->st.spin : c->st.m0;
-    if (g.rpw == 2) pack_sys_kernel<2><<<grid, 128, 0, c->stream>>>((const int8_t*)st.dev, d0, c->st.m1, sg, g.n_replicas, kind);
-    else            pack_sys_kernel<1><<<grid, 128, 0, c->stream>>>((const int8_t*)st.dev, d0, c->st.m1, sg, g.n_replicas, kind);
+    uint32_t* d0 = kind == 0 ? c->st.spin : family_m0(c, c->sel);
+    uint32_t* d1 = family_m1(c, c->sel);
+    if (g.rpw == 2) pack_sys_kernel<2><<<grid, 128, 0, c->stream>>>((const int8_t*)st.dev, d0, d1, sg, g.n_replicas, kind);
+    else            pack_sys_kernel<1><<<grid, 128, 0, c->stream>>>((const int8_t*)st.dev, d0, d1, sg, g.n_replicas, kind);
     rc = post_launch(c); if (rc) return rc;
     CK(c, cudaStreamSynchronize(c->stream));
     return MICSA_OK;
@@ -741,7 +777,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->use_pdl = 1;
     c->pipe_planes = (g.n_words == 1 && (g.L / 4) * (g.Lh / 4) >= 512) ? 4 : 1;   // measured: DESIGN.md 6.1
     c->fuse_measure = 1;
-    c->walkers = 0; c->t = 0; c->fuse_walk = 1;
+    c->walkers = 0; c->t = 0; c->fuse_walk = 1; c->gamma = 1; c->sel = 0;
     c->attempts = c->rns = c->launches = 0;
     c->sticky = 0;
     if (dev_workspace) {
@@ -798,6 +834,8 @@ int micsa_destroy(micsa_ctx* c) {
     if (!c) return MICSA_OK;
     cudaStreamSynchronize(c->stream);
     destroy_side(c);
+    for (uint32_t* p : c->xm0) cudaFree(p);
+    for (uint32_t* p : c->xm1) cudaFree(p);
     if (c->owns_ws) cudaFree(c->ws);
     cudaFreeHost(c->host_row);
     delete c;
@@ -850,9 +888,10 @@ int micsa_get_state(micsa_ctx* c, int8_t* s, uint8_t* m, int8_t* J) {
         void* dst = kind == 0 ? (void*)s : (void*)m;
         if (!dst) continue;
         const dim3 grid = site_blocks(g, g.n_words * 2);
-        const uint32_t* d0 = kind == 0 ? c->st.spin : c->st.m0;
-        if (g.rpw == 2) unpack_sys_kernel<2><<<grid, 128, 0, c->stream>>>((int8_t*)st.dev, d0, c->st.m1, sg, g.n_replicas, kind);
-        else            unpack_sys_kernel<1><<<grid, 128, 0, c->stream>>>((int8_t*)st.dev, d0, c->st.m1, sg, g.n_replicas, kind);
+        const uint32_t* d0 = kind == 0 ? c->st.spin : family_m0(c, c->sel);
+        const uint32_t* d1 = family_m1(c, c->sel);
+        if (g.rpw == 2) unpack_sys_kernel<2><<<grid, 128, 0, c->stream>>>((int8_t*)st.dev, d0, d1, sg, g.n_replicas, kind);
+        else            unpack_sys_kernel<1><<<grid, 128, 0, c->stream>>>((int8_t*)st.dev, d0, d1, sg, g.n_replicas, kind);
         rc = post_launch(c); if (rc) return rc;
         CK(c, cudaMemcpyAsync(dst, st.dev, sys_bytes, cudaMemcpyDeviceToHost, c->stream));
         CK(c, cudaStreamSynchronize(c->stream));
@@ -888,8 +927,39 @@ int micsa_wander(micsa_ctx* c, int axis, int sign, int parity) {
     return launch_wander(c, axis, sign, parity);
 }
 
+int micsa_set_gamma(micsa_ctx* c, int gamma) {
+    int rc = check_ctx(c); if (rc) return rc;
+    if (gamma < 1 || gamma > 6) { set_err("gamma must be 1..6"); return MICSA_ERR_INVALID; }
+    if (gamma > 1 && c->walkers) { set_err("walkers are wired for gamma = 1 only"); return MICSA_ERR_INVALID; }
+    CK(c, cudaStreamSynchronize(c->stream));
+    CK(c, cudaStreamSynchronize(c->side));
+    while ((int)c->xm0.size() > gamma - 1) {
+        cudaFree(c->xm0.back()); cudaFree(c->xm1.back()); c->xm0.pop_back(); c->xm1.pop_back();
+    }
+    while ((int)c->xm0.size() < gamma - 1) {       // new families start at level 0, like family 0 at create
+        void* a = nullptr; void* b = nullptr;
+        if (cudaMalloc(&a, c->plan.plane_bytes) != cudaSuccess || cudaMalloc(&b, c->plan.plane_bytes) != cudaSuccess) {
+            cudaGetLastError(); if (a) cudaFree(a); set_err("out of device memory (daemon families)"); return MICSA_ERR_NOMEM;
+        }
+        CK(c, cudaMemsetAsync(a, 0, c->plan.plane_bytes, c->stream));
+        CK(c, cudaMemsetAsync(b, 0, c->plan.plane_bytes, c->stream));
+        c->xm0.push_back((uint32_t*)a); c->xm1.push_back((uint32_t*)b);
+    }
+    c->gamma = gamma; c->sel = std::min(c->sel, gamma - 1);
+    c->pending = false;                           // a prefetched refresh belongs to the single-family path
+    return MICSA_OK;
+}
+
+int micsa_select_daemon_set(micsa_ctx* c, int alpha) {
+    int rc = check_ctx(c); if (rc) return rc;
+    if (alpha < 0 || alpha >= c->gamma) { set_err("alpha must be 0 .. gamma-1"); return MICSA_ERR_INVALID; }
+    c->sel = alpha;
+    return MICSA_OK;
+}
+
 int micsa_set_walkers(micsa_ctx* c, int mode) {
     int rc = check_ctx(c); if (rc) return rc;
+    if (mode == 1 && c->gamma > 1) { set_err("walkers are wired for gamma = 1 only"); return MICSA_ERR_INVALID; }
     if (mode != 0 && mode != 1) { set_err("walkers mode must be 0 (daemons) or 1 (one forward-X walker per spin)"); return MICSA_ERR_INVALID; }
     c->walkers = mode;
     return MICSA_OK;

@@ -104,7 +104,7 @@ template <int RPW>
 __global__ void __launch_bounds__(kRefreshBlock)
 refresh_kernel(uint32_t* __restrict__ m0, uint32_t* __restrict__ m1, SiteGrid g,
                PhiloxKeys ks, uint32_t step, RefreshThr thr,
-               unsigned long long* __restrict__ n_calls)
+               unsigned long long* __restrict__ n_calls, uint32_t alpha_bits)
 {
     constexpr int SPW = 32 / RPW;
     __shared__ uint32_t q_tid[2][kRefreshBlock];
@@ -123,7 +123,7 @@ refresh_kernel(uint32_t* __restrict__ m0, uint32_t* __restrict__ m1, SiteGrid g,
     const long long plane0 = ((long long)blockIdx.z) * g.half + (long long)z * g.L * g.Lh;
     RefreshWord wd;
     wd.blk_a = blk; wd.blk_b = (RPW == 2) ? blk : blk + 1u;
-    wd.rep_a = kTagRefresh | (uint32_t)(rg * RPW);
+    wd.rep_a = kTagRefresh | alpha_bits | (uint32_t)(rg * RPW);     // alpha_bits = daemon family << 20
     wd.rep_b = (RPW == 2) ? wd.rep_a + 1u : wd.rep_a;
     wd.has_b = (vm >> 16) != 0u;                  // block-uniform
     const unsigned per_chunk = wd.has_b ? 2u : 1u;

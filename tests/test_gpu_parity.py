@@ -615,3 +615,48 @@ def test_config4_walkers_and_metropolis_sampled(micsa, oracle):
         np.testing.assert_array_equal(out["Q"][:, k:k + 1], ref["Q"])
         oracle.metropolis_checkerboard(L, s, J, cfg.seed, 0.9, tau0=0, n_sweeps=3, sample_offset=k)
         np.testing.assert_array_equal(ms[k:k + 1], s)
+
+
+# ---------------------------------------------------------------- gamma daemons per spin
+@pytest.mark.parametrize("gamma", [2, 4, 6])
+@pytest.mark.parametrize("L,ns,nr", [(8, 40, 2), (6, 5, 3), (16, 17, 2), (8, 33, 1)])
+def test_gamma_daemons_bit_exact(micsa, oracle, L, ns, nr, gamma):
+    """Timesteps of gamma sweeps, the alpha-th with its own daemon family: every
+    family, the spins and the measurement rows against the oracle driver."""
+    N, seed = L ** 3, 13
+    s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+    m = np.zeros((gamma, ns, nr, N), np.uint8)
+    sched = [(1.4, 3, 1), (0.9, 4, 2)]
+    ref = driver.anneal(L, s, m, J, seed, sched, step0=5)
+    with micsa.MicSA(L, ns, nr, seed) as g:
+        g.set_gamma(gamma)
+        out = g.anneal(sched, step0=5)
+        for k in ("E", "Edem", "Q"):
+            np.testing.assert_array_equal(out[k], ref[k])
+        for alpha in range(gamma):
+            g.select_daemon_set(alpha)
+            _assert_state(g, s, m[alpha])
+        assert g.get_time() == 7
+        c = g.counters()
+        assert c["attempts"] == 7 * gamma * N * ns * nr and c["rns_drawn"] == 2 * gamma * N * ns * nr
+        # single calls: refresh, timesteps, measurement
+        g.refresh_demons(2.0, 9); g.sweep(2)
+        for alpha in range(gamma):
+            oracle.refresh_alpha(L, m[alpha], seed, 2.0, 9, alpha)
+        for _ in range(2):
+            for alpha in range(gamma):
+                oracle.sweep(L, s, m[alpha], J, 1)
+        E, Ed, Q = g.measure_i64()
+        oE = oracle.measure(L, s, m[0], J)[0]
+        oEd = sum(oracle.measure(L, s, m[alpha], J)[1] for alpha in range(gamma))
+        np.testing.assert_array_equal(E, oE); np.testing.assert_array_equal(Ed, oEd)
+        with pytest.raises(micsa.MicsaError):
+            g.set_walkers(1)
+        with pytest.raises(micsa.MicsaError):
+            g.select_daemon_set(gamma)
+        g.set_gamma(1)                                 # back to one family: family 0 is kept
+        g.select_daemon_set(0)
+        _assert_state(g, s, m[0])
+        g.set_walkers(1)
+        with pytest.raises(micsa.MicsaError):
+            g.set_gamma(2)
