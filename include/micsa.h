@@ -142,8 +142,8 @@ int micsa_half_sweep(micsa_ctx *ctx, int parity);
  * micsa_anneal then run TIMESTEPS -- a sweep, then micsa_wander(0, +1, t & 1),
  * then t += 1.  t is the context's time index: sweeps done
  * through those calls since create, settable with micsa_set_time (a refresh
- * does not reset it; micsa_half_sweep does not advance it).  gamma > 1 and the
- * other five directions of Eq. (13) are not wired into the timestep yet. */
+ * does not reset it; micsa_half_sweep does not advance it).  For gamma > 1 see
+ * micsa_set_gamma. */
 /* gamma daemons per spin: micsa_set_gamma(gamma), gamma = 1..6
  * (the paper tests 1, 2, 4, 6), keeps gamma families n_{x,alpha} of auxiliary
  * variables; a new family starts at level 0.  micsa_sweep / micsa_sweep_measure
@@ -153,9 +153,11 @@ int micsa_half_sweep(micsa_ctx *ctx, int parity);
  * replica, so family 0 is the gamma = 1 refresh and n_replicas < 2^20);
  * E_daemon sums over the families; refreshes are not prefetched.
  * micsa_set_daemons / micsa_get_state address the family chosen with
- * micsa_select_daemon_set(alpha) (default 0).  Walkers are wired for gamma = 1
- * only: gamma > 1 with walkers on, or walkers with gamma > 1 -> MICSA_ERR_INVALID.
- * Synchronises the stream. */
+ * micsa_select_daemon_set(alpha) (default 0).  With walkers on
+ * (micsa_set_walkers(1)) family alpha wanders along the alpha-th direction of
+ * PAPER.md:204 Eq. (13) -- forward X, Y, Z, backward X, Y, Z -- after the gamma
+ * sweeps of a timestep (the paper uses gamma = 6 for all six; smaller gamma
+ * takes the first gamma rows).  Synchronises the stream. */
 int micsa_set_gamma(micsa_ctx *ctx, int gamma);
 int micsa_select_daemon_set(micsa_ctx *ctx, int alpha);
 int micsa_wander(micsa_ctx *ctx, int axis, int sign, int parity);

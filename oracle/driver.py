@@ -15,7 +15,10 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import measure, refresh, refresh_alpha, sweep, timesteps_walkers
+from . import measure, refresh, refresh_alpha, sweep, timesteps_walkers, wander
+
+# PAPER.md:204 Eq. (13): walker family alpha -> (axis, direction)
+EQ13 = [(0, +1), (1, +1), (2, +1), (0, -1), (1, -1), (2, -1)]
 
 
 def anneal(L, s, m, J, seed, schedule, step0=0, sample_offset=0, walkers=False, t0=0):
@@ -26,10 +29,13 @@ def anneal(L, s, m, J, seed, schedule, step0=0, sample_offset=0, walkers=False, 
     :215), t = t0 + sweeps done; a refresh does not reset t.
     gamma daemons per spin: m has shape [gamma, ns, nr, N]; a
     timestep is gamma sweeps, the alpha-th one uses m[alpha]; n_sweeps and
-    `every` then count timesteps, E_daemon sums over the families."""
+    `every` then count timesteps, E_daemon sums over the families.  With
+    walkers, family alpha wanders along Eq. (13)'s alpha-th direction after the
+    gamma sweeps of a timestep (the paper uses all six with gamma = 6; for
+    2 <= gamma < 6 the first gamma rows are taken, R17)."""
     ns, nr, N = s.shape
     gamma = m.shape[0] if m.ndim == 4 else 1
-    assert not (walkers and gamma > 1), "walkers are wired for gamma = 1 only"
+    assert gamma <= 6
     rows = {"sweep": [], "T": [], "E": [], "Edem": [], "Q": []}
     min_e = np.full(ns * nr, np.inf)
     t = 0
@@ -40,11 +46,14 @@ def anneal(L, s, m, J, seed, schedule, step0=0, sample_offset=0, walkers=False, 
         else:
             refresh(L, m, seed, T, step0 + k, sample_offset)
         for j in range(1, n_sweeps + 1):
-            if walkers:
-                timesteps_walkers(L, s, m, J, 1, t0 + t)
-            elif gamma > 1:
+            if gamma > 1:
                 for alpha in range(gamma):
                     sweep(L, s, m[alpha], J, 1)
+                if walkers:      # after the gamma sweeps every family wanders its own way (Eq. 13)
+                    for alpha in range(gamma):
+                        wander(L, m[alpha], EQ13[alpha][0], EQ13[alpha][1], (t0 + t) & 1)
+            elif walkers:
+                timesteps_walkers(L, s, m, J, 1, t0 + t)
             else:
                 sweep(L, s, m, J, 1)
             t += 1

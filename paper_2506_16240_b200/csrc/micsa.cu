@@ -398,6 +398,14 @@ int launch_sweeps(micsa_ctx* c, int n) {
                 c->st.m1 = alpha == 0 ? h1 : c->xm1[alpha - 1];
                 rc = launch_plain_sweeps(c, 1);
             }
+            if (c->walkers) {                       // PAPER.md:204 Eq. (13): family alpha -> its wandering direction
+                static const int kAxis[6] = { 0, 1, 2, 0, 1, 2 }, kSign[6] = { +1, +1, +1, -1, -1, -1 };
+                for (int alpha = 0; alpha < c->gamma && rc == MICSA_OK; ++alpha) {
+                    c->st.m0 = alpha == 0 ? h0 : c->xm0[alpha - 1];
+                    c->st.m1 = alpha == 0 ? h1 : c->xm1[alpha - 1];
+                    rc = launch_wander(c, kAxis[alpha], kSign[alpha], (int)(c->t & 1));
+                }
+            }
             c->t += 1;
         }
         c->st.m0 = h0; c->st.m1 = h1;
@@ -930,7 +938,6 @@ int micsa_wander(micsa_ctx* c, int axis, int sign, int parity) {
 int micsa_set_gamma(micsa_ctx* c, int gamma) {
     int rc = check_ctx(c); if (rc) return rc;
     if (gamma < 1 || gamma > 6) { set_err("gamma must be 1..6"); return MICSA_ERR_INVALID; }
-    if (gamma > 1 && c->walkers) { set_err("walkers are wired for gamma = 1 only"); return MICSA_ERR_INVALID; }
     CK(c, cudaStreamSynchronize(c->stream));
     CK(c, cudaStreamSynchronize(c->side));
     while ((int)c->xm0.size() > gamma - 1) {
@@ -959,7 +966,7 @@ int micsa_select_daemon_set(micsa_ctx* c, int alpha) {
 
 int micsa_set_walkers(micsa_ctx* c, int mode) {
     int rc = check_ctx(c); if (rc) return rc;
-    if (mode == 1 && c->gamma > 1) { set_err("walkers are wired for gamma = 1 only"); return MICSA_ERR_INVALID; }
+
     if (mode != 0 && mode != 1) { set_err("walkers mode must be 0 (daemons) or 1 (one forward-X walker per spin)"); return MICSA_ERR_INVALID; }
     c->walkers = mode;
     return MICSA_OK;

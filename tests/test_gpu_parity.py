@@ -651,12 +651,19 @@ def test_gamma_daemons_bit_exact(micsa, oracle, L, ns, nr, gamma):
         oEd = sum(oracle.measure(L, s, m[alpha], J)[1] for alpha in range(gamma))
         np.testing.assert_array_equal(E, oE); np.testing.assert_array_equal(Ed, oEd)
         with pytest.raises(micsa.MicsaError):
-            g.set_walkers(1)
-        with pytest.raises(micsa.MicsaError):
             g.select_daemon_set(gamma)
+        # the same families as walkers: Eq. (13) directions after the gamma sweeps of a timestep
+        g.set_walkers(1)
+        t0 = g.get_time()
+        sched2 = [(1.1, 3, 1)]
+        out2 = g.anneal(sched2, step0=20)
+        ref2 = driver.anneal(L, s, m, J, seed, sched2, step0=20, walkers=True, t0=t0)
+        for k in ("E", "Edem", "Q"):
+            np.testing.assert_array_equal(out2[k], ref2[k])
+        for alpha in range(gamma):
+            g.select_daemon_set(alpha)
+            _assert_state(g, s, m[alpha])
+        g.set_walkers(0)
         g.set_gamma(1)                                 # back to one family: family 0 is kept
         g.select_daemon_set(0)
         _assert_state(g, s, m[0])
-        g.set_walkers(1)
-        with pytest.raises(micsa.MicsaError):
-            g.set_gamma(2)

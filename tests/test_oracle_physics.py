@@ -442,3 +442,27 @@ def test_gamma_daemons_conserve_energy_and_reach_boltzmann_on_2x2x2(oracle, gamm
     per_rep = e.mean(axis=0)
     mean, err = per_rep.mean(), per_rep.std(ddof=1) / math.sqrt(nr)
     assert err < 0.012 and abs(mean - exact) < 3 * err, (mean, exact, err)
+
+
+def test_six_walkers_conserve_energy_and_reach_boltzmann_on_2x2x2(oracle):
+    """gamma = 6 walkers with the six wandering directions of Eq. (13)."""
+    L, N, nr, T, seed = 2, 8, 64, 2.0, 58
+    J = random_pm1((1, 3, N), seed)
+    exact = _boltzmann_2x2x2(J[0].tolist(), T)
+    s = oracle.init_spins(L, 1, nr, seed)
+    m = np.zeros((6, 1, nr, N), dtype=np.uint8)
+    out = driver.anneal(L, s, m, J, seed, [(T, 10, 1)] * 400, walkers=True)
+    tot = out["E"] + out["Edem"]
+    for k in range(400):
+        blk = tot[10 * k:10 * k + 10]
+        assert np.all(blk == blk[0])
+    per_rep = (out["E"][200:] / float(N)).mean(axis=0)
+    mean, err = per_rep.mean(), per_rep.std(ddof=1) / math.sqrt(nr)
+    assert err < 0.012 and abs(mean - exact) < 3 * err, (mean, exact, err)
+    # on a larger lattice the walkers change the trajectory (they are not daemons)
+    L2 = 6
+    s1 = oracle.init_spins(L2, 2, 2, 3); Jb = oracle.init_bonds(L2, 2, 3); s2 = s1.copy()
+    m1 = np.zeros((6, 2, 2, L2 ** 3), np.uint8); m2 = m1.copy()
+    driver.anneal(L2, s1, m1, Jb, 3, [(1.5, 4, 0)], walkers=True)
+    driver.anneal(L2, s2, m2, Jb, 3, [(1.5, 4, 0)], walkers=False)
+    assert not np.array_equal(s1, s2)
