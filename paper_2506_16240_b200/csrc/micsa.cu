@@ -227,19 +227,31 @@ void launch_half_sweep_pipe(micsa_ctx* c, int parity, int dir = 0) {
         const int pp4 = (c->g.L / 4) * (c->g.Lh / 4);
         cfg.gridDim = (zw == 4) ? dim3((unsigned)((pp4 + 31) / 32), (unsigned)(c->g.L / 4), (unsigned)c->g.n_words)
                                 : dim3((unsigned)((pp4 + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
-        if (zw == 4) {
-            if (dir > 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, +1>, a, parity);
-            else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, -1>, a, parity);
+        // dir = +-1: along X; +-2: along Y; +-3: along Z (Y and Z share the DIR = +-2 kernels)
+        const int axis = (dir > 0 ? dir : -dir) - 1, walk_z = (axis == 2) ? 1 : 0;
+        if (axis == 0) {
+            if (zw == 4) {
+                if (dir > 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, +1>, a, parity, 0);
+                else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, -1>, a, parity, 0);
+            } else {
+                if (dir > 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, +1>, a, parity, 0);
+                else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, -1>, a, parity, 0);
+            }
         } else {
-            if (dir > 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, +1>, a, parity);
-            else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, -1>, a, parity);
+            if (zw == 4) {
+                if (dir > 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, +2>, a, parity, walk_z);
+                else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, -2>, a, parity, walk_z);
+            } else {
+                if (dir > 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, +2>, a, parity, walk_z);
+                else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, -2>, a, parity, walk_z);
+            }
         }
     } else if (zw == 4) {
-        if (yc == 8) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8, 4>, a, parity);
-        else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4>, a, parity);
+        if (yc == 8) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8, 4>, a, parity, 0);
+        else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4>, a, parity, 0);
     } else {
-        if (yc == 8) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8, 1>, a, parity);
-        else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1>, a, parity);
+        if (yc == 8) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8, 1>, a, parity, 0);
+        else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1>, a, parity, 0);
     }
 }
 
@@ -390,16 +402,26 @@ bool fused_walk(const micsa_ctx* c) { return c->walkers && c->fuse_walk && c->V 
 int launch_sweeps(micsa_ctx* c, int n) {
     if (n <= 0) return MICSA_OK;
     if (c->gamma > 1) {                         // a timestep = gamma sweeps, the alpha-th with family alpha
+        static const int kAxis[6] = { 0, 1, 2, 0, 1, 2 }, kSign[6] = { +1, +1, +1, -1, -1, -1 };   // Eq. (13)
         uint32_t* const h0 = c->st.m0; uint32_t* const h1 = c->st.m1;
         int rc = MICSA_OK;
         for (int k = 0; k < n && rc == MICSA_OK; ++k) {
             for (int alpha = 0; alpha < c->gamma && rc == MICSA_OK; ++alpha) {
                 c->st.m0 = alpha == 0 ? h0 : c->xm0[alpha - 1];
                 c->st.m1 = alpha == 0 ? h1 : c->xm1[alpha - 1];
-                rc = launch_plain_sweeps(c, 1);
+                if (fused_walk(c)) {
+                    // the family's own odd half-sweep does its exchange: sources (parity t & 1) swap with their
+                    // +sign*axis neighbour, i.e. an odd site with +sign*axis if t is odd, else with -sign*axis
+                    rc = launch_half_sweep(c, 0); if (rc) break;
+                    const int dir = ((c->t & 1) ? kSign[alpha] : -kSign[alpha]) * (kAxis[alpha] + 1);
+                    if (c->g.rpw == 2) launch_half_sweep_pipe<2>(c, 1, dir); else launch_half_sweep_pipe<1>(c, 1, dir);
+                    c->attempts += (uint64_t)(c->g.N / 2) * (uint64_t)c->g.n_sys;
+                    rc = post_launch(c);
+                } else {
+                    rc = launch_plain_sweeps(c, 1);
+                }
             }
-            if (c->walkers) {                       // PAPER.md:204 Eq. (13): family alpha -> its wandering direction
-                static const int kAxis[6] = { 0, 1, 2, 0, 1, 2 }, kSign[6] = { +1, +1, +1, -1, -1, -1 };
+            if (c->walkers && !fused_walk(c)) {     // PAPER.md:204 Eq. (13): family alpha -> its wandering direction
                 for (int alpha = 0; alpha < c->gamma && rc == MICSA_OK; ++alpha) {
                     c->st.m0 = alpha == 0 ? h0 : c->xm0[alpha - 1];
                     c->st.m1 = alpha == 0 ? h1 : c->xm1[alpha - 1];

@@ -321,7 +321,8 @@ struct RowRegs {                 // everything one row step reads
     uint32_t e;
     typename B4::elem eJ;
     uint4 w0, w1;                // walkers: the exchange partners' planes, same quad ...
-    uint32_t we0, we1;           // ... and the word just outside it
+    uint32_t we0, we1;           // ... and the word just outside it (X), or
+    uint32_t po;                 // the partner quad's byte offset (Y, Z)
 };
 
 // o, o_prev, o_next: byte offsets (inside a parity array of spin words) of
@@ -336,6 +337,7 @@ struct XNb {
     unsigned mask;          // lanes taking part (all of them run the same row step)
     int lane_up, lane_dn;   // lanes owning quads xv+1 and xv-1 (periodic) of the same row
     bool in_up, in_dn;      // ... and whether they can be reached by a shuffle
+    int walk_z;             // walkers along Y (0) or Z (1) when the launch's DIR is +-2
 };
 
 template <int RPW, int C, int DIR = 0>
@@ -359,7 +361,11 @@ __device__ __forceinline__ void load_row(RowRegs<RPW>& r, const PipeBase& P, uin
     r.jyq = ld_off<typename B4::raw>(P.jyq, ojm);
     r.jzq = ld_off<typename B4::raw>(P.jzq, (o + dzm) / 4u * JS);
     r.jxq = ld_off<typename B4::raw>(P.jxq, oj);
-    if (DIR != 0) {              // walkers: the planes of the sites these sites exchange with (see exchange_walkers)
+    if (DIR == 2 || DIR == -2) { // walkers along Y or Z: the partner is the same quad of the next / previous row or plane
+        r.po = nb.walk_z ? o + (DIR > 0 ? dzp : dzm) : (DIR > 0 ? o_next : o_prev);
+        r.w0 = ld_off<uint4>(P.m0q, r.po);
+        r.w1 = ld_off<uint4>(P.m1q, r.po);
+    } else if (DIR != 0) {       // walkers along X: the planes of the sites these sites exchange with (see exchange_walkers)
         r.w0 = ld_off<uint4>(P.m0q, o);
         r.w1 = ld_off<uint4>(P.m1q, o);
         if (DIR > 0 && C)  { r.we0 = ld_off<uint32_t>(P.m0q, rowstart + xe_up); r.we1 = ld_off<uint32_t>(P.m1q, rowstart + xe_up); }
@@ -431,14 +437,22 @@ __device__ __forceinline__ void count6x4(const uint32_t (&f)[6][4], uint32_t (&o
 // the even half-sweep) in return.  In the x-compressed arrays the partner of
 // word xh is word xh of the other parity's planes, or xh+1 (DIR > 0, rows with
 // C = 1) / xh-1 (DIR < 0, rows with C = 0): the same edge word as the spin
-// neighbour's.  Every word is written by exactly one thread.
+// neighbour's.  Along Y and Z (DIR = +-2, axis in XNb::walk_z) the partner is the
+// same quad of the next / previous row or plane.  Every word is written by
+// exactly one thread, and a row's partner words are loaded one row step ahead
+// of the exchange that overwrites a DIFFERENT row's (or plane's) words.
 template <int RPW, int C, int DIR>
 __device__ __forceinline__ void exchange_walkers(const RowRegs<RPW>& r, const PipeBase& P, uint32_t o,
                                                  uint32_t rowstart, uint32_t xe_up, uint32_t xe_dn,
                                                  uint32_t (&v0)[4], uint32_t (&v1)[4])
 {
     const uint32_t a0[4] = { r.w0.x, r.w0.y, r.w0.z, r.w0.w }, a1[4] = { r.w1.x, r.w1.y, r.w1.z, r.w1.w };
-    if ((DIR > 0 && !C) || (DIR < 0 && C)) {              // partner words = the same quad
+    if (DIR == 2 || DIR == -2) {                          // Y / Z: the same quad of the neighbouring row / plane
+        st_off<uint4>(P.m0q, r.po, make_uint4(v0[0], v0[1], v0[2], v0[3]));
+        st_off<uint4>(P.m1q, r.po, make_uint4(v1[0], v1[1], v1[2], v1[3]));
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { v0[k] = a0[k]; v1[k] = a1[k]; }
+    } else if ((DIR > 0 && !C) || (DIR < 0 && C)) {       // X, partner words = the same quad
         st_off<uint4>(P.m0q, o, make_uint4(v0[0], v0[1], v0[2], v0[3]));
         st_off<uint4>(P.m1q, o, make_uint4(v1[0], v1[1], v1[2], v1[3]));
 #pragma unroll
@@ -599,6 +613,7 @@ __device__ __forceinline__ XNb x_neighbours(int idx, int xv, int nxv, unsigned m
     nb.lane_up = up & 31; nb.lane_dn = dn & 31;
     nb.in_up = use_shuffle && (up >> 5) == (idx >> 5) && ((mask >> nb.lane_up) & 1u);
     nb.in_dn = use_shuffle && (dn >> 5) == (idx >> 5) && ((mask >> nb.lane_dn) & 1u);
+    nb.walk_z = 0;
     return nb;
 }
 
@@ -632,7 +647,7 @@ __device__ __forceinline__ PipeBase pipe_base(const SweepArgs& a, int w, int p)
 // (exchange_walkers).
 template <int RPW, int YC, int ZW, int DIR = 0>
 __global__ void __launch_bounds__(128)
-half_sweep_pipe_kernel(SweepArgs a, int p)
+half_sweep_pipe_kernel(SweepArgs a, int p, int walk_z)
 {
     const int L = a.L, Lh = a.Lh;
     const int nxv = Lh >> 2;
@@ -646,7 +661,8 @@ half_sweep_pipe_kernel(SweepArgs a, int p)
     const int chunk = t / nxv, xv = t - chunk * nxv;
     const int w = blockIdx.z;
     const PipeBase P = pipe_base<RPW>(a, w, p);
-    const XNb nb = x_neighbours(t, xv, nxv, mask, true);          // z is warp-uniform: one code path per warp
+    XNb nb = x_neighbours(t, xv, nxv, mask, true);                // z is warp-uniform: one code path per warp
+    nb.walk_z = walk_z;
     // programmatic dependent launch: this grid may have been scheduled while the
     // previous half-sweep was still draining; its results are needed from here on,
     // and the next grid may be scheduled as soon as every CTA of this one got here
