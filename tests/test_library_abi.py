@@ -103,3 +103,12 @@ def test_product_does_not_import_oracle():
         if p.suffix in (".py", ".cu", ".cuh", ".h"):
             txt = p.read_text()
             assert "oracle" not in txt.lower().replace("no cpu fallback", ""), p
+
+
+@pytest.mark.parametrize("T", [50.0, 3.0, 2.0, 1.1019, 0.9, 0.7, 0.3, 0.2, 0.05, 1e6])
+def test_metropolis_thresholds_equal_oracle(micsa, oracle, T):
+    """The Boltzmann factors exp(-4k/T) * 2^32 of the canonical comparator are
+    computed on the host on both sides; bit-exact parity rests on their equality."""
+    np.testing.assert_array_equal(micsa.debug_metropolis_thresholds(T), oracle.metropolis_thresholds(T))
+    with pytest.raises(micsa.MicsaError):
+        micsa.debug_metropolis_thresholds(0.0)
