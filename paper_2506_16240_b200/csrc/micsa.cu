@@ -123,6 +123,8 @@ struct micsa_ctx {
     cudaEvent_t ev_main, ev_side;
     bool pending; double pending_T; uint32_t pending_step;
     bool measure_queued;                      // micsa_measure_begin without its _end yet
+    void* stage_dev; size_t stage_bytes;      // canonical-layout staging of set_* / get_state (grow-only)
+    void* trace_dev; size_t trace_bytes;      // measurement rows of micsa_anneal (grow-only)
     long long* host_row;        // pinned host staging for one measurement row
     unsigned long long* calls;  // Philox calls made by the refresh kernels (device counter)
     int V;
@@ -713,13 +715,29 @@ struct Staging {
     ~Staging() { if (dev) cudaFree(dev); }
 };
 
+// Device staging for the canonical (one byte per spin / bond / daemon) boundary layouts: owned by the
+// context and grow-only, so that the set / get calls do not pay a cudaMalloc + cudaFree each time.
+int stage_reserve(micsa_ctx* c, size_t bytes, void** out) {
+    if (bytes > c->stage_bytes) {
+        CK(c, cudaStreamSynchronize(c->stream));
+        if (c->stage_dev) cudaFree(c->stage_dev);
+        c->stage_dev = nullptr; c->stage_bytes = 0;
+        if (cudaMalloc(&c->stage_dev, bytes) != cudaSuccess) {
+            cudaGetLastError(); set_err("out of device memory (staging)"); return MICSA_ERR_NOMEM;
+        }
+        c->stage_bytes = bytes;
+    }
+    *out = c->stage_dev;
+    return MICSA_OK;
+}
+
 int set_sys(micsa_ctx* c, const int8_t* src, int kind) {
     int rc = check_ctx(c); if (rc) return rc;
     if (!src) { set_err("null pointer"); return MICSA_ERR_INVALID; }
     const Geom& g = c->g;
     const size_t bytes = (size_t)g.n_sys * (size_t)g.N;
-    Staging st;
-    if (cudaMalloc(&st.dev, bytes) != cudaSuccess) { cudaGetLastError(); set_err("out of device memory (staging)"); return MICSA_ERR_NOMEM; }
+    struct { void* dev; } st = { nullptr };
+    rc = stage_reserve(c, bytes, &st.dev); if (rc) return rc;
     CK(c, cudaMemcpyAsync(st.dev, src, bytes, cudaMemcpyHostToDevice, c->stream));
     CK(c, cudaMemsetAsync(c->bad, 0, sizeof(int), c->stream));
     validate_kernel<<<148 * 4, 256, 0, c->stream>>>((const int8_t*)st.dev, (long long)bytes, kind, c->bad);
@@ -839,6 +857,8 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->progress = (int*)(c->ws + c->plan.progress);
     c->task_ticket = (unsigned long long*)(c->ws + c->plan.task_ticket);
     c->ticket0 = 0; c->progress_base = 0;
+    c->trace_dev = nullptr; c->trace_bytes = 0;
+    c->stage_dev = nullptr; c->stage_bytes = 0;
     c->host_row = nullptr; c->side = nullptr; c->ev_main = nullptr; c->ev_side = nullptr;
     if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_main, cudaEventDisableTiming) != cudaSuccess ||
@@ -864,6 +884,8 @@ int micsa_destroy(micsa_ctx* c) {
     if (!c) return MICSA_OK;
     cudaStreamSynchronize(c->stream);
     destroy_side(c);
+    if (c->trace_dev) cudaFree(c->trace_dev);
+    if (c->stage_dev) cudaFree(c->stage_dev);
     for (uint32_t* p : c->xm0) cudaFree(p);
     for (uint32_t* p : c->xm1) cudaFree(p);
     if (c->owns_ws) cudaFree(c->ws);
@@ -887,8 +909,8 @@ int micsa_set_couplings(micsa_ctx* c, const int8_t* J) {
     if (!J) { set_err("null pointer"); return MICSA_ERR_INVALID; }
     const Geom& g = c->g;
     const size_t bytes = (size_t)g.n_samples * 3 * (size_t)g.N;
-    Staging st;
-    if (cudaMalloc(&st.dev, bytes) != cudaSuccess) { cudaGetLastError(); set_err("out of device memory (staging)"); return MICSA_ERR_NOMEM; }
+    struct { void* dev; } st = { nullptr };
+    rc = stage_reserve(c, bytes, &st.dev); if (rc) return rc;
     CK(c, cudaMemcpyAsync(st.dev, J, bytes, cudaMemcpyHostToDevice, c->stream));
     CK(c, cudaMemsetAsync(c->bad, 0, sizeof(int), c->stream));
     validate_kernel<<<148 * 4, 256, 0, c->stream>>>((const int8_t*)st.dev, (long long)bytes, 0, c->bad);
@@ -912,8 +934,8 @@ int micsa_get_state(micsa_ctx* c, int8_t* s, uint8_t* m, int8_t* J) {
     const SiteGrid sg = site_grid(g);
     const size_t sys_bytes = (size_t)g.n_sys * (size_t)g.N;
     const size_t J_bytes = (size_t)g.n_samples * 3 * (size_t)g.N;
-    Staging st;
-    if (cudaMalloc(&st.dev, std::max(sys_bytes, J_bytes)) != cudaSuccess) { cudaGetLastError(); set_err("out of device memory (staging)"); return MICSA_ERR_NOMEM; }
+    struct { void* dev; } st = { nullptr };
+    rc = stage_reserve(c, std::max(sys_bytes, J_bytes), &st.dev); if (rc) return rc;
     for (int kind = 0; kind < 2; ++kind) {
         void* dst = kind == 0 ? (void*)s : (void*)m;
         if (!dst) continue;
@@ -1150,11 +1172,21 @@ int micsa_anneal(micsa_ctx* c, const micsa_step* sched, int n_steps, uint32_t st
     if (trace && trace->capacity < 0) { set_err("negative trace capacity"); return MICSA_ERR_INVALID; }
     const long long keep = trace ? std::min<long long>(rows, trace->capacity) : 0;
     const size_t row_len = c->plan.row_len;
-    Staging dev_rows;
-    if (keep > 0) {
-        if (cudaMalloc(&dev_rows.dev, (size_t)keep * row_len * 8) != cudaSuccess) {
+    // the trace rows live in a context-owned device buffer that only grows: no cudaMalloc / cudaFree
+    // (and their implicit synchronisation) per call
+    struct { void* dev; } dev_rows = { c->trace_dev };
+    if ((size_t)keep * row_len * 8 > c->trace_bytes) {
+        CK(c, cudaStreamSynchronize(c->stream));
+        if (c->trace_dev) cudaFree(c->trace_dev);
+    if (c->stage_dev) cudaFree(c->stage_dev);
+        c->trace_dev = nullptr; c->trace_bytes = 0;
+    c->stage_dev = nullptr; c->stage_bytes = 0;
+        const size_t want = std::max<size_t>((size_t)keep * row_len * 8, 4096);
+        if (cudaMalloc(&c->trace_dev, want) != cudaSuccess) {
             cudaGetLastError(); set_err("out of device memory (trace)"); return MICSA_ERR_NOMEM;
         }
+        c->trace_bytes = want;
+        dev_rows.dev = c->trace_dev;
     }
     fill_i64_kernel<<<(g.n_sys + 127) / 128, 128, 0, c->stream>>>(c->minE, std::numeric_limits<long long>::max(), g.n_sys);
     rc = post_launch(c); if (rc) return rc;
