@@ -294,13 +294,16 @@ int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
  *   the observables inside the last sweep, 0 = separate measurement kernel.
  * key MICSA_TUNE_FUSE_WALK: 1 (default) = with walkers the wandering exchange is done by the odd
  *   half-sweep of kernel 2 itself, 0 = by a separate kernel after the sweep.
+ * key MICSA_TUNE_L2_GROUPS: 1 (default) = when the packed state exceeds the L2 cache, a call of several
+ *   sweeps runs all of them on one group of word lattices (independent systems) that fits in L2 before
+ *   touching the next group, 0 = every half-sweep over all lattices.
  * key MICSA_TUNE_PDL: 1 (default) = kernel 2 is launched with programmatic
  *   stream serialization (the next half-sweep's grid is scheduled while this
  *   one drains and waits on the device for its completion), 0 = plain launches.
  * Unknown key or value: MICSA_ERR_INVALID, nothing changes. */
 enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_TILE_TZ = 1, MICSA_TUNE_PIPE_ROWS = 2, MICSA_TUNE_PDL = 3,
        MICSA_TUNE_PIPE_PLANES = 4, MICSA_TUNE_FUSE_MEASURE = 5,
-       MICSA_TUNE_FUSE_WALK = 6 };
+       MICSA_TUNE_FUSE_WALK = 6, MICSA_TUNE_L2_GROUPS = 7 };
 int micsa_set_tuning(micsa_ctx *ctx, int key, int value);
 
 #ifdef __cplusplus

@@ -337,7 +337,7 @@ class MicSA:
     def set_tuning(self, key, value):
         """micsa_set_tuning: 'sweep_kernel' (0 tiled, 1 row-marching, 2 pipelined
         row-marching, 3 persistent), 'tile_tz' (2, 4, 8), 'pipe_rows' (4, 8), 'pdl' (0, 1), 'pipe_planes' (1, 4) 'fuse_measure' (0, 1) or 'fuse_walk' (0, 1)."""
-        k = {"sweep_kernel": 0, "tile_tz": 1, "pipe_rows": 2, "pdl": 3, "pipe_planes": 4, "fuse_measure": 5, "fuse_walk": 6}[key]
+        k = {"sweep_kernel": 0, "tile_tz": 1, "pipe_rows": 2, "pdl": 3, "pipe_planes": 4, "fuse_measure": 5, "fuse_walk": 6, "l2_groups": 7}[key]
         _check(_lib.micsa_set_tuning(self._h, k, int(value)))
 
     def layout_info(self):

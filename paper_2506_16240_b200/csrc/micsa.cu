@@ -137,6 +137,7 @@ struct micsa_ctx {
     int gamma;                 // daemon families per spin; family 0 lives in st.m0/m1
     int sel;                   // family that set_daemons / get_state address
     std::vector<uint32_t*> xm0, xm1;   // families 1 .. gamma-1 (library-owned)
+    int l2_groups;             // run multi-sweep calls lattice group by lattice group when the state exceeds L2
     int fuse_walk;             // walkers: exchange inside the odd half-sweep instead of a separate kernel
     int walkers;               // 0 = daemons stay on their site, 1 = one forward-X walker per spin
     long long t;               // time index (timesteps = sweeps done since create / micsa_set_time)
@@ -188,7 +189,7 @@ template <int V, int RPW>
 void launch_half_sweep_t(micsa_ctx* c, int parity) {
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half;
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = 0;
     const int per_plane = c->g.L * (c->g.Lh / V);
     dim3 grid((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
     half_sweep_kernel<V, RPW><<<grid, 128, 0, c->stream>>>(a, parity);
@@ -200,7 +201,7 @@ template <int RPW>
 void launch_half_sweep_rows(micsa_ctx* c, int parity) {
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half;
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = 0;
     const int per_plane = (c->g.L / kRowsPerThread) * (c->g.Lh / 4);
     dim3 grid((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
     half_sweep_rows_kernel<RPW, kRowsPerThread><<<grid, 128, 0, c->stream>>>(a, parity);
@@ -208,15 +209,16 @@ void launch_half_sweep_rows(micsa_ctx* c, int parity) {
 
 // dir != 0 (odd launches of walker timesteps): the launch also does the wandering exchange
 template <int RPW>
-void launch_half_sweep_pipe(micsa_ctx* c, int parity, int dir = 0) {
+void launch_half_sweep_pipe(micsa_ctx* c, int parity, int dir = 0, int w0 = 0, int nw = -1) {
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half;
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = w0;
+    const unsigned gz = (unsigned)(nw < 0 ? c->g.n_words : nw);
     const int yc = c->pipe_rows;
     const int per_plane = (c->g.L / yc) * (c->g.Lh / 4);
     const int zw = c->pipe_planes;
-    dim3 grid = (zw == 4) ? dim3((unsigned)((per_plane + 31) / 32), (unsigned)(c->g.L / 4), (unsigned)c->g.n_words)
-                          : dim3((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
+    dim3 grid = (zw == 4) ? dim3((unsigned)((per_plane + 31) / 32), (unsigned)(c->g.L / 4), gz)
+                          : dim3((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, gz);
     // programmatic dependent launch (the kernel waits with griddepcontrol.wait before
     // its first load): launch latency and ramp overlap the previous grid's tail
     cudaLaunchConfig_t cfg = {};
@@ -227,8 +229,8 @@ void launch_half_sweep_pipe(micsa_ctx* c, int parity, int dir = 0) {
     cfg.attrs = attr; cfg.numAttrs = 1;
     if (dir != 0) {                                  // 4 rows per thread only (grid was sized for yc; redo it)
         const int pp4 = (c->g.L / 4) * (c->g.Lh / 4);
-        cfg.gridDim = (zw == 4) ? dim3((unsigned)((pp4 + 31) / 32), (unsigned)(c->g.L / 4), (unsigned)c->g.n_words)
-                                : dim3((unsigned)((pp4 + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
+        cfg.gridDim = (zw == 4) ? dim3((unsigned)((pp4 + 31) / 32), (unsigned)(c->g.L / 4), gz)
+                                : dim3((unsigned)((pp4 + 127) / 128), (unsigned)c->g.L, gz);
         // dir = +-1: along X; +-2: along Y; +-3: along Z (Y and Z share the DIR = +-2 kernels)
         const int axis = (dir > 0 ? dir : -dir) - 1, walk_z = (axis == 2) ? 1 : 0;
         if (axis == 0) {
@@ -261,7 +263,7 @@ template <int RPW, int TY, int TZ>
 int launch_half_sweep_tile(micsa_ctx* c, int parity) {
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half;
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = 0;
     const int items = TY * TZ * (c->g.Lh / 4);
     const int block = std::min((items + 31) / 32 * 32, 640);
     const size_t smem = TileSmem<RPW, TY, TZ>::bytes(c->g.Lh);
@@ -340,7 +342,7 @@ int launch_persistent(micsa_ctx* c, int n_hs, int p_first) {
         }
         PersistArgs A;
         A.a.spin = c->st.spin; A.a.m0 = c->st.m0; A.a.m1 = c->st.m1; A.a.J = c->st.J;
-        A.a.L = g.L; A.a.Lh = g.Lh; A.a.n_rg = g.n_rg; A.a.half = g.half;
+        A.a.L = g.L; A.a.Lh = g.Lh; A.a.n_rg = g.n_rg; A.a.half = g.half; A.a.w0 = 0;
         A.n_hs = n; A.p_first = p_first; A.ZT = pp.ZT; A.n_slabs = g.L / pp.ZT; A.n_words = g.n_words;
         A.n_sub = pp.n_sub; A.sub_items = pp.sub_items; A.n_groups = pp.n_groups;
         A.base = c->progress_base; A.progress = c->progress;
@@ -459,6 +461,28 @@ int launch_plain_sweeps(micsa_ctx* c, int n) {
     if (n <= 0) return MICSA_OK;
     if (use_persistent(c))
         return (c->g.rpw == 2) ? launch_persistent<2>(c, 2 * n, 0) : launch_persistent<1>(c, 2 * n, 0);
+    const Geom& g = c->g;
+    // State larger than L2 (config 5: 201 MB): lattices never interact, so run all n sweeps on a group of
+    // lattices that fits in L2 before touching the next group -- each group is read from HBM once per call
+    // instead of once per half-sweep.
+    if (n >= 2 && c->l2_groups && c->V == 4 && c->sweep_kernel == 2 && g.n_words > 1) {
+        const double per_lattice = (double)g.N * (12.0 + 3.0 * (g.rpw == 2 ? 2 : 4) / g.n_rg);
+        const int fit = (int)std::max(1.0, 96e6 / per_lattice);
+        if (fit < g.n_words) {
+            const int n_groups = (g.n_words + fit - 1) / fit, per = (g.n_words + n_groups - 1) / n_groups;
+            for (int w0 = 0; w0 < g.n_words; w0 += per) {
+                const int nw = std::min(per, g.n_words - w0);
+                for (int t = 0; t < n; ++t)
+                    for (int parity = 0; parity < 2; ++parity) {
+                        if (g.rpw == 2) launch_half_sweep_pipe<2>(c, parity, 0, w0, nw);
+                        else            launch_half_sweep_pipe<1>(c, parity, 0, w0, nw);
+                        const int rc = post_launch(c); if (rc) return rc;
+                    }
+            }
+            c->attempts += (uint64_t)n * (uint64_t)g.N * (uint64_t)g.n_sys;
+            return MICSA_OK;
+        }
+    }
     for (int t = 0; t < n; ++t) {
         int rc = launch_half_sweep(c, 0); if (rc) return rc;
         rc = launch_half_sweep(c, 1); if (rc) return rc;
@@ -663,7 +687,7 @@ int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min, int dir)
     const Geom& g = c->g;
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg; a.half = g.half;
+    a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg; a.half = g.half; a.w0 = 0;
     MeasureArgs ma; FinalizeArgs fa;
     make_measure_args(c, row, fold_min, ma, fa);
     const int per_plane = (g.L / 4) * (g.Lh / 4);
@@ -825,7 +849,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->use_pdl = 1;
     c->pipe_planes = (g.n_words == 1 && (g.L / 4) * (g.Lh / 4) >= 512) ? 4 : 1;   // measured: DESIGN.md 6.1
     c->fuse_measure = 1;
-    c->walkers = 0; c->t = 0; c->fuse_walk = 1; c->gamma = 1; c->sel = 0;
+    c->walkers = 0; c->t = 0; c->fuse_walk = 1; c->l2_groups = 1; c->gamma = 1; c->sel = 0;
     c->attempts = c->rns = c->launches = 0;
     c->sticky = 0;
     if (dev_workspace) {
@@ -1265,6 +1289,9 @@ int micsa_set_tuning(micsa_ctx* c, int key, int value) {
         case MICSA_TUNE_PIPE_PLANES:
             if (value != 1 && value != 4) { set_err("pipe_planes must be 1 or 4"); return MICSA_ERR_INVALID; }
             c->pipe_planes = value; return MICSA_OK;
+        case MICSA_TUNE_L2_GROUPS:
+            if (value != 0 && value != 1) { set_err("l2_groups must be 0 or 1"); return MICSA_ERR_INVALID; }
+            c->l2_groups = value; return MICSA_OK;
         case MICSA_TUNE_FUSE_WALK:
             if (value != 0 && value != 1) { set_err("fuse_walk must be 0 or 1"); return MICSA_ERR_INVALID; }
             c->fuse_walk = value; return MICSA_OK;

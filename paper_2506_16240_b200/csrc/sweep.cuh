@@ -36,6 +36,7 @@ struct SweepArgs {
     uint32_t* spin; uint32_t* m0; uint32_t* m1; const void* J;
     int L, Lh, n_rg;
     long long half;
+    int w0;                 // first word lattice of this launch (pipelined kernel: blockIdx.z + w0)
 };
 
 // One thread updates V consecutive words of one row (y,z) of the parity-p
@@ -659,7 +660,7 @@ half_sweep_pipe_kernel(SweepArgs a, int p, int walk_z)
     const unsigned mask = __ballot_sync(0xFFFFFFFFu, active);
     if (!active) return;
     const int chunk = t / nxv, xv = t - chunk * nxv;
-    const int w = blockIdx.z;
+    const int w = blockIdx.z + a.w0;
     const PipeBase P = pipe_base<RPW>(a, w, p);
     XNb nb = x_neighbours(t, xv, nxv, mask, true);                // z is warp-uniform: one code path per warp
     nb.walk_z = walk_z;
