@@ -2,10 +2,12 @@
  * micsa.h -- C ABI of the B200-native MicSA library (libmicsa.so).
  *
  * Microcanonical simulated annealing for the 3D +-J Edwards-Anderson spin
- * glass, arxiv/paper_2506_16240 (citations are PAPER.md:<line>).  One capped
- * daemon per spin (gamma = 1, n in {0,4,8,12}); checkerboard sweeps without
- * random numbers; sporadic Philox-driven daemon refresh; E / E_daemon / q
- * reductions.  Every step runs in hand-written CUDA kernels for sm_100a; there
+ * glass, arxiv/paper_2506_16240 (citations are PAPER.md:<line>).  Capped
+ * daemons n in {0,4,8,12}, one per spin by default (gamma = 1; up to 6
+ * families and walkers: micsa_set_gamma, micsa_set_walkers); checkerboard
+ * sweeps without random numbers; sporadic Philox-driven daemon refresh; E /
+ * E_daemon / q reductions and C4; a Metropolis comparator on the same layout.
+ * Every step runs in hand-written CUDA kernels for sm_100a; there
  * is no CPU fallback: every call fails with MICSA_ERR_CUDA when no device is
  * usable.
  *
@@ -54,8 +56,10 @@ typedef struct micsa_ctx micsa_ctx;
 
 /* One step of an annealing schedule (Sec. 2.8.1, with an
  * explicit list of steps instead of the 2^s rule):
- * refresh all daemons at temperature T, then n_sweeps sweeps; after every
- * measure_every-th sweep of the step (0 = never) one measurement row is taken. */
+ * refresh all daemons at temperature T, then n_sweeps sweeps (timesteps of
+ * gamma sweeps plus wandering when micsa_set_gamma / micsa_set_walkers are in
+ * force); after every measure_every-th of them (0 = never) one measurement row
+ * is taken. */
 typedef struct micsa_step {
     double  T;
     int32_t n_sweeps;
@@ -141,9 +145,10 @@ int micsa_half_sweep(micsa_ctx *ctx, int parity);
  * walker variant): micsa_sweep, micsa_sweep_measure and
  * micsa_anneal then run TIMESTEPS -- a sweep, then micsa_wander(0, +1, t & 1),
  * then t += 1.  t is the context's time index: sweeps done
- * through those calls since create, settable with micsa_set_time (a refresh
- * does not reset it; micsa_half_sweep does not advance it).  For gamma > 1 see
- * micsa_set_gamma. */
+ * through those calls since create (timesteps, when gamma > 1), settable with
+ * micsa_set_time (a refresh does not reset it; micsa_half_sweep does not advance
+ * it).  micsa_wander acts on the daemon family chosen with
+ * micsa_select_daemon_set.  For gamma > 1 see micsa_set_gamma. */
 /* gamma daemons per spin: micsa_set_gamma(gamma), gamma = 1..6
  * (the paper tests 1, 2, 4, 6), keeps gamma families n_{x,alpha} of auxiliary
  * variables; a new family starts at level 0.  micsa_sweep / micsa_sweep_measure
@@ -202,7 +207,10 @@ int micsa_refresh_demons(micsa_ctx *ctx, double T, uint32_t step);
  * directly as usual, and the prefetched planes stay valid until consumed or
  * replaced by another prefetch.  Results are bit-identical either way.
  * micsa_anneal prefetches step k+1 under the sweeps of step k by itself.
- * Asynchronous.  T must be finite and > 0. */
+ * The side stream has the lowest priority: give the context a stream of higher
+ * priority than the default (bench.py does) so that the generation only fills
+ * what the sweeps leave idle.  A no-op when gamma > 1.  Asynchronous.  T must be
+ * finite and > 0. */
 int micsa_prefetch_refresh(micsa_ctx *ctx, double T, uint32_t step);
 
 /* The thresholds micsa_refresh_demons uses: thr[k] = floor(cdf_k * 2^32),

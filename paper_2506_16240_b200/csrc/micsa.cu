@@ -1000,7 +1000,11 @@ int micsa_wander(micsa_ctx* c, int axis, int sign, int parity) {
     if (axis < 0 || axis > 2 || (sign != 1 && sign != -1) || (parity != 0 && parity != 1)) {
         set_err("axis must be 0..2, sign +1 or -1, parity 0 or 1"); return MICSA_ERR_INVALID;
     }
-    return launch_wander(c, axis, sign, parity);
+    uint32_t* const h0 = c->st.m0; uint32_t* const h1 = c->st.m1;      // the selected family
+    c->st.m0 = family_m0(c, c->sel); c->st.m1 = family_m1(c, c->sel);
+    rc = launch_wander(c, axis, sign, parity);
+    c->st.m0 = h0; c->st.m1 = h1;
+    return rc;
 }
 
 int micsa_set_gamma(micsa_ctx* c, int gamma) {

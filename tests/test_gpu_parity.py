@@ -664,6 +664,9 @@ def test_gamma_daemons_bit_exact(micsa, oracle, L, ns, nr, gamma):
             g.select_daemon_set(alpha)
             _assert_state(g, s, m[alpha])
         g.set_walkers(0)
+        g.select_daemon_set(gamma - 1)                 # a single half-cycle on a chosen family
+        g.wander(2, -1, 1); oracle.wander(L, m[gamma - 1], 2, -1, 1)
+        _assert_state(g, s, m[gamma - 1])
         g.set_gamma(1)                                 # back to one family: family 0 is kept
         g.select_daemon_set(0)
         _assert_state(g, s, m[0])
