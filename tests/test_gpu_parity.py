@@ -6,6 +6,8 @@ compared element by element after every sweep; BASELINE's full-size configs are
 compared on sampled systems (systems never interact, so the oracle can run any
 subset of samples on its own) plus exact invariants on all of them.
 """
+from pathlib import Path
+
 import numpy as np
 import pytest
 
@@ -670,3 +672,31 @@ def test_gamma_daemons_bit_exact(micsa, oracle, L, ns, nr, gamma):
         g.set_gamma(1)                                 # back to one family: family 0 is kept
         g.select_daemon_set(0)
         _assert_state(g, s, m[0])
+
+
+def test_energy_at_T14_agrees_with_the_papers_asymptote(micsa):
+    """Soft pin P9: PAPER.md:326 prints e_inf(T = 1.4) = -1.607026(4) for the authors' L = 160
+    sample.  Our 16 random samples of the same size, 3 x 10^4 MicSA sweeps (refresh every 10): the sample-averaged
+    energy per spin must sit within the sample-to-sample scatter (3.5e-4 per sample) plus what is left of the
+    relaxation (measured: -1.60618 at this length, -1.60666 after 2 x 10^5 sweeps)."""
+    gold = {}
+    for line in (Path(__file__).parent / "golden" / "paper_table2_einf.txt").read_text().splitlines():
+        if line and not line.startswith("#"):
+            k, v = line.split()
+            gold[k] = float(v)
+    cfg = CONFIGS[4]
+    N = cfg.L ** 3
+    with micsa.MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, 14) as g:
+        out = g.anneal([(gold["T"], 10, 10)] * 3000)
+    e = out["E"][1500:] / N
+    per_sample = e.mean(axis=0).reshape(cfg.n_samples, cfg.n_replicas).mean(axis=1)
+    mean, scatter = float(per_sample.mean()), float(per_sample.std(ddof=1))
+    assert 2e-4 < scatter < 6e-4                                   # self-averaging: ~ (3N)^-1/2 = 2.9e-4
+    assert abs(mean - gold["e_inf"]) < 1.5e-3, (mean, gold["e_inf"])
+    assert mean > gold["e_inf"] - 3 * scatter                      # relaxing from above, never far below the asymptote
+    # conservation check on the way: total energy constant inside every refresh interval is covered elsewhere;
+    # here the demon energy just before a refresh sits near Eq. (12) once equilibrated (P10)
+    b = 1.0 / gold["T"]
+    eq12 = 4 * np.exp(-4 * b) / (1 - np.exp(-4 * b)) - 16 * np.exp(-16 * b) / (1 - np.exp(-16 * b))
+    ed = (out["Edem"][1500:] / N).mean()
+    assert abs(ed - eq12) < 0.01, (ed, eq12)
