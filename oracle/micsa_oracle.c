@@ -34,6 +34,11 @@
  *   thresholds/refresh histogram vs Eq. (11), mean vs Eq. (12) closed forms
  *   wander             period L, involution, conservation, 2x2x2
  *                      Boltzmann average with walkers
+ *   refresh_alpha      family 0 == refresh, families uncorrelated, conservation and the
+ *                      2x2x2 Boltzmann average with gamma = 2, 6 daemons and 6 walkers
+ *   metropolis_*       acceptance rates exp(-dH/T), 2x2x2 Boltzmann average, the
+ *                      independent typewriter Metropolis (metropolis_oracle.c)
+ *   c4                 np.roll, line-sum identity, S(r) = S(L-r), special replicas
  * Unpinned by the paper: low-temperature quench curves (configs 3, 4) and the
  * final annealed energies (config 5) -- see DESIGN.md "parity unpinned".
  */
