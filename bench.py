@@ -146,7 +146,7 @@ def run_reference(args, rank):
     line = {
         "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32-bitsliced",
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32",
         "data": "synthetic",
         "config": {"workload": CFG.name, "L": CFG.L, "n_samples": CFG.n_samples,
                    "n_replicas": CFG.n_replicas, "T": T_RUN, "sweeps_per_step": SWEEPS_PER_STEP},
@@ -341,7 +341,7 @@ def main():
             "metric": METRIC + (" [gamma=1 forward-X walkers]" if args.walkers else ""),
             "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": t_step_ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "u32-bitsliced", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
             "config": {"workload": CFG.name, "L": L, "n_samples": ns, "n_replicas": nr, "T": T_RUN,
                        "sweeps_per_step": SWEEPS_PER_STEP, "state_bytes": info["state_bytes"],
                        "l2": "flushed between timed steps (256 MiB write); state 73.7 MB < 126 MB L2",
