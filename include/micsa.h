@@ -213,6 +213,13 @@ int micsa_refresh_demons(micsa_ctx *ctx, double T, uint32_t step);
  * finite and > 0. */
 int micsa_prefetch_refresh(micsa_ctx *ctx, double T, uint32_t step);
 
+/* micsa_effective_temperature (host arithmetic only): the temperature at which
+ * Eq. (12) gives the measured daemon energy per auxiliary
+ * variable, <H_aux>/(gamma N) = E_daemon / (gamma N) -- the instantaneous
+ * temperature of the daemons / walkers.  The argument must lie
+ * strictly between 0 (T -> 0) and 6 (T -> infinity). */
+int micsa_effective_temperature(double e_daemon_per_variable, double *T);
+
 /* The thresholds micsa_refresh_demons uses: thr[k] = floor(cdf_k * 2^32),
  * k = 0,1,2, each in [0, 2^32]; level m = #{k : u >= thr[k]}.               */
 int micsa_debug_thresholds(double T, uint64_t thr[3]);

@@ -91,6 +91,13 @@ def schedule_for(cfg: Config, T=None, interval=None, n_sweeps=None, measure_ever
     return fixed_interval_schedule(T, n, R, measure_every)
 
 
+def pow2_schedule(T, s_max, measure_at_end=True):
+    """The paper's own refresh rule (Sec. 2.8.1): refresh at
+    t_s = 2^s, i.e. step s = refresh then 2^s timesteps, s = 0 .. s_max; one
+    measurement at the end of every step."""
+    return [(float(T), 1 << s, (1 << s) if measure_at_end else 0) for s in range(int(s_max) + 1)]
+
+
 def random_pm1(shape, seed) -> np.ndarray:
     """i.i.d. fair +-1 int8 array (numpy PCG64) for tests that inject state
     through set_spins / set_couplings instead of the built-in Philox init."""

@@ -32,7 +32,7 @@ EXPORTS = (
     "micsa_measure", "micsa_anneal", "micsa_counters", "micsa_layout_info",
     "micsa_set_tuning",
     "micsa_prefetch_refresh", "micsa_measure_begin", "micsa_measure_end", "micsa_sweep_measure",
-    "micsa_measure_c4", "micsa_metropolis_sweep", "micsa_metropolis_half_sweep", "micsa_debug_metropolis_thresholds",
+    "micsa_measure_c4", "micsa_effective_temperature", "micsa_metropolis_sweep", "micsa_metropolis_half_sweep", "micsa_debug_metropolis_thresholds",
     "micsa_set_gamma", "micsa_select_daemon_set",
     "micsa_wander", "micsa_set_walkers", "micsa_set_time", "micsa_get_time",
 )
@@ -100,7 +100,7 @@ def _bind() -> ctypes.CDLL:
             ("micsa_set_time", [vp, ctypes.c_int64]), ("micsa_get_time", [vp, vp]), ("micsa_half_sweep", [vp, i32]),
             ("micsa_refresh_demons", [vp, f64, u32]),
             ("micsa_prefetch_refresh", [vp, f64, u32]),
-            ("micsa_debug_thresholds", [f64, vp]),
+            ("micsa_debug_thresholds", [f64, vp]), ("micsa_effective_temperature", [f64, vp]),
             ("micsa_measure_i64", [vp, vp, vp, vp]),
             ("micsa_measure_c4", [vp, vp]), ("micsa_measure_begin", [vp]), ("micsa_measure_end", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
             ("micsa_anneal", [vp, vp, i32, u32, vp, vp]),
@@ -133,6 +133,13 @@ def debug_thresholds(T: float) -> np.ndarray:
     thr = np.zeros(3, dtype=np.uint64)
     _check(_lib.micsa_debug_thresholds(float(T), _ptr(thr)))
     return thr
+
+
+def effective_temperature(e_daemon_per_variable: float) -> float:
+    """Invert Eq. (12): the temperature of daemons holding this energy per auxiliary variable."""
+    T = ctypes.c_double(0.0)
+    _check(_lib.micsa_effective_temperature(float(e_daemon_per_variable), ctypes.byref(T)))
+    return float(T.value)
 
 
 def debug_metropolis_thresholds(T: float) -> np.ndarray:

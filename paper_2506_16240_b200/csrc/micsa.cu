@@ -1084,6 +1084,26 @@ int micsa_debug_metropolis_thresholds(double T, uint64_t thr[3]) {
     return MICSA_OK;
 }
 
+int micsa_effective_temperature(double e_daemon_per_variable, double* T) {
+    // invert Eq. (12): <H_aux>/(gamma N) = 4x/(1-x) - 16x^4/(1-x^4), x = exp(-4/T), is
+    // increasing in T from 0 (T -> 0) to 6 (T -> infinity, uniform levels): bisection on x in float64
+    if (!T) { set_err("null pointer"); return MICSA_ERR_INVALID; }
+    if (!(e_daemon_per_variable > 0.0) || !(e_daemon_per_variable < 6.0)) {
+        set_err("the daemon energy per auxiliary variable must lie strictly between 0 and 6"); return MICSA_ERR_INVALID;
+    }
+    auto f = [](double x) {           // regular at x -> 1: 4(x + 2x^2 + 3x^3)/(1 + x + x^2 + x^3)
+        return 4.0 * (x + 2.0 * x * x + 3.0 * x * x * x) / (1.0 + x + x * x + x * x * x);
+    };
+    double lo = 0.0, hi = 1.0;
+    for (int it = 0; it < 200; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (f(mid) < e_daemon_per_variable) lo = mid; else hi = mid;
+    }
+    const double x = 0.5 * (lo + hi);
+    *T = -4.0 / std::log(x);
+    return MICSA_OK;
+}
+
 int micsa_debug_thresholds(double T, uint64_t thr[3]) {
     if (!thr) { set_err("null pointer"); return MICSA_ERR_INVALID; }
     if (thresholds_host(T, thr) != MICSA_OK) { set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID; }

@@ -700,3 +700,26 @@ def test_energy_at_T14_agrees_with_the_papers_asymptote(micsa):
     eq12 = 4 * np.exp(-4 * b) / (1 - np.exp(-4 * b)) - 16 * np.exp(-16 * b) / (1 - np.exp(-16 * b))
     ed = (out["Edem"][1500:] / N).mean()
     assert abs(ed - eq12) < 0.01, (ed, eq12)
+
+
+def test_pow2_refresh_schedule_and_effective_temperature(micsa, oracle):
+    """The paper's own refresh rule t_s = 2^s (Sec. 2.8.1) through micsa_anneal, and the daemons'
+    effective temperature from Eq. (12) right after a refresh (= T) and after relaxation (> T: the spins heat them)."""
+    from micsa_workloads import pow2_schedule
+    L, ns, nr, seed, T = 16, 8, 2, 23, 0.9
+    N = L ** 3
+    sched = pow2_schedule(T, 6)
+    s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+    m = np.zeros_like(s, dtype=np.uint8)
+    ref = driver.anneal(L, s, m, J, seed, sched)
+    with micsa.MicSA(L, ns, nr, seed) as g:
+        out = g.anneal(sched)
+        _assert_state(g, s, m)
+        for k in ("sweep", "E", "Edem", "Q"):
+            np.testing.assert_array_equal(out[k], ref[k])
+        assert out["sweep"].tolist() == [1, 3, 7, 15, 31, 63, 127]
+        t_hot = micsa.effective_temperature(float(out["Edem"][0].mean()) / N)     # after 1 sweep of a random start
+        assert t_hot > 1.5 * T
+        g.refresh_demons(T, 99)
+        t_fresh = micsa.effective_temperature(float(g.measure_i64()[1].mean()) / N)
+        assert abs(t_fresh - T) < 0.02

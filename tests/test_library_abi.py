@@ -112,3 +112,22 @@ def test_metropolis_thresholds_equal_oracle(micsa, oracle, T):
     np.testing.assert_array_equal(micsa.debug_metropolis_thresholds(T), oracle.metropolis_thresholds(T))
     with pytest.raises(micsa.MicsaError):
         micsa.debug_metropolis_thresholds(0.0)
+
+
+@pytest.mark.parametrize("T", [0.3, 0.7, 0.9, 1.1019, 1.4, 2.0, 3.0, 10.0, 100.0])
+def test_effective_temperature_inverts_eq12(micsa, T):
+    """Eq. (12) as printed, and its inverse."""
+    import math
+    b = 1.0 / T
+    e = 4 * math.exp(-4 * b) / (1 - math.exp(-4 * b)) - 16 * math.exp(-16 * b) / (1 - math.exp(-16 * b))
+    assert abs(micsa.effective_temperature(e) - T) < 1e-9 * max(1.0, T * T)
+    for bad in (0.0, 6.0, -1.0, float("nan")):
+        with pytest.raises(micsa.MicsaError):
+            micsa.effective_temperature(bad)
+
+
+def test_pow2_schedule_is_the_papers_rule():
+    from micsa_workloads import pow2_schedule
+    sch = pow2_schedule(0.7, 5)
+    assert [n for _, n, _ in sch] == [1, 2, 4, 8, 16, 32] and sum(n for _, n, _ in sch) == 63
+    assert all(T == 0.7 and every == n for T, n, every in sch)
