@@ -723,3 +723,33 @@ def test_pow2_refresh_schedule_and_effective_temperature(micsa, oracle):
         g.refresh_demons(T, 99)
         t_fresh = micsa.effective_temperature(float(g.measure_i64()[1].mean()) / N)
         assert abs(t_fresh - T) < 0.02
+
+
+def test_config4_full_size_invariants(micsa):
+    """Properties that hold at any size, on the headline lattice in the launch configuration bench.py times
+    (pipelined kernel, 4 planes per CTA, dependent launches, prefetched refresh, fused measurement):
+    H_EA + H_aux is conserved between refreshes in every one of the 32 systems, and the move is
+    its own inverse: 40 sweeps forward, then 40 with the half-sweeps in the opposite order,
+    restore all 4.1 M spins and daemons of every system."""
+    cfg = CONFIGS[4]
+    with micsa.MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed) as g:
+        tot = None
+        for k in range(4):
+            g.refresh_demons(0.9, k)
+            g.prefetch_refresh(0.9, k + 1)
+            E0, Ed0, _ = g.measure_i64()
+            for _ in range(3):
+                g.sweep(9); g.sweep_measure(1)
+                E, Ed, Q = g.measure_end()
+                np.testing.assert_array_equal(E + Ed, E0 + Ed0)
+                assert np.all(np.abs(Q) <= cfg.N)
+            assert tot is None or np.all(E < tot)                 # every refresh at T = 0.9 cools a random start further
+            tot = E
+        s0, m0, _ = g.get_state(couplings=False)
+        g.sweep(40)
+        assert not np.array_equal(g.get_state(daemons=False, couplings=False)[0], s0)
+        for _ in range(40):
+            g.half_sweep(1); g.half_sweep(0)
+        s1, m1, _ = g.get_state(couplings=False)
+        np.testing.assert_array_equal(s1, s0)
+        np.testing.assert_array_equal(m1, m0)
