@@ -43,6 +43,11 @@ UNIT = "attempts/ns"
 # (cold L2: ncu flushes caches before every replay; in a real step the 73.7 MB
 # state stays in the 126 MB L2 after the first sweep)
 NCU_TRAFFIC_BYTES_PER_LAUNCH = 57_401_600 + 172_288
+# lts__t_sectors_srcunit_tex.sum * 32 B of the same capture: what crosses the L2 <-> SM path per launch -- the
+# path that actually bounds the kernel (the state is L2-resident); the microarchitecture guide's full-chip L2
+# throughput cap is ~6300 B/clk = 12.4 TB/s at 1.965 GHz
+NCU_L2_BYTES_PER_LAUNCH = 3_355_957 * 32
+L2_CAP_GBS = 6300 * 1.965
 
 
 def measured_peaks():
@@ -287,6 +292,11 @@ def main():
                 "us_per_launch": t_launch_s * 1e6,
                 "convention": "compulsory one-pass traffic: 7.5 bits/attempt (spin 1r+1w, daemon 2r+2w, "
                               "bonds 1.5r shared by the replica pair)",
+                "l2_path": {"bytes_per_launch": NCU_L2_BYTES_PER_LAUNCH,
+                            "achieved_gbs": NCU_L2_BYTES_PER_LAUNCH / t_launch_s / 1e9, "cap_gbs": L2_CAP_GBS,
+                            "frac": NCU_L2_BYTES_PER_LAUNCH / t_launch_s / 1e9 / L2_CAP_GBS,
+                            "note": "secondary roofline: L2 <-> SM bytes of the ncu capture over the live launch "
+                                    "time, against the guide's full-chip L2 throughput cap"},
                 "sweep_share_of_step": t_sweep_ms_max / t_step_ms,
                 "note": "share = the 18 plain half-sweep launches of a step; the 2 launches of the last sweep "
                         "also do the measurement and are timed with the rest of the step"}
