@@ -445,7 +445,7 @@ __device__ __forceinline__ void count6x4(const uint32_t (&f)[6][4], uint32_t (&o
 template <int RPW, int C, int DIR>
 __device__ __forceinline__ void exchange_walkers(const RowRegs<RPW>& r, const PipeBase& P, uint32_t o,
                                                  uint32_t rowstart, uint32_t xe_up, uint32_t xe_dn,
-                                                 uint32_t (&v0)[4], uint32_t (&v1)[4])
+                                                 uint32_t (&v0)[4], uint32_t (&v1)[4], const XNb& nb)
 {
     const uint32_t a0[4] = { r.w0.x, r.w0.y, r.w0.z, r.w0.w }, a1[4] = { r.w1.x, r.w1.y, r.w1.z, r.w1.w };
     if (DIR == 2 || DIR == -2) {                          // Y / Z: the same quad of the neighbouring row / plane
@@ -459,22 +459,40 @@ __device__ __forceinline__ void exchange_walkers(const RowRegs<RPW>& r, const Pi
 #pragma unroll
         for (int k = 0; k < 4; ++k) { v0[k] = a0[k]; v1[k] = a1[k]; }
     } else if (DIR > 0) {                                 // partner words xh0+1 .. xh0+4 (periodic)
+        // word xh0 of the partner planes belongs to the left neighbour's exchange: take its last new level by
+        // shuffle and write one aligned quad; lanes whose neighbour is in another warp fall back to 32-bit stores
+        const uint32_t l0 = __shfl_sync(nb.mask, v0[3], nb.lane_dn), l1 = __shfl_sync(nb.mask, v1[3], nb.lane_dn);
+        if (nb.in_dn) {
+            st_off<uint4>(P.m0q, o, make_uint4(l0, v0[0], v0[1], v0[2]));
+            st_off<uint4>(P.m1q, o, make_uint4(l1, v1[0], v1[1], v1[2]));
+        } else {
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            st_off<uint32_t>(P.m0q, o + 4u * (k + 1), v0[k]);
-            st_off<uint32_t>(P.m1q, o + 4u * (k + 1), v1[k]);
+            for (int k = 0; k < 3; ++k) {
+                st_off<uint32_t>(P.m0q, o + 4u * (k + 1), v0[k]);
+                st_off<uint32_t>(P.m1q, o + 4u * (k + 1), v1[k]);
+            }
         }
-        st_off<uint32_t>(P.m0q, rowstart + xe_up, v0[3]);
-        st_off<uint32_t>(P.m1q, rowstart + xe_up, v1[3]);
+        if (!nb.in_up) {                                  // nobody will fetch my last level: store it myself
+            st_off<uint32_t>(P.m0q, rowstart + xe_up, v0[3]);
+            st_off<uint32_t>(P.m1q, rowstart + xe_up, v1[3]);
+        }
         v0[0] = a0[1]; v0[1] = a0[2]; v0[2] = a0[3]; v0[3] = r.we0;
         v1[0] = a1[1]; v1[1] = a1[2]; v1[2] = a1[3]; v1[3] = r.we1;
     } else {                                              // partner words xh0-1 .. xh0+2 (periodic)
-        st_off<uint32_t>(P.m0q, rowstart + xe_dn, v0[0]);
-        st_off<uint32_t>(P.m1q, rowstart + xe_dn, v1[0]);
+        const uint32_t r0 = __shfl_sync(nb.mask, v0[0], nb.lane_up), r1 = __shfl_sync(nb.mask, v1[0], nb.lane_up);
+        if (nb.in_up) {
+            st_off<uint4>(P.m0q, o, make_uint4(v0[1], v0[2], v0[3], r0));
+            st_off<uint4>(P.m1q, o, make_uint4(v1[1], v1[2], v1[3], r1));
+        } else {
 #pragma unroll
-        for (int k = 1; k < 4; ++k) {
-            st_off<uint32_t>(P.m0q, o + 4u * (k - 1), v0[k]);
-            st_off<uint32_t>(P.m1q, o + 4u * (k - 1), v1[k]);
+            for (int k = 1; k < 4; ++k) {
+                st_off<uint32_t>(P.m0q, o + 4u * (k - 1), v0[k]);
+                st_off<uint32_t>(P.m1q, o + 4u * (k - 1), v1[k]);
+            }
+        }
+        if (!nb.in_dn) {
+            st_off<uint32_t>(P.m0q, rowstart + xe_dn, v0[0]);
+            st_off<uint32_t>(P.m1q, rowstart + xe_dn, v1[0]);
         }
         v0[3] = a0[2]; v0[2] = a0[1]; v0[1] = a0[0]; v0[0] = r.we0;
         v1[3] = a1[2]; v1[2] = a1[1]; v1[1] = a1[0]; v1[0] = r.we1;
@@ -554,7 +572,7 @@ __device__ __forceinline__ void update_row(const RowRegs<RPW>& r, const uint4& A
         }
     }
     if (DIR != 0) {              // walkers: hand the new levels to the partner sites, keep theirs
-        exchange_walkers<RPW, C, DIR>(r, P, o, o - x4, xe_up, xe_dn, v0, v1);
+        exchange_walkers<RPW, C, DIR>(r, P, o, o - x4, xe_up, xe_dn, v0, v1, nb);
         st_off<uint4>(P.m0, o, make_uint4(v0[0], v0[1], v0[2], v0[3]));
         st_off<uint4>(P.m1, o, make_uint4(v1[0], v1[1], v1[2], v1[3]));
     }
