@@ -753,3 +753,17 @@ def test_config4_full_size_invariants(micsa):
         s1, m1, _ = g.get_state(couplings=False)
         np.testing.assert_array_equal(s1, s0)
         np.testing.assert_array_equal(m1, m0)
+
+
+def test_run_configs_script(micsa, capsys):
+    """The full-length runner of the five BASELINE configs (shortened here) prints one JSON line per case."""
+    import json
+    from paper_2506_16240_b200 import run_configs
+    run_configs.run(1, 1.0)
+    run_configs.run(2, 0.01)
+    run_configs.run(5, 0.01)
+    lines = [json.loads(ln) for ln in capsys.readouterr().out.splitlines() if ln.startswith("{")]
+    assert [d["config"] for d in lines] == [1, 2, 2, 2, 5]
+    assert lines[0]["sweeps"] == 1000 and lines[0]["refreshes"] == 100 and lines[0]["rns_defined_per_attempt"] == 0.1
+    assert all(d["attempts_per_ns"] > 0 and -3.0 < d["e_final_mean"] < 0.0 for d in lines)
+    assert "min_energy_best" in lines[-1] and lines[-1]["min_energy_best"] <= lines[-1]["min_energy_mean"]
