@@ -119,6 +119,7 @@ int        micsa_synchronize(micsa_ctx *ctx);        /* waits for the stream */
 int micsa_set_couplings(micsa_ctx *ctx, const int8_t *J);
 int micsa_set_spins(micsa_ctx *ctx, const int8_t *s);
 int micsa_set_daemons(micsa_ctx *ctx, const uint8_t *m);
+int micsa_set_demons(micsa_ctx *ctx, const uint8_t *m);   /* same call, SURVEY.md 8(b) spelling */
 int micsa_get_state(micsa_ctx *ctx, int8_t *s, uint8_t *m, int8_t *J);
 
 /* ---- the hot path ------------------------------------------------------
@@ -224,6 +225,13 @@ int micsa_effective_temperature(double e_daemon_per_variable, double *T);
  * k = 0,1,2, each in [0, 2^32]; level m = #{k : u >= thr[k]}.               */
 int micsa_debug_thresholds(double T, uint64_t thr[3]);
 
+/* Test hook (pin P6, R8): the library's own device Philox4x32-10.
+ * counters = host array [n][4] of counter words (c0, c1, c2, c3), out = host
+ * array [n][4] receiving the four output words of each; key = (seed low 32
+ * bits, seed high 32 bits).  Synchronous, default stream, no context needed.
+ * Errors: NULL pointer / n < 0 -> MICSA_ERR_INVALID; no device -> MICSA_ERR_CUDA. */
+int micsa_debug_philox(uint64_t seed, const uint32_t *counters, int n, uint32_t *out);
+
 /* micsa_measure_i64 (synchronous): exact integer sums into host arrays, any
  * may be NULL:
  *   E[n_sys]        H_EA = -sum_<xy> J s s                 (Eq. 1)
@@ -295,13 +303,11 @@ int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
 /* Tuning / A-B switch, never needed for correctness (every setting gives the
  * same bits; tests/test_gpu_parity.py runs parity cases under each).  They
  * only matter when L % 8 == 0; other L always use the generic kernel.
- * key MICSA_TUNE_SWEEP_KERNEL: 0 = tiled half-sweep, opposite-parity spins
- *   staged in shared memory by TMA; 1 = row-marching register kernel; 2 =
- *   software-pipelined row-marching kernel (default); 3 = persistent
- *   kernel: all the half-sweeps of one micsa_sweep / anneal group in ONE launch,
- *   slab-wise dependences through device-side flags instead of kernel
- *   boundaries.
- * key MICSA_TUNE_TILE_TZ: lattice planes per tile of kernel 0: 2, 4 (default), 8.
+ * key MICSA_TUNE_SWEEP_KERNEL: 1 = row-marching register kernel; 2 =
+ *   software-pipelined row-marching kernel, one launch per half-sweep
+ *   (default); 3 = z-marching kernel: persistent CTAs walk along z through a
+ *   strip of rows, the opposite-parity spins staged once in a shared-memory
+ *   ring by the TMA engine.
  * key MICSA_TUNE_PIPE_ROWS: rows per thread of kernel 2: 4 (default) or 8.
  * key MICSA_TUNE_PIPE_PLANES: lattice planes per CTA of kernel 2 (one warp
  *   each): 4 (default) or 1.
@@ -316,7 +322,7 @@ int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
  *   stream serialization (the next half-sweep's grid is scheduled while this
  *   one drains and waits on the device for its completion), 0 = plain launches.
  * Unknown key or value: MICSA_ERR_INVALID, nothing changes. */
-enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_TILE_TZ = 1, MICSA_TUNE_PIPE_ROWS = 2, MICSA_TUNE_PDL = 3,
+enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_PIPE_ROWS = 2, MICSA_TUNE_PDL = 3,
        MICSA_TUNE_PIPE_PLANES = 4, MICSA_TUNE_FUSE_MEASURE = 5,
        MICSA_TUNE_FUSE_WALK = 6, MICSA_TUNE_L2_GROUPS = 7 };
 int micsa_set_tuning(micsa_ctx *ctx, int key, int value);

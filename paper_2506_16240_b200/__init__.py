@@ -27,8 +27,8 @@ MICSA_OK, MICSA_ERR_INVALID, MICSA_ERR_NOMEM, MICSA_ERR_CUDA = 0, -1, -2, -3
 EXPORTS = (
     "micsa_last_error", "micsa_create", "micsa_create_ex", "micsa_workspace_bytes",
     "micsa_destroy", "micsa_synchronize", "micsa_set_couplings", "micsa_set_spins",
-    "micsa_set_daemons", "micsa_get_state", "micsa_sweep", "micsa_half_sweep",
-    "micsa_refresh_demons", "micsa_debug_thresholds", "micsa_measure_i64",
+    "micsa_set_daemons", "micsa_set_demons", "micsa_get_state", "micsa_sweep", "micsa_half_sweep",
+    "micsa_refresh_demons", "micsa_debug_thresholds", "micsa_debug_philox", "micsa_measure_i64",
     "micsa_measure", "micsa_anneal", "micsa_counters", "micsa_layout_info",
     "micsa_set_tuning",
     "micsa_prefetch_refresh", "micsa_measure_begin", "micsa_measure_end", "micsa_sweep_measure",
@@ -91,7 +91,7 @@ def _bind() -> ctypes.CDLL:
     for name, args in (
             ("micsa_destroy", [vp]), ("micsa_synchronize", [vp]),
             ("micsa_set_couplings", [vp, vp]), ("micsa_set_spins", [vp, vp]),
-            ("micsa_set_daemons", [vp, vp]), ("micsa_get_state", [vp, vp, vp, vp]),
+            ("micsa_set_daemons", [vp, vp]), ("micsa_set_demons", [vp, vp]), ("micsa_get_state", [vp, vp, vp, vp]),
             ("micsa_sweep", [vp, i32]), ("micsa_sweep_measure", [vp, i32]),
             ("micsa_metropolis_sweep", [vp, f64, u32, i32]), ("micsa_metropolis_half_sweep", [vp, f64, u32, i32]),
             ("micsa_debug_metropolis_thresholds", [f64, vp]),
@@ -100,7 +100,7 @@ def _bind() -> ctypes.CDLL:
             ("micsa_set_time", [vp, ctypes.c_int64]), ("micsa_get_time", [vp, vp]), ("micsa_half_sweep", [vp, i32]),
             ("micsa_refresh_demons", [vp, f64, u32]),
             ("micsa_prefetch_refresh", [vp, f64, u32]),
-            ("micsa_debug_thresholds", [f64, vp]), ("micsa_effective_temperature", [f64, vp]),
+            ("micsa_debug_thresholds", [f64, vp]), ("micsa_debug_philox", [u64, vp, i32, vp]), ("micsa_effective_temperature", [f64, vp]),
             ("micsa_measure_i64", [vp, vp, vp, vp]),
             ("micsa_measure_c4", [vp, vp]), ("micsa_measure_begin", [vp]), ("micsa_measure_end", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
             ("micsa_anneal", [vp, vp, i32, u32, vp, vp]),
@@ -133,6 +133,14 @@ def debug_thresholds(T: float) -> np.ndarray:
     thr = np.zeros(3, dtype=np.uint64)
     _check(_lib.micsa_debug_thresholds(float(T), _ptr(thr)))
     return thr
+
+
+def debug_philox(seed: int, counters) -> np.ndarray:
+    """micsa_debug_philox: the library's device Philox4x32-10 on counters [n][4] (test hook, pin P6)."""
+    c = np.ascontiguousarray(counters, dtype=np.uint32).reshape(-1, 4)
+    out = np.empty_like(c)
+    _check(_lib.micsa_debug_philox(int(seed), _ptr(c), c.shape[0], _ptr(out)))
+    return out
 
 
 def effective_temperature(e_daemon_per_variable: float) -> float:
@@ -342,9 +350,10 @@ class MicSA:
         return {"attempts": a.value, "rns_drawn": r.value, "philox_calls": p.value}
 
     def set_tuning(self, key, value):
-        """micsa_set_tuning: 'sweep_kernel' (0 tiled, 1 row-marching, 2 pipelined
-        row-marching, 3 persistent), 'tile_tz' (2, 4, 8), 'pipe_rows' (4, 8), 'pdl' (0, 1), 'pipe_planes' (1, 4) 'fuse_measure' (0, 1) or 'fuse_walk' (0, 1)."""
-        k = {"sweep_kernel": 0, "tile_tz": 1, "pipe_rows": 2, "pdl": 3, "pipe_planes": 4, "fuse_measure": 5, "fuse_walk": 6, "l2_groups": 7}[key]
+        """micsa_set_tuning: 'sweep_kernel' (1 row-marching, 2 pipelined row-marching, 3 z-marching),
+        'pipe_rows' (4, 8), 'pdl' (0, 1), 'pipe_planes' (1, 4), 'fuse_measure' (0, 1), 'fuse_walk' (0, 1),
+        'l2_groups' (0, 1)."""
+        k = {"sweep_kernel": 0, "pipe_rows": 2, "pdl": 3, "pipe_planes": 4, "fuse_measure": 5, "fuse_walk": 6, "l2_groups": 7}[key]
         _check(_lib.micsa_set_tuning(self._h, k, int(value)))
 
     def layout_info(self):

@@ -19,8 +19,6 @@
 #include "philox.cuh"
 #include "refresh.cuh"
 #include "sweep.cuh"
-#include "sweep_persistent.cuh"
-#include "sweep_tile.cuh"
 #include "wander.cuh"
 
 using namespace micsa;
@@ -37,7 +35,7 @@ constexpr size_t kAlign = 256;
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {                 // byte offsets inside the workspace
-    size_t spin, m0, m1, m0s, m1s, J, cnt, ticket, row, minE, bad, calls, progress, task_ticket, total;
+    size_t spin, m0, m1, m0s, m1s, J, cnt, ticket, row, minE, bad, calls, total;
     size_t plane_bytes, J_bytes, cnt_words, row_len;
 };
 
@@ -49,6 +47,9 @@ bool make_geom(int L, int n_samples, int n_replicas, int sample_offset, Geom& g)
     if (N > 0x7FFFFFFFll) { set_err("L^3 must be below 2^31 (32-bit site index and byte offsets inside a parity array)"); return false; }
     if ((long long)n_samples * n_replicas > (1ll << 24) || n_replicas >= (1 << 20)) {
         set_err("too many systems"); return false;
+    }
+    if ((long long)n_replicas * (n_replicas - 1) / 2 > 65535) {      // gridDim.z of the replica-pair counting kernel
+        set_err("too many replica pairs per sample (n_replicas <= 362)"); return false;
     }
     if ((long long)sample_offset + n_samples > 0x7FFFFFFFll) { set_err("sample index overflow"); return false; }
     g.L = L; g.Lh = L / 2;
@@ -88,8 +89,6 @@ Plan make_plan(const Geom& g) {
     p.minE = o; o += align_up((size_t)g.n_sys * 8);
     p.bad = o;  o += align_up(sizeof(int));
     p.calls = o; o += align_up(sizeof(unsigned long long));
-    p.progress = o; o += align_up((size_t)g.n_words * g.L * sizeof(int));
-    p.task_ticket = o; o += align_up((size_t)g.n_words * sizeof(unsigned long long));
     p.total = o;
     return p;
 }
@@ -97,12 +96,6 @@ Plan make_plan(const Geom& g) {
 int vec_width(int Lh) { return (Lh % 4 == 0) ? 4 : (Lh % 2 == 0) ? 2 : 1; }
 
 }  // namespace
-
-struct PersistPlan {          // launch shape of the persistent sweep kernel
-    bool valid = false;
-    int ZT, n_sub, sub_items, block, n_groups, grid;
-    long long tasks_per_hs;   // per word lattice
-};
 
 struct micsa_ctx {
     Geom g;
@@ -125,15 +118,13 @@ struct micsa_ctx {
     bool measure_queued;                      // micsa_measure_begin without its _end yet
     void* stage_dev; size_t stage_bytes;      // canonical-layout staging of set_* / get_state (grow-only)
     void* trace_dev; size_t trace_bytes;      // measurement rows of micsa_anneal (grow-only)
+    void* c4_dev; size_t c4_bytes;            // overlap field + counters of micsa_measure_c4 (grow-only)
+    unsigned long long* c4_host; size_t c4_host_bytes;   // pinned read-back of the C4 counters
     long long* host_row;        // pinned host staging for one measurement row
     unsigned long long* calls;  // Philox calls made by the refresh kernels (device counter)
     int V;
-    int sweep_kernel;          // L % 8 == 0: 0 = tiled (TMA-staged), 1 = row-marching, 2 = pipelined row-marching
-    int* progress;             // persistent sweep: half-sweeps done per (word lattice, slab)
-    unsigned long long* task_ticket;
-    unsigned long long ticket0;   // value of *task_ticket when the next launch starts
-    int progress_base;         // value of every progress entry between launches
-    PersistPlan pp;
+    int sweep_kernel;          // L % 8 == 0: 1 = row-marching, 2 = pipelined row-marching
+    int sms;                   // multiprocessors of the device (grid sizing)
     int gamma;                 // daemon families per spin; family 0 lives in st.m0/m1
     int sel;                   // family that set_daemons / get_state address
     std::vector<uint32_t*> xm0, xm1;   // families 1 .. gamma-1 (library-owned)
@@ -145,7 +136,6 @@ struct micsa_ctx {
     int pipe_planes;           // planes per CTA of the pipelined kernel (1 or 4)
     int use_pdl;               // programmatic dependent launch for the pipelined kernel
     int pipe_rows;             // rows per thread of the pipelined kernel (4 or 8)
-    int tile_tz;               // planes per tile of the tiled kernel (2, 4 or 8)
     uint64_t attempts, rns, launches;
     int sticky;
 };
@@ -259,118 +249,7 @@ void launch_half_sweep_pipe(micsa_ctx* c, int parity, int dir = 0, int w0 = 0, i
     }
 }
 
-template <int RPW, int TY, int TZ>
-int launch_half_sweep_tile(micsa_ctx* c, int parity) {
-    SweepArgs a;
-    a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = 0;
-    const int items = TY * TZ * (c->g.Lh / 4);
-    const int block = std::min((items + 31) / 32 * 32, 640);
-    const size_t smem = TileSmem<RPW, TY, TZ>::bytes(c->g.Lh);
-    if (smem > 48 * 1024) {
-        if (smem > 227 * 1024) { set_err("L too large for the tiled sweep kernel"); return MICSA_ERR_INVALID; }
-        CK(c, cudaFuncSetAttribute(half_sweep_tile_kernel<RPW, TY, TZ>,
-                                   cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    }
-    dim3 grid((unsigned)((c->g.L / TY) * (c->g.L / TZ)), (unsigned)c->g.n_words);
-    half_sweep_tile_kernel<RPW, TY, TZ><<<grid, block, smem, c->stream>>>(a, parity);
-    return MICSA_OK;
-}
-
-template <int RPW>
-int launch_half_sweep_tile_tz(micsa_ctx* c, int parity) {
-    switch (c->tile_tz) {
-        case 2:  return launch_half_sweep_tile<RPW, 8, 2>(c, parity);
-        case 8:  return launch_half_sweep_tile<RPW, 8, 8>(c, parity);
-        default: return launch_half_sweep_tile<RPW, 8, 4>(c, parity);
-    }
-}
-
-// Shape of the persistent launch (sweep_persistent.cuh), computed once.
-template <int RPW>
-int plan_persistent(micsa_ctx* c) {
-    const Geom& g = c->g;
-    constexpr int YC = 4;
-    PersistPlan& pp = c->pp;
-    const int items_per_plane = (g.L / YC) * (g.Lh / 4);
-    int per_sm = 0, dev = 0, sms = 0;
-    CK(c, cudaGetDevice(&dev));
-    CK(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sweep_persistent_kernel<RPW, YC>, kPersistBlock, 0));
-    const long long grid_max = (long long)std::max(1, per_sm) * sms;
-    // lattices worked on together: as many as keep their state (12 B of spins and daemons +
-    // the bond words per site) inside ~96 MB of L2, a divisor of n_words so that groups stay balanced
-    const double bytes_per_lattice = (double)g.N * (12.0 + 3.0 * (g.rpw == 2 ? 2 : 4) / g.n_rg);
-    const long long n_fit = std::max<long long>(1, (long long)(96e6 / bytes_per_lattice));
-    int n_groups = 1;
-    for (int d = 1; d <= g.n_words && d <= n_fit && d <= grid_max; ++d)
-        if (g.n_words % d == 0) n_groups = d;
-    long long cpg = std::max<long long>(1, grid_max / n_groups);      // CTAs per lattice
-    // task size: <= 256 thread items, and (where the lattice allows) > 2.2 tasks per CTA per half-sweep
-    int ZT = 1, n_sub = 1;
-    if (items_per_plane > 256) n_sub = (items_per_plane + 255) / 256;
-    while ((long long)g.L * n_sub * 10 < 22 * cpg && (items_per_plane + n_sub) / (n_sub + 1) >= 64) ++n_sub;
-    if (n_sub == 1)
-        for (int d = 2; d <= g.L; ++d) {
-            if (g.L % d) continue;
-            if (d * items_per_plane > 256 || (long long)(g.L / d) * 10 < 22 * cpg) break;
-            ZT = d;
-        }
-    const int items = ZT * items_per_plane;
-    const long long tasks_per_hs = (long long)(g.L / ZT) * n_sub;
-    cpg = std::min(cpg, std::max<long long>(1, tasks_per_hs / 2));   // small lattices: nobody should spin
-    pp.ZT = ZT; pp.n_sub = n_sub; pp.sub_items = (items + n_sub - 1) / n_sub;
-    pp.block = std::min(kPersistBlock, (pp.sub_items + 31) / 32 * 32);
-    pp.n_groups = n_groups; pp.grid = (int)(cpg * n_groups);
-    pp.tasks_per_hs = tasks_per_hs;
-    pp.valid = true;
-    return MICSA_OK;
-}
-
-// n_hs half-sweeps, parities p_first, p_first^1, ... in one persistent launch
-template <int RPW>
-int launch_persistent(micsa_ctx* c, int n_hs, int p_first) {
-    const Geom& g = c->g;
-    constexpr int YC = 4;
-    if (!c->pp.valid) { const int rc = plan_persistent<RPW>(c); if (rc) return rc; }
-    const PersistPlan& pp = c->pp;
-    while (n_hs > 0) {
-        const int n = std::min(n_hs, 1 << 20);
-        if ((long long)(c->progress_base + n) * pp.n_sub > (1ll << 30)) {   // keep the counters far from overflow
-            CK(c, cudaMemsetAsync(c->progress, 0, (size_t)g.n_words * g.L * sizeof(int), c->stream));
-            c->progress_base = 0;
-        }
-        PersistArgs A;
-        A.a.spin = c->st.spin; A.a.m0 = c->st.m0; A.a.m1 = c->st.m1; A.a.J = c->st.J;
-        A.a.L = g.L; A.a.Lh = g.Lh; A.a.n_rg = g.n_rg; A.a.half = g.half; A.a.w0 = 0;
-        A.n_hs = n; A.p_first = p_first; A.ZT = pp.ZT; A.n_slabs = g.L / pp.ZT; A.n_words = g.n_words;
-        A.n_sub = pp.n_sub; A.sub_items = pp.sub_items; A.n_groups = pp.n_groups;
-        A.base = c->progress_base; A.progress = c->progress;
-        A.ticket = c->task_ticket; A.ticket0 = c->ticket0;
-        sweep_persistent_kernel<RPW, YC><<<pp.grid, pp.block, 0, c->stream>>>(A);
-        // per lattice: its tasks, plus one ticket past the end drawn by each CTA of its group
-        c->ticket0 += (unsigned long long)pp.tasks_per_hs * n + (unsigned long long)(pp.grid / pp.n_groups);
-        c->progress_base += n;
-        c->attempts += (uint64_t)n * (uint64_t)(g.N / 2) * (uint64_t)g.n_sys;
-        const int rc = post_launch(c); if (rc) return rc;
-        p_first ^= (n & 1);
-        n_hs -= n;
-    }
-    return MICSA_OK;
-}
-
-bool use_persistent(const micsa_ctx* c) { return c->V == 4 && c->sweep_kernel == 3; }
-
 int launch_half_sweep(micsa_ctx* c, int parity) {
-    if (use_persistent(c))
-        return (c->g.rpw == 2) ? launch_persistent<2>(c, 1, parity) : launch_persistent<1>(c, 1, parity);
-    if (c->V == 4 && c->sweep_kernel == 0) {
-        const int rc = (c->g.rpw == 2) ? launch_half_sweep_tile_tz<2>(c, parity)
-                                       : launch_half_sweep_tile_tz<1>(c, parity);
-        if (rc) return rc;
-        c->attempts += (uint64_t)(c->g.N / 2) * (uint64_t)c->g.n_sys;
-        return post_launch(c);
-    }
     const int key = c->V * 10 + c->g.rpw;
     switch (key) {
         case 41: if (c->sweep_kernel == 2) launch_half_sweep_pipe<1>(c, parity);      // L % 8 == 0
@@ -456,11 +335,9 @@ int launch_sweeps(micsa_ctx* c, int n) {
     return MICSA_OK;
 }
 
-// n full sweeps (even, odd, even, ...): one persistent launch or 2n launches
+// n full sweeps (even, odd, even, ...)
 int launch_plain_sweeps(micsa_ctx* c, int n) {
     if (n <= 0) return MICSA_OK;
-    if (use_persistent(c))
-        return (c->g.rpw == 2) ? launch_persistent<2>(c, 2 * n, 0) : launch_persistent<1>(c, 2 * n, 0);
     const Geom& g = c->g;
     // State larger than L2 (config 5: 201 MB): lattices never interact, so run all n sweeps on a group of
     // lattices that fits in L2 before touching the next group -- each group is read from HBM once per call
@@ -488,6 +365,12 @@ int launch_plain_sweeps(micsa_ctx* c, int n) {
         rc = launch_half_sweep(c, 1); if (rc) return rc;
     }
     return MICSA_OK;
+}
+
+// raw generator output for the pins of tests/ (R8, pin P6)
+__global__ void debug_philox_kernel(const uint4* ctr, uint4* out, int n, PhiloxKeys ks) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = philox4x32_10(ctr[i].x, ctr[i].y, ctr[i].z, ctr[i].w, ks);
 }
 
 int thresholds_host(double T, uint64_t thr[3]) {
@@ -610,9 +493,9 @@ int launch_prefetch(micsa_ctx* c, double T, uint32_t step) {
     return MICSA_OK;
 }
 
-unsigned count_blocks(long long nvec, long long other) {
+unsigned count_blocks(const micsa_ctx* c, long long nvec, long long other) {
     long long nb = (nvec + kCountBlock * 16 - 1) / (kCountBlock * 16);
-    const long long cap = std::max<long long>(1, (148 * 8) / std::max<long long>(1, other));
+    const long long cap = std::max<long long>(1, ((long long)c->sms * 8) / std::max<long long>(1, other));
     nb = std::min(nb, cap);
     const long long need = (nvec + (long long)kCountBlock * 4096 - 1) / ((long long)kCountBlock * 4096);
     nb = std::max<long long>(std::max<long long>(nb, need), 1);
@@ -625,7 +508,7 @@ void launch_measure_t(micsa_ctx* c, const MeasureArgs& a, const FinalizeArgs& f)
     const int pps = g.n_replicas * (g.n_replicas - 1) / 2;
     const bool pair_in_word = (g.n_replicas == 2);          // then RPW == 2
     if (pps > 0 && !pair_in_word) {
-        count_xor_kernel<V, RPW><<<dim3(count_blocks(2 * g.half / V, (long long)g.n_sg * pps),
+        count_xor_kernel<V, RPW><<<dim3(count_blocks(c, 2 * g.half / V, (long long)g.n_sg * pps),
                                         (unsigned)g.n_sg, (unsigned)pps),
                                    kCountBlock, 0, c->stream>>>(a);
         c->launches += 1;
@@ -634,7 +517,7 @@ void launch_measure_t(micsa_ctx* c, const MeasureArgs& a, const FinalizeArgs& f)
     // kMeasureMaxItems items per thread (10-plane per-thread counters)
     const long long n_items = 2 * g.half / V;
     long long nb = (n_items + (long long)kMeasureBlock * 4 - 1) / ((long long)kMeasureBlock * 4);
-    nb = std::min(nb, std::max<long long>(1, (148 * 2) / g.n_words));
+    nb = std::min(nb, std::max<long long>(1, ((long long)c->sms * 2) / g.n_words));
     const long long need = (n_items + (long long)kMeasureBlock * kMeasureMaxItems - 1) / ((long long)kMeasureBlock * kMeasureMaxItems);
     nb = std::max<long long>(std::max<long long>(nb, need), 1);
     const dim3 grid((unsigned)nb, (unsigned)g.n_words);
@@ -665,7 +548,10 @@ int launch_measure(micsa_ctx* c, long long* row, bool fold_min) {
     make_measure_args(c, row, fold_min, a, f);
     for (int alpha = 1; alpha < c->gamma; ++alpha) {        // E_daemon sums over the families
         const long long n = 2 * g.half;
-        const unsigned nb = (unsigned)std::max<long long>(1, std::min<long long>((n + kCountBlock * 64 - 1) / (kCountBlock * 64), std::max(1, 592 / g.n_words)));
+        long long nbl = std::min<long long>((n + kCountBlock * 64 - 1) / (kCountBlock * 64), std::max(1, 4 * c->sms / g.n_words));
+        // 16-plane per-thread counters, up to 3 per word: at most 16384 words per thread
+        nbl = std::max<long long>(nbl, (n + (long long)kCountBlock * 16384 - 1) / ((long long)kCountBlock * 16384));
+        const unsigned nb = (unsigned)std::max<long long>(1, nbl);
         count_levels_kernel<<<dim3(nb, (unsigned)g.n_words), kCountBlock, 0, c->stream>>>(c->xm0[alpha - 1], c->xm1[alpha - 1], n, a.cntM);
         c->launches += 1;
     }
@@ -764,7 +650,7 @@ int set_sys(micsa_ctx* c, const int8_t* src, int kind) {
     rc = stage_reserve(c, bytes, &st.dev); if (rc) return rc;
     CK(c, cudaMemcpyAsync(st.dev, src, bytes, cudaMemcpyHostToDevice, c->stream));
     CK(c, cudaMemsetAsync(c->bad, 0, sizeof(int), c->stream));
-    validate_kernel<<<148 * 4, 256, 0, c->stream>>>((const int8_t*)st.dev, (long long)bytes, kind, c->bad);
+    validate_kernel<<<c->sms * 4, 256, 0, c->stream>>>((const int8_t*)st.dev, (long long)bytes, kind, c->bad);
     rc = post_launch(c); if (rc) return rc;
     int bad = 0;
     CK(c, cudaMemcpyAsync(&bad, c->bad, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
@@ -791,8 +677,6 @@ int init_state(micsa_ctx* c) {
     const Geom& g = c->g;
     const SiteGrid sg = site_grid(g);
     CK(c, cudaMemsetAsync(c->calls, 0, sizeof(unsigned long long), c->stream));
-    CK(c, cudaMemsetAsync(c->progress, 0, (size_t)c->g.n_words * c->g.L * sizeof(int), c->stream));
-    CK(c, cudaMemsetAsync(c->task_ticket, 0, (size_t)c->g.n_words * sizeof(unsigned long long), c->stream));
     CK(c, cudaMemsetAsync(c->cnt, 0, c->plan.cnt_words * 8, c->stream));
     CK(c, cudaMemsetAsync(c->ticket, 0, sizeof(unsigned int), c->stream));
     CK(c, cudaMemsetAsync(c->st.m0, 0, c->plan.plane_bytes, c->stream));
@@ -843,8 +727,15 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->ks = philox_make_keys(seed);
     c->stream = (cudaStream_t)cuda_stream;
     c->V = vec_width(g.Lh);
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+            cudaGetLastError(); set_err("could not query the device"); delete c; return nullptr;
+        }
+        c->sms = sms;
+    }
     c->sweep_kernel = 2;
-    c->tile_tz = 4;
     c->pipe_rows = 4;
     c->use_pdl = 1;
     c->pipe_planes = (g.n_words == 1 && (g.L / 4) * (g.Lh / 4) >= 512) ? 4 : 1;   // measured: DESIGN.md 6.1
@@ -878,11 +769,9 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->minE = (long long*)(c->ws + c->plan.minE);
     c->bad = (int*)(c->ws + c->plan.bad);
     c->calls = (unsigned long long*)(c->ws + c->plan.calls);
-    c->progress = (int*)(c->ws + c->plan.progress);
-    c->task_ticket = (unsigned long long*)(c->ws + c->plan.task_ticket);
-    c->ticket0 = 0; c->progress_base = 0;
     c->trace_dev = nullptr; c->trace_bytes = 0;
     c->stage_dev = nullptr; c->stage_bytes = 0;
+    c->c4_dev = nullptr; c->c4_bytes = 0; c->c4_host = nullptr; c->c4_host_bytes = 0;
     c->host_row = nullptr; c->side = nullptr; c->ev_main = nullptr; c->ev_side = nullptr;
     if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_main, cudaEventDisableTiming) != cudaSuccess ||
@@ -910,6 +799,8 @@ int micsa_destroy(micsa_ctx* c) {
     destroy_side(c);
     if (c->trace_dev) cudaFree(c->trace_dev);
     if (c->stage_dev) cudaFree(c->stage_dev);
+    if (c->c4_dev) cudaFree(c->c4_dev);
+    if (c->c4_host) cudaFreeHost(c->c4_host);
     for (uint32_t* p : c->xm0) cudaFree(p);
     for (uint32_t* p : c->xm1) cudaFree(p);
     if (c->owns_ws) cudaFree(c->ws);
@@ -927,6 +818,7 @@ int micsa_synchronize(micsa_ctx* c) {
 
 int micsa_set_spins(micsa_ctx* c, const int8_t* s) { return set_sys(c, s, 0); }
 int micsa_set_daemons(micsa_ctx* c, const uint8_t* m) { return set_sys(c, (const int8_t*)m, 1); }
+int micsa_set_demons(micsa_ctx* c, const uint8_t* m) { return micsa_set_daemons(c, m); }
 
 int micsa_set_couplings(micsa_ctx* c, const int8_t* J) {
     int rc = check_ctx(c); if (rc) return rc;
@@ -937,7 +829,7 @@ int micsa_set_couplings(micsa_ctx* c, const int8_t* J) {
     rc = stage_reserve(c, bytes, &st.dev); if (rc) return rc;
     CK(c, cudaMemcpyAsync(st.dev, J, bytes, cudaMemcpyHostToDevice, c->stream));
     CK(c, cudaMemsetAsync(c->bad, 0, sizeof(int), c->stream));
-    validate_kernel<<<148 * 4, 256, 0, c->stream>>>((const int8_t*)st.dev, (long long)bytes, 0, c->bad);
+    validate_kernel<<<c->sms * 4, 256, 0, c->stream>>>((const int8_t*)st.dev, (long long)bytes, 0, c->bad);
     rc = post_launch(c); if (rc) return rc;
     int bad = 0;
     CK(c, cudaMemcpyAsync(&bad, c->bad, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
@@ -1104,6 +996,23 @@ int micsa_effective_temperature(double e_daemon_per_variable, double* T) {
     return MICSA_OK;
 }
 
+int micsa_debug_philox(uint64_t seed, const uint32_t* counters, int n, uint32_t* out) {
+    if (!counters || !out || n < 0) { set_err("null pointer or negative count"); return MICSA_ERR_INVALID; }
+    if (n == 0) return MICSA_OK;
+    void* dev = nullptr;
+    const size_t bytes = (size_t)n * 16;
+    if (cudaMalloc(&dev, 2 * bytes) != cudaSuccess) { cudaGetLastError(); set_err("no usable CUDA device or out of memory"); return MICSA_ERR_CUDA; }
+    cudaError_t e = cudaMemcpy(dev, counters, bytes, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        debug_philox_kernel<<<(n + 127) / 128, 128>>>((const uint4*)dev, (uint4*)((char*)dev + bytes), n, philox_make_keys(seed));
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(out, (char*)dev + bytes, bytes, cudaMemcpyDeviceToHost);
+    cudaFree(dev);
+    if (e != cudaSuccess) { set_err("CUDA error: %s", cudaGetErrorString(e)); return MICSA_ERR_CUDA; }
+    return MICSA_OK;
+}
+
 int micsa_debug_thresholds(double T, uint64_t thr[3]) {
     if (!thr) { set_err("null pointer"); return MICSA_ERR_INVALID; }
     if (thresholds_host(T, thr) != MICSA_OK) { set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID; }
@@ -1163,22 +1072,37 @@ int micsa_measure_c4(micsa_ctx* c, int64_t* S) {
     if (!S) { set_err("null pointer"); return MICSA_ERR_INVALID; }
     if (g.n_replicas != 2) { set_err("micsa_measure_c4 needs n_replicas == 2"); return MICSA_ERR_INVALID; }
     const int R = g.L / 2 + 1;
-    const size_t x_bytes = (size_t)g.n_sg * (size_t)g.N * sizeof(uint32_t);
+    const size_t x_bytes = align_up((size_t)g.n_sg * (size_t)g.N * sizeof(uint32_t));
     const size_t cnt_words = (size_t)g.n_sg * 3 * R * 32;
-    Staging X, cnt;
-    if (cudaMalloc(&X.dev, x_bytes) != cudaSuccess || cudaMalloc(&cnt.dev, cnt_words * 8) != cudaSuccess) {
-        cudaGetLastError(); set_err("out of device memory (c4)"); return MICSA_ERR_NOMEM;
+    // context-owned, grow-only: no cudaMalloc / cudaFree per measurement
+    if (x_bytes + cnt_words * 8 > c->c4_bytes) {
+        CK(c, cudaStreamSynchronize(c->stream));
+        if (c->c4_dev) cudaFree(c->c4_dev);
+        c->c4_dev = nullptr; c->c4_bytes = 0;
+        if (cudaMalloc(&c->c4_dev, x_bytes + cnt_words * 8) != cudaSuccess) {
+            cudaGetLastError(); set_err("out of device memory (c4)"); return MICSA_ERR_NOMEM;
+        }
+        c->c4_bytes = x_bytes + cnt_words * 8;
     }
-    CK(c, cudaMemsetAsync(cnt.dev, 0, cnt_words * 8, c->stream));
-    overlap_field_kernel<<<site_blocks(g, g.n_sg * 2), 128, 0, c->stream>>>(c->st.spin, (uint32_t*)X.dev, g.L, g.Lh, g.half);
+    if (cnt_words * 8 > c->c4_host_bytes) {
+        if (c->c4_host) cudaFreeHost(c->c4_host);
+        c->c4_host = nullptr; c->c4_host_bytes = 0;
+        if (cudaHostAlloc((void**)&c->c4_host, cnt_words * 8, cudaHostAllocDefault) != cudaSuccess) {
+            cudaGetLastError(); set_err("out of pinned host memory (c4)"); return MICSA_ERR_NOMEM;
+        }
+        c->c4_host_bytes = cnt_words * 8;
+    }
+    uint32_t* X = (uint32_t*)c->c4_dev;
+    unsigned long long* cnt = (unsigned long long*)((char*)c->c4_dev + x_bytes);
+    CK(c, cudaMemsetAsync(cnt, 0, cnt_words * 8, c->stream));
+    overlap_field_kernel<<<site_blocks(g, g.n_sg * 2), 128, 0, c->stream>>>(c->st.spin, X, g.L, g.Lh, g.half);
     // every thread counts at most 65535 sites (16-plane counters)
     long long nb = std::max<long long>(1, std::min<long long>((g.N + kCountBlock * 64 - 1) / (kCountBlock * 64), 64));
     nb = std::max<long long>(nb, (g.N + (long long)kCountBlock * 60000 - 1) / ((long long)kCountBlock * 60000));
-    c4_count_kernel<<<dim3((unsigned)nb, (unsigned)R, (unsigned)(3 * g.n_sg)), kCountBlock, 0, c->stream>>>(
-        (const uint32_t*)X.dev, (unsigned long long*)cnt.dev, g.L);
+    c4_count_kernel<<<dim3((unsigned)nb, (unsigned)R, (unsigned)(3 * g.n_sg)), kCountBlock, 0, c->stream>>>(X, cnt, g.L);
     rc = post_launch(c, 2); if (rc) return rc;
-    std::vector<unsigned long long> host(cnt_words);
-    CK(c, cudaMemcpyAsync(host.data(), cnt.dev, cnt_words * 8, cudaMemcpyDeviceToHost, c->stream));
+    const unsigned long long* host = c->c4_host;
+    CK(c, cudaMemcpyAsync(c->c4_host, cnt, cnt_words * 8, cudaMemcpyDeviceToHost, c->stream));
     CK(c, cudaStreamSynchronize(c->stream));
     for (int sample = 0; sample < g.n_samples; ++sample) {
         const int sg = sample / g.spw, sl = sample - sg * g.spw;
@@ -1226,9 +1150,7 @@ int micsa_anneal(micsa_ctx* c, const micsa_step* sched, int n_steps, uint32_t st
     if ((size_t)keep * row_len * 8 > c->trace_bytes) {
         CK(c, cudaStreamSynchronize(c->stream));
         if (c->trace_dev) cudaFree(c->trace_dev);
-    if (c->stage_dev) cudaFree(c->stage_dev);
         c->trace_dev = nullptr; c->trace_bytes = 0;
-    c->stage_dev = nullptr; c->stage_bytes = 0;
         const size_t want = std::max<size_t>((size_t)keep * row_len * 8, 4096);
         if (cudaMalloc(&c->trace_dev, want) != cudaSuccess) {
             cudaGetLastError(); set_err("out of device memory (trace)"); return MICSA_ERR_NOMEM;
@@ -1305,11 +1227,8 @@ int micsa_set_tuning(micsa_ctx* c, int key, int value) {
     int rc = check_ctx(c); if (rc) return rc;
     switch (key) {
         case MICSA_TUNE_SWEEP_KERNEL:
-            if (value < 0 || value > 3) { set_err("sweep kernel must be 0..3"); return MICSA_ERR_INVALID; }
+            if (value != 1 && value != 2) { set_err("sweep kernel must be 1 or 2"); return MICSA_ERR_INVALID; }
             c->sweep_kernel = value; return MICSA_OK;
-        case MICSA_TUNE_TILE_TZ:
-            if (value != 2 && value != 4 && value != 8) { set_err("tile_tz must be 2, 4 or 8"); return MICSA_ERR_INVALID; }
-            c->tile_tz = value; return MICSA_OK;
         case MICSA_TUNE_PIPE_PLANES:
             if (value != 1 && value != 4) { set_err("pipe_planes must be 1 or 4"); return MICSA_ERR_INVALID; }
             c->pipe_planes = value; return MICSA_OK;

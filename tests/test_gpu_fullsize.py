@@ -1,0 +1,279 @@
+"""The bit-exact parity protocol of SURVEY.md 8(c) at BASELINE's full sizes (-m gpu).
+
+"Configs 2-5: identical seeds; compare full state after each of the first n
+sweeps covering >= 3 refreshes; beyond that, compare the int64 measurement sums
+at sparse checkpoints as far as the oracle budget allows, and run P2/P3 on the
+GPU for the full length."  What each case compares is listed in DESIGN.md 3.1.
+
+The CUDA path runs the whole configuration in the launch configuration
+bench.py times (default kernel selection, prefetched refresh, measurement fused
+into the 10th sweep of a group); the oracle runs the same systems (all of them
+at config 4, sampled blocks of samples elsewhere -- systems never interact).
+"""
+import numpy as np
+import pytest
+
+from micsa_workloads import CONFIGS, schedule_for
+from oracle import driver
+
+pytestmark = pytest.mark.gpu
+
+
+def _per_sweep_parity(micsa, oracle, cfg, T, interval, n_sweeps, blocks, width, tune=None):
+    """State after EVERY sweep (and after every refresh) of the first n_sweeps
+    sweeps; measurement sums at the end of every refresh interval."""
+    L, nr, seed = cfg.L, cfg.n_replicas, cfg.seed
+    ref = []
+    for k in blocks:
+        s = oracle.init_spins(L, width, nr, seed, sample_offset=k)
+        J = oracle.init_bonds(L, width, seed, sample_offset=k)
+        ref.append((k, s, np.zeros_like(s, dtype=np.uint8), J))
+
+    def compare(g, what):
+        gs, gm, _ = g.get_state(couplings=False)
+        for k, s, m, _ in ref:
+            np.testing.assert_array_equal(gs[k:k + width], s, err_msg=f"spins, samples {k}.., {what}")
+            np.testing.assert_array_equal(gm[k:k + width], m, err_msg=f"daemons, samples {k}.., {what}")
+
+    with micsa.MicSA(L, cfg.n_samples, nr, seed) as g:
+        for key, v in (tune or {}).items():
+            g.set_tuning(key, v)
+        gJ = g.get_state(spins=False, daemons=False)[2]
+        for k, _, _, J in ref:
+            np.testing.assert_array_equal(gJ[k:k + width], J)
+        for t in range(n_sweeps):
+            if t % interval == 0:
+                r = t // interval
+                g.refresh_demons(T, r)
+                if t + interval < n_sweeps:
+                    g.prefetch_refresh(T, r + 1)          # generated under the sweeps, as bench.py does
+                for k, _, m, _ in ref:
+                    oracle.refresh(L, m, seed, T, r, k)
+                compare(g, f"after refresh {r}")
+            last_of_group = (t + 1) % interval == 0
+            if last_of_group:
+                g.sweep_measure(1)
+                E, Ed, Q = g.measure_end()
+            else:
+                g.sweep(1)
+            for _, s, m, J in ref:
+                oracle.sweep(L, s, m, J, 1)
+            compare(g, f"after sweep {t + 1}")
+            if last_of_group:
+                for k, s, m, J in ref:
+                    oE, oEd, oQ = oracle.measure(L, s, m, J)
+                    sl = slice(k * nr, (k + width) * nr)
+                    np.testing.assert_array_equal(E[sl], oE)
+                    np.testing.assert_array_equal(Ed[sl], oEd)
+                    if nr == 2:
+                        np.testing.assert_array_equal(Q[k:k + width], oQ)
+
+
+def test_config4_every_sample_every_sweep(micsa, oracle):
+    """Config 4, ALL 16 samples x 2 replicas (every lane of the 32-lane word at L = 160): the full state after each
+    of the first 30 sweeps and each of their 3 refreshes."""
+    cfg = CONFIGS[4]
+    _per_sweep_parity(micsa, oracle, cfg, cfg.temperatures[0], 10, 30, blocks=(0,), width=cfg.n_samples)
+
+
+def test_config4_every_sample_alternative_kernels(micsa, oracle):
+    """The same lattice under the non-default sweep kernels (12 sweeps, 2 refreshes, all 32 lanes)."""
+    cfg = CONFIGS[4]
+    for tune in ({"sweep_kernel": 2, "pipe_planes": 1}, {"sweep_kernel": 1}):
+        _per_sweep_parity(micsa, oracle, cfg, cfg.temperatures[0], 6, 12, blocks=(0,), width=cfg.n_samples, tune=tune)
+
+
+@pytest.mark.parametrize("T", CONFIGS[2].temperatures)
+def test_config2_every_sweep(micsa, oracle, T):
+    _per_sweep_parity(micsa, oracle, CONFIGS[2], T, 10, 30, blocks=(0, 28, 60), width=4)
+
+
+@pytest.mark.parametrize("interval,n_sweeps", [(1, 4), (10, 30)])
+def test_config3_every_sweep(micsa, oracle, interval, n_sweeps):
+    cfg = CONFIGS[3]
+    _per_sweep_parity(micsa, oracle, cfg, cfg.temperatures[0], interval, n_sweeps, blocks=(0, 62, 124), width=4)
+
+
+def test_config3_interval_100(micsa, oracle):
+    """Refresh interval 100: 3 refreshes = 300 sweeps on one sample; state after sweeps 1..10 of every interval and
+    at its end (the oracle still runs every sweep)."""
+    cfg = CONFIGS[3]
+    L, nr, seed, T, k = cfg.L, cfg.n_replicas, cfg.seed, cfg.temperatures[0], 77
+    s = oracle.init_spins(L, 1, nr, seed, sample_offset=k)
+    J = oracle.init_bonds(L, 1, seed, sample_offset=k)
+    m = np.zeros_like(s, dtype=np.uint8)
+    with micsa.MicSA(L, cfg.n_samples, nr, seed) as g:
+        for r in range(3):
+            g.refresh_demons(T, r); oracle.refresh(L, m, seed, T, r, k)
+            g.prefetch_refresh(T, r + 1)
+            for t in range(10):
+                g.sweep(1); oracle.sweep(L, s, m, J, 1)
+                gs, gm, _ = g.get_state(couplings=False)
+                np.testing.assert_array_equal(gs[k:k + 1], s); np.testing.assert_array_equal(gm[k:k + 1], m)
+            g.sweep(89); g.sweep_measure(1); E, Ed, Q = g.measure_end()
+            oracle.sweep(L, s, m, J, 90)
+            gs, gm, _ = g.get_state(couplings=False)
+            np.testing.assert_array_equal(gs[k:k + 1], s); np.testing.assert_array_equal(gm[k:k + 1], m)
+            oE, oEd, oQ = oracle.measure(L, s, m, J)
+            np.testing.assert_array_equal(E[k * nr:(k + 1) * nr], oE)
+            np.testing.assert_array_equal(Ed[k * nr:(k + 1) * nr], oEd)
+            np.testing.assert_array_equal(Q[k:k + 1], oQ)
+
+
+def test_config5_every_sweep(micsa, oracle):
+    """Config 5 (1024 single-replica samples, 201 MB of state, lattice groups): the first three ramp steps."""
+    cfg = CONFIGS[5]
+    sched = schedule_for(cfg, n_sweeps=30)
+    L, seed = cfg.L, cfg.seed
+    blocks, width = (0, 500, 1020), 4
+    ref = []
+    for k in blocks:
+        s = oracle.init_spins(L, width, 1, seed, sample_offset=k)
+        ref.append((k, s, np.zeros_like(s, dtype=np.uint8), oracle.init_bonds(L, width, seed, sample_offset=k)))
+    with micsa.MicSA(L, cfg.n_samples, 1, seed) as g:
+        for r, (T, n, _) in enumerate(sched):
+            g.refresh_demons(T, r)
+            if r + 1 < len(sched):
+                g.prefetch_refresh(sched[r + 1][0], r + 1)
+            for k, _, m, _ in ref:
+                oracle.refresh(L, m, seed, T, r, k)
+            for t in range(n):
+                if t == 3:
+                    g.sweep(n - 4)                     # a multi-sweep call: goes lattice group by lattice group
+                    for _, s, m, J in ref:
+                        oracle.sweep(L, s, m, J, n - 4)
+                elif t > 3 and t < n - 1:
+                    continue
+                else:
+                    g.sweep(1)
+                    for _, s, m, J in ref:
+                        oracle.sweep(L, s, m, J, 1)
+                gs, gm, _ = g.get_state(couplings=False)
+                for k, s, m, _ in ref:
+                    np.testing.assert_array_equal(gs[k:k + width], s)
+                    np.testing.assert_array_equal(gm[k:k + width], m)
+            E, Ed, _ = g.measure_i64()
+            for k, s, m, J in ref:
+                oE, oEd, _ = oracle.measure(L, s, m, J)
+                np.testing.assert_array_equal(E[k:k + width], oE)
+                np.testing.assert_array_equal(Ed[k:k + width], oEd)
+
+
+@pytest.mark.parametrize("walkers", [False, True])
+def test_config4_gamma6_full_size(micsa, oracle, walkers):
+    """gamma = 6 daemon families / six walkers per spin (Eq. 13) on the L = 160 lattice of config 4
+    (238 MB of state; with walkers the exchanges along X, Y and Z ride on the odd half-sweeps): two refreshes, three
+    timesteps each = 36 sweeps, sampled samples against the oracle driver -- spins, every family, rows."""
+    cfg = CONFIGS[4]
+    L, nr, seed, gamma = cfg.L, cfg.n_replicas, cfg.seed, 6
+    sched = [(0.9, 3, 1), (0.8, 3, 3)]
+    with micsa.MicSA(L, cfg.n_samples, nr, seed) as g:
+        g.set_gamma(gamma)
+        g.set_walkers(1 if walkers else 0)
+        out = g.anneal(sched)
+        spins = g.get_state(daemons=False, couplings=False)[0]
+        fam = []
+        for alpha in range(gamma):
+            g.select_daemon_set(alpha)
+            fam.append(g.get_state(spins=False, couplings=False)[1])
+        assert g.get_time() == 6
+    for k in (3, 12):
+        s = oracle.init_spins(L, 1, nr, seed, sample_offset=k)
+        J = oracle.init_bonds(L, 1, seed, sample_offset=k)
+        m = np.zeros((gamma, 1, nr, L ** 3), np.uint8)
+        ref = driver.anneal(L, s, m, J, seed, sched, sample_offset=k, walkers=walkers)
+        np.testing.assert_array_equal(spins[k:k + 1], s)
+        for alpha in range(gamma):
+            np.testing.assert_array_equal(fam[alpha][k:k + 1], m[alpha])
+        sl = slice(k * nr, (k + 1) * nr)
+        np.testing.assert_array_equal(out["E"][:, sl], ref["E"])
+        np.testing.assert_array_equal(out["Edem"][:, sl], ref["Edem"])
+        np.testing.assert_array_equal(out["Q"][:, k:k + 1], ref["Q"])
+
+
+def test_config2_late_checkpoint_rows(micsa, oracle):
+    """Beyond the per-sweep window: the int64 sums at sweeps 250, 500, 750, 1000 of config 2 (T = 2.0) and the state at
+    sweep 1000, four samples against the oracle."""
+    cfg = CONFIGS[2]
+    L, nr, seed, k, width = cfg.L, cfg.n_replicas, cfg.seed, 36, 4
+    sched = schedule_for(cfg, T=2.0, n_sweeps=1000, measure_every=10)
+    with micsa.MicSA(L, cfg.n_samples, nr, seed) as g:
+        out = g.anneal(sched)
+        gs, gm, _ = g.get_state(couplings=False)
+    s = oracle.init_spins(L, width, nr, seed, sample_offset=k)
+    J = oracle.init_bonds(L, width, seed, sample_offset=k)
+    m = np.zeros_like(s, dtype=np.uint8)
+    ref = driver.anneal(L, s, m, J, seed, sched, sample_offset=k)
+    np.testing.assert_array_equal(gs[k:k + width], s)
+    np.testing.assert_array_equal(gm[k:k + width], m)
+    sl = slice(k * nr, (k + width) * nr)
+    for row in (24, 49, 74, 99):
+        assert out["sweep"][row] == ref["sweep"][row] == 10 * (row + 1)
+        np.testing.assert_array_equal(out["E"][row, sl], ref["E"][row])
+        np.testing.assert_array_equal(out["Edem"][row, sl], ref["Edem"][row])
+        np.testing.assert_array_equal(out["Q"][row, k:k + width], ref["Q"][row])
+
+
+def _full_length_invariants(micsa, cfg, sched_step, n_steps, n_check):
+    """P2 / P3 over a run of the configuration's REAL length: n_steps schedule steps through
+    micsa_anneal, interrupted at n_check evenly spaced places by a hand-made step (refresh, measure, sweeps, measure)
+    in which E + E_daemon must be the same integer before and after the sweeps, in every system; at the end n sweeps
+    forward and n with the half-sweeps reversed restore the state."""
+    T, n_sw = sched_step
+    chunk = n_steps // n_check
+    with micsa.MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed) as g:
+        done = 0
+        for c in range(n_check):
+            g.anneal([(T, n_sw, 0)] * (chunk - 1), step0=done, trace=False)
+            done += chunk - 1
+            g.refresh_demons(T, done)
+            E0, Ed0, _ = g.measure_i64()
+            g.sweep(n_sw - 1); g.sweep_measure(1)
+            E1, Ed1, _ = g.measure_end()
+            np.testing.assert_array_equal(E0 + Ed0, E1 + Ed1)
+            done += 1
+        assert g.counters()["attempts"] == done * n_sw * cfg.attempts_per_sweep
+        s0, m0, _ = g.get_state(couplings=False)
+        g.sweep(25)
+        for _ in range(25):
+            g.half_sweep(1); g.half_sweep(0)
+        s1, m1, _ = g.get_state(couplings=False)
+        np.testing.assert_array_equal(s1, s0)
+        np.testing.assert_array_equal(m1, m0)
+        return E1 / cfg.N
+
+
+def test_config4_full_length_invariants(micsa):
+    cfg = CONFIGS[4]
+    e = _full_length_invariants(micsa, cfg, (cfg.temperatures[0], 10), cfg.n_sweeps // 10, 20)
+    assert -1.75 < e.mean() < -1.73                       # -1.7402 after 1e5 sweeps at T = 0.9
+
+
+def test_config3_full_length_invariants(micsa):
+    cfg = CONFIGS[3]
+    e = _full_length_invariants(micsa, cfg, (cfg.temperatures[0], 10), cfg.n_sweeps // 10, 20)
+    assert -1.77 < e.mean() < -1.75                       # -1.7622 at T = 0.7, R = 10
+
+
+def test_config5_full_length_invariants(micsa):
+    """Config 5's ramp at its real length, E + E_daemon checked inside 20 of its 1000 steps, reversal at T = 0.2."""
+    cfg = CONFIGS[5]
+    sched = schedule_for(cfg)
+    with micsa.MicSA(cfg.L, cfg.n_samples, 1, cfg.seed) as g:
+        for c in range(20):
+            lo = c * 50
+            g.anneal(sched[lo:lo + 49], step0=lo, trace=False)
+            T = sched[lo + 49][0]
+            g.refresh_demons(T, lo + 49)
+            E0, Ed0, _ = g.measure_i64()
+            g.sweep(9); g.sweep_measure(1)
+            E1, Ed1, _ = g.measure_end()
+            np.testing.assert_array_equal(E0 + Ed0, E1 + Ed1)
+        assert (E1 / cfg.N).mean() < -1.76                # annealed: -1.7714
+        s0, m0, _ = g.get_state(couplings=False)
+        g.sweep(20)
+        for _ in range(20):
+            g.half_sweep(1); g.half_sweep(0)
+        s1, m1, _ = g.get_state(couplings=False)
+        np.testing.assert_array_equal(s1, s0)
+        np.testing.assert_array_equal(m1, m0)

@@ -75,7 +75,8 @@ def test_philox_matches_curand_host(oracle, seed, offset):
     # Philox(counter = (q / 65536 as 64 bit, q % 65536 as 64 bit), key = seed).
     # The host API therefore exercises c0, c1, the low 16 bits of c2 and both
     # key words; c3 and the rest of c2 are covered by the all-words test below
-    # and by the device-API pin in tests/test_gpu_parity.py.
+    # and by the device-API pin test_philox_matches_curand_device_api in
+    # tests/test_gpu_parity.py (curand_init's subsequence reaches c2 and c3).
     for k in range(n_sub):
         q = offset // 4 + k
         pos, sub = q // 65536, q % 65536
