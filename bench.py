@@ -6,18 +6,28 @@
 One STEP = one pass of the whole hot path over BASELINE
 config 4 (L=160, 16 samples x 2 replicas, T=0.9): daemon refresh at T, then
 10 checkerboard sweeps, then the E / E_daemon / q reductions.  Prints ONE JSON
-line (rank 0).  `value` = spin-flip attempts per ns with the state resident in
-HBM, timed with CUDA events on the library's stream, L2 flushed between steps;
-the refresh of step k+1 is generated on the library's side stream during step
-k (micsa_prefetch_refresh), so every timed step contains one generation;
-`e2e` = the same step through the C ABI with HOST buffers (couplings + spins
-uploaded from pinned host memory, observables read back) inside the timed
-region.  N > 1: one process per GPU (torchrun), samples sharded by rank with
-global sample offsets, no data-path collective (weak scaling).
+line (rank 0).
+
+`value` (attempts per ns, state resident in HBM / L2) is the LOWER of two
+device-timed figures, both with a closed timed window:
+  * back_to_back: the K steps through ONE micsa_anneal call, one CUDA-event
+    pair on the library's stream around all of them (rows read back inside);
+  * l2_flushed: K separately timed steps with a 256 MiB write between them
+    (outside the events); the window of step k = generation of refresh k+1 on
+    the side stream (queued first, consumed last) + 20 half-sweeps + the
+    measurement, so no refresh work runs between two windows.
+`e2e` = upload of spins and couplings from pinned host int8 arrays once, then
+the K steps through micsa_anneal with the rows copied back, wall clock.
+`roofline` = the plain half-sweep launches inside the flushed steps;
+`hbm_resident` = the same kernels on 160^3 x 128 systems (the shape of the
+paper's Table 3; 295 MB of state, larger than L2).
+N > 1: one process per GPU (torchrun), samples sharded by rank with global
+sample offsets, no data-path collective (weak scaling).
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -38,16 +48,24 @@ SWEEPS_PER_STEP = CFG.refresh_intervals[0]          # refresh every 10 sweeps
 T_RUN = CFG.temperatures[0]
 METRIC = "spin-flip attempts/ns (refresh + 10 sweeps + measure per step)"
 UNIT = "attempts/ns"
-# dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch from the
-# ncu --set full capture summarised in profiles/r1c_final_launches_and_sweep.md
-# (cold L2: ncu flushes caches before every replay; in a real step the 73.7 MB
-# state stays in the 126 MB L2 after the first sweep)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 57_401_600 + 172_288
-# lts__t_sectors_srcunit_tex.sum * 32 B of the same capture: what crosses the L2 <-> SM path per launch -- the
-# path that actually bounds the kernel (the state is L2-resident); the microarchitecture guide's full-chip L2
-# throughput cap is ~6300 B/clk = 12.4 TB/s at 1.965 GHz
-NCU_L2_BYTES_PER_LAUNCH = 3_355_957 * 32
-L2_CAP_GBS = 6300 * 1.965
+# the microarchitecture guide's full-chip L2 throughput cap: ~6300 B/clk at the SM clock
+L2_CAP_BYTES_PER_CLK = 6300.0
+NCU_CSV = ROOT / "profiles" / "r2_ncu_metrics.csv"
+
+
+def ncu_metrics(kernel_prefix, workload):
+    """Per-launch counters of an ncu capture, from the committed summary
+    profiles/r2_ncu_metrics.csv (columns: kernel, workload, metric, value, commit; written from the capture named in
+    profiles/r2_ncu_metrics.md).  Returns ({metric: value}, commit) or ({}, None)."""
+    if not NCU_CSV.exists():
+        return {}, None
+    out, commit = {}, None
+    with open(NCU_CSV) as f:
+        for row in csv.DictReader(f):
+            if row["kernel"].startswith(kernel_prefix) and row["workload"] == workload:
+                out[row["metric"]] = float(row["value"])
+                commit = row["commit"]
+    return out, commit
 
 
 def measured_peaks():
@@ -121,11 +139,18 @@ class ClockSampler(threading.Thread):
                 "source": "nvml" if self.nvml is not None else "nvidia-smi"}
 
 
-def oracle_step_rate(n_samples, steps, warmup):
-    """The oracle, as it stands, on the host cores: same step on the first
-    n_samples samples of config 4.  Returns (attempts/ns, cores, seconds)."""
+def oracle_step_rate(n_samples, steps, warmup, threads=None):
+    """The oracle, as it stands, on the host cores: the same step on the first n_samples samples of config 4.  Its
+    OpenMP loop spreads SYSTEMS over threads (oracle/micsa_oracle.c), so n_samples * n_replicas systems keep at most
+    that many cores busy.  Returns (attempts/ns, threads busy, seconds)."""
     import oracle
     L, nr, seed = CFG.L, CFG.n_replicas, CFG.seed
+    avail = os.cpu_count() or 1
+    if threads is not None:
+        oracle.set_num_threads(threads)
+    else:
+        oracle.set_num_threads(avail)
+    busy = min(oracle.num_threads(), n_samples * nr)
     s = oracle.init_spins(L, n_samples, nr, seed)
     J = oracle.init_bonds(L, n_samples, seed)
     m = np.zeros_like(s, dtype=np.uint8)
@@ -138,16 +163,37 @@ def oracle_step_rate(n_samples, steps, warmup):
         oracle.measure(L, s, m, J)
         if k >= warmup:
             t_total += time.perf_counter() - t0
-    return attempts * steps / t_total / 1e9, oracle.num_threads(), t_total
+    oracle.set_num_threads(avail)
+    return attempts * steps / t_total / 1e9, busy, t_total
+
+
+def oracle_sample_size():
+    """Samples of config 4 the oracle legs run: one system per host core (2 replicas per sample)."""
+    cores = os.cpu_count() or 1
+    return max(1, min(CFG.n_samples, cores // CFG.n_replicas)), cores
+
+
+def cpu_baseline_record(steps=1):
+    n_s, cores = oracle_sample_size()
+    rate_all, busy, secs = oracle_step_rate(n_s, steps, 0)
+    rate_1, _, secs1 = oracle_step_rate(1, 1, 0, threads=1)
+    rate_1 /= 1.0                                        # 2 systems, one thread
+    return {"value": rate_all, "unit": UNIT, "cores": busy, "kind": "oracle",
+            "host_cores": cores, "value_allcores": rate_all, "cores_used": busy,
+            "value_1core": rate_1,
+            "sample": f"{steps} step(s) (refresh + {SWEEPS_PER_STEP} sweeps + measure) of config 4 restricted to its "
+                      f"first {n_s} samples x {CFG.n_replicas} replicas at L={CFG.L} = {n_s * CFG.n_replicas} systems, "
+                      f"one OpenMP thread per system ({secs:.1f} s); value_1core: the first sample's 2 systems on "
+                      f"one thread ({secs1:.1f} s)"}
 
 
 def run_reference(args, rank):
     if rank != 0:
         return
-    n_samples = 1                       # 2 systems of L=160: ~2-3 s of CPU work per step
-    rate, cores, secs = oracle_step_rate(n_samples, args.steps, min(args.warmup, 1))
-    sample = (f"config 4 restricted to its first {n_samples} sample(s) x {CFG.n_replicas} replicas "
-              f"(L={CFG.L}); each step = refresh + {SWEEPS_PER_STEP} sweeps + measure")
+    n_s, cores = oracle_sample_size()
+    rate, busy, secs = oracle_step_rate(n_s, args.steps, min(args.warmup, 1))
+    sample = (f"config 4 restricted to its first {n_s} sample(s) x {CFG.n_replicas} replicas (L={CFG.L}), one OpenMP "
+              f"thread per system on {cores} host cores; each step = refresh + {SWEEPS_PER_STEP} sweeps + measure")
     line = {
         "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3,
@@ -155,7 +201,8 @@ def run_reference(args, rank):
         "data": "synthetic",
         "config": {"workload": CFG.name, "L": CFG.L, "n_samples": CFG.n_samples,
                    "n_replicas": CFG.n_replicas, "T": T_RUN, "sweeps_per_step": SWEEPS_PER_STEP},
-        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": busy, "host_cores": cores, "kind": "oracle",
+                         "sample": sample},
         "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -170,8 +217,9 @@ def main():
     ap.add_argument("--impl", default="micsa", choices=["micsa", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-hbm-resident", action="store_true")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
-                    help="micsa_set_tuning for A/B runs, e.g. --tune pipe_smem_kb=48")
+                    help="micsa_set_tuning for A/B runs, e.g. --tune sweep_kernel=2")
     ap.add_argument("--walkers", action="store_true",
                     help="one forward-X walker per spin instead of a daemon (PAPER.md Sec. 2.6): every sweep is "
                          "followed by a wandering half-cycle; reported under its own metric name")
@@ -220,147 +268,235 @@ def main():
     stream = torch.cuda.Stream(device=dev, priority=-1)
     torch.cuda.set_stream(stream)
     from paper_2506_16240_b200.sharding import sample_offset
-    g = micsa.MicSA(L, ns, nr, CFG.seed, sample_offset=sample_offset(rank, ns), device=local_rank,
-                    stream=stream)
-    if args.no_fuse_measure:
-        g.set_tuning("fuse_measure", 0)
-    if args.walkers:
-        g.set_walkers(1)
-    for kv in args.tune:
-        k, v = kv.split("=")
-        g.set_tuning(k, int(v))
+
+    def tuned(g):
+        if args.no_fuse_measure:
+            g.set_tuning("fuse_measure", 0)
+        if args.walkers:
+            g.set_walkers(1)
+        for kv in args.tune:
+            k, v = kv.split("=")
+            g.set_tuning(k, int(v))
+        return g
+
+    g = tuned(micsa.MicSA(L, ns, nr, CFG.seed, sample_offset=sample_offset(rank, ns), device=local_rank,
+                          stream=stream))
     info = g.layout_info()
     attempts_step = CFG.attempts_per_sweep * SWEEPS_PER_STEP
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+    K, W = args.steps, args.warmup
+    sched_step = (T_RUN, SWEEPS_PER_STEP, SWEEPS_PER_STEP)
 
+    # ---- (1) l2_flushed: separately timed steps, closed window -------------------------------------------------
+    # window of step k: [queue the generation of refresh k+1 on the side stream] [9 plain sweeps]
+    # [measuring sweep, row D2H] [consume refresh k+1: wait for the side stream, swap the planes]
     def step(k, ev=None):
-        g.refresh_demons(T_RUN, k)              # consumes the planes prefetched during step k-1
-        g.prefetch_refresh(T_RUN, k + 1)        # generated on the side stream under this step's sweeps
+        if ev:
+            ev[0].record(stream)
+        g.prefetch_refresh(T_RUN, k + 1)
         if ev:
             ev[1].record(stream)
         g.sweep(SWEEPS_PER_STEP - 1)            # 18 plain half-sweep launches: the roofline kernel
         if ev:
             ev[2].record(stream)
         g.sweep_measure(1)                      # the last sweep also counts E, E_daemon, q; row D2H queued
+        g.refresh_demons(T_RUN, k + 1)          # the refresh the next step starts from
         if ev:
             ev[3].record(stream)
         return g.measure_end()                  # host waits for the row (after the timed region)
 
-    for k in range(args.warmup):
+    g.refresh_demons(T_RUN, 0)
+    for k in range(W):
         step(k)
     barrier()
     launches0 = g.layout_info()["launches"]
     calls0 = g.counters()["philox_calls"]
     sampler = ClockSampler(local_rank)
     sampler.start()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
     barrier()
     wall0 = time.perf_counter()
-    for k in range(args.steps):
-        flush.zero_()                                   # evict the state from L2 (untimed)
-        ev = evs[k]
-        ev[0].record(stream)
-        step(args.warmup + k, ev)
+    for k in range(K):
+        flush.zero_()                                   # evict the state from L2 (untimed; nothing else is queued)
+        step(W + k, evs[k])
     barrier()
     wall = time.perf_counter() - wall0
-    clocks = sampler.stop()
-    launches = g.layout_info()["launches"] - launches0
+    launches_flushed = g.layout_info()["launches"] - launches0
     philox_words = 4.0 * (g.counters()["philox_calls"] - calls0)
-    t_step_ms = sum(e[0].elapsed_time(e[3]) for e in evs)
+    t_flushed_ms = max_over_ranks(sum(e[0].elapsed_time(e[3]) for e in evs))
     t_sweep_ms = sum(e[1].elapsed_time(e[2]) for e in evs)
-    t_step_ms = max_over_ranks(t_step_ms)
     t_sweep_ms_max = max_over_ranks(t_sweep_ms)
-    value = attempts_step * args.steps * world / (t_step_ms * 1e6)
+    value_flushed = attempts_step * K * world / (t_flushed_ms * 1e6)
 
-    # steady state, no flush, back-to-back sweeps only (what a long run looks like)
+    # ---- (2) back_to_back: the K steps in ONE micsa_anneal call, one event pair --------------------------------
+    g.anneal([sched_step] * W, step0=W + K + 1)                      # warm-up of this path (rows, trace buffer)
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches1 = g.layout_info()["launches"]
+    e0.record(stream)
+    out = g.anneal([sched_step] * K, step0=2 * W + K + 1)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    launches_b2b = g.layout_info()["launches"] - launches1
+    t_b2b_ms = max_over_ranks(e0.elapsed_time(e1))
+    value_b2b = attempts_step * K * world / (t_b2b_ms * 1e6)
+    assert out["E"].shape[0] == K
+    if value_b2b <= value_flushed:
+        value, t_step_ms, which, launches = value_b2b, t_b2b_ms, "back_to_back", launches_b2b
+    else:
+        value, t_step_ms, which, launches = value_flushed, t_flushed_ms, "l2_flushed", launches_flushed
+
+    # steady state, no flush, back-to-back sweeps only
+    barrier()
     e0.record(stream); g.sweep(100); e1.record(stream)
     torch.cuda.synchronize()
     sweep_only = CFG.attempts_per_sweep * 100 / (e0.elapsed_time(e1) * 1e6)
 
-    # roofline of the dominant kernel (half-sweep), live from the timed region
+    # ---- roofline of the dominant kernel (plain half-sweep), live from the flushed steps ------------------------
     peak, peak_src = measured_peaks()
-    n_launch = 2 * (SWEEPS_PER_STEP - 1) * args.steps        # the plain launches between events 1 and 2
+    sm_mhz = clocks.get("sm_mhz") or 1965.0
+    l2_cap_gbs = L2_CAP_BYTES_PER_CLK * sm_mhz * 1e6 / 1e9
+    n_launch = 2 * (SWEEPS_PER_STEP - 1) * K                 # the plain launches between events 1 and 2
     t_launch_s = t_sweep_ms * 1e-3 / n_launch
     alg_bytes = info["compulsory_bytes_per_sweep"] / 2          # per half-sweep launch
     achieved = alg_bytes / t_launch_s / 1e9
+    kname = g.sweep_kernel_name() if hasattr(g, "sweep_kernel_name") else "half_sweep_pipe_kernel"
+    ncu, ncu_commit = ncu_metrics(kname, CFG.name)
+    traffic = None
+    if "dram__bytes_read.sum" in ncu:
+        traffic = ncu["dram__bytes_read.sum"] + ncu.get("dram__bytes_write.sum", 0.0)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
-                "kernel": "half_sweep_pipe_kernel<2,4,4>", "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic, "traffic_source": f"{NCU_CSV.name} @ {ncu_commit}" if ncu else None,
+                "kernel": kname, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "us_per_launch": t_launch_s * 1e6,
                 "convention": "compulsory one-pass traffic: 7.5 bits/attempt (spin 1r+1w, daemon 2r+2w, "
                               "bonds 1.5r shared by the replica pair)",
-                "l2_path": {"bytes_per_launch": NCU_L2_BYTES_PER_LAUNCH,
-                            "achieved_gbs": NCU_L2_BYTES_PER_LAUNCH / t_launch_s / 1e9, "cap_gbs": L2_CAP_GBS,
-                            "frac": NCU_L2_BYTES_PER_LAUNCH / t_launch_s / 1e9 / L2_CAP_GBS,
-                            "note": "secondary roofline: L2 <-> SM bytes of the ncu capture over the live launch "
-                                    "time, against the guide's full-chip L2 throughput cap"},
-                "sweep_share_of_step": t_sweep_ms_max / t_step_ms,
-                "note": "share = the 18 plain half-sweep launches of a step; the 2 launches of the last sweep "
-                        "also do the measurement and are timed with the rest of the step"}
+                "real_bound": "L2 <-> SM path: the 73.7 MB state of config 4 is L2-resident after the first sweep of a "
+                              "step, DRAM traffic is ~0 warm; see l2_path and hbm_resident",
+                "sweep_share_of_step": t_sweep_ms_max / t_flushed_ms,
+                "note": "share = the 18 plain half-sweep launches of an l2_flushed step; the 2 launches of the last "
+                        "sweep also do the measurement and are timed with the rest of the step"}
+    if "lts__t_sectors_srcunit_tex.sum" in ncu:
+        l2b = ncu["lts__t_sectors_srcunit_tex.sum"] * 32.0
+        roofline["l2_path"] = {"bytes_per_launch": l2b, "achieved_gbs": l2b / t_launch_s / 1e9, "cap_gbs": l2_cap_gbs,
+                               "frac": l2b / t_launch_s / 1e9 / l2_cap_gbs, "source": f"{NCU_CSV.name} @ {ncu_commit}",
+                               "note": "secondary roofline: L2 <-> SM bytes of the ncu capture over the live launch "
+                                       "time, against the guide's full-chip L2 throughput cap (6300 B/clk)"}
 
-    # end to end through the C ABI with host buffers
+    # ---- end to end through the C ABI with host buffers ---------------------------------------------------------
     e2e = None
     if not args.no_e2e:
         s_host = torch.from_numpy(g.get_state(daemons=False, couplings=False)[0]).pin_memory()
         J_host = torch.from_numpy(g.get_state(spins=False, daemons=False)[2]).pin_memory()
         s_np, J_np = s_host.numpy(), J_host.numpy()
-        n_e2e = max(3, min(args.steps, 5))
+        n_run = max(K, 100)
         barrier()
         t0 = time.perf_counter()
-        for k in range(n_e2e):
-            g.set_couplings(J_np)
-            g.set_spins(s_np)
-            out = g.anneal([(T_RUN, SWEEPS_PER_STEP, SWEEPS_PER_STEP)], step0=1000 + k)
+        g.set_couplings(J_np)
+        g.set_spins(s_np)
+        out = g.anneal([sched_step] * n_run, step0=5000)
         barrier()
         dt = max_over_ranks(time.perf_counter() - t0)
-        h2d = s_np.nbytes + J_np.nbytes + 16
-        d2h = (2 * g.n_sys + g.n_pairs + g.n_sys) * 8
-        # the same host call with the state left on the device between steps (what a long run does:
-        # the only per-step input is the 16-byte schedule entry, the output the measurement row)
-        n_res = max(20, args.steps)
+        row_bytes = (2 * g.n_sys + g.n_pairs) * 8
+        h2d = (s_np.nbytes + J_np.nbytes) / n_run + 16
+        d2h = row_bytes + g.n_sys * 8 / n_run
+        # the upload-every-step figure of round 1 (PCIe-bound by the one-byte-per-spin boundary layout)
+        n_up = 3
         barrier()
         t1 = time.perf_counter()
-        for k in range(n_res):
-            out = g.anneal([(T_RUN, SWEEPS_PER_STEP, SWEEPS_PER_STEP)], step0=2000 + k)
+        for k in range(n_up):
+            g.set_couplings(J_np)
+            g.set_spins(s_np)
+            g.anneal([sched_step], step0=6000 + k)
         barrier()
-        dt_res = max_over_ranks(time.perf_counter() - t1)
-        e2e = {"value": attempts_step * n_e2e * world / (dt * 1e9), "unit": UNIT,
-               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e,
-               "what": "micsa_set_couplings + micsa_set_spins from pinned host int8 (one byte per spin / bond: "
-                       "the canonical boundary layout), micsa_anneal (refresh + 10 sweeps + measure), rows copied "
-                       "back; PCIe-bound by construction",
-               "state_resident": {"value": attempts_step * n_res * world / (dt_res * 1e9), "unit": UNIT,
-                                  "h2d_bytes_per_step": 16, "d2h_bytes_per_step": d2h, "steps": n_res,
-                                  "what": "micsa_anneal of one schedule step per host call, state left on the "
-                                          "device, wall clock including launch, synchronisation and row read-back"}}
+        dt_up = max_over_ranks(time.perf_counter() - t1)
+        # one host call per step, state left on the device
+        n_res = max(20, K)
+        barrier()
+        t2 = time.perf_counter()
+        for k in range(n_res):
+            g.anneal([sched_step], step0=7000 + k)
+        barrier()
+        dt_res = max_over_ranks(time.perf_counter() - t2)
+        e2e = {"value": attempts_step * n_run * world / (dt * 1e9), "unit": UNIT,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_run,
+               "what": f"wall clock of: micsa_set_couplings + micsa_set_spins from pinned host int8 arrays (one byte "
+                       f"per spin / bond, {s_np.nbytes + J_np.nbytes} B once), micsa_anneal of {n_run} steps "
+                       f"(refresh + 10 sweeps + measure each), measurement rows and min energies copied back",
+               "upload_every_step": {"value": attempts_step * n_up * world / (dt_up * 1e9), "unit": UNIT,
+                                     "h2d_bytes_per_step": s_np.nbytes + J_np.nbytes + 16,
+                                     "d2h_bytes_per_step": row_bytes + g.n_sys * 8, "steps": n_up},
+               "one_call_per_step": {"value": attempts_step * n_res * world / (dt_res * 1e9), "unit": UNIT,
+                                     "h2d_bytes_per_step": 16, "d2h_bytes_per_step": row_bytes + g.n_sys * 8,
+                                     "steps": n_res}}
     g.destroy()
+    del flush
+
+    # ---- the same kernels on a state larger than L2: 160^3 x 128 systems (Table 3 shape) ------
+    hbm = None
+    if not args.no_hbm_resident and not args.walkers:
+        ns_big = 64
+        gb = tuned(micsa.MicSA(L, ns_big, nr, CFG.seed, sample_offset=sample_offset(rank, ns_big), device=local_rank,
+                               stream=stream))
+        big = gb.layout_info()
+        att_sweep = L ** 3 * ns_big * nr
+        hbm = {"workload": f"table3_L{L}_{ns_big}x{nr}", "state_bytes": big["state_bytes"],
+               "algorithmic_bytes_per_sweep": big["compulsory_bytes_per_sweep"], "peak": peak, "unit": "GB/s"}
+        gb.refresh_demons(T_RUN, 0)
+        for l2g in (0, 1):
+            gb.set_tuning("l2_groups", l2g)
+            gb.sweep(10)
+            barrier()
+            reps = []
+            for _ in range(3):
+                e0.record(stream); gb.sweep(10); e1.record(stream)
+                torch.cuda.synchronize()
+                reps.append(e0.elapsed_time(e1) / 10.0)
+            ms = max_over_ranks(float(np.median(reps)))
+            gbs = big["compulsory_bytes_per_sweep"] / (ms * 1e-3) / 1e9
+            hbm[f"l2_groups_{l2g}"] = {"us_per_sweep": ms * 1e3, "attempts_per_ns": att_sweep * world / (ms * 1e6),
+                                       "achieved": gbs, "frac": gbs / peak}
+        gb.set_tuning("l2_groups", 1)
+        gb.anneal([sched_step] * 3, step0=1)
+        barrier()
+        e0.record(stream); gb.anneal([sched_step] * 20, step0=4); e1.record(stream)
+        barrier()
+        hbm["whole_step_attempts_per_ns"] = att_sweep * SWEEPS_PER_STEP * 20 * world / (max_over_ranks(e0.elapsed_time(e1)) * 1e6)
+        nb, nb_commit = ncu_metrics(kname, hbm["workload"])
+        if "dram__bytes_read.sum" in nb:
+            hbm["traffic_per_half_sweep"] = nb["dram__bytes_read.sum"] + nb.get("dram__bytes_write.sum", 0.0)
+            hbm["traffic_source"] = f"{NCU_CSV.name} @ {nb_commit}"
+        hbm["note"] = ("sweeps only, 10 per call; l2_groups_0 = every half-sweep over all 4 word lattices (each launch "
+                       "streams the state through HBM), l2_groups_1 = the 10 sweeps lattice group by lattice group; "
+                       "frac = 7.5 bits/attempt over time against the measured HBM copy peak")
+        gb.destroy()
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        n_s = 2
-        rate, cores, secs = oracle_step_rate(n_s, 1, 0)
-        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"one step (refresh + {SWEEPS_PER_STEP} sweeps + measure) of config 4 restricted "
-                         f"to its first {n_s} samples x {nr} replicas at L={L}; {secs:.1f} s"}
+        cpu = cpu_baseline_record()
 
     if rank == 0:
         line = {
             "metric": METRIC + (" [gamma=1 forward-X walkers]" if args.walkers else ""),
-            "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": t_step_ms / args.steps, "higher_is_better": True,
+            "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
+            "warmup": W, "ms_per_step": t_step_ms / K, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
             "config": {"workload": CFG.name, "L": L, "n_samples": ns, "n_replicas": nr, "T": T_RUN,
                        "sweeps_per_step": SWEEPS_PER_STEP, "state_bytes": info["state_bytes"],
-                       "l2": "flushed between timed steps (256 MiB write); state 73.7 MB < 126 MB L2",
+                       "l2": "value = the lower of back_to_back (no flush: the 73.7 MB state is L2-resident in any "
+                             "long run) and l2_flushed (256 MiB write between separately timed steps); inputs larger "
+                             "than L2: see hbm_resident",
                        "sharding": "samples by rank, global sample offsets, no collective"},
+            "value_is": which,
+            "value_back_to_back": value_b2b, "ms_per_step_back_to_back": t_b2b_ms / K,
+            "value_l2_flushed": value_flushed, "ms_per_step_l2_flushed": t_flushed_ms / K,
             "rns_per_attempt": 1.0 / SWEEPS_PER_STEP,
-            "philox_words_generated_per_attempt": philox_words / (attempts_step * args.steps),
+            "philox_words_generated_per_attempt": philox_words / (attempts_step * K),
             "sweep_only_attempts_per_ns": sweep_only,
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
-            "roofline": roofline, "cpu_baseline": cpu, "wall_s": wall,
+            "roofline": roofline, "hbm_resident": hbm, "cpu_baseline": cpu, "wall_s": wall,
         }
         print(json.dumps(line), flush=True)
     if world > 1:

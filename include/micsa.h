@@ -305,9 +305,7 @@ int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
  * only matter when L % 8 == 0; other L always use the generic kernel.
  * key MICSA_TUNE_SWEEP_KERNEL: 1 = row-marching register kernel; 2 =
  *   software-pipelined row-marching kernel, one launch per half-sweep
- *   (default); 3 = z-marching kernel: persistent CTAs walk along z through a
- *   strip of rows, the opposite-parity spins staged once in a shared-memory
- *   ring by the TMA engine.
+ *   (default).
  * key MICSA_TUNE_PIPE_ROWS: rows per thread of kernel 2: 4 (default) or 8.
  * key MICSA_TUNE_PIPE_PLANES: lattice planes per CTA of kernel 2 (one warp
  *   each): 4 (default) or 1.

@@ -350,7 +350,7 @@ class MicSA:
         return {"attempts": a.value, "rns_drawn": r.value, "philox_calls": p.value}
 
     def set_tuning(self, key, value):
-        """micsa_set_tuning: 'sweep_kernel' (1 row-marching, 2 pipelined row-marching, 3 z-marching),
+        """micsa_set_tuning: 'sweep_kernel' (1 row-marching, 2 pipelined row-marching),
         'pipe_rows' (4, 8), 'pdl' (0, 1), 'pipe_planes' (1, 4), 'fuse_measure' (0, 1), 'fuse_walk' (0, 1),
         'l2_groups' (0, 1)."""
         k = {"sweep_kernel": 0, "pipe_rows": 2, "pdl": 3, "pipe_planes": 4, "fuse_measure": 5, "fuse_walk": 6, "l2_groups": 7}[key]
