@@ -109,3 +109,10 @@ def random_levels(shape, seed) -> np.ndarray:
     """i.i.d. uniform demon levels 0..3 (uint8) for state-injection tests."""
     rng = np.random.default_rng(seed)
     return rng.integers(0, 4, size=shape, dtype=np.uint8)
+
+
+def gaussian_couplings(shape, seed) -> np.ndarray:
+    """i.i.d. N(0, 1) float64 couplings (numpy PCG64) for the continuous-daemon workload of the paper's Appendix C
+    ("couplings are drawn from a Gaussian distribution J ~ N(0,1)").  Inputs only: both the CUDA
+    library and the oracle receive the same array through their set-couplings calls."""
+    return np.random.default_rng(seed).standard_normal(size=shape).astype(np.float64)

@@ -38,12 +38,12 @@ def build(force: bool = False) -> Path:
     """Compile the oracle's C sources with gcc into oracle/_build/liboracle.so."""
     _BUILD.mkdir(exist_ok=True)
     so = _BUILD / "liboracle.so"
-    srcs = [_HERE / "micsa_oracle.c", _HERE / "metropolis_oracle.c"]
+    srcs = [_HERE / "micsa_oracle.c", _HERE / "metropolis_oracle.c", _HERE / "gauss_oracle.c"]
     if (not force and so.exists()
             and all(so.stat().st_mtime >= p.stat().st_mtime for p in srcs)):
         return so
     tmp = _BUILD / f"liboracle.{os.getpid()}.tmp.so"
-    cmd = ["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", str(tmp)] + \
+    cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-o", str(tmp)] + \
           [str(p) for p in srcs] + ["-lm"]
     subprocess.run(cmd, check=True)
     os.replace(tmp, so)
@@ -64,6 +64,8 @@ def lib() -> ctypes.CDLL:
         _LIB.oracle_metropolis_half_sweep.restype = ctypes.c_int
         _LIB.oracle_refresh_uniform.restype = ctypes.c_uint32
         _LIB.oracle_num_threads.restype = ctypes.c_int
+        _LIB.oracle_gauss_refresh.restype = ctypes.c_int
+        _LIB.oracle_gauss_uniform.restype = ctypes.c_double
     return _LIB
 
 
@@ -257,3 +259,64 @@ def metropolis(L, s, J, T, n_sweeps, seed):
                          ctypes.c_uint64(seed), _p(s, _c_i8p), _p(J, _c_i8p),
                          _p(e, _c_f64p))
     return e
+
+
+# ---------------------------------------------------------------- continuous daemons, Gaussian couplings
+# (gauss_oracle.c; PAPER.md:136-140 Eq. 9, :436-454 Appendix C).  s int8 [ns, nr, N], n float64 [ns, nr, N],
+# J float64 [ns, 3, N].
+def _check_gauss(L, s, n, J):
+    ns, nr, N = s.shape
+    assert N == L ** 3 and s.dtype == np.int8 and s.flags.c_contiguous
+    if n is not None:
+        assert n.shape == s.shape and n.dtype == np.float64 and n.flags.c_contiguous
+    if J is not None:
+        assert J.shape == (ns, 3, N) and J.dtype == np.float64 and J.flags.c_contiguous
+    return ns, nr
+
+
+def gauss_refresh(L, n, seed, T, step, sample_offset=0) -> None:
+    ns, nr, N = n.shape
+    assert n.dtype == np.float64 and n.flags.c_contiguous and N == L ** 3
+    rc = lib().oracle_gauss_refresh(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr), ctypes.c_uint64(seed),
+                                    ctypes.c_double(T), ctypes.c_uint32(step), ctypes.c_int(sample_offset),
+                                    _p(n, _c_f64p))
+    if rc != 0:
+        raise ValueError("temperature must be finite and > 0")
+
+
+def gauss_uniform(i, gsample, rep, step, seed) -> float:
+    return float(lib().oracle_gauss_uniform(ctypes.c_int64(i), ctypes.c_int(gsample), ctypes.c_int(rep),
+                                            ctypes.c_uint32(step), ctypes.c_uint64(seed)))
+
+
+def gauss_half_sweep(L, s, n, J, parity) -> None:
+    ns, nr = _check_gauss(L, s, n, J)
+    lib().oracle_gauss_half_sweep(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr), _p(s, _c_i8p),
+                                  _p(n, _c_f64p), _p(J, _c_f64p), ctypes.c_int(parity))
+
+
+def gauss_sweep(L, s, n, J, n_sweeps=1, walkers=False, t0=0) -> None:
+    """n_sweeps timesteps: even half-sweep, odd half-sweep; with walkers the forward-X wandering
+    half-cycle of parity t mod 2 follows every sweep (Appendix C step 1(b); R15)."""
+    for k in range(n_sweeps):
+        gauss_half_sweep(L, s, n, J, 0)
+        gauss_half_sweep(L, s, n, J, 1)
+        if walkers:
+            gauss_wander(L, n, 0, +1, (t0 + k) & 1)
+
+
+def gauss_wander(L, n, axis=0, sign=+1, parity=0) -> None:
+    ns, nr, N = n.shape
+    assert n.dtype == np.float64 and n.flags.c_contiguous
+    lib().oracle_gauss_wander(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr), _p(n, _c_f64p),
+                              ctypes.c_int(axis), ctypes.c_int(sign), ctypes.c_int(parity))
+
+
+def gauss_measure(L, s, n, J):
+    ns, nr = _check_gauss(L, s, n, J)
+    E = np.zeros(ns * nr, np.float64)
+    Ed = np.zeros(ns * nr, np.float64)
+    Q = np.zeros(ns * (nr * (nr - 1) // 2), np.int64)
+    lib().oracle_gauss_measure(ctypes.c_int(L), ctypes.c_int(ns), ctypes.c_int(nr), _p(s, _c_i8p), _p(n, _c_f64p),
+                               _p(J, _c_f64p), _p(E, _c_f64p), _p(Ed, _c_f64p), _p(Q, _c_i64p))
+    return E, Ed, Q
