@@ -325,6 +325,47 @@ enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_PIPE_ROWS = 2, MICSA_TUNE_PDL = 3
        MICSA_TUNE_FUSE_WALK = 6, MICSA_TUNE_L2_GROUPS = 7 };
 int micsa_set_tuning(micsa_ctx *ctx, int key, int value);
 
+/* ---- continuous daemons / walkers with real couplings -------------
+ * PAPER.md:136-140 (Sec. 2.4, Eq. 9: in the continuous case the n are exponentially
+ * distributed, Prob(0 < n < R) = 1 - exp(-R/T)) and :436-454 (Appendix C: Gaussian couplings
+ * J ~ N(0,1), "continuous walker variables", no cap: the elementary move of Sec. 2.3,
+ * n <- n - dH, legal iff n >= 0).  A context of its own; float64 arithmetic without fused
+ * multiply-add in the order DESIGN.md R20 fixes, so that the accept decision is taken on the
+ * same number as in the oracle.
+ * Canonical host layouts (site i = x + L (y + L z)):
+ *   s  int8    [n_samples][n_replicas][N]   spins +-1
+ *   n  float64 [n_samples][n_replicas][N]   daemon / walker energies, >= 0
+ *   J  float64 [n_samples][3][N]            bond from site i to its +d neighbour; replicas share it
+ * micsa_gauss_create: spins = the Philox start of micsa_create (same seed, same counters), n = 0,
+ *   J = 0 until micsa_gauss_set_couplings (the Gaussian couplings are an INPUT: a caller-owned host
+ *   array, finite values; copied).  NULL on error (L odd or < 2, sizes, no device, out of memory).
+ * micsa_gauss_set_state / get_state: any pointer may be NULL; spins must be +-1, n finite and >= 0
+ *   (else MICSA_ERR_INVALID, state unchanged).  Synchronous.
+ * micsa_gauss_refresh: every n <- -T log(u), u = (x + 1/2) 2^-32, x = word 0 of Philox4x32-10 at counter
+ *   (i, sample_offset + sample, (5 << 24) | replica, step), key = seed (Eq. 9).  T finite and > 0.
+ * micsa_gauss_sweep: n timesteps = even half-sweep, odd half-sweep and, with walkers
+ *   (micsa_gauss_set_walkers(ctx, 1, t)), the forward-X wandering half-cycle of parity t mod 2 after each
+ *   (Appendix C step 1(b); R15), t += 1.  Asynchronous on the context's stream.
+ * micsa_gauss_wander: one half-cycle, walkers on sites of `parity` exchange with the neighbour at +sign along axis.
+ * micsa_gauss_measure: E[n_sys] = H_EA (Eq. 1), E_daemon[n_sys] = sum of n (Eq. 4) as float64 sums (fixed
+ *   summation tree: reproducible run to run; equal to the oracle's site-ordered sum to ~1e-13 relative),
+ *   Q[n_samples * n_replicas (n_replicas - 1) / 2] = N q (exact); any pointer may be NULL.  Synchronises. */
+typedef struct micsa_gauss_ctx micsa_gauss_ctx;
+micsa_gauss_ctx *micsa_gauss_create(int L, int n_samples, int n_replicas, uint64_t seed,
+                                    int sample_offset, void *cuda_stream);
+int micsa_gauss_destroy(micsa_gauss_ctx *ctx);
+int micsa_gauss_set_couplings(micsa_gauss_ctx *ctx, const double *J);
+int micsa_gauss_set_state(micsa_gauss_ctx *ctx, const int8_t *s, const double *n);
+int micsa_gauss_get_state(micsa_gauss_ctx *ctx, int8_t *s, double *n, double *J);
+int micsa_gauss_refresh(micsa_gauss_ctx *ctx, double T, uint32_t step);
+int micsa_gauss_sweep(micsa_gauss_ctx *ctx, int n);
+int micsa_gauss_half_sweep(micsa_gauss_ctx *ctx, int parity);
+int micsa_gauss_wander(micsa_gauss_ctx *ctx, int axis, int sign, int parity);
+int micsa_gauss_set_walkers(micsa_gauss_ctx *ctx, int mode, int64_t t);
+int micsa_gauss_measure(micsa_gauss_ctx *ctx, double *E, double *E_daemon, int64_t *Q);
+int micsa_gauss_counters(micsa_gauss_ctx *ctx, uint64_t *attempts, uint64_t *rns_drawn);
+int micsa_gauss_synchronize(micsa_gauss_ctx *ctx);
+
 #ifdef __cplusplus
 }
 #endif

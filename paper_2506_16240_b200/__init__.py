@@ -35,6 +35,10 @@ EXPORTS = (
     "micsa_measure_c4", "micsa_effective_temperature", "micsa_metropolis_sweep", "micsa_metropolis_half_sweep", "micsa_debug_metropolis_thresholds",
     "micsa_set_gamma", "micsa_select_daemon_set",
     "micsa_wander", "micsa_set_walkers", "micsa_set_time", "micsa_get_time",
+    "micsa_gauss_create", "micsa_gauss_destroy", "micsa_gauss_set_couplings", "micsa_gauss_set_state",
+    "micsa_gauss_get_state", "micsa_gauss_refresh", "micsa_gauss_sweep", "micsa_gauss_half_sweep",
+    "micsa_gauss_wander", "micsa_gauss_set_walkers", "micsa_gauss_measure", "micsa_gauss_counters",
+    "micsa_gauss_synchronize",
 )
 
 
@@ -86,6 +90,8 @@ def _bind() -> ctypes.CDLL:
     lib.micsa_create.argtypes = [i32, i32, i32, u64]
     lib.micsa_create_ex.restype = vp
     lib.micsa_create_ex.argtypes = [i32, i32, i32, u64, i32, vp, ctypes.c_size_t, vp]
+    lib.micsa_gauss_create.restype = vp
+    lib.micsa_gauss_create.argtypes = [i32, i32, i32, u64, i32, vp]
     lib.micsa_workspace_bytes.restype = ctypes.c_size_t
     lib.micsa_workspace_bytes.argtypes = [i32, i32, i32]
     for name, args in (
@@ -105,7 +111,13 @@ def _bind() -> ctypes.CDLL:
             ("micsa_measure_c4", [vp, vp]), ("micsa_measure_begin", [vp]), ("micsa_measure_end", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
             ("micsa_anneal", [vp, vp, i32, u32, vp, vp]),
             ("micsa_counters", [vp, vp, vp, vp]), ("micsa_layout_info", [vp, vp]),
-            ("micsa_set_tuning", [vp, i32, i32])):
+            ("micsa_set_tuning", [vp, i32, i32]),
+            ("micsa_gauss_destroy", [vp]), ("micsa_gauss_set_couplings", [vp, vp]),
+            ("micsa_gauss_set_state", [vp, vp, vp]), ("micsa_gauss_get_state", [vp, vp, vp, vp]),
+            ("micsa_gauss_refresh", [vp, f64, u32]), ("micsa_gauss_sweep", [vp, i32]),
+            ("micsa_gauss_half_sweep", [vp, i32]), ("micsa_gauss_wander", [vp, i32, i32, i32]),
+            ("micsa_gauss_set_walkers", [vp, i32, ctypes.c_int64]), ("micsa_gauss_measure", [vp, vp, vp, vp]),
+            ("micsa_gauss_counters", [vp, vp, vp]), ("micsa_gauss_synchronize", [vp])):
         fn = getattr(lib, name)
         fn.restype = i32
         fn.argtypes = args
@@ -362,3 +374,88 @@ class MicSA:
         return {"state_bytes": int(info[0]), "compulsory_bytes_per_sweep": int(info[1]),
                 "words_per_site": int(info[2]), "bond_bits": int(info[3]),
                 "launches": int(info[4])}
+
+
+class GaussMicSA:
+    """Continuous daemons / walkers with real couplings (micsa_gauss_*; Sec. 2.4 Eq. 9, Appendix C).
+    Argument marshalling only; the library allocates its own device memory, `stream` is a torch stream or None."""
+
+    def __init__(self, L, n_samples, n_replicas, seed, sample_offset=0, stream=None):
+        self.L, self.n_samples, self.n_replicas = int(L), int(n_samples), int(n_replicas)
+        self.N = self.L ** 3
+        self.n_sys = self.n_samples * self.n_replicas
+        self.n_pairs = self.n_samples * (self.n_replicas * (self.n_replicas - 1) // 2)
+        self._stream = stream
+        h = _lib.micsa_gauss_create(self.L, self.n_samples, self.n_replicas, int(seed), int(sample_offset),
+                                    stream.cuda_stream if stream is not None else None)
+        if not h:
+            raise MicsaError(MICSA_ERR_INVALID, last_error())
+        self._h = ctypes.c_void_p(h)
+
+    def destroy(self):
+        if self._h is not None:
+            _lib.micsa_gauss_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def set_couplings(self, J):
+        J = np.ascontiguousarray(J, dtype=np.float64)
+        assert J.shape == (self.n_samples, 3, self.N), J.shape
+        _check(_lib.micsa_gauss_set_couplings(self._h, _ptr(J)))
+
+    def set_state(self, s=None, n=None):
+        if s is not None:
+            s = np.ascontiguousarray(s, dtype=np.int8)
+            assert s.shape == (self.n_samples, self.n_replicas, self.N)
+        if n is not None:
+            n = np.ascontiguousarray(n, dtype=np.float64)
+            assert n.shape == (self.n_samples, self.n_replicas, self.N)
+        _check(_lib.micsa_gauss_set_state(self._h, _ptr(s), _ptr(n)))
+
+    def get_state(self, spins=True, daemons=True, couplings=True):
+        s = np.empty((self.n_samples, self.n_replicas, self.N), np.int8) if spins else None
+        n = np.empty((self.n_samples, self.n_replicas, self.N), np.float64) if daemons else None
+        J = np.empty((self.n_samples, 3, self.N), np.float64) if couplings else None
+        _check(_lib.micsa_gauss_get_state(self._h, _ptr(s), _ptr(n), _ptr(J)))
+        return s, n, J
+
+    def refresh(self, T, step):
+        _check(_lib.micsa_gauss_refresh(self._h, float(T), int(step)))
+
+    def sweep(self, n=1):
+        _check(_lib.micsa_gauss_sweep(self._h, int(n)))
+
+    def half_sweep(self, parity):
+        _check(_lib.micsa_gauss_half_sweep(self._h, int(parity)))
+
+    def wander(self, axis=0, sign=+1, parity=0):
+        _check(_lib.micsa_gauss_wander(self._h, int(axis), int(sign), int(parity)))
+
+    def set_walkers(self, mode, t=0):
+        _check(_lib.micsa_gauss_set_walkers(self._h, int(mode), int(t)))
+
+    def measure(self):
+        E = np.empty(self.n_sys, np.float64)
+        Ed = np.empty(self.n_sys, np.float64)
+        Q = np.empty(self.n_pairs, np.int64) if self.n_replicas >= 2 else None
+        _check(_lib.micsa_gauss_measure(self._h, _ptr(E), _ptr(Ed), _ptr(Q)))
+        return E, Ed, (Q if Q is not None else np.empty(0, np.int64))
+
+    def counters(self):
+        a, r = ctypes.c_uint64(), ctypes.c_uint64()
+        _check(_lib.micsa_gauss_counters(self._h, ctypes.byref(a), ctypes.byref(r)))
+        return {"attempts": a.value, "rns_drawn": r.value}
+
+    def synchronize(self):
+        _check(_lib.micsa_gauss_synchronize(self._h))

@@ -39,7 +39,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cu, _ = sources()
     tmp = PKG / f"libmicsa.{os.getpid()}.tmp.so"
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    cmd = [nvcc, "--threads", "0"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
           ["-I", str(INCLUDE), "-o", str(tmp)] + [str(p) for p in cu]
     subprocess.run(cmd, check=True)
     os.replace(tmp, LIB)

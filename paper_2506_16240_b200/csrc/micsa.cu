@@ -31,6 +31,13 @@ void set_err(const char* fmt, const char* detail = "") {
     snprintf(g_err, sizeof g_err, fmt, detail);
 }
 
+}  // namespace
+
+// for the other translation units of the library (gauss.cu): the same thread-local message
+void micsa_internal_set_error(const char* fmt, const char* detail) { snprintf(g_err, sizeof g_err, fmt, detail); }
+
+namespace {
+
 constexpr size_t kAlign = 256;
 size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
