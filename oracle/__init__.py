@@ -248,6 +248,29 @@ def c4(L, s) -> np.ndarray:
     return S
 
 
+def c4_normalised(L, S) -> np.ndarray:
+    """Eq. (16) with its normalisation: C4(r) of ONE sample from the sums of all its replica pairs,
+    S[pairs_of_the_sample, axis, r] -> sum over pairs and axes / (3 N N_R (N_R - 1) / 2) = mean over pairs and axes / N."""
+    S = np.asarray(S, dtype=np.float64)
+    return S.sum(axis=(0, 1)) / (3.0 * S.shape[0] * L ** 3)
+
+
+def xi(C4, c_min=0.0):
+    """Eq. (17)-(18) on the lattice, reading R22 of DESIGN.md (the paper defers the technical details
+    of estimating I_n to its refs. [61, 46]): C4 is known at r = 0, 1, ..., L/2; the integral over [0, r_cut] is taken
+    with the trapezoidal rule, r_cut = the last r before C4 first drops to c_min or below (noise floor chosen by the
+    caller, e.g. three times the sample error), no tail added.  Returns (I_1, I_2, I_3, xi_12 = I_2 / I_1,
+    xi_23 / xi_12 = I_3 I_1 / I_2^2)."""
+    C4 = np.asarray(C4, dtype=np.float64)
+    below = np.nonzero(C4 <= c_min)[0]
+    n = int(below[0]) if below.size else C4.size
+    if n < 2:
+        raise ValueError("C4 is at or below the cut-off from r = 1 on")
+    r = np.arange(n, dtype=np.float64)
+    I = [float(np.trapezoid(r ** k * C4[:n], r)) for k in (1, 2, 3)]
+    return I[0], I[1], I[2], I[1] / I[0], (I[2] / I[1]) / (I[1] / I[0])
+
+
 def metropolis(L, s, J, T, n_sweeps, seed):
     """Independent textbook Metropolis (metropolis_oracle.c); s updated in
     place; returns the energy per spin after each sweep, float64

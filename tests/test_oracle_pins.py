@@ -289,3 +289,63 @@ def test_c4_against_numpy_roll_and_identities(oracle, L, ns, nr):
     pair = np.concatenate([stag, np.ones((1, 1, N), np.int8)], axis=1)                  # q = staggered field
     want = np.array([N * (-1) ** r for r in range(L // 2 + 1)])
     assert np.all(oracle.c4(L, pair)[0] == want[None, :])
+
+
+# ---------------------------------------------------------------- I_n, xi_12, xi_23 / xi_12 (Eq. 17-18)
+def test_xi_closed_forms(oracle):
+    """Eq. (17)-(18) under reading R22 (trapezoid on the lattice, cut where C4 first drops to the floor, no tail).
+    For C4(r) = exp(-r / xi) the continuum integrals are I_n = n! xi^(n+1), so xi_12 = 2 xi and xi_23 / xi_12 = 3/2;
+    the trapezoid on integer r differs at relative order 1 / xi^2.  The trapezoid itself has a closed form for a
+    triangle C4(r) = 1 - r / R."""
+    for x in (6.0, 10.0, 25.0):
+        r = np.arange(40 * int(x))
+        I1, I2, I3, xi12, ratio = oracle.xi(np.exp(-r / x))
+        tol = 0.5 / x ** 2
+        assert abs(I1 / x ** 2 - 1.0) < tol and abs(I2 / (2 * x ** 3) - 1.0) < tol and abs(I3 / (6 * x ** 4) - 1.0) < tol
+        assert abs(xi12 / (2 * x) - 1.0) < tol and abs(ratio / 1.5 - 1.0) < tol
+    R = 12
+    tri = 1.0 - np.arange(R + 1) / R
+    I1 = oracle.xi(tri, c_min=-1.0)[0]                       # trapezoid of r (1 - r/R) on [0, R]: sum_{r=1}^{R-1} r (1 - r/R)
+    assert abs(I1 - sum(k * (1 - k / R) for k in range(1, R))) < 1e-12
+    # the cut-off: values after the first one at or below the floor do not enter, wherever they are
+    c = np.exp(-np.arange(30) / 3.0)
+    noisy = c.copy(); noisy[14] = -1e-3; noisy[15:] = 5.0
+    np.testing.assert_allclose(oracle.xi(noisy), oracle.xi(c[:14]), rtol=1e-15)
+    np.testing.assert_allclose(oracle.xi(c, c_min=c[9]), oracle.xi(c[:9]), rtol=1e-15)
+    with pytest.raises(ValueError):
+        oracle.xi(np.array([1.0, 0.0, 0.5]))
+
+
+def test_c4_normalisation_over_all_replica_pairs(oracle):
+    """Eq. (16) sums over every pair a != b with N~ = N N_R (N_R - 1) / 2: with three replicas of
+    which two are identical and one independent, C4(0) = 1 and the pair of identical replicas contributes exactly 1 at
+    every r, so C4(r) = (1 + 2 c(r)) / 3 with c the two-replica value of the mixed pairs."""
+    L, N = 8, 512
+    a = random_pm1((1, 1, N), 101); b = random_pm1((1, 1, N), 102)
+    s3 = np.ascontiguousarray(np.concatenate([a, a, b], axis=1))
+    S3 = oracle.c4(L, s3)
+    assert S3.shape == (3, 3, L // 2 + 1)                    # pairs (0,1), (0,2), (1,2)
+    assert np.all(S3[0] == N) and np.array_equal(S3[1], S3[2])
+    c2 = oracle.c4_normalised(L, oracle.c4(L, np.ascontiguousarray(np.concatenate([a, b], axis=1))))
+    c3 = oracle.c4_normalised(L, S3)
+    np.testing.assert_allclose(c3, (1.0 + 2.0 * c2) / 3.0, rtol=1e-14)
+    assert c3[0] == 1.0
+
+
+def test_xi_grows_in_a_quench(oracle):
+    """PAPER.md:283, Fig. 2: below T_c the coherence length xi_12(t) grows with time.  L = 12, T = 0.7, 8 samples x 2
+    replicas of the oracle's MicSA dynamics: xi_12 after 64 sweeps exceeds xi_12 after 4, and C4(0) = 1."""
+    from oracle import driver
+    L, ns, nr, seed = 12, 8, 2, 5
+    s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+    m = np.zeros_like(s, dtype=np.uint8)
+    out = []
+    done = 0
+    for t_end in (4, 64):
+        driver.anneal(L, s, m, J, seed, [(0.7, 4, 0)] * ((t_end - done) // 4), step0=done // 4)
+        done = t_end
+        S = oracle.c4(L, s)                                  # one pair per sample
+        c4 = np.mean([oracle.c4_normalised(L, S[k:k + 1]) for k in range(ns)], axis=0)
+        assert c4[0] == 1.0
+        out.append(oracle.xi(c4, c_min=0.01)[3])
+    assert out[1] > 1.15 * out[0] > 0.0, out
