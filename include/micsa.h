@@ -244,14 +244,25 @@ int micsa_debug_philox(uint64_t seed, const uint32_t *counters, int n, uint32_t 
 int micsa_measure_i64(micsa_ctx *ctx, int64_t *E, int64_t *E_daemon, int64_t *Q);
 
 /* micsa_measure_c4 (synchronous): four-point replica correlation along the
- * lattice axes, Eq. (16), as exact integer sums for the
- * replica pair of every sample (n_replicas must be 2, else MICSA_ERR_INVALID):
- *   S[n_samples][3][L/2 + 1],  S[s][d][r] = sum_x q_x q_{x + r e_d},  q = s^a s^b,
- * periodic; d = 0,1,2 = x,y,z.  C4(r) of Eq. (16) for one pair =
- * (S[s][0][r] + S[s][1][r] + S[s][2][r]) / (3N).  The integrals I_n and xi_12
- * (Eq. 17-18) need the cut-off procedure of the paper's refs. [61,46] and are
- * left to the caller.  Caller-owned host array. */
+ * lattice axes, Eq. (16), as exact integer sums for EVERY
+ * replica pair a < b of every sample (pairs ordered like Q of micsa_measure;
+ * n_replicas < 2 -> MICSA_ERR_INVALID):
+ *   S[n_samples][n_replicas (n_replicas - 1) / 2][3][L/2 + 1],
+ *   S[s][pair][d][r] = sum_x q_x q_{x + r e_d},  q = s^a s^b, periodic; d = 0,1,2 = x,y,z.
+ * C4(r) of Eq. (16) for a sample = sum over its pairs and the three axes /
+ * (3 N n_replicas (n_replicas - 1) / 2).  Caller-owned host array.
+ *
+ * micsa_xi (host arithmetic on L/2 + 1 numbers, no context): the integrals
+ * I_n = int r^n C4(r) dr, n = 1, 2, 3 (Eq. 17) and the lengths
+ * xi_12 = I_2 / I_1, xi_23 / xi_12 = I_3 I_1 / I_2^2 (Eq. 18).
+ * The paper defers the estimation of I_n to its refs. [61, 46]; the reading
+ * taken here (R22): C4[r] is given at r = 0 .. n_r - 1, trapezoidal
+ * rule, integration stops before the first C4[r] <= c_min (the caller's noise
+ * floor, e.g. three times the sample error), no tail.  I = double[3] or NULL.
+ * Fewer than two points above the floor -> MICSA_ERR_INVALID. */
 int micsa_measure_c4(micsa_ctx *ctx, int64_t *S);
+int micsa_xi(const double *C4, int n_r, double c_min, double I[3], double *xi12,
+             double *xi23_over_xi12);
 
 /* The same measurement split in two, so that the caller can queue more work
  * (or stop a timer on the stream) before waiting: micsa_measure_begin queues
@@ -316,13 +327,18 @@ int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
  * key MICSA_TUNE_L2_GROUPS: 1 (default) = when the packed state exceeds the L2 cache, a call of several
  *   sweeps runs all of them on one group of word lattices (independent systems) that fits in L2 before
  *   touching the next group, 0 = every half-sweep over all lattices.
+ * key MICSA_TUNE_SMALL_PATH: 1 (default) = on small lattices (L a multiple of 8, L*L*L/8 <= 8192 quad rows,
+ *   n_replicas <= 2, one daemon per spin) micsa_sweep, micsa_sweep_measure and every schedule step of
+ *   micsa_anneal run as ONE launch in which each word lattice is walked by a thread-block cluster (refresh, all
+ *   sweeps and the measurement rows; cluster barriers instead of kernel boundaries), 0 = the general path.
  * key MICSA_TUNE_PDL: 1 (default) = kernel 2 is launched with programmatic
  *   stream serialization (the next half-sweep's grid is scheduled while this
  *   one drains and waits on the device for its completion), 0 = plain launches.
  * Unknown key or value: MICSA_ERR_INVALID, nothing changes. */
 enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_PIPE_ROWS = 2, MICSA_TUNE_PDL = 3,
        MICSA_TUNE_PIPE_PLANES = 4, MICSA_TUNE_FUSE_MEASURE = 5,
-       MICSA_TUNE_FUSE_WALK = 6, MICSA_TUNE_L2_GROUPS = 7 };
+       MICSA_TUNE_FUSE_WALK = 6, MICSA_TUNE_L2_GROUPS = 7,
+       MICSA_TUNE_SMALL_PATH = 8 };
 int micsa_set_tuning(micsa_ctx *ctx, int key, int value);
 
 /* ---- continuous daemons / walkers with real couplings -------------

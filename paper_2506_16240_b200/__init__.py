@@ -32,7 +32,7 @@ EXPORTS = (
     "micsa_measure", "micsa_anneal", "micsa_counters", "micsa_layout_info",
     "micsa_set_tuning",
     "micsa_prefetch_refresh", "micsa_measure_begin", "micsa_measure_end", "micsa_sweep_measure",
-    "micsa_measure_c4", "micsa_effective_temperature", "micsa_metropolis_sweep", "micsa_metropolis_half_sweep", "micsa_debug_metropolis_thresholds",
+    "micsa_measure_c4", "micsa_xi", "micsa_effective_temperature", "micsa_metropolis_sweep", "micsa_metropolis_half_sweep", "micsa_debug_metropolis_thresholds",
     "micsa_set_gamma", "micsa_select_daemon_set",
     "micsa_wander", "micsa_set_walkers", "micsa_set_time", "micsa_get_time",
     "micsa_gauss_create", "micsa_gauss_destroy", "micsa_gauss_set_couplings", "micsa_gauss_set_state",
@@ -108,7 +108,7 @@ def _bind() -> ctypes.CDLL:
             ("micsa_prefetch_refresh", [vp, f64, u32]),
             ("micsa_debug_thresholds", [f64, vp]), ("micsa_debug_philox", [u64, vp, i32, vp]), ("micsa_effective_temperature", [f64, vp]),
             ("micsa_measure_i64", [vp, vp, vp, vp]),
-            ("micsa_measure_c4", [vp, vp]), ("micsa_measure_begin", [vp]), ("micsa_measure_end", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
+            ("micsa_measure_c4", [vp, vp]), ("micsa_xi", [vp, i32, f64, vp, vp, vp]), ("micsa_measure_begin", [vp]), ("micsa_measure_end", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
             ("micsa_anneal", [vp, vp, i32, u32, vp, vp]),
             ("micsa_counters", [vp, vp, vp, vp]), ("micsa_layout_info", [vp, vp]),
             ("micsa_set_tuning", [vp, i32, i32]),
@@ -153,6 +153,15 @@ def debug_philox(seed: int, counters) -> np.ndarray:
     out = np.empty_like(c)
     _check(_lib.micsa_debug_philox(int(seed), _ptr(c), c.shape[0], _ptr(out)))
     return out
+
+
+def xi(C4, c_min=0.0):
+    """micsa_xi: (I_1, I_2, I_3, xi_12, xi_23 / xi_12) of Eq. (17)-(18) from C4(r), r = 0 .. len - 1."""
+    C4 = np.ascontiguousarray(C4, dtype=np.float64)
+    I = np.zeros(3, np.float64)
+    a, b = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(_lib.micsa_xi(_ptr(C4), C4.size, float(c_min), _ptr(I), ctypes.byref(a), ctypes.byref(b)))
+    return float(I[0]), float(I[1]), float(I[2]), float(a.value), float(b.value)
 
 
 def effective_temperature(e_daemon_per_variable: float) -> float:
@@ -303,8 +312,9 @@ class MicSA:
         return E, Ed, (Q if Q is not None else np.empty(0, np.int64))
 
     def measure_c4(self):
-        """S[sample, axis, r] = sum_x q_x q_{x + r e_axis} (exact int64), r = 0..L/2."""
-        S = np.empty((self.n_samples, 3, self.L // 2 + 1), np.int64)
+        """S[pair, axis, r] = sum_x q_x q_{x + r e_axis} (exact int64), r = 0..L/2, for every replica pair a < b of
+        every sample, pairs ordered like Q of measure()."""
+        S = np.empty((self.n_pairs, 3, self.L // 2 + 1), np.int64)
         _check(_lib.micsa_measure_c4(self._h, _ptr(S)))
         return S
 
@@ -364,8 +374,8 @@ class MicSA:
     def set_tuning(self, key, value):
         """micsa_set_tuning: 'sweep_kernel' (1 row-marching, 2 pipelined row-marching),
         'pipe_rows' (4, 8), 'pdl' (0, 1), 'pipe_planes' (1, 4), 'fuse_measure' (0, 1), 'fuse_walk' (0, 1),
-        'l2_groups' (0, 1)."""
-        k = {"sweep_kernel": 0, "pipe_rows": 2, "pdl": 3, "pipe_planes": 4, "fuse_measure": 5, "fuse_walk": 6, "l2_groups": 7}[key]
+        'l2_groups' (0, 1), 'small_path' (0, 1)."""
+        k = {"sweep_kernel": 0, "pipe_rows": 2, "pdl": 3, "pipe_planes": 4, "fuse_measure": 5, "fuse_walk": 6, "l2_groups": 7, "small_path": 8}[key]
         _check(_lib.micsa_set_tuning(self._h, k, int(value)))
 
     def layout_info(self):

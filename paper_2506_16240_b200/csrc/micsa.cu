@@ -18,6 +18,7 @@
 #include "pack.cuh"
 #include "philox.cuh"
 #include "refresh.cuh"
+#include "small.cuh"
 #include "sweep.cuh"
 #include "wander.cuh"
 
@@ -136,6 +137,7 @@ struct micsa_ctx {
     int sel;                   // family that set_daemons / get_state address
     std::vector<uint32_t*> xm0, xm1;   // families 1 .. gamma-1 (library-owned)
     int l2_groups;             // run multi-sweep calls lattice group by lattice group when the state exceeds L2
+    int small_path;            // small lattices: whole groups of sweeps (+ refresh, + rows) in one cluster launch
     int fuse_walk;             // walkers: exchange inside the odd half-sweep instead of a separate kernel
     int walkers;               // 0 = daemons stay on their site, 1 = one forward-X walker per spin
     long long t;               // time index (timesteps = sweeps done since create / micsa_set_time)
@@ -608,9 +610,61 @@ int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min, int dir)
     return post_launch(c, 2);
 }
 
+// ---- small lattices: one cluster per word lattice walks through refresh + sweeps + rows (small.cuh) ----
+bool small_eligible(const micsa_ctx* c) {
+    const Geom& g = c->g;
+    return c->small_path && c->V == 4 && g.n_replicas <= 2 && c->gamma == 1 && !c->walkers &&
+           (long long)g.L * g.L * (g.Lh / 4) <= 8192;
+}
+
+// do_refresh: Eq. (11) at (T, step) first; then n_sweeps sweeps; a measurement row after every measure_every-th
+// sweep (0 = none) into rows[row0 ...] (row index >= rows_cap: into the context's scratch row)
+int launch_small_step(micsa_ctx* c, bool do_refresh, double T, uint32_t step, int n_sweeps, int measure_every,
+                      long long* rows, long long row0, long long rows_cap, bool fold_min) {
+    const Geom& g = c->g;
+    SmallArgs A;
+    A.a.spin = c->st.spin; A.a.m0 = c->st.m0; A.a.m1 = c->st.m1; A.a.J = c->st.J;
+    A.a.L = g.L; A.a.Lh = g.Lh; A.a.n_rg = g.n_rg; A.a.half = g.half; A.a.w0 = 0;
+    A.sg = site_grid(g);
+    MeasureArgs ma; FinalizeArgs fa;
+    make_measure_args(c, c->row, fold_min, ma, fa);
+    A.ma = ma;
+    A.rows = rows; A.scratch_row = c->row; A.min_E = fold_min ? c->minE : nullptr;
+    A.row_len = (long long)c->plan.row_len; A.row0 = row0; A.rows_cap = rows_cap;
+    A.n_calls = c->calls;
+    A.n_words = g.n_words;
+    A.do_refresh = do_refresh ? 1 : 0; A.step = step; A.alpha_bits = 0u;
+    A.n_sweeps = n_sweeps; A.measure_every = measure_every;
+    A.n_samples = g.n_samples; A.n_replicas = g.n_replicas; A.rpw = g.rpw; A.spw = g.spw; A.N = g.N;
+    RefreshThr rt = {};
+    if (do_refresh) {
+        uint64_t thr[3];
+        if (thresholds_host(T, thr) != MICSA_OK || thr[0] == 0) { set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID; }
+        rt = make_thr(thr);
+    }
+    const int items = g.L * g.L * (g.Lh / 4);
+    const int bt = items >= 512 ? 512 : std::max(32, (items + 31) / 32 * 32);
+    int cs = 1;
+    while (cs < 8 && cs * bt < items) cs *= 2;
+    A.cs = cs;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(g.n_words * cs)); cfg.blockDim = dim3((unsigned)bt);
+    cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)cs; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (g.rpw == 2) CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<2>, A, c->ks, rt));
+    else            CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<1>, A, c->ks, rt));
+    c->attempts += (uint64_t)n_sweeps * (uint64_t)g.N * (uint64_t)g.n_sys;
+    c->t += n_sweeps;
+    return post_launch(c);
+}
+
 // n sweeps, then one measurement into `row`
 int launch_sweeps_measured(micsa_ctx* c, int n, long long* row, bool fold_min) {
     const Geom& g = c->g;
+    if (n >= 1 && small_eligible(c)) return launch_small_step(c, false, 0.0, 0u, n, n, row, 0, 1, fold_min);
     const bool fused = n >= 1 && c->fuse_measure && c->V == 4 && c->sweep_kernel == 2 && g.n_replicas <= 2 && c->gamma == 1;
     if (!fused) {
         const int rc = launch_sweeps(c, n); if (rc) return rc;
@@ -747,7 +801,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->use_pdl = 1;
     c->pipe_planes = (g.n_words == 1 && (g.L / 4) * (g.Lh / 4) >= 512) ? 4 : 1;   // measured: DESIGN.md 6.1
     c->fuse_measure = 1;
-    c->walkers = 0; c->t = 0; c->fuse_walk = 1; c->l2_groups = 1; c->gamma = 1; c->sel = 0;
+    c->walkers = 0; c->t = 0; c->fuse_walk = 1; c->l2_groups = 1; c->small_path = 1; c->gamma = 1; c->sel = 0;
     c->attempts = c->rns = c->launches = 0;
     c->sticky = 0;
     if (dev_workspace) {
@@ -891,6 +945,7 @@ int micsa_half_sweep(micsa_ctx* c, int parity) {
 int micsa_sweep(micsa_ctx* c, int n) {
     int rc = check_ctx(c); if (rc) return rc;
     if (n < 0) { set_err("n must be >= 0"); return MICSA_ERR_INVALID; }
+    if (n >= 1 && small_eligible(c)) return launch_small_step(c, false, 0.0, 0u, n, 0, c->row, 0, 0, false);
     return launch_sweeps(c, n);
 }
 
@@ -1077,10 +1132,11 @@ int micsa_measure_c4(micsa_ctx* c, int64_t* S) {
     int rc = check_ctx(c); if (rc) return rc;
     const Geom& g = c->g;
     if (!S) { set_err("null pointer"); return MICSA_ERR_INVALID; }
-    if (g.n_replicas != 2) { set_err("micsa_measure_c4 needs n_replicas == 2"); return MICSA_ERR_INVALID; }
+    if (g.n_replicas < 2) { set_err("micsa_measure_c4 needs n_replicas >= 2"); return MICSA_ERR_INVALID; }
     const int R = g.L / 2 + 1;
+    const int pps = g.n_replicas * (g.n_replicas - 1) / 2;
     const size_t x_bytes = align_up((size_t)g.n_sg * (size_t)g.N * sizeof(uint32_t));
-    const size_t cnt_words = (size_t)g.n_sg * 3 * R * 32;
+    const size_t pair_words = (size_t)g.n_sg * 3 * R * 32, cnt_words = pair_words * pps;
     // context-owned, grow-only: no cudaMalloc / cudaFree per measurement
     if (x_bytes + cnt_words * 8 > c->c4_bytes) {
         CK(c, cudaStreamSynchronize(c->stream));
@@ -1102,22 +1158,50 @@ int micsa_measure_c4(micsa_ctx* c, int64_t* S) {
     uint32_t* X = (uint32_t*)c->c4_dev;
     unsigned long long* cnt = (unsigned long long*)((char*)c->c4_dev + x_bytes);
     CK(c, cudaMemsetAsync(cnt, 0, cnt_words * 8, c->stream));
-    overlap_field_kernel<<<site_blocks(g, g.n_sg * 2), 128, 0, c->stream>>>(c->st.spin, X, g.L, g.Lh, g.half);
     // every thread counts at most 65535 sites (16-plane counters)
     long long nb = std::max<long long>(1, std::min<long long>((g.N + kCountBlock * 64 - 1) / (kCountBlock * 64), 64));
     nb = std::max<long long>(nb, (g.N + (long long)kCountBlock * 60000 - 1) / ((long long)kCountBlock * 60000));
-    c4_count_kernel<<<dim3((unsigned)nb, (unsigned)R, (unsigned)(3 * g.n_sg)), kCountBlock, 0, c->stream>>>(X, cnt, g.L);
-    rc = post_launch(c, 2); if (rc) return rc;
+    const uint32_t mask = (g.rpw == 2) ? 0xFFFFu : 0xFFFFFFFFu;
+    int k = 0;
+    for (int ra = 0; ra < g.n_replicas; ++ra)
+        for (int rb = ra + 1; rb < g.n_replicas; ++rb, ++k) {        // pairs a < b, lexicographic (Eq. 16 sums all of them)
+            overlap_field_kernel<<<site_blocks(g, g.n_sg * 2), 128, 0, c->stream>>>(
+                c->st.spin, X, g.L, g.Lh, g.half, g.n_rg, ra / g.rpw, 16 * (ra % g.rpw), rb / g.rpw, 16 * (rb % g.rpw), mask);
+            c4_count_kernel<<<dim3((unsigned)nb, (unsigned)R, (unsigned)(3 * g.n_sg)), kCountBlock, 0, c->stream>>>(
+                X, cnt + (size_t)k * pair_words, g.L);
+            rc = post_launch(c, 2); if (rc) return rc;
+        }
     const unsigned long long* host = c->c4_host;
     CK(c, cudaMemcpyAsync(c->c4_host, cnt, cnt_words * 8, cudaMemcpyDeviceToHost, c->stream));
     CK(c, cudaStreamSynchronize(c->stream));
     for (int sample = 0; sample < g.n_samples; ++sample) {
         const int sg = sample / g.spw, sl = sample - sg * g.spw;
-        for (int d = 0; d < 3; ++d)
-            for (int r = 0; r < R; ++r)
-                S[((size_t)sample * 3 + d) * R + r] =
-                    (int64_t)g.N - 2 * (int64_t)host[(((size_t)sg * 3 + d) * R + r) * 32 + sl];
+        for (int pk = 0; pk < pps; ++pk)
+            for (int d = 0; d < 3; ++d)
+                for (int r = 0; r < R; ++r)
+                    S[(((size_t)sample * pps + pk) * 3 + d) * R + r] =
+                        (int64_t)g.N - 2 * (int64_t)host[(size_t)pk * pair_words + (((size_t)sg * 3 + d) * R + r) * 32 + sl];
     }
+    return MICSA_OK;
+}
+
+int micsa_xi(const double* C4, int n_r, double c_min, double I[3], double* xi12, double* xi23_over_xi12) {
+    // Eq. (17)-(18), reading R22 of DESIGN.md: trapezoidal rule on r = 0, 1, ..., cut before the
+    // first value at or below c_min, no tail
+    if (!C4 || n_r < 2) { set_err("C4 must hold at least r = 0 and r = 1"); return MICSA_ERR_INVALID; }
+    int n = n_r;
+    for (int r = 0; r < n_r; ++r)
+        if (!(C4[r] > c_min)) { n = r; break; }
+    if (n < 2) { set_err("C4 is at or below the cut-off from r = 1 on"); return MICSA_ERR_INVALID; }
+    double In[3] = { 0.0, 0.0, 0.0 };
+    for (int k = 0; k < 3; ++k)
+        for (int r = 0; r + 1 < n; ++r) {
+            const double f0 = std::pow((double)r, k + 1) * C4[r], f1 = std::pow((double)(r + 1), k + 1) * C4[r + 1];
+            In[k] += 0.5 * (f0 + f1);
+        }
+    if (I) { I[0] = In[0]; I[1] = In[1]; I[2] = In[2]; }
+    if (xi12) *xi12 = In[1] / In[0];
+    if (xi23_over_xi12) *xi23_over_xi12 = (In[2] / In[1]) / (In[1] / In[0]);
     return MICSA_OK;
 }
 
@@ -1172,6 +1256,20 @@ int micsa_anneal(micsa_ctx* c, const micsa_step* sched, int n_steps, uint32_t st
     std::vector<double> row_T;
     long long r = 0, t = 0;
     for (int k = 0; k < n_steps; ++k) {
+        if (small_eligible(c) && sched[k].n_sweeps > 0) {     // small lattice: the whole step in one cluster launch
+            const int me = sched[k].measure_every, n_rows = me > 0 ? sched[k].n_sweeps / me : 0;
+            const bool prefetched = c->pending && c->pending_step == step0 + (uint32_t)k &&
+                                    memcmp(&c->pending_T, &sched[k].T, sizeof(double)) == 0;
+            if (prefetched) { rc = launch_refresh(c, sched[k].T, step0 + (uint32_t)k); if (rc) return rc; }
+            else c->rns += (uint64_t)g.N * (uint64_t)g.n_sys;
+            rc = launch_small_step(c, !prefetched, sched[k].T, step0 + (uint32_t)k, sched[k].n_sweeps, me,
+                                   (long long*)dev_rows.dev, r, keep, true);
+            if (rc) return rc;
+            for (int i = 1; i <= n_rows; ++i)
+                if (r + i - 1 < keep) { row_sweep.push_back(t + (long long)i * me); row_T.push_back(sched[k].T); }
+            r += n_rows; t += sched[k].n_sweeps;
+            continue;
+        }
         rc = launch_refresh(c, sched[k].T, step0 + (uint32_t)k); if (rc) return rc;
         if (k + 1 < n_steps && sched[k].n_sweeps > 0) {       // generated under this step's sweeps
             rc = launch_prefetch(c, sched[k + 1].T, step0 + (uint32_t)k + 1u); if (rc) return rc;
@@ -1242,6 +1340,9 @@ int micsa_set_tuning(micsa_ctx* c, int key, int value) {
         case MICSA_TUNE_L2_GROUPS:
             if (value != 0 && value != 1) { set_err("l2_groups must be 0 or 1"); return MICSA_ERR_INVALID; }
             c->l2_groups = value; return MICSA_OK;
+        case MICSA_TUNE_SMALL_PATH:
+            if (value != 0 && value != 1) { set_err("small_path must be 0 or 1"); return MICSA_ERR_INVALID; }
+            c->small_path = value; return MICSA_OK;
         case MICSA_TUNE_FUSE_WALK:
             if (value != 0 && value != 1) { set_err("fuse_walk must be 0 or 1"); return MICSA_ERR_INVALID; }
             c->fuse_walk = value; return MICSA_OK;

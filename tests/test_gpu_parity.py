@@ -613,9 +613,26 @@ def test_c4_exact(micsa, oracle, L, ns):
         S = g.measure_c4()
         np.testing.assert_array_equal(S, oracle.c4(L, gs))
         assert np.all(S[:, :, 0] == N)
-    with micsa.MicSA(L, ns, 3, 1) as g3:
+    with micsa.MicSA(L, ns, 1, 1) as g1:
         with pytest.raises(micsa.MicsaError):
-            g3.measure_c4()
+            g1.measure_c4()
+
+
+@pytest.mark.parametrize("L,ns,nr", [(6, 5, 3), (8, 3, 4), (4, 40, 4), (8, 33, 5), (10, 2, 6)])
+def test_c4_all_replica_pairs(micsa, oracle, L, ns, nr):
+    """Eq. (16) sums over every pair a != b: replicas in the same word, in different words, with
+    one and with two replicas per word, against the oracle's pair-by-pair triple loop; then C4(r) and xi_12."""
+    with micsa.MicSA(L, ns, nr, 7) as g:
+        g.refresh_demons(0.8, 0); g.sweep(4)
+        gs = g.get_state(daemons=False, couplings=False)[0]
+        S = g.measure_c4()
+        ref = oracle.c4(L, gs)
+        assert S.shape == ref.shape == (ns * nr * (nr - 1) // 2, 3, L // 2 + 1)
+        np.testing.assert_array_equal(S, ref)
+        pps = nr * (nr - 1) // 2
+        c4 = np.mean([oracle.c4_normalised(L, S[k * pps:(k + 1) * pps]) for k in range(ns)], axis=0)
+        assert c4[0] == 1.0
+        np.testing.assert_allclose(micsa.xi(c4, 0.0), oracle.xi(c4, 0.0), rtol=1e-13)
 
 
 def test_c4_config3_shape(micsa, oracle):
@@ -806,3 +823,49 @@ def test_run_configs_script(micsa, capsys):
     assert lines[0]["sweeps"] == 1000 and lines[0]["refreshes"] == 100 and lines[0]["rns_defined_per_attempt"] == 0.1
     assert all(d["attempts_per_ns"] > 0 and -3.0 < d["e_final_mean"] < 0.0 for d in lines)
     assert "min_energy_best" in lines[-1] and lines[-1]["min_energy_best"] <= lines[-1]["min_energy_mean"]
+
+
+# ---------------------------------------------------------------- small lattices: one cluster launch per step
+@pytest.mark.parametrize("L,ns,nr", [(8, 1, 2), (8, 40, 2), (8, 33, 1), (16, 17, 2), (24, 2, 2), (32, 6, 2), (32, 35, 1)])
+def test_small_lattice_path_bit_exact(micsa, oracle, L, ns, nr):
+    """The cluster-per-lattice path of small lattices (micsa_set_tuning small_path, default on): sweep, sweep_measure
+    and anneal (refresh + sweeps + rows in one launch) against the oracle, state after every call, and the same calls
+    on the general path; a prefetched refresh is consumed, rows beyond the trace capacity are dropped."""
+    N, seed = L ** 3, 17
+    sched = [(1.3, 4, 1), (0.9, 6, 3), (0.6, 5, 0), (0.4, 4, 4)]
+    for small in (1, 0):
+        s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+        m = np.zeros_like(s, dtype=np.uint8)
+        with micsa.MicSA(L, ns, nr, seed) as g:
+            g.set_tuning("small_path", small)
+            launches0 = g.layout_info()["launches"]
+            out = g.anneal(sched, step0=3)
+            n_launch = g.layout_info()["launches"] - launches0
+            ref = driver.anneal(L, s, m, J, seed, sched, step0=3)
+            _assert_state(g, s, m, J)
+            for k in ("sweep", "E", "Edem", "Q"):
+                np.testing.assert_array_equal(out[k], ref[k])
+            np.testing.assert_allclose(out["min_energy"], ref["min_energy"], rtol=1e-12)
+            assert out["sweep"].tolist() == [1, 2, 3, 4, 7, 10, 19]
+            if small:
+                assert n_launch == 1 + len(sched)                      # min-energy fill + one launch per step
+            c = g.counters()
+            assert c["attempts"] == 19 * N * ns * nr and c["rns_drawn"] == 4 * N * ns * nr and c["philox_calls"] > 0
+            g.sweep(3); oracle.sweep(L, s, m, J, 3)
+            _assert_state(g, s, m)
+            g.prefetch_refresh(0.8, 50)
+            g.sweep_measure(2); E, Ed, Q = g.measure_end()
+            oracle.sweep(L, s, m, J, 2)
+            oE, oEd, oQ = oracle.measure(L, s, m, J)
+            np.testing.assert_array_equal(E, oE); np.testing.assert_array_equal(Ed, oEd); np.testing.assert_array_equal(Q, oQ)
+            out2 = g.anneal([(0.8, 3, 3), (0.7, 2, 1)], step0=50)       # the first refresh was prefetched
+            ref2 = driver.anneal(L, s, m, J, seed, [(0.8, 3, 3), (0.7, 2, 1)], step0=50)
+            _assert_state(g, s, m)
+            np.testing.assert_array_equal(out2["E"], ref2["E"]); np.testing.assert_array_equal(out2["Edem"], ref2["Edem"])
+            assert g.get_time() == 19 + 3 + 2 + 5
+            # involution through single half-sweeps (general kernels) after small-path sweeps
+            s0, m0, _ = g.get_state(couplings=False)
+            g.sweep(4)
+            for _ in range(4):
+                g.half_sweep(1); g.half_sweep(0)
+            _assert_state(g, s0, m0)

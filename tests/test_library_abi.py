@@ -131,3 +131,23 @@ def test_pow2_schedule_is_the_papers_rule():
     sch = pow2_schedule(0.7, 5)
     assert [n for _, n, _ in sch] == [1, 2, 4, 8, 16, 32] and sum(n for _, n, _ in sch) == 63
     assert all(T == 0.7 and every == n for T, n, every in sch)
+
+
+def test_xi_equals_oracle(micsa, oracle):
+    """micsa_xi (host arithmetic of the library) against the oracle's numpy trapezoid (Eq. 17-18, reading R22)."""
+    rng = np.random.default_rng(5)
+    for n in (2, 5, 41, 81):
+        c = np.exp(-np.arange(n) / 7.3) * (1.0 + 0.05 * rng.standard_normal(n))
+        c[0] = 1.0
+        for c_min in (0.0, 0.01, 0.2):
+            try:
+                want = oracle.xi(c, c_min)
+            except ValueError:
+                with pytest.raises(micsa.MicsaError):
+                    micsa.xi(c, c_min)
+                continue
+            np.testing.assert_allclose(micsa.xi(c, c_min), want, rtol=1e-13)
+    with pytest.raises(micsa.MicsaError):
+        micsa.xi(np.array([1.0]), 0.0)
+    with pytest.raises(micsa.MicsaError):
+        micsa.xi(np.array([1.0, -0.5, 0.3]), 0.0)
