@@ -611,10 +611,29 @@ int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min, int dir)
 }
 
 // ---- small lattices: one cluster per word lattice walks through refresh + sweeps + rows (small.cuh) ----
+// cluster size (CTAs per word lattice, each holding L/cs planes in shared memory), threads per CTA, shared bytes
+struct SmallShape { bool ok; int cs, block; size_t smem; };
+
+SmallShape small_shape(const micsa_ctx* c) {
+    const Geom& g = c->g;
+    SmallShape sh; sh.ok = false; sh.cs = 1; sh.block = 32; sh.smem = 0;
+    if (c->V != 4 || g.L > 64) return sh;
+    for (int cs = 1; cs <= 8; cs *= 2) {
+        if (g.L % cs) break;
+        const size_t smem = (g.rpw == 2) ? SlabLayout<2>(g.L / cs, g.L * g.Lh).total() : SlabLayout<1>(g.L / cs, g.L * g.Lh).total();
+        const int items = (g.L / cs) * g.L * (g.Lh / 4);
+        if (smem <= 200 * 1024 && (items <= 512 || (cs == 8 && items <= 1024))) {
+            sh.ok = true; sh.cs = cs; sh.smem = smem;
+            sh.block = items >= 512 ? 512 : std::max(32, (items + 31) / 32 * 32);
+            return sh;
+        }
+    }
+    return sh;
+}
+
 bool small_eligible(const micsa_ctx* c) {
     const Geom& g = c->g;
-    return c->small_path && c->V == 4 && g.n_replicas <= 2 && c->gamma == 1 && !c->walkers &&
-           (long long)g.L * g.L * (g.Lh / 4) <= 8192;
+    return c->small_path && g.n_replicas <= 2 && c->gamma == 1 && !c->walkers && small_shape(c).ok;
 }
 
 // do_refresh: Eq. (11) at (T, step) first; then n_sweeps sweeps; a measurement row after every measure_every-th
@@ -642,20 +661,22 @@ int launch_small_step(micsa_ctx* c, bool do_refresh, double T, uint32_t step, in
         if (thresholds_host(T, thr) != MICSA_OK || thr[0] == 0) { set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID; }
         rt = make_thr(thr);
     }
-    const int items = g.L * g.L * (g.Lh / 4);
-    const int bt = items >= 512 ? 512 : std::max(32, (items + 31) / 32 * 32);
-    int cs = 1;
-    while (cs < 8 && cs * bt < items) cs *= 2;
-    A.cs = cs;
+    const SmallShape sh = small_shape(c);
+    A.cs = sh.cs;
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)(g.n_words * cs)); cfg.blockDim = dim3((unsigned)bt);
-    cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
+    cfg.gridDim = dim3((unsigned)(g.n_words * sh.cs)); cfg.blockDim = dim3((unsigned)sh.block);
+    cfg.dynamicSmemBytes = sh.smem; cfg.stream = c->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = (unsigned)cs; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    attr[0].val.clusterDim.x = (unsigned)sh.cs; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    if (g.rpw == 2) CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<2>, A, c->ks, rt));
-    else            CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<1>, A, c->ks, rt));
+    if (g.rpw == 2) {
+        CK(c, cudaFuncSetAttribute(small_step_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
+        CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<2>, A, c->ks, rt));
+    } else {
+        CK(c, cudaFuncSetAttribute(small_step_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
+        CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<1>, A, c->ks, rt));
+    }
     c->attempts += (uint64_t)n_sweeps * (uint64_t)g.N * (uint64_t)g.n_sys;
     c->t += n_sweeps;
     return post_launch(c);

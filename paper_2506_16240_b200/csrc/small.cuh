@@ -8,8 +8,10 @@
 // word lattice gets ONE THREAD-BLOCK CLUSTER (1, 2, 4 or 8 CTAs): the cluster walks through the
 // whole step by itself and the hardware cluster barrier (barrier.cluster, release / acquire)
 // replaces the kernel boundary between half-sweeps; no grid-wide synchronisation exists at all.
-// The state stays in L2 (opposite-parity spins are read with ld.global.cg, everything else a
-// thread reads in a half-sweep it wrote itself); the update is the same 20-operation Boolean
+// The lattice is held ON CHIP for the whole launch: every CTA of the cluster loads a slab of L/cs planes (spins,
+// daemon planes, bonds; both parities) into its shared memory, the opposite-parity planes just across a slab
+// boundary are read from the neighbouring CTA's shared memory (distributed shared memory, ld.shared::cluster), and
+// the slabs go back to global memory once at the end; the update is the same 20-operation Boolean
 // core as the large-lattice kernels (creutz_word20, sweep.cuh), the refresh the same lazy
 // bit-plane compare (refresh_chunk, refresh.cuh), the counting the same carry-save trees
 // (measure_item, measure.cuh).
@@ -38,71 +40,174 @@ struct SmallArgs {
 
 __device__ __forceinline__ void cluster_sync_all() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-    __threadfence();       // gpu-scope fence: also drops whatever this SM's L1 still holds of other CTAs' words
+}
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+// shared::cta address -> the same offset in the shared memory of CTA `rank` of this cluster
+__device__ __forceinline__ uint32_t dsmem_addr(uint32_t local, uint32_t rank) {
+    uint32_t r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ uint4 ld_cluster4(uint32_t a) {
+    uint4 v; asm volatile("ld.shared::cluster.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint4 lds4(uint32_t a) {
+    uint4 v; asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds1(uint32_t a) {
+    uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts4(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" :: "r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
 
-__device__ __forceinline__ uint4 ldcg4(const uint32_t* p) { return __ldcg(reinterpret_cast<const uint4*>(p)); }
+// Shared-memory image of the ZP planes a CTA owns (both parities): byte offsets from the start of dynamic smem.
+// PW = words per parity plane (L * Lh).  The z-bond arrays carry one more plane in front (plane z0 - 1, periodic):
+// the bond towards -z of a site in the CTA's first plane is owned by the plane below, and bonds never change.
+template <int RPW> struct SlabLayout {
+    typedef typename BondT<RPW>::type JT;
+    uint32_t ZP, PW, ZPW, ZPJ;
+    __host__ __device__ SlabLayout(int zp, int pw) : ZP((uint32_t)zp), PW((uint32_t)pw), ZPW((uint32_t)zp * pw * 4u), ZPJ((uint32_t)zp * pw * (uint32_t)sizeof(JT)) {}
+    __host__ __device__ uint32_t spin(int p) const { return (uint32_t)p * ZPW; }
+    __host__ __device__ uint32_t m0(int p) const { return 2u * ZPW + (uint32_t)p * ZPW; }
+    __host__ __device__ uint32_t m1(int p) const { return 4u * ZPW + (uint32_t)p * ZPW; }
+    __host__ __device__ uint32_t jx(int p) const { return 6u * ZPW + (uint32_t)p * ZPJ; }
+    __host__ __device__ uint32_t jy(int p) const { return 6u * ZPW + (2u + (uint32_t)p) * ZPJ; }
+    __host__ __device__ uint32_t jz(int p) const { return 6u * ZPW + 4u * ZPJ + (uint32_t)p * (ZP + 1u) * PW * (uint32_t)sizeof(JT); }   // plane -1 first
+    __host__ __device__ uint32_t total() const { return 6u * ZPW + 4u * ZPJ + 2u * (ZP + 1u) * PW * (uint32_t)sizeof(JT); }
+};
 
-// one item = the quad xq of row (y, z) of the parity-p array of one lattice
+template <int RPW> __device__ __forceinline__ void lds_bonds4(uint32_t addr, uint32_t (&o)[4]);
+template <> __device__ __forceinline__ void lds_bonds4<2>(uint32_t addr, uint32_t (&o)[4]) {
+    uint2 t; asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(t.x), "=r"(t.y) : "r"(addr));
+    Bond4<2>::expand(t, o);
+}
+template <> __device__ __forceinline__ void lds_bonds4<1>(uint32_t addr, uint32_t (&o)[4]) {
+    const uint4 t = lds4(addr); Bond4<1>::expand(t, o);
+}
+template <int RPW> __device__ __forceinline__ uint32_t lds_bond1(uint32_t addr);
+template <> __device__ __forceinline__ uint32_t lds_bond1<2>(uint32_t addr) {
+    uint32_t v; asm volatile("{ .reg .u16 t; ld.shared.u16 t, [%1]; cvt.u32.u16 %0, t; }" : "=r"(v) : "r"(addr));
+    return __byte_perm(v, 0u, 0x1010);
+}
+template <> __device__ __forceinline__ uint32_t lds_bond1<1>(uint32_t addr) { return lds1(addr); }
+
+// one item = the quad xq of row y of the CTA's plane zl (lattice plane z0 + zl), parity p; everything in shared
+// memory, the opposite-parity planes z +- 1 possibly in the neighbouring CTA's (distributed shared memory)
 template <int RPW>
-__device__ __forceinline__ void small_update_item(const SweepArgs& a, int w, int p, int it)
+__device__ __forceinline__ void slab_update_item(const SlabLayout<RPW>& S, uint32_t sm, int L, int Lh, int z0, int rank, int cs,
+                                                 int p, int it)
 {
     typedef typename BondT<RPW>::type JT;
-    const int L = a.L, Lh = a.Lh, nq = Lh >> 2, q = 1 - p;
-    const int xq = it % nq, yz = it / nq, y = yz % L, z = yz / L;
-    const long long half = a.half;
-    uint32_t* sp = a.spin + ((long long)w * 2 + p) * half;
-    const uint32_t* sq = a.spin + ((long long)w * 2 + q) * half;
-    uint32_t* m0p = a.m0 + ((long long)w * 2 + p) * half;
-    uint32_t* m1p = a.m1 + ((long long)w * 2 + p) * half;
-    const JT* Jb = reinterpret_cast<const JT*>(a.J) + (long long)(w / a.n_rg) * 6 * half;
+    constexpr uint32_t JS = sizeof(JT);
+    const int nq = Lh >> 2, q = 1 - p, ZP = (int)S.ZP;
+    const int xq = it % nq, r2 = it / nq, y = r2 % L, zl = r2 / L;
+    const int z = z0 + zl;
     const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
-    const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
     const int xh0 = 4 * xq;
-    const int row = (z * L + y) * Lh, h = row + xh0;
-    const int h_yp = (z * L + yp) * Lh + xh0, h_ym = (z * L + ym) * Lh + xh0;
-    const int h_zp = (zp * L + y) * Lh + xh0, h_zm = (zm * L + y) * Lh + xh0;
-    // c = 1: x = 2xh+1, the -x neighbour has the same xh, the +x one xh+1;  c = 0: x = 2xh, +x same xh, -x at xh-1
+    const uint32_t row = (uint32_t)(zl * L + y) * Lh, h = row + xh0;
+    const uint32_t h_yp = (uint32_t)(zl * L + yp) * Lh + xh0, h_ym = (uint32_t)(zl * L + ym) * Lh + xh0;
     const int c = (y + z + p) & 1;
     const uint32_t cm = 0u - (uint32_t)c;
     const int xe = c ? ((xh0 + 4 == Lh) ? 0 : xh0 + 4) : ((xh0 == 0) ? Lh - 1 : xh0 - 1);
 
-    Vec<4> s = ldg_vec<4>(sp + h), d0 = ldg_vec<4>(m0p + h), d1 = ldg_vec<4>(m1p + h);      // written by this thread
-    const uint4 A4 = ldcg4(sq + h), yp4 = ldcg4(sq + h_yp), ym4 = ldcg4(sq + h_ym);           // written by other CTAs
-    const uint4 zp4 = ldcg4(sq + h_zp), zm4 = ldcg4(sq + h_zm);
-    const uint32_t e = __ldcg(sq + row + xe);
-    const Vec<4> jxo = ldg_bonds<4, RPW>(Jb + (0 * 2 + p) * half + h);
-    const Vec<4> jyo = ldg_bonds<4, RPW>(Jb + (1 * 2 + p) * half + h);
-    const Vec<4> jzo = ldg_bonds<4, RPW>(Jb + (2 * 2 + p) * half + h);
-    const Vec<4> B   = ldg_bonds<4, RPW>(Jb + (0 * 2 + q) * half + h);
-    const uint32_t eJ = bond_expand<RPW>(Jb[(0 * 2 + q) * half + row + xe]);
-    const Vec<4> jym = ldg_bonds<4, RPW>(Jb + (1 * 2 + q) * half + h_ym);
-    const Vec<4> jzm = ldg_bonds<4, RPW>(Jb + (2 * 2 + q) * half + h_zm);
+    const uint32_t a_s = sm + S.spin(p) + h * 4u, a_0 = sm + S.m0(p) + h * 4u, a_1 = sm + S.m1(p) + h * 4u;
+    const uint4 s4 = lds4(a_s), d04 = lds4(a_0), d14 = lds4(a_1);
+    const uint32_t sq = sm + S.spin(q);
+    const uint4 A4 = lds4(sq + h * 4u), yp4 = lds4(sq + h_yp * 4u), ym4 = lds4(sq + h_ym * 4u);
+    const uint32_t e = lds1(sq + (row + xe) * 4u);
+    // planes z + 1 and z - 1 of the opposite parity: in this CTA, or in the next / previous one of the cluster
+    const uint32_t in_plane = ((uint32_t)y * Lh + xh0) * 4u;
+    uint4 zp4, zm4;
+    if (zl + 1 < ZP) zp4 = lds4(sq + ((uint32_t)(zl + 1) * S.PW) * 4u + in_plane);
+    else             zp4 = ld_cluster4(dsmem_addr(sq + in_plane, (uint32_t)((rank + 1 == cs) ? 0 : rank + 1)));
+    if (zl > 0)      zm4 = lds4(sq + ((uint32_t)(zl - 1) * S.PW) * 4u + in_plane);
+    else             zm4 = ld_cluster4(dsmem_addr(sq + ((uint32_t)(ZP - 1) * S.PW) * 4u + in_plane, (uint32_t)((rank == 0) ? cs - 1 : rank - 1)));
+    uint32_t jxo[4], jyo[4], jzo[4], Bx[4], jym[4], jzm[4];
+    lds_bonds4<RPW>(sm + S.jx(p) + h * JS, jxo);
+    lds_bonds4<RPW>(sm + S.jy(p) + h * JS, jyo);
+    lds_bonds4<RPW>(sm + S.jz(p) + (S.PW + h) * JS, jzo);           // the z arrays start at plane -1
+    lds_bonds4<RPW>(sm + S.jx(q) + h * JS, Bx);
+    lds_bonds4<RPW>(sm + S.jy(q) + h_ym * JS, jym);
+    lds_bonds4<RPW>(sm + S.jz(q) + h * JS, jzm);                    // plane zl - 1
+    const uint32_t eJ = lds_bond1<RPW>(sm + S.jx(q) + (row + xe) * JS);
     const uint32_t aw[4] = { A4.x, A4.y, A4.z, A4.w };
+    uint32_t sv[4] = { s4.x, s4.y, s4.z, s4.w }, v0[4] = { d04.x, d04.y, d04.z, d04.w }, v1[4] = { d14.x, d14.y, d14.z, d14.w };
     const uint32_t ypv[4] = { yp4.x, yp4.y, yp4.z, yp4.w }, ymv[4] = { ym4.x, ym4.y, ym4.z, ym4.w };
     const uint32_t zpv[4] = { zp4.x, zp4.y, zp4.z, zp4.w }, zmv[4] = { zm4.x, zm4.y, zm4.z, zm4.w };
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
+        // c = 1: x = 2xh+1, the -x neighbour has the same xh, the +x one xh+1;  c = 0: x = 2xh, +x same xh, -x at xh-1
         const uint32_t up = (k < 3) ? aw[k + 1] : e, dn = (k > 0) ? aw[k - 1] : e;
-        const uint32_t bdn = (k > 0) ? B.v[k - 1] : eJ;
+        const uint32_t bdn = (k > 0) ? Bx[k - 1] : eJ;
         const uint32_t nxp = (cm & up) | (~cm & aw[k]);
         const uint32_t nxm = (cm & aw[k]) | (~cm & dn);
-        const uint32_t jxm = (cm & B.v[k]) | (~cm & bdn);
-        const uint32_t g = s.v[k];
-        creutz_word20(g ^ nxp ^ jxo.v[k], g ^ nxm ^ jxm,
-                      g ^ ypv[k] ^ jyo.v[k], g ^ ymv[k] ^ jym.v[k],
-                      g ^ zpv[k] ^ jzo.v[k], g ^ zmv[k] ^ jzm.v[k],
-                      s.v[k], d0.v[k], d1.v[k]);
+        const uint32_t jxm = (cm & Bx[k]) | (~cm & bdn);
+        const uint32_t g = sv[k];
+        creutz_word20(g ^ nxp ^ jxo[k], g ^ nxm ^ jxm,
+                      g ^ ypv[k] ^ jyo[k], g ^ ymv[k] ^ jym[k],
+                      g ^ zpv[k] ^ jzo[k], g ^ zmv[k] ^ jzm[k],
+                      sv[k], v0[k], v1[k]);
     }
-    stg_vec<4>(sp + h, s);
-    stg_vec<4>(m0p + h, d0);
-    stg_vec<4>(m1p + h, d1);
+    sts4(a_s, sv[0], sv[1], sv[2], sv[3]);
+    sts4(a_0, v0[0], v0[1], v0[2], v0[3]);
+    sts4(a_1, v1[0], v1[1], v1[2], v1[3]);
 }
 
-// Eq. (11) for one word: the lazy bit-plane compare of refresh.cuh, all chunks in this thread
+// counting of one item (quad of row y, plane zl, parity p): unsatisfied own +x, +y, +z bonds, levels, replica differences
+template <int RPW, bool PAIR>
+__device__ __forceinline__ void slab_measure_item(const SlabLayout<RPW>& S, uint32_t sm, int L, int Lh, int z0, int rank, int cs,
+                                                  int p, int it, ItemSums& r)
+{
+    typedef typename BondT<RPW>::type JT;
+    constexpr uint32_t JS = sizeof(JT);
+    const int nq = Lh >> 2, q = 1 - p, ZP = (int)S.ZP;
+    const int xq = it % nq, r2 = it / nq, y = r2 % L, zl = r2 / L;
+    const int z = z0 + zl;
+    const int yp = (y + 1 == L) ? 0 : y + 1;
+    const int xh0 = 4 * xq;
+    const uint32_t row = (uint32_t)(zl * L + y) * Lh, h = row + xh0;
+    const int c = (y + z + p) & 1;                      // c = 1: the +x neighbour is word xh+1, else the same xh
+    const uint32_t sq = sm + S.spin(q);
+    const uint4 s4 = lds4(sm + S.spin(p) + h * 4u), A4 = lds4(sq + h * 4u);
+    const uint32_t e = lds1(sq + (row + ((xh0 + 4 == Lh) ? 0 : xh0 + 4)) * 4u);
+    const uint4 ny4 = lds4(sq + ((uint32_t)(zl * L + yp) * Lh + xh0) * 4u);
+    const uint32_t in_plane = ((uint32_t)y * Lh + xh0) * 4u;
+    uint4 nz4;
+    if (zl + 1 < ZP) nz4 = lds4(sq + ((uint32_t)(zl + 1) * S.PW) * 4u + in_plane);
+    else             nz4 = ld_cluster4(dsmem_addr(sq + in_plane, (uint32_t)((rank + 1 == cs) ? 0 : rank + 1)));
+    uint32_t jx[4], jy[4], jz[4];
+    lds_bonds4<RPW>(sm + S.jx(p) + h * JS, jx);
+    lds_bonds4<RPW>(sm + S.jy(p) + h * JS, jy);
+    lds_bonds4<RPW>(sm + S.jz(p) + (S.PW + h) * JS, jz);
+    const uint4 b04 = lds4(sm + S.m0(p) + h * 4u), b14 = lds4(sm + S.m1(p) + h * 4u);
+    const uint32_t sv[4] = { s4.x, s4.y, s4.z, s4.w }, aw[4] = { A4.x, A4.y, A4.z, A4.w };
+    const uint32_t ny[4] = { ny4.x, ny4.y, ny4.z, ny4.w }, nz[4] = { nz4.x, nz4.y, nz4.z, nz4.w };
+    uint32_t us[4], uc[4], xs[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const uint32_t up = (k < 3) ? aw[k + 1] : e;
+        const uint32_t nx = c ? up : aw[k];
+        full_add(sv[k] ^ nx ^ jx[k], sv[k] ^ ny[k] ^ jy[k], sv[k] ^ nz[k] ^ jz[k], us[k], uc[k]);
+        xs[k] = PAIR ? ((sv[k] ^ (sv[k] >> 16)) & 0xFFFFu) : 0u;
+    }
+    const uint32_t m_lo[4] = { b04.x, b04.y, b04.z, b04.w }, m_hi[4] = { b14.x, b14.y, b14.z, b14.w };
+    csa_4x1_4x2(us, uc, r.u);
+    csa_4x1_4x2(m_lo, m_hi, r.m);
+    if (PAIR) {
+        uint32_t a2, b2, b3;
+        full_add(xs[0], xs[1], xs[2], a2, b2);
+        half_add(a2, xs[3], r.x[0], b3);
+        r.x[1] = b2 ^ b3; r.x[2] = b2 & b3;
+    } else { r.x[0] = r.x[1] = r.x[2] = 0u; }
+}
+
+// Eq. (11) for one word of the CTA's slab: the lazy bit-plane compare of refresh.cuh, all chunks in this thread
 template <int RPW>
-__device__ __forceinline__ unsigned small_refresh_word(const SmallArgs& A, const PhiloxKeys& ks, const RefreshThr& thr,
-                                                       int w, int p, int word)
+__device__ __forceinline__ unsigned slab_refresh_word(const SmallArgs& A, const PhiloxKeys& ks, const RefreshThr& thr,
+                                                      const SlabLayout<RPW>& S, unsigned char* smem, int w, int z0, int p, int word)
 {
     constexpr int SPW = 32 / RPW;
     const SiteGrid& g = A.sg;
@@ -114,8 +219,8 @@ __device__ __forceinline__ unsigned small_refresh_word(const SmallArgs& A, const
     wd.rep_a = kTagRefresh | A.alpha_bits | (uint32_t)(rg * RPW);
     wd.rep_b = (RPW == 2) ? wd.rep_a + 1u : wd.rep_a;
     wd.has_b = (vm >> 16) != 0u;
-    const int rowi = word / g.Lh, xh = word - rowi * g.Lh, z = rowi / g.L, y = rowi - z * g.L;
-    wd.i = canonical_site(g.L, p, z, y, xh);
+    const int rowi = word / g.Lh, xh = word - rowi * g.Lh, zl = rowi / g.L, y = rowi - zl * g.L;
+    wd.i = canonical_site(g.L, p, z0 + zl, y, xh);
     uint32_t EQ[3], gt[3] = { 0u, 0u, 0u };
 #pragma unroll
     for (int k = 0; k < 3; ++k) EQ[k] = thr.never[k] ? 0u : vm;
@@ -127,9 +232,8 @@ __device__ __forceinline__ unsigned small_refresh_word(const SmallArgs& A, const
         if ((EQ[0] | EQ[1] | EQ[2]) == 0u) break;
     }
     const uint32_t ge0 = gt[0] | EQ[0], ge1 = gt[1] | EQ[1], ge2 = gt[2] | EQ[2];
-    const long long o = ((long long)w * 2 + p) * g.half + word;
-    A.a.m0[o] = (ge0 ^ ge1 ^ ge2) & vm;
-    A.a.m1[o] = ge1 & vm;
+    reinterpret_cast<uint32_t*>(smem + S.m0(p))[word] = (ge0 ^ ge1 ^ ge2) & vm;
+    reinterpret_cast<uint32_t*>(smem + S.m1(p))[word] = ge1 & vm;
     return calls;
 }
 
@@ -160,51 +264,76 @@ __device__ __forceinline__ void small_finalize_lattice(const SmallArgs& A, int w
     }
 }
 
-// grid = n_words * cs CTAs in clusters of cs; block = a multiple of 32, at most 512
+// grid = n_words * cs CTAs in clusters of cs (cs divides L); block = a multiple of 32, at most 512;
+// dynamic shared memory = SlabLayout(L / cs, L * Lh).total()
 template <int RPW>
 __global__ void __launch_bounds__(512)
 small_step_kernel(SmallArgs A, PhiloxKeys ks, RefreshThr thr)
 {
     typedef typename BondT<RPW>::type JT;
+    extern __shared__ __align__(16) unsigned char smem[];
     __shared__ unsigned int s_cnt[32];
-    const int w = blockIdx.x / A.cs, rank = blockIdx.x - w * A.cs;
-    const int tid = rank * (int)blockDim.x + (int)threadIdx.x, nthr = A.cs * (int)blockDim.x;
+    const int w = blockIdx.x / A.cs, rank = blockIdx.x - w * A.cs, cs = A.cs;
     const int L = A.a.L, Lh = A.a.Lh, nq = Lh >> 2;
+    const int ZP = L / cs, z0 = rank * ZP, PW = L * Lh;
+    const SlabLayout<RPW> S(ZP, PW);
+    const uint32_t sm = smem_u32(smem);
     const long long half = A.a.half;
-    const int items = L * L * nq;                  // quad-rows per parity
+    const int tid = threadIdx.x, nthr = blockDim.x;
     const bool pair = (RPW == 2) && A.n_replicas == 2;
+    const int slab_words = ZP * PW;                                   // words per parity of this CTA
+    const JT* Jb = reinterpret_cast<const JT*>(A.a.J) + (long long)(w / A.a.n_rg) * 6 * half;
+
+    // ---- global -> shared: the CTA's planes of every array (both parities); 128-bit copies
+    for (int p = 0; p < 2; ++p) {
+        const long long go = ((long long)w * 2 + p) * half + (long long)z0 * PW;
+        const uint4* gs = reinterpret_cast<const uint4*>(A.a.spin + go);
+        const uint4* g0 = reinterpret_cast<const uint4*>(A.a.m0 + go);
+        const uint4* g1 = reinterpret_cast<const uint4*>(A.a.m1 + go);
+        uint4* ss = reinterpret_cast<uint4*>(smem + S.spin(p));
+        uint4* s0 = reinterpret_cast<uint4*>(smem + S.m0(p));
+        uint4* s1 = reinterpret_cast<uint4*>(smem + S.m1(p));
+        for (int i = tid; i < slab_words / 4; i += nthr) { ss[i] = gs[i]; s0[i] = g0[i]; s1[i] = g1[i]; }
+        // bonds: PW * sizeof(JT) bytes per plane, a multiple of 16 (Lh % 4 == 0 and L even)
+        const int jq = (int)((size_t)slab_words * sizeof(JT) / 16), pq = (int)((size_t)PW * sizeof(JT) / 16);
+        const uint4* gx = reinterpret_cast<const uint4*>(Jb + (0 * 2 + p) * half + (long long)z0 * PW);
+        const uint4* gy = reinterpret_cast<const uint4*>(Jb + (1 * 2 + p) * half + (long long)z0 * PW);
+        const uint4* gz = reinterpret_cast<const uint4*>(Jb + (2 * 2 + p) * half + (long long)z0 * PW);
+        const uint4* gzm = reinterpret_cast<const uint4*>(Jb + (2 * 2 + p) * half + (long long)((z0 == 0) ? L - 1 : z0 - 1) * PW);
+        uint4* sx = reinterpret_cast<uint4*>(smem + S.jx(p));
+        uint4* sy = reinterpret_cast<uint4*>(smem + S.jy(p));
+        uint4* sz = reinterpret_cast<uint4*>(smem + S.jz(p));
+        for (int i = tid; i < jq; i += nthr) { sx[i] = gx[i]; sy[i] = gy[i]; sz[pq + i] = gz[i]; }
+        for (int i = tid; i < pq; i += nthr) sz[i] = gzm[i];
+    }
+    __syncthreads();
 
     if (A.do_refresh) {
         unsigned calls = 0;
-        for (int u = tid; u < 2 * (int)half; u += nthr) {
-            const int p = (u >= (int)half) ? 1 : 0;
-            calls += small_refresh_word<RPW>(A, ks, thr, w, p, u - p * (int)half);
+        for (int u = tid; u < 2 * slab_words; u += nthr) {
+            const int p = (u >= slab_words) ? 1 : 0;
+            calls += slab_refresh_word<RPW>(A, ks, thr, S, smem, w, z0, p, u - p * slab_words);
         }
         calls = __reduce_add_sync(0xFFFFFFFFu, calls);
         if ((threadIdx.x & 31) == 0 && calls) atomicAdd(A.n_calls, (unsigned long long)calls);
-        cluster_sync_all();
     }
+    cluster_sync_all();                                               // every CTA's slab is in place
+    const int items = ZP * L * nq;                                    // quad rows per parity of this CTA
     long long r = A.row0;
     for (int t = 1; t <= A.n_sweeps; ++t) {
         for (int p = 0; p < 2; ++p) {
-            for (int it = tid; it < items; it += nthr) small_update_item<RPW>(A.a, w, p, it);
+            for (int it = tid; it < items; it += nthr) slab_update_item<RPW>(S, sm, L, Lh, z0, rank, cs, p, it);
             cluster_sync_all();
         }
         if (A.measure_every > 0 && t % A.measure_every == 0) {
-            // every thread counts its share of the lattice (L1 holds nothing stale: other CTAs' data were only
-            // ever read through ld.global.cg, and a cluster barrier with acquire semantics came in between)
-            const uint32_t items_p = (uint32_t)(half / 4), n_items = 2u * items_p;
-            const uint32_t* s0 = A.a.spin + (long long)w * 2 * half;
-            const uint32_t* d0 = A.a.m0 + (long long)w * 2 * half;
-            const uint32_t* d1 = A.a.m1 + (long long)w * 2 * half;
-            const JT* Jb = reinterpret_cast<const JT*>(A.a.J) + (long long)(w / A.a.n_rg) * 6 * half;
             VCount<kMeasurePlanes> accU, accM, accX; accU.clear(); accM.clear(); accX.clear();
-            for (uint32_t it = (uint32_t)tid; it < n_items; it += (uint32_t)nthr) {
-                ItemSums S;
-                if (pair) measure_item<4, RPW, true>(S, it, items_p, (uint32_t)nq, (uint32_t)L, (uint32_t)Lh, half, s0, d0, d1, Jb);
-                else      measure_item<4, RPW, false>(S, it, items_p, (uint32_t)nq, (uint32_t)L, (uint32_t)Lh, half, s0, d0, d1, Jb);
-                accU.add(S.u); accM.add(S.m);
-                if (pair) accX.add(S.x);
+            for (int u = tid; u < 2 * items; u += nthr) {
+                const int p = (u >= items) ? 1 : 0;
+                ItemSums Sm;
+                if (pair) slab_measure_item<RPW, true>(S, sm, L, Lh, z0, rank, cs, p, u - p * items, Sm);
+                else      slab_measure_item<RPW, false>(S, sm, L, Lh, z0, rank, cs, p, u - p * items, Sm);
+                accU.add(Sm.u); accM.add(Sm.m);
+                if (pair) accX.add(Sm.x);
             }
             block_warp_lane_counts<kMeasurePlanes, 512>(accU.c, s_cnt, A.ma.cntU + (long long)w * 32);
             block_warp_lane_counts<kMeasurePlanes, 512>(accM.c, s_cnt, A.ma.cntM + (long long)w * 32);
@@ -219,6 +348,18 @@ small_step_kernel(SmallArgs A, PhiloxKeys ks, RefreshThr thr)
             // the counters are zero again before anybody adds to them: two cluster barriers (the next sweep) lie between
         }
     }
+    // ---- shared -> global: spins and daemon planes
+    for (int p = 0; p < 2; ++p) {
+        const long long go = ((long long)w * 2 + p) * half + (long long)z0 * PW;
+        uint4* gs = reinterpret_cast<uint4*>(A.a.spin + go);
+        uint4* g0 = reinterpret_cast<uint4*>(A.a.m0 + go);
+        uint4* g1 = reinterpret_cast<uint4*>(A.a.m1 + go);
+        const uint4* ss = reinterpret_cast<const uint4*>(smem + S.spin(p));
+        const uint4* s0 = reinterpret_cast<const uint4*>(smem + S.m0(p));
+        const uint4* s1 = reinterpret_cast<const uint4*>(smem + S.m1(p));
+        for (int i = tid; i < slab_words / 4; i += nthr) { gs[i] = ss[i]; g0[i] = s0[i]; g1[i] = s1[i]; }
+    }
+    cluster_sync_all();          // no CTA leaves while a neighbour may still read its shared memory
 }
 
 }  // namespace micsa
