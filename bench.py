@@ -53,16 +53,16 @@ L2_CAP_BYTES_PER_CLK = 6300.0
 NCU_CSV = ROOT / "profiles" / "r2_ncu_metrics.csv"
 
 
-def ncu_metrics(kernel_prefix, workload):
-    """Per-launch counters of an ncu capture, from the committed summary
-    profiles/r2_ncu_metrics.csv (columns: kernel, workload, metric, value, commit; written from the capture named in
-    profiles/r2_ncu_metrics.md).  Returns ({metric: value}, commit) or ({}, None)."""
+def ncu_metrics(kernel_prefix, workload, capture="single pass"):
+    """Per-launch counters of an ncu capture, from the committed summary profiles/r2_ncu_metrics.csv (columns: kernel,
+    workload, metric, value in bytes / ns / counts, capture, commit; the commands are in profiles/r2_ncu_metrics.md).
+    `capture` selects the rows whose capture column contains it.  Returns ({metric: value}, commit) or ({}, None)."""
     if not NCU_CSV.exists():
         return {}, None
     out, commit = {}, None
     with open(NCU_CSV) as f:
         for row in csv.DictReader(f):
-            if row["kernel"].startswith(kernel_prefix) and row["workload"] == workload:
+            if row["kernel"].startswith(kernel_prefix) and row["workload"] == workload and capture in row["capture"]:
                 out[row["metric"]] = float(row["value"])
                 commit = row["commit"]
     return out, commit
@@ -187,6 +187,54 @@ def cpu_baseline_record(steps=1):
                       f"one thread ({secs1:.1f} s)"}
 
 
+def hbm_resident_record(micsa, tuned, stream, local_rank, rank, world, barrier, max_over_ranks, peak, e0, e1, kname):
+    """The same kernels on a state larger than L2: 160^3 x 128 systems (the shape of the paper's timing table,
+    PAPER.md:341-350), sweeps only and whole steps; frac = 7.5 bits per attempt over time against the HBM copy peak."""
+    import torch
+    from paper_2506_16240_b200.sharding import sample_offset
+    L, nr, ns_big = CFG.L, CFG.n_replicas, 64
+    sched_step = (T_RUN, SWEEPS_PER_STEP, SWEEPS_PER_STEP)
+    gb = tuned(micsa.MicSA(L, ns_big, nr, CFG.seed, sample_offset=sample_offset(rank, ns_big), device=local_rank,
+                           stream=stream))
+    big = gb.layout_info()
+    att_sweep = L ** 3 * ns_big * nr
+    hbm = {"workload": f"table3_L{L}_{ns_big}x{nr}", "state_bytes": big["state_bytes"],
+           "algorithmic_bytes_per_sweep": big["compulsory_bytes_per_sweep"], "peak": peak, "unit": "GB/s"}
+    gb.refresh_demons(T_RUN, 0)
+    for l2g in (0, 1):
+        gb.set_tuning("l2_groups", l2g)
+        gb.sweep(10)
+        barrier()
+        reps = []
+        for _ in range(3):
+            e0.record(stream); gb.sweep(10); e1.record(stream)
+            torch.cuda.synchronize()
+            reps.append(e0.elapsed_time(e1) / 10.0)
+        ms = max_over_ranks(float(np.median(reps)))
+        gbs = big["compulsory_bytes_per_sweep"] / (ms * 1e-3) / 1e9
+        hbm[f"l2_groups_{l2g}"] = {"us_per_sweep": ms * 1e3, "attempts_per_ns": att_sweep * world / (ms * 1e6),
+                                   "achieved": gbs, "frac": gbs / peak}
+    gb.set_tuning("l2_groups", 1)
+    gb.anneal([sched_step] * 20, step0=1)
+    reps = []
+    for rep in range(3):
+        barrier()
+        e0.record(stream); gb.anneal([sched_step] * 20, step0=21 + 20 * rep); e1.record(stream)
+        barrier()
+        reps.append(max_over_ranks(e0.elapsed_time(e1)))
+    hbm["whole_step_attempts_per_ns"] = att_sweep * SWEEPS_PER_STEP * 20 * world / (float(np.median(reps)) * 1e6)
+    hbm["whole_step_ms_repetitions"] = [t / 20 for t in reps]
+    nb, nb_commit = ncu_metrics(kname, hbm["workload"])
+    if "dram__bytes_read.sum" in nb:
+        hbm["traffic_per_half_sweep"] = nb["dram__bytes_read.sum"] + nb.get("dram__bytes_write.sum", 0.0)
+        hbm["traffic_source"] = f"{NCU_CSV.name} @ {nb_commit}"
+    hbm["note"] = ("sweeps only, 10 per call; l2_groups_0 = every half-sweep over all 4 word lattices (each launch "
+                   "streams the state through HBM), l2_groups_1 = the 10 sweeps lattice group by lattice group; "
+                   "frac = 7.5 bits/attempt over time against the measured HBM copy peak")
+    gb.destroy()
+    return hbm
+
+
 def run_reference(args, rank):
     if rank != 0:
         return
@@ -218,6 +266,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-hbm-resident", action="store_true")
+    ap.add_argument("--only-hbm-resident", action="store_true",
+                    help="profiling aid: run only the 160^3 x 128-system section (state larger than L2) and print it")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
                     help="micsa_set_tuning for A/B runs, e.g. --tune sweep_kernel=2")
     ap.add_argument("--walkers", action="store_true",
@@ -279,6 +329,15 @@ def main():
             g.set_tuning(k, int(v))
         return g
 
+    if args.only_hbm_resident:
+        peak, _ = measured_peaks()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        hbm = hbm_resident_record(micsa, tuned, stream, local_rank, rank, world, barrier, max_over_ranks, peak, e0, e1,
+                                  "half_sweep_pipe_kernel")
+        if rank == 0:
+            print(json.dumps({"hbm_resident": hbm}), flush=True)
+        return
+
     g = tuned(micsa.MicSA(L, ns, nr, CFG.seed, sample_offset=sample_offset(rank, ns), device=local_rank,
                           stream=stream))
     info = g.layout_info()
@@ -329,17 +388,21 @@ def main():
     value_flushed = attempts_step * K * world / (t_flushed_ms * 1e6)
 
     # ---- (2) back_to_back: the K steps in ONE micsa_anneal call, one event pair --------------------------------
-    g.anneal([sched_step] * W, step0=W + K + 1)                      # warm-up of this path (rows, trace buffer)
+    g.anneal([sched_step] * max(W, K), step0=W + K + 1)              # warm-up of this path (rows, trace buffer)
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches1 = g.layout_info()["launches"]
-    e0.record(stream)
-    out = g.anneal([sched_step] * K, step0=2 * W + K + 1)
-    e1.record(stream)
-    barrier()
+    reps_b2b = []
+    for rep in range(3):                                             # K steps each; the median repetition is reported
+        barrier()
+        e0.record(stream)
+        out = g.anneal([sched_step] * K, step0=(2 + rep) * (W + K) + 1)
+        e1.record(stream)
+        barrier()
+        reps_b2b.append(max_over_ranks(e0.elapsed_time(e1)))
     clocks = sampler.stop()
-    launches_b2b = g.layout_info()["launches"] - launches1
-    t_b2b_ms = max_over_ranks(e0.elapsed_time(e1))
+    launches_b2b = (g.layout_info()["launches"] - launches1) // 3
+    t_b2b_ms = float(np.median(reps_b2b))
     value_b2b = attempts_step * K * world / (t_b2b_ms * 1e6)
     assert out["E"].shape[0] == K
     if value_b2b <= value_flushed:
@@ -366,8 +429,13 @@ def main():
     traffic = None
     if "dram__bytes_read.sum" in ncu:
         traffic = ncu["dram__bytes_read.sum"] + ncu.get("dram__bytes_write.sum", 0.0)
+    cold, _ = ncu_metrics(kname, CFG.name, capture="caches flushed")
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "traffic_source": f"{NCU_CSV.name} @ {ncu_commit}" if ncu else None,
+                "frac": achieved / peak, "traffic": traffic,
+                "traffic_source": f"{NCU_CSV.name} @ {ncu_commit}: dram__bytes_read.sum + dram__bytes_write.sum per launch, "
+                                  "single-pass ncu of this command (L2 as the run leaves it)" if ncu else None,
+                "traffic_cold": (cold["dram__bytes_read.sum"] + cold.get("dram__bytes_write.sum", 0.0))
+                                if "dram__bytes_read.sum" in cold else None,
                 "kernel": kname, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "us_per_launch": t_launch_s * 1e6,
@@ -434,44 +502,9 @@ def main():
     g.destroy()
     del flush
 
-    # ---- the same kernels on a state larger than L2: 160^3 x 128 systems (Table 3 shape) ------
     hbm = None
     if not args.no_hbm_resident and not args.walkers:
-        ns_big = 64
-        gb = tuned(micsa.MicSA(L, ns_big, nr, CFG.seed, sample_offset=sample_offset(rank, ns_big), device=local_rank,
-                               stream=stream))
-        big = gb.layout_info()
-        att_sweep = L ** 3 * ns_big * nr
-        hbm = {"workload": f"table3_L{L}_{ns_big}x{nr}", "state_bytes": big["state_bytes"],
-               "algorithmic_bytes_per_sweep": big["compulsory_bytes_per_sweep"], "peak": peak, "unit": "GB/s"}
-        gb.refresh_demons(T_RUN, 0)
-        for l2g in (0, 1):
-            gb.set_tuning("l2_groups", l2g)
-            gb.sweep(10)
-            barrier()
-            reps = []
-            for _ in range(3):
-                e0.record(stream); gb.sweep(10); e1.record(stream)
-                torch.cuda.synchronize()
-                reps.append(e0.elapsed_time(e1) / 10.0)
-            ms = max_over_ranks(float(np.median(reps)))
-            gbs = big["compulsory_bytes_per_sweep"] / (ms * 1e-3) / 1e9
-            hbm[f"l2_groups_{l2g}"] = {"us_per_sweep": ms * 1e3, "attempts_per_ns": att_sweep * world / (ms * 1e6),
-                                       "achieved": gbs, "frac": gbs / peak}
-        gb.set_tuning("l2_groups", 1)
-        gb.anneal([sched_step] * 3, step0=1)
-        barrier()
-        e0.record(stream); gb.anneal([sched_step] * 20, step0=4); e1.record(stream)
-        barrier()
-        hbm["whole_step_attempts_per_ns"] = att_sweep * SWEEPS_PER_STEP * 20 * world / (max_over_ranks(e0.elapsed_time(e1)) * 1e6)
-        nb, nb_commit = ncu_metrics(kname, hbm["workload"])
-        if "dram__bytes_read.sum" in nb:
-            hbm["traffic_per_half_sweep"] = nb["dram__bytes_read.sum"] + nb.get("dram__bytes_write.sum", 0.0)
-            hbm["traffic_source"] = f"{NCU_CSV.name} @ {nb_commit}"
-        hbm["note"] = ("sweeps only, 10 per call; l2_groups_0 = every half-sweep over all 4 word lattices (each launch "
-                       "streams the state through HBM), l2_groups_1 = the 10 sweeps lattice group by lattice group; "
-                       "frac = 7.5 bits/attempt over time against the measured HBM copy peak")
-        gb.destroy()
+        hbm = hbm_resident_record(micsa, tuned, stream, local_rank, rank, world, barrier, max_over_ranks, peak, e0, e1, kname)
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -491,6 +524,7 @@ def main():
                        "sharding": "samples by rank, global sample offsets, no collective"},
             "value_is": which,
             "value_back_to_back": value_b2b, "ms_per_step_back_to_back": t_b2b_ms / K,
+            "ms_per_step_back_to_back_repetitions": [t / K for t in reps_b2b],
             "value_l2_flushed": value_flushed, "ms_per_step_l2_flushed": t_flushed_ms / K,
             "rns_per_attempt": 1.0 / SWEEPS_PER_STEP,
             "philox_words_generated_per_attempt": philox_words / (attempts_step * K),

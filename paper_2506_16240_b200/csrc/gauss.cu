@@ -66,11 +66,13 @@ int gcheck(micsa_gauss_ctx* c) {
 
 struct GGeom { int L, Lh; long long half; };
 
-// thread -> site of parity p: t = (z L + y) Lh + xh
+// thread -> site of parity p: t = (z L + y) Lh + xh (32-bit arithmetic: half = L^3 / 2 < 2^30)
 __device__ __forceinline__ bool site_of(const GGeom& g, long long t, int p, int& xh, int& y, int& z, int& c) {
     if (t >= g.half) return false;
-    xh = (int)(t % g.Lh); const long long r = t / g.Lh;
-    y = (int)(r % g.L); z = (int)(r / g.L);
+    const uint32_t tt = (uint32_t)t, Lh = (uint32_t)g.Lh, L = (uint32_t)g.L;
+    const uint32_t r = tt / Lh;
+    xh = (int)(tt - r * Lh);
+    z = (int)(r / L); y = (int)(r - (uint32_t)z * L);
     c = (y + z + p) & 1;
     return true;
 }
@@ -90,15 +92,15 @@ gauss_half_sweep_kernel(int8_t* __restrict__ spin, double* __restrict__ nd, cons
     const int8_t* sq = spin + ((long long)sys * 2 + q) * half;
     double* np_ = nd + ((long long)sys * 2 + p) * half;
     const double* Jb = J + (long long)sample * 6 * half;
-    const long long row = ((long long)z * L + y) * Lh;
+    const uint32_t row = (uint32_t)(z * L + y) * (uint32_t)Lh;
     const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
     const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
     // x = 2 xh + c: the +x neighbour sits at xh + c, the -x neighbour at xh + c - 1 of the other parity's row
     const int xp = (xh + c == Lh) ? 0 : xh + c;
     const int xm = (xh + c - 1 < 0) ? Lh - 1 : xh + c - 1;
-    const long long h_xp = row + xp, h_xm = row + xm;
-    const long long h_yp = ((long long)z * L + yp) * Lh + xh, h_ym = ((long long)z * L + ym) * Lh + xh;
-    const long long h_zp = ((long long)zp * L + y) * Lh + xh, h_zm = ((long long)zm * L + y) * Lh + xh;
+    const uint32_t h_xp = row + (uint32_t)xp, h_xm = row + (uint32_t)xm;
+    const uint32_t h_yp = (uint32_t)(z * L + yp) * (uint32_t)Lh + (uint32_t)xh, h_ym = (uint32_t)(z * L + ym) * (uint32_t)Lh + (uint32_t)xh;
+    const uint32_t h_zp = (uint32_t)(zp * L + y) * (uint32_t)Lh + (uint32_t)xh, h_zm = (uint32_t)(zm * L + y) * (uint32_t)Lh + (uint32_t)xh;
     const double s0 = (double)sp[t];
     double h = __dmul_rn(Jb[(0 * 2 + p) * half + t], (double)sq[h_xp]);
     h = __dadd_rn(h, __dmul_rn(Jb[(0 * 2 + q) * half + h_xm], (double)sq[h_xm]));

@@ -820,7 +820,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->sweep_kernel = 2;
     c->pipe_rows = 4;
     c->use_pdl = 1;
-    c->pipe_planes = (g.n_words == 1 && (g.L / 4) * (g.Lh / 4) >= 512) ? 4 : 1;   // measured: DESIGN.md 6.1
+    c->pipe_planes = ((g.L / 4) * (g.Lh / 4) >= 512) ? 4 : 1;   // big lattices, measured: DESIGN.md 6.1
     c->fuse_measure = 1;
     c->walkers = 0; c->t = 0; c->fuse_walk = 1; c->l2_groups = 1; c->small_path = 1; c->gamma = 1; c->sel = 0;
     c->attempts = c->rns = c->launches = 0;

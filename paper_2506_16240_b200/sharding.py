@@ -16,8 +16,9 @@ import numpy as np
 
 
 def sample_offset(rank: int, n_samples_per_rank: int) -> int:
-    """Global index of the first sample of `rank`: a multiple of 32, the
-    Philox block width of the refresh, so blocks stay whole."""
+    """Global index of the first sample of `rank`.  The library needs a multiple of 16, the sample block that shares
+    the Philox calls of a refresh; the stride is rounded up to a multiple of 32 (a whole word of
+    single-replica samples), which satisfies it."""
     if rank < 0 or n_samples_per_rank < 1:
         raise ValueError("rank must be >= 0 and n_samples_per_rank >= 1")
     stride = (int(n_samples_per_rank) + 31) // 32 * 32

@@ -277,3 +277,28 @@ def test_config5_full_length_invariants(micsa):
         s1, m1, _ = g.get_state(couplings=False)
         np.testing.assert_array_equal(s1, s0)
         np.testing.assert_array_equal(m1, m0)
+
+
+@pytest.mark.parametrize("l2_groups", [1, 0])
+def test_table3_shape_sampled(micsa, oracle, l2_groups):
+    """The state-larger-than-L2 workload of bench.py's `hbm_resident` record (160^3 x 128 systems, the shape of the
+    paper's Table 3; four word lattices, 295 MB): two refresh intervals in the launch configuration
+    the bench times (multi-sweep calls lattice group by lattice group, or every half-sweep over all lattices), three
+    sampled samples from different word lattices against the oracle -- state, rows, counters."""
+    L, ns, nr, seed, T = 160, 64, 2, 4, 0.9
+    sched = [(T, 10, 10)] * 2
+    with micsa.MicSA(L, ns, nr, seed) as g:
+        g.set_tuning("l2_groups", l2_groups)
+        assert g.layout_info()["state_bytes"] == 294912000
+        out = g.anneal(sched)
+        gs, gm, _ = g.get_state(couplings=False)
+        assert g.counters()["attempts"] == 20 * L ** 3 * ns * nr
+    for k in (0, 17, 63):
+        s = oracle.init_spins(L, 1, nr, seed, sample_offset=k); J = oracle.init_bonds(L, 1, seed, sample_offset=k)
+        m = np.zeros_like(s, dtype=np.uint8)
+        ref = driver.anneal(L, s, m, J, seed, sched, sample_offset=k)
+        np.testing.assert_array_equal(gs[k:k + 1], s)
+        np.testing.assert_array_equal(gm[k:k + 1], m)
+        np.testing.assert_array_equal(out["E"][:, k * nr:(k + 1) * nr], ref["E"])
+        np.testing.assert_array_equal(out["Edem"][:, k * nr:(k + 1) * nr], ref["Edem"])
+        np.testing.assert_array_equal(out["Q"][:, k:k + 1], ref["Q"])
