@@ -235,6 +235,41 @@ def hbm_resident_record(micsa, tuned, stream, local_rank, rank, world, barrier, 
     return hbm
 
 
+def gauss_record(micsa, stream, rank, world, barrier, max_over_ranks, peak, e0, e1):
+    """SURVEY.md 8(f) rank 4, sub-record: continuous walkers with Gaussian couplings (Appendix C step 1),
+    64^3 sites x 64 systems, float64: per EMCS one refresh from Eq. (9) and 10 x (sweep + forward-X wandering).
+    Algorithmic bytes per attempt (one pass per sweep): n 8 r + 8 w, spin 1 r + 1 w (int8), bonds 3 x 8 B per site
+    and sample read once per sweep and shared by the replicas = 24 / n_replicas."""
+    import torch
+    from micsa_workloads import gaussian_couplings
+    L, ns, nr, T, n_emcs = 64, 32, 2, 1.0, 20
+    N = L ** 3
+    g = micsa.GaussMicSA(L, ns, nr, 6, sample_offset=rank * ns, stream=stream)
+    g.set_couplings(gaussian_couplings((ns, 3, N), 7 + rank))
+    g.set_walkers(1, 0)
+    for k in range(3):
+        g.refresh(T, k); g.sweep(10)
+    reps = []
+    for rep in range(3):
+        barrier()
+        e0.record(stream)
+        for k in range(n_emcs):
+            g.refresh(T, 10 + rep * n_emcs + k); g.sweep(10)
+        e1.record(stream)
+        barrier()
+        reps.append(max_over_ranks(e0.elapsed_time(e1)))
+    ms = float(np.median(reps))
+    attempts = 10 * n_emcs * N * ns * nr * world
+    bytes_per_attempt = 16.0 + 2.0 + 24.0 / nr
+    gbs = attempts * bytes_per_attempt / (ms * 1e-3) / 1e9
+    g.destroy()
+    return {"workload": f"gauss_L{L}_{ns}x{nr}", "dtype": "f64", "attempts_per_ns": attempts / (ms * 1e6),
+            "ms_per_emcs": ms / n_emcs, "algorithmic_bytes_per_attempt": bytes_per_attempt,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak},
+            "note": "whole EMCS (refresh + 10 sweeps + 10 wandering half-cycles), one thread per (site, system); "
+                    "state 335 MB, larger than L2"}
+
+
 def run_reference(args, rank):
     if rank != 0:
         return
@@ -506,6 +541,10 @@ def main():
     if not args.no_hbm_resident and not args.walkers:
         hbm = hbm_resident_record(micsa, tuned, stream, local_rank, rank, world, barrier, max_over_ranks, peak, e0, e1, kname)
 
+    gauss = None
+    if not args.no_hbm_resident and not args.walkers:
+        gauss = gauss_record(micsa, stream, rank, world, barrier, max_over_ranks, peak, e0, e1)
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline_record()
@@ -530,7 +569,7 @@ def main():
             "philox_words_generated_per_attempt": philox_words / (attempts_step * K),
             "sweep_only_attempts_per_ns": sweep_only,
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
-            "roofline": roofline, "hbm_resident": hbm, "cpu_baseline": cpu, "wall_s": wall,
+            "roofline": roofline, "hbm_resident": hbm, "continuous_daemons": gauss, "cpu_baseline": cpu, "wall_s": wall,
         }
         print(json.dumps(line), flush=True)
     if world > 1:
