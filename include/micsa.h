@@ -331,6 +331,8 @@ int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
  *   n_replicas <= 2, one daemon per spin) micsa_sweep, micsa_sweep_measure and every schedule step of
  *   micsa_anneal run as ONE launch in which each word lattice is walked by a thread-block cluster (refresh, all
  *   sweeps and the measurement rows; cluster barriers instead of kernel boundaries), 0 = the general path.
+ * key MICSA_TUNE_SMALL_ITEMS: quad rows per CTA and parity the small-lattice path aims at when it chooses the cluster
+ *   size (1 .. 16 CTAs per word lattice): 0 = default, else 1 .. 1024.
  * key MICSA_TUNE_PDL: 1 (default) = kernel 2 is launched with programmatic
  *   stream serialization (the next half-sweep's grid is scheduled while this
  *   one drains and waits on the device for its completion), 0 = plain launches.
@@ -338,7 +340,7 @@ int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
 enum { MICSA_TUNE_SWEEP_KERNEL = 0, MICSA_TUNE_PIPE_ROWS = 2, MICSA_TUNE_PDL = 3,
        MICSA_TUNE_PIPE_PLANES = 4, MICSA_TUNE_FUSE_MEASURE = 5,
        MICSA_TUNE_FUSE_WALK = 6, MICSA_TUNE_L2_GROUPS = 7,
-       MICSA_TUNE_SMALL_PATH = 8 };
+       MICSA_TUNE_SMALL_PATH = 8, MICSA_TUNE_SMALL_ITEMS = 9 };
 int micsa_set_tuning(micsa_ctx *ctx, int key, int value);
 
 /* ---- continuous daemons / walkers with real couplings -------------

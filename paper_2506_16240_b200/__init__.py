@@ -374,8 +374,8 @@ class MicSA:
     def set_tuning(self, key, value):
         """micsa_set_tuning: 'sweep_kernel' (1 row-marching, 2 pipelined row-marching),
         'pipe_rows' (4, 8), 'pdl' (0, 1), 'pipe_planes' (1, 4), 'fuse_measure' (0, 1), 'fuse_walk' (0, 1),
-        'l2_groups' (0, 1), 'small_path' (0, 1)."""
-        k = {"sweep_kernel": 0, "pipe_rows": 2, "pdl": 3, "pipe_planes": 4, "fuse_measure": 5, "fuse_walk": 6, "l2_groups": 7, "small_path": 8}[key]
+        'l2_groups' (0, 1), 'small_path' (0, 1), 'small_items' (0 default, 1..1024)."""
+        k = {"sweep_kernel": 0, "pipe_rows": 2, "pdl": 3, "pipe_planes": 4, "fuse_measure": 5, "fuse_walk": 6, "l2_groups": 7, "small_path": 8, "small_items": 9}[key]
         _check(_lib.micsa_set_tuning(self._h, k, int(value)))
 
     def layout_info(self):

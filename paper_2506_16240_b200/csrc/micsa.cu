@@ -137,6 +137,7 @@ struct micsa_ctx {
     int sel;                   // family that set_daemons / get_state address
     std::vector<uint32_t*> xm0, xm1;   // families 1 .. gamma-1 (library-owned)
     int l2_groups;             // run multi-sweep calls lattice group by lattice group when the state exceeds L2
+    int small_items;           // small lattices: quad rows per CTA aimed at (0 = default)
     int small_path;            // small lattices: whole groups of sweeps (+ refresh, + rows) in one cluster launch
     int fuse_walk;             // walkers: exchange inside the odd half-sweep instead of a separate kernel
     int walkers;               // 0 = daemons stay on their site, 1 = one forward-X walker per spin
@@ -618,13 +619,15 @@ SmallShape small_shape(const micsa_ctx* c) {
     const Geom& g = c->g;
     SmallShape sh; sh.ok = false; sh.cs = 1; sh.block = 32; sh.smem = 0;
     if (c->V != 4 || g.L > 64) return sh;
-    for (int cs = 1; cs <= 8; cs *= 2) {
+    const int target = c->small_items > 0 ? c->small_items : 128;      // quad rows per CTA and parity aimed at (measured: DESIGN.md 6.8)
+    for (int cs = 1; cs <= 16; cs *= 2) {
         if (g.L % cs) break;
         const size_t smem = (g.rpw == 2) ? SlabLayout<2>(g.L / cs, g.L * g.Lh).total() : SlabLayout<1>(g.L / cs, g.L * g.Lh).total();
         const int items = (g.L / cs) * g.L * (g.Lh / 4);
-        if (smem <= 200 * 1024 && (items <= 512 || (cs == 8 && items <= 1024))) {
+        const bool last = (cs == 16) || (g.L % (2 * cs)) != 0;
+        if (smem <= 200 * 1024 && (items <= target || (last && items <= 1024))) {
             sh.ok = true; sh.cs = cs; sh.smem = smem;
-            sh.block = items >= 512 ? 512 : std::max(32, (items + 31) / 32 * 32);
+            sh.block = items >= 512 ? 512 : std::max(256, (items + 31) / 32 * 32);    // refresh and counting use every thread
             return sh;
         }
     }
@@ -671,9 +674,11 @@ int launch_small_step(micsa_ctx* c, bool do_refresh, double T, uint32_t step, in
     attr[0].val.clusterDim.x = (unsigned)sh.cs; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
     if (g.rpw == 2) {
+        if (sh.cs > 8) CK(c, cudaFuncSetAttribute(small_step_kernel<2>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         CK(c, cudaFuncSetAttribute(small_step_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
         CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<2>, A, c->ks, rt));
     } else {
+        if (sh.cs > 8) CK(c, cudaFuncSetAttribute(small_step_kernel<1>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         CK(c, cudaFuncSetAttribute(small_step_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
         CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<1>, A, c->ks, rt));
     }
@@ -822,7 +827,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->use_pdl = 1;
     c->pipe_planes = ((g.L / 4) * (g.Lh / 4) >= 512) ? 4 : 1;   // big lattices, measured: DESIGN.md 6.1
     c->fuse_measure = 1;
-    c->walkers = 0; c->t = 0; c->fuse_walk = 1; c->l2_groups = 1; c->small_path = 1; c->gamma = 1; c->sel = 0;
+    c->walkers = 0; c->t = 0; c->fuse_walk = 1; c->l2_groups = 1; c->small_path = 1; c->small_items = 0; c->gamma = 1; c->sel = 0;
     c->attempts = c->rns = c->launches = 0;
     c->sticky = 0;
     if (dev_workspace) {
@@ -1361,6 +1366,9 @@ int micsa_set_tuning(micsa_ctx* c, int key, int value) {
         case MICSA_TUNE_L2_GROUPS:
             if (value != 0 && value != 1) { set_err("l2_groups must be 0 or 1"); return MICSA_ERR_INVALID; }
             c->l2_groups = value; return MICSA_OK;
+        case MICSA_TUNE_SMALL_ITEMS:
+            if (value < 0 || value > 1024) { set_err("small_items must be 0 (default) .. 1024"); return MICSA_ERR_INVALID; }
+            c->small_items = value; return MICSA_OK;
         case MICSA_TUNE_SMALL_PATH:
             if (value != 0 && value != 1) { set_err("small_path must be 0 or 1"); return MICSA_ERR_INVALID; }
             c->small_path = value; return MICSA_OK;

@@ -50,6 +50,8 @@ def run(ci, scale):
             # measure at the end of every k-th refresh interval: measure_every counts sweeps inside a step
             k = max(1, me // R)
             sched = [(float(T), R, R if (i + 1) % k == 0 or i == steps - 1 else 0) for i in range(steps)]
+        with MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed) as warm:      # load the kernels once (lazy module loading)
+            warm.anneal(sched[:2], trace=False)
         with MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed) as g:
             g.synchronize()
             t0 = time.perf_counter()
