@@ -147,6 +147,7 @@ struct micsa_ctx {
     int use_pdl;               // programmatic dependent launch for the pipelined kernel
     int pipe_rows;             // rows per thread of the pipelined kernel (4 or 8)
     uint64_t attempts, rns, launches;
+    cudaError_t launch_err;    // first failed cudaLaunchKernelEx since the last post_launch()
     int sticky;
 };
 
@@ -180,6 +181,7 @@ dim3 site_blocks(const Geom& g, int nz) {
 
 int post_launch(micsa_ctx* c, int n = 1) {
     c->launches += (uint64_t)n;
+    if (c->launch_err != cudaSuccess) { const cudaError_t e = c->launch_err; c->launch_err = cudaSuccess; cudaGetLastError(); CK(c, e); }
     CK(c, cudaGetLastError());
     return MICSA_OK;
 }
@@ -208,6 +210,9 @@ void launch_half_sweep_rows(micsa_ctx* c, int parity) {
 }
 
 // dir != 0 (odd launches of walker timesteps): the launch also does the wandering exchange
+// a failed launch is remembered on the context and reported by the next post_launch()
+#define LK(call) do { const cudaError_t e_ = (call); if (e_ != cudaSuccess && c->launch_err == cudaSuccess) c->launch_err = e_; } while (0)
+
 template <int RPW>
 void launch_half_sweep_pipe(micsa_ctx* c, int parity, int dir = 0, int w0 = 0, int nw = -1) {
     SweepArgs a;
@@ -235,27 +240,27 @@ void launch_half_sweep_pipe(micsa_ctx* c, int parity, int dir = 0, int w0 = 0, i
         const int axis = (dir > 0 ? dir : -dir) - 1, walk_z = (axis == 2) ? 1 : 0;
         if (axis == 0) {
             if (zw == 4) {
-                if (dir > 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, +1>, a, parity, 0);
-                else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, -1>, a, parity, 0);
+                if (dir > 0) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, +1>, a, parity, 0));
+                else         LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, -1>, a, parity, 0));
             } else {
-                if (dir > 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, +1>, a, parity, 0);
-                else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, -1>, a, parity, 0);
+                if (dir > 0) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, +1>, a, parity, 0));
+                else         LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, -1>, a, parity, 0));
             }
         } else {
             if (zw == 4) {
-                if (dir > 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, +2>, a, parity, walk_z);
-                else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, -2>, a, parity, walk_z);
+                if (dir > 0) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, +2>, a, parity, walk_z));
+                else         LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4, -2>, a, parity, walk_z));
             } else {
-                if (dir > 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, +2>, a, parity, walk_z);
-                else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, -2>, a, parity, walk_z);
+                if (dir > 0) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, +2>, a, parity, walk_z));
+                else         LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1, -2>, a, parity, walk_z));
             }
         }
     } else if (zw == 4) {
-        if (yc == 8) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8, 4>, a, parity, 0);
-        else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4>, a, parity, 0);
+        if (yc == 8) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8, 4>, a, parity, 0));
+        else         LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 4>, a, parity, 0));
     } else {
-        if (yc == 8) cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8, 1>, a, parity, 0);
-        else         cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1>, a, parity, 0);
+        if (yc == 8) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 8, 1>, a, parity, 0));
+        else         LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_kernel<RPW, 4, 1>, a, parity, 0));
     }
 }
 
@@ -597,15 +602,15 @@ int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min, int dir)
     attr[0].val.programmaticStreamSerializationAllowed = c->use_pdl ? 1 : 0;
     cfg.attrs = attr; cfg.numAttrs = 1;
     if (zw == 4) {
-        cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 1>, a, 0, ma, fa);
-        if (dir > 0)      cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2, +1>, a, 1, ma, fa);
-        else if (dir < 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2, -1>, a, 1, ma, fa);
-        else              cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2>, a, 1, ma, fa);
+        LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 1>, a, 0, ma, fa));
+        if (dir > 0)      LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2, +1>, a, 1, ma, fa));
+        else if (dir < 0) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2, -1>, a, 1, ma, fa));
+        else              LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2>, a, 1, ma, fa));
     } else {
-        cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 1>, a, 0, ma, fa);
-        if (dir > 0)      cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2, +1>, a, 1, ma, fa);
-        else if (dir < 0) cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2, -1>, a, 1, ma, fa);
-        else              cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2>, a, 1, ma, fa);
+        LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 1>, a, 0, ma, fa));
+        if (dir > 0)      LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2, +1>, a, 1, ma, fa));
+        else if (dir < 0) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2, -1>, a, 1, ma, fa));
+        else              LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2>, a, 1, ma, fa));
     }
     c->attempts += (uint64_t)g.N * (uint64_t)g.n_sys;
     return post_launch(c, 2);
@@ -829,7 +834,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->fuse_measure = 1;
     c->walkers = 0; c->t = 0; c->fuse_walk = 1; c->l2_groups = 1; c->small_path = 1; c->small_items = 0; c->gamma = 1; c->sel = 0;
     c->attempts = c->rns = c->launches = 0;
-    c->sticky = 0;
+    c->sticky = 0; c->launch_err = cudaSuccess;
     if (dev_workspace) {
         if (workspace_bytes < c->plan.total || ((uintptr_t)dev_workspace % kAlign)) {
             set_err("workspace too small or not 256-byte aligned"); delete c; return nullptr;
