@@ -137,6 +137,7 @@ struct micsa_ctx {
     int sel;                   // family that set_daemons / get_state address
     std::vector<uint32_t*> xm0, xm1;   // families 1 .. gamma-1 (library-owned)
     int l2_groups;             // run multi-sweep calls lattice group by lattice group when the state exceeds L2
+    bool small_attr_set;       // small lattices: kernel attributes (shared memory size, cluster size) set
     int small_items;           // small lattices: quad rows per CTA aimed at (0 = default)
     int small_path;            // small lattices: whole groups of sweeps (+ refresh, + rows) in one cluster launch
     int fuse_walk;             // walkers: exchange inside the odd half-sweep instead of a separate kernel
@@ -678,15 +679,19 @@ int launch_small_step(micsa_ctx* c, bool do_refresh, double T, uint32_t step, in
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = (unsigned)sh.cs; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    if (g.rpw == 2) {
-        if (sh.cs > 8) CK(c, cudaFuncSetAttribute(small_step_kernel<2>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        CK(c, cudaFuncSetAttribute(small_step_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
-        CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<2>, A, c->ks, rt));
-    } else {
-        if (sh.cs > 8) CK(c, cudaFuncSetAttribute(small_step_kernel<1>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        CK(c, cudaFuncSetAttribute(small_step_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
-        CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<1>, A, c->ks, rt));
+    // function attributes are per device and sticky: set them once per context (shape never changes)
+    if (!c->small_attr_set) {
+        if (g.rpw == 2) {
+            if (sh.cs > 8) CK(c, cudaFuncSetAttribute(small_step_kernel<2>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+            CK(c, cudaFuncSetAttribute(small_step_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
+        } else {
+            if (sh.cs > 8) CK(c, cudaFuncSetAttribute(small_step_kernel<1>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+            CK(c, cudaFuncSetAttribute(small_step_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
+        }
+        c->small_attr_set = true;
     }
+    if (g.rpw == 2) CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<2>, A, c->ks, rt));
+    else            CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<1>, A, c->ks, rt));
     c->attempts += (uint64_t)n_sweeps * (uint64_t)g.N * (uint64_t)g.n_sys;
     c->t += n_sweeps;
     return post_launch(c);
@@ -832,7 +837,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->use_pdl = 1;
     c->pipe_planes = ((g.L / 4) * (g.Lh / 4) >= 512) ? 4 : 1;   // big lattices, measured: DESIGN.md 6.1
     c->fuse_measure = 1;
-    c->walkers = 0; c->t = 0; c->fuse_walk = 1; c->l2_groups = 1; c->small_path = 1; c->small_items = 0; c->gamma = 1; c->sel = 0;
+    c->walkers = 0; c->t = 0; c->fuse_walk = 1; c->l2_groups = 1; c->small_path = 1; c->small_items = 0; c->small_attr_set = false; c->gamma = 1; c->sel = 0;
     c->attempts = c->rns = c->launches = 0;
     c->sticky = 0; c->launch_err = cudaSuccess;
     if (dev_workspace) {
@@ -1373,7 +1378,7 @@ int micsa_set_tuning(micsa_ctx* c, int key, int value) {
             c->l2_groups = value; return MICSA_OK;
         case MICSA_TUNE_SMALL_ITEMS:
             if (value < 0 || value > 1024) { set_err("small_items must be 0 (default) .. 1024"); return MICSA_ERR_INVALID; }
-            c->small_items = value; return MICSA_OK;
+            c->small_items = value; c->small_attr_set = false; return MICSA_OK;
         case MICSA_TUNE_SMALL_PATH:
             if (value != 0 && value != 1) { set_err("small_path must be 0 or 1"); return MICSA_ERR_INVALID; }
             c->small_path = value; return MICSA_OK;
