@@ -302,3 +302,28 @@ def test_table3_shape_sampled(micsa, oracle, l2_groups):
         np.testing.assert_array_equal(out["E"][:, k * nr:(k + 1) * nr], ref["E"])
         np.testing.assert_array_equal(out["Edem"][:, k * nr:(k + 1) * nr], ref["Edem"])
         np.testing.assert_array_equal(out["Q"][:, k:k + 1], ref["Q"])
+
+
+def test_largest_lattice_offsets_beyond_2_31_bytes(micsa, oracle):
+    """Maximum size: L = 1040 (N = 1.125e9 sites, just below the 2^31 limit of the 32-bit site index; a parity array
+    holds 2.25 GB, so the kernels' unsigned 32-bit byte offsets go beyond 2^31).  One sample x two replicas: the Philox
+    start, one refresh, one sweep, the separate and the fused measurement against the oracle, every site.  About three
+    minutes, mostly the oracle; 20 GB of host memory."""
+    L, ns, nr, seed, T = 1040, 1, 2, 3, 0.9
+    s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+    m = np.zeros_like(s, dtype=np.uint8)
+    with micsa.MicSA(L, ns, nr, seed) as g:
+        gs, gm, gJ = g.get_state()
+        assert np.array_equal(gs, s) and np.array_equal(gJ, J) and not gm.any()
+        del gJ
+        g.refresh_demons(T, 7); g.sweep(1)
+        oracle.refresh(L, m, seed, T, 7); oracle.sweep(L, s, m, J, 1)
+        gs, gm, _ = g.get_state(couplings=False)
+        assert np.array_equal(gs, s) and np.array_equal(gm, m)
+        del gs, gm
+        E, Ed, Q = g.measure_i64()
+        oE, oEd, oQ = oracle.measure(L, s, m, J)
+        np.testing.assert_array_equal(E, oE); np.testing.assert_array_equal(Ed, oEd); np.testing.assert_array_equal(Q, oQ)
+        g.sweep_measure(1); E2, Ed2, _ = g.measure_end()
+        np.testing.assert_array_equal(E2 + Ed2, E + Ed)           # PAPER.md:124 at this size too
+        assert g.counters()["attempts"] == 2 * L ** 3 * ns * nr

@@ -869,3 +869,26 @@ def test_small_lattice_path_bit_exact(micsa, oracle, L, ns, nr):
             for _ in range(4):
                 g.half_sweep(1); g.half_sweep(0)
             _assert_state(g, s0, m0)
+
+
+def test_empty_and_rowless_schedules(micsa, oracle):
+    """Degenerate calls: an empty schedule, steps without sweeps, measure_every larger than the step -- no rows, the
+    state only sees the refreshes; min_energy is +inf when nothing was measured."""
+    L, ns, nr, seed = 8, 3, 2, 5
+    s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+    m = np.zeros_like(s, dtype=np.uint8)
+    for small in (1, 0):
+        with micsa.MicSA(L, ns, nr, seed) as g:
+            g.set_tuning("small_path", small)
+            out = g.anneal([])
+            assert out["E"].shape == (0, ns * nr) and np.all(np.isinf(out["min_energy"]))
+            _assert_state(g, s, m, J)
+            out = g.anneal([(1.0, 0, 0), (2.0, 0, 5)], step0=3)         # refreshes only
+            m2 = m.copy(); oracle.refresh(L, m2, seed, 2.0, 4)
+            _assert_state(g, s, m2)
+            assert out["E"].shape[0] == 0 and g.counters()["attempts"] == 0 and g.counters()["rns_drawn"] == 2 * L ** 3 * ns * nr
+            out = g.anneal([(1.5, 3, 7)], step0=9)                        # measure_every beyond the step: no row
+            s3, m3 = s.copy(), m2.copy()
+            oracle.refresh(L, m3, seed, 1.5, 9); oracle.sweep(L, s3, m3, J, 3)
+            _assert_state(g, s3, m3)
+            assert out["E"].shape[0] == 0 and np.all(np.isinf(out["min_energy"]))
