@@ -1298,6 +1298,11 @@ int micsa_anneal(micsa_ctx* c, const micsa_step* sched, int n_steps, uint32_t st
                                     memcmp(&c->pending_T, &sched[k].T, sizeof(double)) == 0;
             if (prefetched) { rc = launch_refresh(c, sched[k].T, step0 + (uint32_t)k); if (rc) return rc; }
             else c->rns += (uint64_t)g.N * (uint64_t)g.n_sys;
+            // the clusters of a small lattice leave most SMs idle: the NEXT step's refresh is generated beside them by
+            // the stand-alone kernel on the side stream (into the staging planes) instead of inside the next launch
+            if (k + 1 < n_steps && sched[k + 1].n_sweeps > 0 && c->g.n_words * small_shape(c).cs * 2 <= c->sms) {
+                rc = launch_prefetch(c, sched[k + 1].T, step0 + (uint32_t)k + 1u); if (rc) return rc;
+            }
             rc = launch_small_step(c, !prefetched, sched[k].T, step0 + (uint32_t)k, sched[k].n_sweeps, me,
                                    (long long*)dev_rows.dev, r, keep, true);
             if (rc) return rc;
