@@ -454,7 +454,8 @@ int launch_refresh_into(micsa_ctx* c, double T, uint32_t step, uint32_t* m0, uin
         for (int p = 0; p < 32; ++p) rt.tb[k][p] = ((thr[k] >> (31 - p)) & 1u) ? 0xFFFFFFFFu : 0u;
     }
     const SiteGrid sg = site_grid(c->g);
-    const dim3 grid = site_blocks(c->g, c->g.n_words * 2);
+    dim3 grid = site_blocks(c->g, c->g.n_words * 2);
+    grid.x = (grid.x + kRefreshSub - 1) / kRefreshSub;       // kRefreshSub groups of 128 words per block
     if (c->g.rpw == 2)
         refresh_kernel<2><<<grid, 128, 0, stream>>>(m0, m1, sg, c->ks, step, rt, c->calls, (uint32_t)alpha << 20);
     else

@@ -90,16 +90,17 @@ __device__ __forceinline__ void refresh_chunk(uint32_t c_rt, const RefreshWord& 
 }
 
 constexpr int kRefreshBlock = 128;
+constexpr int kRefreshSub = 4;        // groups of kRefreshBlock words per block
 
 // grid = (ceil(L*Lh/block), L, n_words*2); one thread = one site word in phase 0.
 // A word holds two 16-lane Philox streams a (lanes 0-15) and b (lanes 16-31):
 // RPW = 2: the same sample block, replicas 2rg and 2rg+1;
 // RPW = 1: sample blocks 2sg and 2sg+1 of one replica.
-// Phase 0: every thread runs chunk 0 of its word.  About a quarter of the words
-// still have an undecided lane after 8 planes; they are queued in shared memory
-// and phase 1 runs chunk 1 for the queued words only, on the first threads of
-// the block (so whole warps drop out instead of idling beside one busy lane),
-// and so on.  Measured at config 4: 93 -> 84 us per refresh.
+// Phase 0: every thread runs chunk 0 of its words (kRefreshSub groups of kRefreshBlock words per block).  About a
+// quarter of the words still have an undecided lane after 8 planes; they are queued in shared memory and phase 1
+// runs chunk 1 for the queued words only, densely on the threads of the block (so whole warps drop out instead of
+// idling beside one busy lane), and so on.  Measured at config 4: 93 us with every thread iterating by itself, 84 us
+// with a queue per 128 words, 67 us with the block-wide queue (one barrier per phase and 512 words).
 template <int RPW>
 __global__ void __launch_bounds__(kRefreshBlock)
 refresh_kernel(uint32_t* __restrict__ m0, uint32_t* __restrict__ m1, SiteGrid g,
@@ -107,8 +108,9 @@ refresh_kernel(uint32_t* __restrict__ m0, uint32_t* __restrict__ m1, SiteGrid g,
                unsigned long long* __restrict__ n_calls, uint32_t alpha_bits)
 {
     constexpr int SPW = 32 / RPW;
-    __shared__ uint32_t q_tid[2][kRefreshBlock];
-    __shared__ uint32_t q_st[2][6][kRefreshBlock];
+    constexpr int kQ = kRefreshBlock * kRefreshSub;       // every word of the block may be queued
+    __shared__ uint32_t q_tid[2][kQ];
+    __shared__ uint32_t q_st[2][6][kQ];
     __shared__ int q_n[4];
     __shared__ unsigned int s_calls;
     if (threadIdx.x < 4) q_n[threadIdx.x] = 0;
@@ -129,45 +131,55 @@ refresh_kernel(uint32_t* __restrict__ m0, uint32_t* __restrict__ m1, SiteGrid g,
     const unsigned per_chunk = wd.has_b ? 2u : 1u;
     unsigned int calls = 0;
 
+    // Phase 0 for all kRefreshSub groups of kRefreshBlock words of this block, then ONE barrier; the words that are
+    // still undecided (about a quarter) sit densely in the block-wide queue and phase c runs chunk c for them, a
+    // barrier per phase: three barriers per kRefreshSub * 128 words instead of three per 128 (ncu: 37 % of the stall
+    // samples of the one-group kernel were warps waiting at those barriers).
+    const int n_plane = g.L * g.Lh;
+    auto finish = [&](int word, const uint32_t (&EQ)[3], const uint32_t (&gt)[3]) {
+        // lanes equal to a threshold in all 32 bits are >= it
+        const uint32_t ge0 = gt[0] | EQ[0], ge1 = gt[1] | EQ[1], ge2 = gt[2] | EQ[2];
+        m0[plane0 + word] = (ge0 ^ ge1 ^ ge2) & vm;       // level odd
+        m1[plane0 + word] = ge1 & vm;                     // level >= 2
+    };
+    auto push = [&](int c, int word, const uint32_t (&EQ)[3], const uint32_t (&gt)[3]) {
+        const int slot = atomicAdd(&q_n[c], 1);
+        const int b = c & 1;
+        q_tid[b][slot] = (uint32_t)word;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { q_st[b][k][slot] = EQ[k]; q_st[b][3 + k][slot] = gt[k]; }
+    };
 #pragma unroll 1
-    for (uint32_t c = 0; c < 4; ++c) {
-        // the word this thread works on in phase c, and its compare state so far
-        int word = -1;
+    for (int sub = 0; sub < kRefreshSub; ++sub) {
+        const int word = ((int)blockIdx.x * kRefreshSub + sub) * kRefreshBlock + (int)threadIdx.x;
+        if (word >= n_plane) break;
         uint32_t EQ[3], gt[3] = { 0u, 0u, 0u };
-        if (c == 0) {
-            const int t = blockIdx.x * kRefreshBlock + threadIdx.x;
-            if (t < g.L * g.Lh) word = t;
 #pragma unroll
-            for (int k = 0; k < 3; ++k) EQ[k] = thr.never[k] ? 0u : vm;
-        } else {
-            __syncthreads();                      // queue c-1 is complete
-            const int n = q_n[c - 1];
-            if (n == 0) break;                    // block-uniform
-            if ((int)threadIdx.x < n) {
-                const int b = (c - 1) & 1;
-                word = (int)q_tid[b][threadIdx.x];
+        for (int k = 0; k < 3; ++k) EQ[k] = thr.never[k] ? 0u : vm;
+        const int y = word / g.Lh, xh = word - y * g.Lh;
+        wd.i = canonical_site(g.L, p, z, y, xh);
+        refresh_chunk<0>(0u, wd, step, EQ, gt, thr, ks);
+        calls += per_chunk;
+        if ((EQ[0] | EQ[1] | EQ[2]) != 0u) push(0, word, EQ, gt);      // a lane is still equal to a threshold prefix
+        else finish(word, EQ, gt);
+    }
+#pragma unroll 1
+    for (uint32_t c = 1; c < 4; ++c) {
+        __syncthreads();                          // queue c-1 is complete
+        const int n = q_n[c - 1];
+        if (n == 0) break;                        // block-uniform
+        const int b = (c - 1) & 1;
+        for (int e = threadIdx.x; e < n; e += kRefreshBlock) {
+            const int word = (int)q_tid[b][e];
+            uint32_t EQ[3], gt[3];
 #pragma unroll
-                for (int k = 0; k < 3; ++k) { EQ[k] = q_st[b][k][threadIdx.x]; gt[k] = q_st[b][3 + k][threadIdx.x]; }
-            }
-        }
-        if (word >= 0) {
+            for (int k = 0; k < 3; ++k) { EQ[k] = q_st[b][k][e]; gt[k] = q_st[b][3 + k][e]; }
             const int y = word / g.Lh, xh = word - y * g.Lh;
             wd.i = canonical_site(g.L, p, z, y, xh);
-            if (c == 0) refresh_chunk<0>(0u, wd, step, EQ, gt, thr, ks);
-            else        refresh_chunk<-1>(c, wd, step, EQ, gt, thr, ks);
+            refresh_chunk<-1>(c, wd, step, EQ, gt, thr, ks);
             calls += per_chunk;
-            if (c < 3 && (EQ[0] | EQ[1] | EQ[2]) != 0u) {         // a lane is still equal to a threshold prefix
-                const int slot = atomicAdd(&q_n[c], 1);
-                const int b = c & 1;
-                q_tid[b][slot] = (uint32_t)word;
-#pragma unroll
-                for (int k = 0; k < 3; ++k) { q_st[b][k][slot] = EQ[k]; q_st[b][3 + k][slot] = gt[k]; }
-            } else {
-                // lanes equal to a threshold in all 32 bits are >= it
-                const uint32_t ge0 = gt[0] | EQ[0], ge1 = gt[1] | EQ[1], ge2 = gt[2] | EQ[2];
-                m0[plane0 + word] = (ge0 ^ ge1 ^ ge2) & vm;       // level odd
-                m1[plane0 + word] = ge1 & vm;                     // level >= 2
-            }
+            if (c < 3 && (EQ[0] | EQ[1] | EQ[2]) != 0u) push((int)c, word, EQ, gt);
+            else finish(word, EQ, gt);
         }
     }
     // Philox calls made by this block -> one atomic
