@@ -24,21 +24,24 @@ struct MetropolisArgs {
     long long half;
 };
 
-// grid = (ceil(L*Lh/128), L, n_words); one thread = one word of the parity-p array in phase 0.
-// Phase 0: every thread gathers its word's six "unsatisfied" flags and runs chunk 0 (planes 0..7) of the compare.
-// About a quarter of the words still have a lane equal to its threshold prefix after 8 planes; they are queued in
-// shared memory and phase c runs chunk c for the queued words only, on the first threads of the block, so that whole
-// warps drop out instead of iterating beside one busy lane (the scheme of refresh_kernel).
+constexpr int kMetroBlock = 128;
+constexpr int kMetroSub = 4;          // groups of kMetroBlock words per block
+
+// grid = (ceil(L*Lh / (128 * kMetroSub)), L, n_words).
+// Phase 0: every thread gathers the six "unsatisfied" flags of its words (kMetroSub groups of 128 words per block)
+// and runs chunk 0 (planes 0..7) of the compare.  About a quarter of the words still have a lane equal to its
+// threshold prefix after 8 planes; they are queued in shared memory and phase c runs chunk c for the queued words
+// only, densely on the threads of the block -- one barrier per phase and block (the scheme of refresh_kernel).
 template <int RPW>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(kMetroBlock)
 metropolis_half_sweep_kernel(MetropolisArgs a, int p, PhiloxKeys ks, uint32_t tau, RefreshThr thr,
                              unsigned long long* __restrict__ n_calls)
 {
     typedef typename BondT<RPW>::type JT;
     constexpr int SPW = 32 / RPW;
-    constexpr int B = 128;
-    __shared__ uint32_t q_word[2][B];             // word index inside the plane
-    __shared__ uint32_t q_st[2][10][B];           // EQ[3], gt[3], need[3], s ^ always-part
+    constexpr int B = kMetroBlock, kQ = kMetroBlock * kMetroSub;
+    __shared__ uint32_t q_word[2][kQ];            // word index inside the plane
+    __shared__ uint32_t q_st[2][10][kQ];          // EQ[3], gt[3], need[3], spin word with the sure flips applied
     __shared__ int q_n[4];
     __shared__ unsigned int s_calls;
     if (threadIdx.x < 4) q_n[threadIdx.x] = 0;
@@ -61,85 +64,87 @@ metropolis_half_sweep_kernel(MetropolisArgs a, int p, PhiloxKeys ks, uint32_t ta
     wd.has_b = (vm >> 16) != 0u;
     const unsigned per_chunk = wd.has_b ? 2u : 1u;
     const uint32_t plane = (uint32_t)z * (uint32_t)L * (uint32_t)Lh;
+    const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
     unsigned int calls = 0;
 
+    auto finish = [&](int word, const uint32_t (&EQ)[3], const uint32_t (&gt)[3], const uint32_t (&need)[3], uint32_t s_acc) {
+        // u >= thr_k where the lane is above or equal in all planes seen; accept iff u < thr
+        uint32_t acc = 0u;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) acc |= need[k] & ~(gt[k] | EQ[k]);
+        sp[plane + (uint32_t)word] = s_acc ^ (acc & vm);
+    };
+    auto push = [&](int c, int word, const uint32_t (&EQ)[3], const uint32_t (&gt)[3], const uint32_t (&need)[3], uint32_t s_acc) {
+        const int slot = atomicAdd(&q_n[c], 1);
+        const int b = c & 1;
+        q_word[b][slot] = (uint32_t)word;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { q_st[b][k][slot] = EQ[k]; q_st[b][3 + k][slot] = gt[k]; q_st[b][6 + k][slot] = need[k]; }
+        q_st[b][9][slot] = s_acc;
+    };
+
 #pragma unroll 1
-    for (uint32_t c = 0; c < 4; ++c) {
-        int word = -1;
-        uint32_t EQ[3], gt[3] = { 0u, 0u, 0u }, need[3], s_acc = 0u;     // s_acc = s ^ (lanes that flip for sure)
-        if (c == 0) {
-            const int t = blockIdx.x * B + threadIdx.x;
-            if (t < L * Lh) {
-                word = t;
-                const int y = t / Lh, xh = t - y * Lh;
-                const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
-                const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
-                const uint32_t row = plane + (uint32_t)y * Lh, h = row + xh;
-                const uint32_t h_yp = plane + (uint32_t)yp * Lh + xh, h_ym = plane + (uint32_t)ym * Lh + xh;
-                const uint32_t h_zp = ((uint32_t)zp * L + y) * Lh + xh, h_zm = ((uint32_t)zm * L + y) * Lh + xh;
-                // c = 1: x = 2xh+1, -x neighbour at xh (it owns the bond), +x neighbour at xh+1
-                // c = 0: x = 2xh,   +x neighbour at xh, -x neighbour at xh-1 (it owns the bond)
-                const int cx = (y + z + p) & 1;
-                const int xo = cx ? ((xh + 1 == Lh) ? 0 : xh + 1) : ((xh == 0) ? Lh - 1 : xh - 1);
-                const uint32_t s = sp[h];
-                const uint32_t A = sq[h], E = sq[row + xo];
-                const uint32_t n_xp = cx ? E : A, n_xm = cx ? A : E;
-                const uint32_t j_xp = bond_expand<RPW>(Jb[(0 * 2 + p) * half + h]);
-                const uint32_t j_xm = bond_expand<RPW>(Jb[(0 * 2 + q) * half + (cx ? h : row + xo)]);
-                const uint32_t u1 = s ^ n_xp ^ j_xp, u2 = s ^ n_xm ^ j_xm;
-                const uint32_t u3 = s ^ sq[h_yp] ^ bond_expand<RPW>(Jb[(1 * 2 + p) * half + h]);
-                const uint32_t u4 = s ^ sq[h_ym] ^ bond_expand<RPW>(Jb[(1 * 2 + q) * half + h_ym]);
-                const uint32_t u5 = s ^ sq[h_zp] ^ bond_expand<RPW>(Jb[(2 * 2 + p) * half + h]);
-                const uint32_t u6 = s ^ sq[h_zm] ^ bond_expand<RPW>(Jb[(2 * 2 + q) * half + h_zm]);
-                // U = number of unsatisfied bonds, 3 planes
-                const uint32_t sa = u1 ^ u2 ^ u3, ca = (u1 & u2) | (u3 & (u1 ^ u2));
-                const uint32_t sb = u4 ^ u5 ^ u6, cb = (u4 & u5) | (u6 & (u4 ^ u5));
-                const uint32_t U0 = sa ^ sb, cc = sa & sb;
-                const uint32_t U1 = ca ^ cb ^ cc, U2 = (ca & cb) | (cc & (ca ^ cb));
-                const uint32_t always = U2 | (U1 & U0);                     // U >= 3: dH <= 0
-                need[0] = ~U2 & U1 & ~U0; need[1] = ~U2 & ~U1 & U0; need[2] = ~U2 & ~U1 & ~U0;   // U = 2, 1, 0: dH = 4, 8, 12
-                s_acc = s ^ (always & vm);
+    for (int sub = 0; sub < kMetroSub; ++sub) {
+        const int t = ((int)blockIdx.x * kMetroSub + sub) * B + (int)threadIdx.x;
+        if (t >= L * Lh) break;
+        const int y = t / Lh, xh = t - y * Lh;
+        const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
+        const uint32_t row = plane + (uint32_t)y * Lh, h = row + xh;
+        const uint32_t h_yp = plane + (uint32_t)yp * Lh + xh, h_ym = plane + (uint32_t)ym * Lh + xh;
+        const uint32_t h_zp = ((uint32_t)zp * L + y) * Lh + xh, h_zm = ((uint32_t)zm * L + y) * Lh + xh;
+        // c = 1: x = 2xh+1, -x neighbour at xh (it owns the bond), +x neighbour at xh+1
+        // c = 0: x = 2xh,   +x neighbour at xh, -x neighbour at xh-1 (it owns the bond)
+        const int cx = (y + z + p) & 1;
+        const int xo = cx ? ((xh + 1 == Lh) ? 0 : xh + 1) : ((xh == 0) ? Lh - 1 : xh - 1);
+        const uint32_t s = sp[h];
+        const uint32_t A = sq[h], E = sq[row + xo];
+        const uint32_t n_xp = cx ? E : A, n_xm = cx ? A : E;
+        const uint32_t j_xp = bond_expand<RPW>(Jb[(0 * 2 + p) * half + h]);
+        const uint32_t j_xm = bond_expand<RPW>(Jb[(0 * 2 + q) * half + (cx ? h : row + xo)]);
+        const uint32_t u1 = s ^ n_xp ^ j_xp, u2 = s ^ n_xm ^ j_xm;
+        const uint32_t u3 = s ^ sq[h_yp] ^ bond_expand<RPW>(Jb[(1 * 2 + p) * half + h]);
+        const uint32_t u4 = s ^ sq[h_ym] ^ bond_expand<RPW>(Jb[(1 * 2 + q) * half + h_ym]);
+        const uint32_t u5 = s ^ sq[h_zp] ^ bond_expand<RPW>(Jb[(2 * 2 + p) * half + h]);
+        const uint32_t u6 = s ^ sq[h_zm] ^ bond_expand<RPW>(Jb[(2 * 2 + q) * half + h_zm]);
+        // U = number of unsatisfied bonds, 3 planes
+        const uint32_t sa = u1 ^ u2 ^ u3, ca = (u1 & u2) | (u3 & (u1 ^ u2));
+        const uint32_t sb = u4 ^ u5 ^ u6, cb = (u4 & u5) | (u6 & (u4 ^ u5));
+        const uint32_t U0 = sa ^ sb, cc = sa & sb;
+        const uint32_t U1 = ca ^ cb ^ cc, U2 = (ca & cb) | (cc & (ca ^ cb));
+        const uint32_t always = U2 | (U1 & U0);                     // U >= 3: dH <= 0
+        const uint32_t need[3] = { ~U2 & U1 & ~U0, ~U2 & ~U1 & U0, ~U2 & ~U1 & ~U0 };   // U = 2, 1, 0: dH = 4, 8, 12
+        const uint32_t s_acc = s ^ (always & vm);
+        uint32_t EQ[3], gt[3] = { 0u, 0u, 0u };
 #pragma unroll
-                for (int k = 0; k < 3; ++k) EQ[k] = thr.never[k] ? 0u : (need[k] & vm);
-            }
-        } else {
-            __syncthreads();                      // queue c-1 is complete
-            const int n = q_n[c - 1];
-            if (n == 0) break;                    // block-uniform
-            if ((int)threadIdx.x < n) {
-                const int b = (c - 1) & 1;
-                word = (int)q_word[b][threadIdx.x];
-#pragma unroll
-                for (int k = 0; k < 3; ++k) {
-                    EQ[k] = q_st[b][k][threadIdx.x]; gt[k] = q_st[b][3 + k][threadIdx.x]; need[k] = q_st[b][6 + k][threadIdx.x];
-                }
-                s_acc = q_st[b][9][threadIdx.x];
-            }
+        for (int k = 0; k < 3; ++k) EQ[k] = thr.never[k] ? 0u : (need[k] & vm);
+        bool more = (EQ[0] | EQ[1] | EQ[2]) != 0u;
+        if (more) {
+            wd.i = canonical_site(L, p, z, y, xh);
+            refresh_chunk<0>(0u, wd, tau, EQ, gt, thr, ks);
+            calls += per_chunk;
+            more = (EQ[0] | EQ[1] | EQ[2]) != 0u;
         }
-        if (word >= 0) {
-            bool more = (EQ[0] | EQ[1] | EQ[2]) != 0u;
-            if (more) {
-                const int y = word / Lh, xh = word - y * Lh;
-                wd.i = canonical_site(L, p, z, y, xh);
-                if (c == 0) refresh_chunk<0>(0u, wd, tau, EQ, gt, thr, ks);
-                else        refresh_chunk<-1>(c, wd, tau, EQ, gt, thr, ks);
-                calls += per_chunk;
-                more = c < 3 && (EQ[0] | EQ[1] | EQ[2]) != 0u;
-            }
-            if (more) {
-                const int slot = atomicAdd(&q_n[c], 1);
-                const int b = c & 1;
-                q_word[b][slot] = (uint32_t)word;
+        if (more) push(0, t, EQ, gt, need, s_acc);
+        else finish(t, EQ, gt, need, s_acc);
+    }
+#pragma unroll 1
+    for (uint32_t c = 1; c < 4; ++c) {
+        __syncthreads();                          // queue c-1 is complete
+        const int n = q_n[c - 1];
+        if (n == 0) break;                        // block-uniform
+        const int b = (c - 1) & 1;
+        for (int e = threadIdx.x; e < n; e += B) {
+            const int word = (int)q_word[b][e];
+            uint32_t EQ[3], gt[3], need[3];
 #pragma unroll
-                for (int k = 0; k < 3; ++k) { q_st[b][k][slot] = EQ[k]; q_st[b][3 + k][slot] = gt[k]; q_st[b][6 + k][slot] = need[k]; }
-                q_st[b][9][slot] = s_acc;
-            } else {
-                // u >= thr_k where the lane is above or equal in all planes seen; accept iff u < thr
-                uint32_t acc = 0u;
-#pragma unroll
-                for (int k = 0; k < 3; ++k) acc |= need[k] & ~(gt[k] | EQ[k]);
-                sp[plane + (uint32_t)word] = s_acc ^ (acc & vm);
-            }
+            for (int k = 0; k < 3; ++k) { EQ[k] = q_st[b][k][e]; gt[k] = q_st[b][3 + k][e]; need[k] = q_st[b][6 + k][e]; }
+            const uint32_t s_acc = q_st[b][9][e];
+            const int y = word / Lh, xh = word - y * Lh;
+            wd.i = canonical_site(L, p, z, y, xh);
+            refresh_chunk<-1>(c, wd, tau, EQ, gt, thr, ks);
+            calls += per_chunk;
+            if (c < 3 && (EQ[0] | EQ[1] | EQ[2]) != 0u) push((int)c, word, EQ, gt, need, s_acc);
+            else finish(word, EQ, gt, need, s_acc);
         }
     }
     calls = __reduce_add_sync(0xFFFFFFFFu, calls);

@@ -434,7 +434,8 @@ int launch_metropolis_half_sweep(micsa_ctx* c, const RefreshThr& rt, uint32_t ta
     MetropolisArgs a;
     a.spin = c->st.spin; a.J = c->st.J; a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg;
     a.n_samples = g.n_samples; a.sample_offset = g.sample_offset; a.half = g.half;
-    const dim3 grid = site_blocks(g, g.n_words);
+    dim3 grid = site_blocks(g, g.n_words);
+    grid.x = (grid.x + kMetroSub - 1) / kMetroSub;           // kMetroSub groups of 128 words per block
     if (g.rpw == 2) metropolis_half_sweep_kernel<2><<<grid, 128, 0, c->stream>>>(a, parity, c->ks, tau, rt, c->calls);
     else            metropolis_half_sweep_kernel<1><<<grid, 128, 0, c->stream>>>(a, parity, c->ks, tau, rt, c->calls);
     c->attempts += (uint64_t)(g.N / 2) * (uint64_t)g.n_sys;
