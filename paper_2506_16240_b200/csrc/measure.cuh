@@ -115,6 +115,50 @@ __device__ __forceinline__ void block_warp_lane_counts(const uint32_t (&acc)[P],
     __syncthreads();
 }
 
+// Version for the measuring half-sweep launches (B = 128 threads, P planes per
+// thread): the four warps leave their planes in shared memory, ONE warp adds the
+// four vertical counters of each lane position (P + 2 planes), runs the shuffle
+// butterfly over its 32 threads and issues the 32 global atomics.  The caller
+// gives each of its counters to a different warp, so the block pays one butterfly
+// per counter instead of one per counter and warp, and its tail is one butterfly
+// long instead of three.  pl = [P][128] words of shared memory, filled by every
+// thread before the barrier that precedes this call.
+template <int P>
+__device__ __forceinline__ void warp_sum_lane_counts(const uint32_t (*pl)[128], int lane, unsigned long long* out)
+{
+    uint32_t c[P + 7];
+#pragma unroll
+    for (int k = 0; k < P + 7; ++k) c[k] = (k < P) ? pl[k][lane] : 0u;
+#pragma unroll
+    for (int wv = 1; wv < 4; ++wv) {
+        uint32_t carry = 0;
+#pragma unroll
+        for (int k = 0; k < P + 2; ++k) {
+            const uint32_t x = (k < P) ? pl[k][wv * 32 + lane] : 0u;
+            const uint32_t s = c[k] ^ x ^ carry;
+            carry = maj3(c[k], x, carry);
+            c[k] = s;
+        }
+    }
+#pragma unroll
+    for (int l = 0; l < 5; ++l) {
+        uint32_t carry = 0;
+#pragma unroll
+        for (int k = 0; k < P + 7; ++k) {
+            if (k <= P + 2 + l) {                   // planes above P + 2 + l are still zero
+                const uint32_t x = __shfl_xor_sync(0xFFFFFFFFu, c[k], 1 << l);
+                const uint32_t s = c[k] ^ x ^ carry;
+                carry = maj3(c[k], x, carry);
+                c[k] = s;
+            }
+        }
+    }
+    unsigned int mine = 0;
+#pragma unroll
+    for (int k = 0; k < P + 7; ++k) mine += ((c[k] >> lane) & 1u) << k;
+    if (mine) atomicAdd(&out[lane], (unsigned long long)mine);
+}
+
 struct MeasureArgs {
     const uint32_t* spin; const uint32_t* m0; const uint32_t* m1; const void* J;
     int L, Lh, n_rg, n_replicas, n_samples;

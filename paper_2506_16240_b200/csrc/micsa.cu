@@ -605,18 +605,20 @@ int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min, int dir)
     attr[0].val.programmaticStreamSerializationAllowed = c->use_pdl ? 1 : 0;
     cfg.attrs = attr; cfg.numAttrs = 1;
     if (zw == 4) {
-        LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 1>, a, 0, ma, fa));
-        if (dir > 0)      LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2, +1>, a, 1, ma, fa));
-        else if (dir < 0) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2, -1>, a, 1, ma, fa));
-        else              LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2>, a, 1, ma, fa));
+        LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 1>, a, 0, ma));
+        if (dir > 0)      LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2, +1>, a, 1, ma));
+        else if (dir < 0) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2, -1>, a, 1, ma));
+        else              LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2>, a, 1, ma));
     } else {
-        LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 1>, a, 0, ma, fa));
-        if (dir > 0)      LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2, +1>, a, 1, ma, fa));
-        else if (dir < 0) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2, -1>, a, 1, ma, fa));
-        else              LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2>, a, 1, ma, fa));
+        LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 1>, a, 0, ma));
+        if (dir > 0)      LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2, +1>, a, 1, ma));
+        else if (dir < 0) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2, -1>, a, 1, ma));
+        else              LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2>, a, 1, ma));
     }
+    cfg.gridDim = dim3(1);
+    LK(cudaLaunchKernelEx(&cfg, finalize_kernel, fa));
     c->attempts += (uint64_t)g.N * (uint64_t)g.n_sys;
-    return post_launch(c, 2);
+    return post_launch(c, 3);
 }
 
 // ---- small lattices: one cluster per word lattice walks through refresh + sweeps + rows (small.cuh) ----

@@ -696,14 +696,13 @@ half_sweep_pipe_kernel(SweepArgs a, int p, int walk_z)
 // differences); MEAS = 2: odd launch (also unsatisfied bonds) whose last CTA turns
 // the counts into the measurement row (finalize_rows) and re-zeroes them.
 // Same grids as half_sweep_pipe_kernel<RPW, 4, ZW>; every thread stays for the
-// block-wide reduction.
+// block-wide reduction (warp_sum_lane_counts: one shuffle butterfly per counter and block).
 template <int RPW, int ZW, int MEAS, int DIR = 0>
 __global__ void __launch_bounds__(128, 4)
-half_sweep_pipe_meas_kernel(SweepArgs a, int p, MeasureArgs ma, FinalizeArgs fa)
+half_sweep_pipe_meas_kernel(SweepArgs a, int p, MeasureArgs ma)
 {
     constexpr int YC = 4;
-    __shared__ unsigned int s_cnt[32];
-    __shared__ unsigned int s_last;
+    __shared__ uint32_t s_pl[MeasAcc<YC>::PU + MeasAcc<YC>::PM + MeasAcc<YC>::PX][128];
     const int L = a.L, Lh = a.Lh;
     const int nxv = Lh >> 2;
     const int t = (ZW == 1) ? (int)(blockIdx.x * blockDim.x + threadIdx.x)
@@ -723,23 +722,33 @@ half_sweep_pipe_meas_kernel(SweepArgs a, int p, MeasureArgs ma, FinalizeArgs fa)
         if ((z + p) & 1) march_rows_pipe<RPW, YC, 1, MEAS, DIR>(P, L, Lh, z, chunk * YC, xv * 4, nb, &acc, pair);
         else             march_rows_pipe<RPW, YC, 0, MEAS, DIR>(P, L, Lh, z, chunk * YC, xv * 4, nb, &acc, pair);
     }
-    if (MEAS == 2) block_warp_lane_counts<MeasAcc<YC>::PU, 128>(acc.u.c, s_cnt, ma.cntU + (long long)w * 32);
-    block_warp_lane_counts<MeasAcc<YC>::PM, 128>(acc.m.c, s_cnt, ma.cntM + (long long)w * 32);
-    if (pair) block_warp_lane_counts<MeasAcc<YC>::PX, 128>(acc.x.c, s_cnt, ma.cntX + (long long)(w / a.n_rg) * 32);
+    // planes -> shared memory; warp 0 sums the unsatisfied bonds, warp 1 the levels, warp 2 the replica differences
+    typedef MeasAcc<YC> Acc;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (MEAS == 2) {
-        // the last block to arrive finalises (its reads see every block's atomics)
-        __threadfence();
-        if (threadIdx.x == 0) {
-            const unsigned int total = gridDim.x * gridDim.y * gridDim.z;
-            s_last = (atomicAdd(fa.ticket, 1u) == total - 1u);
-        }
-        __syncthreads();
-        if (s_last) {
-            __threadfence();
-            finalize_rows(fa);
-            if (threadIdx.x == 0) *fa.ticket = 0u;
-        }
+#pragma unroll
+        for (int k = 0; k < Acc::PU; ++k) s_pl[k][tid] = acc.u.c[k];
     }
+#pragma unroll
+    for (int k = 0; k < Acc::PM; ++k) s_pl[Acc::PU + k][tid] = acc.m.c[k];
+    if (pair) {
+#pragma unroll
+        for (int k = 0; k < Acc::PX; ++k) s_pl[Acc::PU + Acc::PM + k][tid] = acc.x.c[k];
+    }
+    __syncthreads();
+    if (MEAS == 2 && warp == 0) warp_sum_lane_counts<Acc::PU>(s_pl, lane, ma.cntU + (long long)w * 32);
+    if (warp == 1) warp_sum_lane_counts<Acc::PM>(s_pl + Acc::PU, lane, ma.cntM + (long long)w * 32);
+    if (pair && warp == 2) warp_sum_lane_counts<Acc::PX>(s_pl + Acc::PU + Acc::PM, lane, ma.cntX + (long long)(w / a.n_rg) * 32);
+}
+
+// counts -> measurement row, after the odd measuring launch (one block; a ticket in that launch would cost every one
+// of its blocks a __threadfence behind its row stores)
+__global__ void __launch_bounds__(128)
+finalize_kernel(FinalizeArgs fa)
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    finalize_rows(fa);
 }
 
 }  // namespace micsa
