@@ -157,7 +157,7 @@ int micsa_half_sweep(micsa_ctx *ctx, int parity);
  * timestep using family alpha; micsa_refresh_demons redraws every family (the
  * family index sits in bits 20..23 of the Philox counter word that carries the
  * replica, so family 0 is the gamma = 1 refresh and n_replicas < 2^20);
- * E_daemon sums over the families; refreshes are not prefetched.
+ * E_daemon sums over the families; a prefetched refresh covers every family.
  * micsa_set_daemons / micsa_get_state address the family chosen with
  * micsa_select_daemon_set(alpha) (default 0).  With walkers on
  * (micsa_set_walkers(1)) family alpha wanders along the alpha-th direction of
@@ -210,8 +210,9 @@ int micsa_refresh_demons(micsa_ctx *ctx, double T, uint32_t step);
  * micsa_anneal prefetches step k+1 under the sweeps of step k by itself.
  * The side stream has the lowest priority: give the context a stream of higher
  * priority than the default (bench.py does) so that the generation only fills
- * what the sweeps leave idle.  A no-op when gamma > 1.  Asynchronous.  T must be
- * finite and > 0. */
+ * what the sweeps leave idle.  With gamma > 1 every family gets its own staging
+ * pair (allocated at the first prefetch: MICSA_ERR_NOMEM if that fails, nothing
+ * changed).  Asynchronous.  T must be finite and > 0. */
 int micsa_prefetch_refresh(micsa_ctx *ctx, double T, uint32_t step);
 
 /* micsa_effective_temperature (host arithmetic only): the temperature at which

@@ -136,6 +136,7 @@ struct micsa_ctx {
     int gamma;                 // daemon families per spin; family 0 lives in st.m0/m1
     int sel;                   // family that set_daemons / get_state address
     std::vector<uint32_t*> xm0, xm1;   // families 1 .. gamma-1 (library-owned)
+    std::vector<uint32_t*> xm0s, xm1s; // their staging planes for a prefetched refresh (allocated at the first one)
     int l2_groups;             // run multi-sweep calls lattice group by lattice group when the state exceeds L2
     bool small_attr_set;       // small lattices: kernel attributes (shared memory size, cluster size) set
     int small_items;           // small lattices: quad rows per CTA aimed at (0 = default)
@@ -472,40 +473,49 @@ uint32_t* family_m0(micsa_ctx* c, int alpha) { return alpha == 0 ? c->st.m0 : c-
 uint32_t* family_m1(micsa_ctx* c, int alpha) { return alpha == 0 ? c->st.m1 : c->xm1[alpha - 1]; }
 
 int launch_refresh(micsa_ctx* c, double T, uint32_t step) {
-    if (c->gamma > 1) {                         // every family, its index in the counter; no prefetch
-        for (int alpha = 0; alpha < c->gamma; ++alpha) {
-            const int rc = launch_refresh_into(c, T, step, family_m0(c, alpha), family_m1(c, alpha), c->stream, alpha);
-            if (rc) return rc;
-        }
-        c->rns += (uint64_t)c->gamma * (uint64_t)c->g.N * (uint64_t)c->g.n_sys;
-        return MICSA_OK;
-    }
+    const uint64_t drawn = (uint64_t)c->gamma * (uint64_t)c->g.N * (uint64_t)c->g.n_sys;
     if (c->pending && c->pending_step == step && memcmp(&c->pending_T, &T, sizeof T) == 0) {
         CK(c, cudaStreamWaitEvent(c->stream, c->ev_side, 0));
         std::swap(c->st.m0, c->m0s);
         std::swap(c->st.m1, c->m1s);
+        for (int alpha = 1; alpha < c->gamma; ++alpha) {
+            std::swap(c->xm0[alpha - 1], c->xm0s[alpha - 1]);
+            std::swap(c->xm1[alpha - 1], c->xm1s[alpha - 1]);
+        }
         c->pending = false;
-    } else {
-        const int rc = launch_refresh_into(c, T, step, c->st.m0, c->st.m1, c->stream);
-        if (rc) return rc;
+    } else {                                    // every family in place, its index in the counter
+        for (int alpha = 0; alpha < c->gamma; ++alpha) {
+            const int rc = launch_refresh_into(c, T, step, family_m0(c, alpha), family_m1(c, alpha), c->stream, alpha);
+            if (rc) return rc;
+        }
     }
-    c->rns += (uint64_t)c->g.N * (uint64_t)c->g.n_sys;
+    c->rns += drawn;
     return MICSA_OK;
 }
 
-// Queue the generation of refresh (T, step) into the staging planes on the side
-// stream; it starts once the main stream has reached this point (everything
-// that still reads the staging planes' previous role has finished).
+// Queue the generation of refresh (T, step) into the staging planes (of every
+// family) on the side stream; it starts once the main stream has reached this
+// point (everything that still reads the staging planes' previous role has
+// finished).
 int launch_prefetch(micsa_ctx* c, double T, uint32_t step) {
-    if (c->gamma > 1) return MICSA_OK;          // one staging pair only: gamma > 1 refreshes in place
     uint64_t thr[3];
     if (thresholds_host(T, thr) != MICSA_OK || thr[0] == 0) {
         set_err("temperature must be finite and > 0"); return MICSA_ERR_INVALID;
     }
+    while ((int)c->xm0s.size() < c->gamma - 1) {
+        void* a = nullptr; void* b = nullptr;
+        if (cudaMalloc(&a, c->plan.plane_bytes) != cudaSuccess || cudaMalloc(&b, c->plan.plane_bytes) != cudaSuccess) {
+            cudaGetLastError(); if (a) cudaFree(a); set_err("out of device memory (daemon family staging)"); return MICSA_ERR_NOMEM;
+        }
+        c->xm0s.push_back((uint32_t*)a); c->xm1s.push_back((uint32_t*)b);
+    }
     CK(c, cudaEventRecord(c->ev_main, c->stream));
     CK(c, cudaStreamWaitEvent(c->side, c->ev_main, 0));
-    const int rc = launch_refresh_into(c, T, step, c->m0s, c->m1s, c->side);
-    if (rc) return rc;
+    for (int alpha = 0; alpha < c->gamma; ++alpha) {
+        const int rc = launch_refresh_into(c, T, step, alpha == 0 ? c->m0s : c->xm0s[alpha - 1],
+                                           alpha == 0 ? c->m1s : c->xm1s[alpha - 1], c->side, alpha);
+        if (rc) return rc;
+    }
     CK(c, cudaEventRecord(c->ev_side, c->side));
     c->pending = true; c->pending_T = T; c->pending_step = step;
     return MICSA_OK;
@@ -904,6 +914,8 @@ int micsa_destroy(micsa_ctx* c) {
     if (c->c4_host) cudaFreeHost(c->c4_host);
     for (uint32_t* p : c->xm0) cudaFree(p);
     for (uint32_t* p : c->xm1) cudaFree(p);
+    for (uint32_t* p : c->xm0s) cudaFree(p);
+    for (uint32_t* p : c->xm1s) cudaFree(p);
     if (c->owns_ws) cudaFree(c->ws);
     cudaFreeHost(c->host_row);
     delete c;
@@ -1009,6 +1021,9 @@ int micsa_set_gamma(micsa_ctx* c, int gamma) {
     while ((int)c->xm0.size() > gamma - 1) {
         cudaFree(c->xm0.back()); cudaFree(c->xm1.back()); c->xm0.pop_back(); c->xm1.pop_back();
     }
+    while ((int)c->xm0s.size() > gamma - 1) {
+        cudaFree(c->xm0s.back()); cudaFree(c->xm1s.back()); c->xm0s.pop_back(); c->xm1s.pop_back();
+    }
     while ((int)c->xm0.size() < gamma - 1) {       // new families start at level 0, like family 0 at create
         void* a = nullptr; void* b = nullptr;
         if (cudaMalloc(&a, c->plan.plane_bytes) != cudaSuccess || cudaMalloc(&b, c->plan.plane_bytes) != cudaSuccess) {
@@ -1019,7 +1034,7 @@ int micsa_set_gamma(micsa_ctx* c, int gamma) {
         c->xm0.push_back((uint32_t*)a); c->xm1.push_back((uint32_t*)b);
     }
     c->gamma = gamma; c->sel = std::min(c->sel, gamma - 1);
-    c->pending = false;                           // a prefetched refresh belongs to the single-family path
+    c->pending = false;                           // a prefetched refresh was generated for the old number of families
     return MICSA_OK;
 }
 
