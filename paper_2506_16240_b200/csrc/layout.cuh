@@ -100,6 +100,12 @@ template <> __device__ __forceinline__ Vec<4> ldg_bonds<4, 2>(const uint16_t* p)
     return r;
 }
 
+// n / d by one multiply: m = ceil(2^32 / d) (host, d >= 2), q = umulhi(n, m) is exact whenever n * d <= 2^32
+// (the error of n * m / 2^32 against n / d is below n * d / (d * 2^32) <= 1 / d).  Every use here divides an index
+// inside one lattice plane (< L * L/2 < 2^20) by a row length (< 2^10).  d = 1: m = 0 and the quotient is n.
+inline uint32_t fastdiv_magic(uint32_t d) { return d >= 2 ? (uint32_t)(((1ull << 32) + d - 1) / d) : 0u; }
+__device__ __forceinline__ uint32_t fastdiv(uint32_t n, uint32_t m) { return m ? __umulhi(n, m) : n; }
+
 // canonical site index i = x + L*(y + L*z) of element xh of row (y,z), parity p
 __device__ __forceinline__ uint32_t canonical_site(int L, int p, int z, int y, int xh) {
     const int x = 2 * xh + ((y + z + p) & 1);

@@ -22,6 +22,7 @@ struct MetropolisArgs {
     uint32_t* spin; const void* J;
     int L, Lh, n_rg, n_samples, sample_offset;
     long long half;
+    uint32_t inv_Lh;         // fastdiv_magic(Lh)
 };
 
 constexpr int kMetroBlock = 128;
@@ -87,7 +88,7 @@ metropolis_half_sweep_kernel(MetropolisArgs a, int p, PhiloxKeys ks, uint32_t ta
     for (int sub = 0; sub < kMetroSub; ++sub) {
         const int t = ((int)blockIdx.x * kMetroSub + sub) * B + (int)threadIdx.x;
         if (t >= L * Lh) break;
-        const int y = t / Lh, xh = t - y * Lh;
+        const int y = (int)fastdiv((uint32_t)t, a.inv_Lh), xh = t - y * Lh;
         const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
         const uint32_t row = plane + (uint32_t)y * Lh, h = row + xh;
         const uint32_t h_yp = plane + (uint32_t)yp * Lh + xh, h_ym = plane + (uint32_t)ym * Lh + xh;
@@ -139,7 +140,7 @@ metropolis_half_sweep_kernel(MetropolisArgs a, int p, PhiloxKeys ks, uint32_t ta
 #pragma unroll
             for (int k = 0; k < 3; ++k) { EQ[k] = q_st[b][k][e]; gt[k] = q_st[b][3 + k][e]; need[k] = q_st[b][6 + k][e]; }
             const uint32_t s_acc = q_st[b][9][e];
-            const int y = word / Lh, xh = word - y * Lh;
+            const int y = (int)fastdiv((uint32_t)word, a.inv_Lh), xh = word - y * Lh;
             wd.i = canonical_site(L, p, z, y, xh);
             refresh_chunk<-1>(c, wd, tau, EQ, gt, thr, ks);
             calls += per_chunk;

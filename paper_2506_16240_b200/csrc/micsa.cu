@@ -173,7 +173,7 @@ int check_ctx(micsa_ctx* c) {
 
 SiteGrid site_grid(const Geom& g) {
     SiteGrid s; s.L = g.L; s.Lh = g.Lh; s.n_rg = g.n_rg; s.n_samples = g.n_samples;
-    s.sample_offset = g.sample_offset; s.half = g.half;
+    s.sample_offset = g.sample_offset; s.half = g.half; s.inv_Lh = fastdiv_magic((uint32_t)g.Lh);
     return s;
 }
 
@@ -193,7 +193,7 @@ template <int V, int RPW>
 void launch_half_sweep_t(micsa_ctx* c, int parity) {
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = 0;
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = 0; a.inv_nxv = fastdiv_magic((uint32_t)c->g.Lh / 4u);
     const int per_plane = c->g.L * (c->g.Lh / V);
     dim3 grid((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
     half_sweep_kernel<V, RPW><<<grid, 128, 0, c->stream>>>(a, parity);
@@ -205,7 +205,7 @@ template <int RPW>
 void launch_half_sweep_rows(micsa_ctx* c, int parity) {
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = 0;
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = 0; a.inv_nxv = fastdiv_magic((uint32_t)c->g.Lh / 4u);
     const int per_plane = (c->g.L / kRowsPerThread) * (c->g.Lh / 4);
     dim3 grid((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
     half_sweep_rows_kernel<RPW, kRowsPerThread><<<grid, 128, 0, c->stream>>>(a, parity);
@@ -219,7 +219,7 @@ template <int RPW>
 void launch_half_sweep_pipe(micsa_ctx* c, int parity, int dir = 0, int w0 = 0, int nw = -1) {
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = w0;
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = w0; a.inv_nxv = fastdiv_magic((uint32_t)c->g.Lh / 4u);
     const unsigned gz = (unsigned)(nw < 0 ? c->g.n_words : nw);
     const int yc = c->pipe_rows;
     const int per_plane = (c->g.L / yc) * (c->g.Lh / 4);
@@ -434,7 +434,7 @@ int launch_metropolis_half_sweep(micsa_ctx* c, const RefreshThr& rt, uint32_t ta
     const Geom& g = c->g;
     MetropolisArgs a;
     a.spin = c->st.spin; a.J = c->st.J; a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg;
-    a.n_samples = g.n_samples; a.sample_offset = g.sample_offset; a.half = g.half;
+    a.n_samples = g.n_samples; a.sample_offset = g.sample_offset; a.half = g.half; a.inv_Lh = fastdiv_magic((uint32_t)g.Lh);
     dim3 grid = site_blocks(g, g.n_words);
     grid.x = (grid.x + kMetroSub - 1) / kMetroSub;           // kMetroSub groups of 128 words per block
     if (g.rpw == 2) metropolis_half_sweep_kernel<2><<<grid, 128, 0, c->stream>>>(a, parity, c->ks, tau, rt, c->calls);
@@ -601,7 +601,7 @@ int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min, int dir)
     const Geom& g = c->g;
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg; a.half = g.half; a.w0 = 0;
+    a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg; a.half = g.half; a.w0 = 0; a.inv_nxv = fastdiv_magic((uint32_t)g.Lh / 4u);
     MeasureArgs ma; FinalizeArgs fa;
     make_measure_args(c, row, fold_min, ma, fa);
     const int per_plane = (g.L / 4) * (g.Lh / 4);
@@ -666,7 +666,7 @@ int launch_small_step(micsa_ctx* c, bool do_refresh, double T, uint32_t step, in
     const Geom& g = c->g;
     SmallArgs A;
     A.a.spin = c->st.spin; A.a.m0 = c->st.m0; A.a.m1 = c->st.m1; A.a.J = c->st.J;
-    A.a.L = g.L; A.a.Lh = g.Lh; A.a.n_rg = g.n_rg; A.a.half = g.half; A.a.w0 = 0;
+    A.a.L = g.L; A.a.Lh = g.Lh; A.a.n_rg = g.n_rg; A.a.half = g.half; A.a.w0 = 0; A.a.inv_nxv = fastdiv_magic((uint32_t)g.Lh / 4u);
     A.sg = site_grid(g);
     MeasureArgs ma; FinalizeArgs fa;
     make_measure_args(c, c->row, fold_min, ma, fa);

@@ -30,6 +30,7 @@ namespace micsa {
 struct SiteGrid {            // thread -> (plane index, z, lattice), see kernels
     int L, Lh, n_rg, n_samples, sample_offset;
     long long half;
+    uint32_t inv_Lh;         // fastdiv_magic(Lh)
 };
 
 // lanes of word-lattice sample group sg that hold a real sample
@@ -156,7 +157,7 @@ refresh_kernel(uint32_t* __restrict__ m0, uint32_t* __restrict__ m1, SiteGrid g,
         uint32_t EQ[3], gt[3] = { 0u, 0u, 0u };
 #pragma unroll
         for (int k = 0; k < 3; ++k) EQ[k] = thr.never[k] ? 0u : vm;
-        const int y = word / g.Lh, xh = word - y * g.Lh;
+        const int y = (int)fastdiv((uint32_t)word, g.inv_Lh), xh = word - y * g.Lh;
         wd.i = canonical_site(g.L, p, z, y, xh);
         refresh_chunk<0>(0u, wd, step, EQ, gt, thr, ks);
         calls += per_chunk;
@@ -174,7 +175,7 @@ refresh_kernel(uint32_t* __restrict__ m0, uint32_t* __restrict__ m1, SiteGrid g,
             uint32_t EQ[3], gt[3];
 #pragma unroll
             for (int k = 0; k < 3; ++k) { EQ[k] = q_st[b][k][e]; gt[k] = q_st[b][3 + k][e]; }
-            const int y = word / g.Lh, xh = word - y * g.Lh;
+            const int y = (int)fastdiv((uint32_t)word, g.inv_Lh), xh = word - y * g.Lh;
             wd.i = canonical_site(g.L, p, z, y, xh);
             refresh_chunk<-1>(c, wd, step, EQ, gt, thr, ks);
             calls += per_chunk;

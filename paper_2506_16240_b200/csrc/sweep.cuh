@@ -37,6 +37,7 @@ struct SweepArgs {
     int L, Lh, n_rg;
     long long half;
     int w0;                 // first word lattice of this launch (pipelined kernel: blockIdx.z + w0)
+    uint32_t inv_nxv;       // fastdiv_magic(Lh / 4) (pipelined kernels)
 };
 
 // One thread updates V consecutive words of one row (y,z) of the parity-p
@@ -677,7 +678,7 @@ half_sweep_pipe_kernel(SweepArgs a, int p, int walk_z)
     const bool active = t < (L / YC) * nxv;
     const unsigned mask = __ballot_sync(0xFFFFFFFFu, active);
     if (!active) return;
-    const int chunk = t / nxv, xv = t - chunk * nxv;
+    const int chunk = (int)fastdiv((uint32_t)t, a.inv_nxv), xv = t - chunk * nxv;
     const int w = blockIdx.z + a.w0;
     const PipeBase P = pipe_base<RPW>(a, w, p);
     XNb nb = x_neighbours(t, xv, nxv, mask, true);                // z is warp-uniform: one code path per warp
@@ -716,7 +717,7 @@ half_sweep_pipe_meas_kernel(SweepArgs a, int p, MeasureArgs ma)
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if (active) {
-        const int chunk = t / nxv, xv = t - chunk * nxv;
+        const int chunk = (int)fastdiv((uint32_t)t, a.inv_nxv), xv = t - chunk * nxv;
         const PipeBase P = pipe_base<RPW>(a, w, p);
         const XNb nb = x_neighbours(t, xv, nxv, mask, true);
         if ((z + p) & 1) march_rows_pipe<RPW, YC, 1, MEAS, DIR>(P, L, Lh, z, chunk * YC, xv * 4, nb, &acc, pair);

@@ -400,6 +400,41 @@ def test_prefetched_refresh_is_bit_identical(micsa, oracle):
         assert 0 < c["philox_calls"] <= 10 * L ** 3 * ns * nr // 4 + 10 * L ** 3 * 4
 
 
+def test_prefetched_refresh_covers_every_family(micsa, oracle):
+    """gamma > 1: a prefetched refresh is generated for every daemon family (own staging pair each) and swapped in
+    family by family; changing gamma drops a pending prefetch."""
+    L, ns, nr, seed, gamma = 8, 18, 2, 23, 3
+    s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+    m = np.zeros((gamma, ns, nr, L ** 3), np.uint8)
+
+    def check(g, n_fam):
+        for alpha in range(n_fam):
+            g.select_daemon_set(alpha)
+            _assert_state(g, s, m[alpha])
+
+    with micsa.MicSA(L, ns, nr, seed) as g:
+        g.set_gamma(gamma)
+        for k in range(3):
+            T = 1.5 - 0.3 * k
+            g.prefetch_refresh(T, k)
+            g.sweep(2)
+            for _ in range(2):
+                for alpha in range(gamma):
+                    oracle.sweep(L, s, m[alpha], J, 1)
+            check(g, gamma)                                   # the staging planes are not the state yet
+            g.refresh_demons(T, k)
+            for alpha in range(gamma):
+                oracle.refresh_alpha(L, m[alpha], seed, T, k, alpha)
+            check(g, gamma)
+        g.prefetch_refresh(0.7, 5)
+        g.set_gamma(2)                                        # the pending planes were made for three families
+        g.refresh_demons(0.7, 5)
+        for alpha in range(2):
+            oracle.refresh_alpha(L, m[alpha], seed, 0.7, 5, alpha)
+        check(g, 2)
+        assert g.counters()["rns_drawn"] == (3 * 3 + 2) * L ** 3 * ns * nr
+
+
 def test_measure_begin_end(micsa, oracle):
     """The split measurement returns the state at the point of _begin."""
     L, ns, nr = 8, 5, 2
