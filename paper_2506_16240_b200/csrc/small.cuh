@@ -142,13 +142,13 @@ __device__ __forceinline__ void slab_update_item(const SlabLayout<RPW>& S, uint3
         // c = 1: x = 2xh+1, the -x neighbour has the same xh, the +x one xh+1;  c = 0: x = 2xh, +x same xh, -x at xh-1
         const uint32_t up = (k < 3) ? aw[k + 1] : e, dn = (k > 0) ? aw[k - 1] : e;
         const uint32_t bdn = (k > 0) ? Bx[k - 1] : eJ;
-        const uint32_t nxp = (cm & up) | (~cm & aw[k]);
-        const uint32_t nxm = (cm & aw[k]) | (~cm & dn);
-        const uint32_t jxm = (cm & Bx[k]) | (~cm & bdn);
+        const uint32_t nxp = lop3<kSel>(cm, up, aw[k]);
+        const uint32_t nxm = lop3<kSel>(cm, aw[k], dn);
+        const uint32_t jxm = lop3<kSel>(cm, Bx[k], bdn);
         const uint32_t g = sv[k];
-        creutz_word20(g ^ nxp ^ jxo[k], g ^ nxm ^ jxm,
-                      g ^ ypv[k] ^ jyo[k], g ^ ymv[k] ^ jym[k],
-                      g ^ zpv[k] ^ jzo[k], g ^ zmv[k] ^ jzm[k],
+        creutz_word20(bond_flag(g, nxp, jxo[k]), bond_flag(g, nxm, jxm),
+                      bond_flag(g, ypv[k], jyo[k]), bond_flag(g, ymv[k], jym[k]),
+                      bond_flag(g, zpv[k], jzo[k]), bond_flag(g, zmv[k], jzm[k]),
                       sv[k], v0[k], v1[k]);
     }
     sts4(a_s, sv[0], sv[1], sv[2], sv[3]);

@@ -292,19 +292,33 @@ half_sweep_rows_kernel(SweepArgs a, int p)
 // V = m + U + 1 in [1, 10]; accept iff 3 <= m + U <= 6 iff 4 <= V <= 7 iff bit 2
 // of V is set and bit 3 is not -- and bit 3 set implies bit 2 clear here, so
 // accept = V2; new level m + U - 3 = V - 4 = bits 1:0 of V.
+// Every line below is one three-input logic operation, written as the LOP3 it is meant to be: left as C++ the
+// compiler re-associates the XOR chains (it forms neighbour ^ bond first and then needs two or three operations for
+// every sum and carry of the first adder level) and the 20 operations per word become 43.
+template <int LUT>
+__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(d) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+    return d;
+}
+constexpr int kXor3 = 0x96, kMaj3 = 0xE8, kSel = 0xCA /* a ? b : c */, kSelNot = 0x3A /* a ? ~b : c */;
+
+// unsatisfied-bond flag of one neighbour: own spin ^ neighbour spin ^ bond
+__device__ __forceinline__ uint32_t bond_flag(uint32_t g, uint32_t n, uint32_t j) { return lop3<kXor3>(g, n, j); }
+
 __device__ __forceinline__ void creutz_word20(uint32_t u1, uint32_t u2, uint32_t u3,
                                               uint32_t u4, uint32_t u5, uint32_t u6,
                                               uint32_t& sigma, uint32_t& m0, uint32_t& m1) {
-    const uint32_t sa = u1 ^ u2 ^ u3, ca = (u1 & u2) | (u3 & (u1 ^ u2));
-    const uint32_t sb = u4 ^ u5 ^ u6, cb = (u4 & u5) | (u6 & (u4 ^ u5));
-    const uint32_t t0 = sa ^ sb ^ m0, cd = (sa & sb) | (m0 & (sa ^ sb));    // weight 1 without the +1
+    const uint32_t sa = lop3<kXor3>(u1, u2, u3), ca = lop3<kMaj3>(u1, u2, u3);
+    const uint32_t sb = lop3<kXor3>(u4, u5, u6), cb = lop3<kMaj3>(u4, u5, u6);
+    const uint32_t t0 = lop3<kXor3>(sa, sb, m0), cd = lop3<kMaj3>(sa, sb, m0);   // weight 1 without the +1
     // + 1: V0 = ~t0 and a carry t0 into weight 2
-    const uint32_t s1 = ca ^ cb ^ cd, c1a = (ca & cb) | (cd & (ca ^ cb));
-    const uint32_t V1 = s1 ^ t0 ^ m1, c1b = (s1 & t0) | (m1 & (s1 ^ t0));
-    const uint32_t acc = c1a ^ c1b;                                         // V2 (V3 = c1a & c1b excludes it)
-    sigma ^= acc;
-    m0 = (acc & ~t0) | (~acc & m0);
-    m1 = (acc & V1) | (~acc & m1);
+    const uint32_t s1 = lop3<kXor3>(ca, cb, cd), c1a = lop3<kMaj3>(ca, cb, cd);
+    const uint32_t V1 = lop3<kXor3>(s1, t0, m1), c1b = lop3<kMaj3>(s1, t0, m1);
+    const uint32_t acc = c1a ^ c1b;                                              // V2 (V3 = c1a & c1b excludes it)
+    sigma = lop3<kXor3>(sigma, c1a, c1b);
+    m0 = lop3<kSelNot>(acc, t0, m0);
+    m1 = lop3<kSel>(acc, V1, m1);
 }
 
 struct PipeBase {           // block-uniform bases of lattice w: plane 0 of each parity array
@@ -536,9 +550,9 @@ __device__ __forceinline__ void update_row(const RowRegs<RPW>& r, const uint4& A
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         const uint32_t g = sv[k];
-        creutz_word20(g ^ nxp[k] ^ jxo[k], g ^ nxm[k] ^ jxm[k],
-                      g ^ yp[k] ^ jyo[k],  g ^ ym[k] ^ jym[k],
-                      g ^ zp[k] ^ jzo[k],  g ^ zm[k] ^ jzm[k],
+        creutz_word20(bond_flag(g, nxp[k], jxo[k]), bond_flag(g, nxm[k], jxm[k]),
+                      bond_flag(g, yp[k], jyo[k]),  bond_flag(g, ym[k], jym[k]),
+                      bond_flag(g, zp[k], jzo[k]),  bond_flag(g, zm[k], jzm[k]),
                       sv[k], v0[k], v1[k]);
     }
     st_off<uint4>(P.sp, o, make_uint4(sv[0], sv[1], sv[2], sv[3]));
