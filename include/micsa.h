@@ -207,10 +207,14 @@ int micsa_refresh_demons(micsa_ctx *ctx, double T, uint32_t step);
  * only waits for it and swaps plane pointers; any other (T, step) is generated
  * directly as usual, and the prefetched planes stay valid until consumed or
  * replaced by another prefetch.  Results are bit-identical either way.
- * micsa_anneal prefetches step k+1 under the sweeps of step k by itself.
- * The side stream has the lowest priority: give the context a stream of higher
- * priority than the default (bench.py does) so that the generation only fills
- * what the sweeps leave idle.  With gamma > 1 every family gets its own staging
+ * micsa_anneal prefetches step k+1 under the sweeps of step k by itself when
+ * the context's stream has a HIGHER priority than the default (bench.py and
+ * run_configs create one): the side stream has the lowest priority, so the
+ * generation then only fills what the sweeps leave idle.  On a stream of
+ * default priority the two grids would take turns block by block (measured:
+ * 366 us per step of config 4 instead of 243), so there micsa_anneal generates
+ * its refreshes in line (251 us); large lattices only -- beside the clusters of
+ * a small lattice most SMs are idle and the prefetch is always used.  With gamma > 1 every family gets its own staging
  * pair (allocated at the first prefetch: MICSA_ERR_NOMEM if that fails, nothing
  * changed).  Asynchronous.  T must be finite and > 0. */
 int micsa_prefetch_refresh(micsa_ctx *ctx, double T, uint32_t step);

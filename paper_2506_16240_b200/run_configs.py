@@ -50,9 +50,13 @@ def run(ci, scale):
             # measure at the end of every k-th refresh interval: measure_every counts sweeps inside a step
             k = max(1, me // R)
             sched = [(float(T), R, R if (i + 1) % k == 0 or i == steps - 1 else 0) for i in range(steps)]
-        with MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed) as warm:      # load the kernels once (lazy module loading)
+        # a stream above the default priority: the library's side stream (the next refresh) then only fills what
+        # the sweeps leave idle (include/micsa.h, micsa_prefetch_refresh)
+        import torch
+        stream = torch.cuda.Stream(priority=-1)
+        with MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed, stream=stream) as warm:   # load the kernels once (lazy module loading)
             warm.anneal(sched[:2], trace=False)
-        with MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed) as g:
+        with MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed, stream=stream) as g:
             g.synchronize()
             t0 = time.perf_counter()
             out = g.anneal(sched)
