@@ -250,11 +250,11 @@ def test_config1_state_after_every_sweep(micsa, oracle):
             _assert_state(g, s, m)
 
 
-def _sampled_parity(micsa, oracle, cfg, sched, samples, width):
+def _sampled_parity(micsa, oracle, cfg, sched, samples, width, stream=None):
     """Run `sched` on the full-size config on the GPU; the oracle re-runs only
     the sample blocks [k, k+width) for k in `samples` (sample_offset = k)."""
     L, nr = cfg.L, cfg.n_replicas
-    with micsa.MicSA(L, cfg.n_samples, nr, cfg.seed) as g:
+    with micsa.MicSA(L, cfg.n_samples, nr, cfg.seed, stream=stream) as g:
         E0, Ed0, _ = g.measure_i64()
         out = g.anneal(sched)
         gs, gm, gJ = g.get_state()
@@ -301,9 +301,35 @@ def test_config3_truncated(micsa, oracle, interval, n_sweeps, width):
 def test_config4_truncated(micsa, oracle):
     """The headline config at full size, in the launch configuration bench.py
     times (refresh + 10 sweeps + measure per step)."""
+    import torch
     cfg = CONFIGS[4]
     sched = schedule_for(cfg, n_sweeps=30, measure_every=10)
+    # on the default stream micsa_anneal generates its refreshes in line; on a stream above the default priority
+    # (what bench.py and run_configs use) it prefetches them on the side stream (include/micsa.h)
     _sampled_parity(micsa, oracle, cfg, sched, samples=(0, 14), width=2)
+    _sampled_parity(micsa, oracle, cfg, sched, samples=(1, 15), width=1, stream=torch.cuda.Stream(priority=-1))
+
+
+def test_anneal_on_a_high_priority_stream(micsa, oracle):
+    """micsa_anneal with its refreshes prefetched on the side stream (the context's stream outranks it): gamma = 1
+    and gamma = 3 with walkers, rows and every family against the oracle driver."""
+    import torch
+    L, ns, nr, seed = 16, 20, 2, 29
+    for gamma, walkers in ((1, False), (3, True)):
+        s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+        m = np.zeros((gamma, ns, nr, L ** 3), np.uint8)
+        sched = [(1.6, 4, 2), (1.2, 3, 3), (0.8, 5, 0), (0.5, 2, 1)]
+        ref = driver.anneal(L, s, m if gamma > 1 else m[0], J, seed, sched, step0=2, walkers=walkers)
+        stream = torch.cuda.Stream(priority=-1)
+        with micsa.MicSA(L, ns, nr, seed, stream=stream) as g:
+            g.set_gamma(gamma); g.set_walkers(1 if walkers else 0)
+            out = g.anneal(sched, step0=2)
+            for k in ("E", "Edem", "Q"):
+                np.testing.assert_array_equal(out[k], ref[k])
+            for alpha in range(gamma):
+                g.select_daemon_set(alpha)
+                _assert_state(g, s, m[alpha])
+            assert g.counters()["rns_drawn"] == len(sched) * gamma * L ** 3 * ns * nr
 
 
 def test_config5_truncated(micsa, oracle):
