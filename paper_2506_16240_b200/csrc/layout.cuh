@@ -100,6 +100,20 @@ template <> __device__ __forceinline__ Vec<4> ldg_bonds<4, 2>(const uint16_t* p)
     return r;
 }
 
+// One three-input logic operation, written as the LOP3 it is meant to be.  Left as C++ (in the update) the
+// compiler re-associates the XOR chains (it forms neighbour ^ bond first and then needs two or three operations for
+// every sum and carry of the first adder level) and the 20 operations per word become 43.
+template <int LUT>
+__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(d) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+    return d;
+}
+constexpr int kXor3 = 0x96, kMaj3 = 0xE8, kSel = 0xCA /* a ? b : c */, kSelNot = 0x3A /* a ? ~b : c */;
+
+// unsatisfied-bond flag of one neighbour: own spin ^ neighbour spin ^ bond
+__device__ __forceinline__ uint32_t bond_flag(uint32_t g, uint32_t n, uint32_t j) { return lop3<kXor3>(g, n, j); }
+
 // n / d by one multiply: m = ceil(2^32 / d) (host, d >= 2), q = umulhi(n, m) is exact whenever n * d <= 2^32
 // (the error of n * m / 2^32 against n / d is below n * d / (d * 2^32) <= 1 / d).  Every use here divides an index
 // inside one lattice plane (< L * L/2 < 2^20) by a row length (< 2^10).  d = 1: m = 0 and the quotient is n.

@@ -102,16 +102,16 @@ metropolis_half_sweep_kernel(MetropolisArgs a, int p, PhiloxKeys ks, uint32_t ta
         const uint32_t n_xp = cx ? E : A, n_xm = cx ? A : E;
         const uint32_t j_xp = bond_expand<RPW>(Jb[(0 * 2 + p) * half + h]);
         const uint32_t j_xm = bond_expand<RPW>(Jb[(0 * 2 + q) * half + (cx ? h : row + xo)]);
-        const uint32_t u1 = s ^ n_xp ^ j_xp, u2 = s ^ n_xm ^ j_xm;
-        const uint32_t u3 = s ^ sq[h_yp] ^ bond_expand<RPW>(Jb[(1 * 2 + p) * half + h]);
-        const uint32_t u4 = s ^ sq[h_ym] ^ bond_expand<RPW>(Jb[(1 * 2 + q) * half + h_ym]);
-        const uint32_t u5 = s ^ sq[h_zp] ^ bond_expand<RPW>(Jb[(2 * 2 + p) * half + h]);
-        const uint32_t u6 = s ^ sq[h_zm] ^ bond_expand<RPW>(Jb[(2 * 2 + q) * half + h_zm]);
-        // U = number of unsatisfied bonds, 3 planes
-        const uint32_t sa = u1 ^ u2 ^ u3, ca = (u1 & u2) | (u3 & (u1 ^ u2));
-        const uint32_t sb = u4 ^ u5 ^ u6, cb = (u4 & u5) | (u6 & (u4 ^ u5));
+        const uint32_t u1 = bond_flag(s, n_xp, j_xp), u2 = bond_flag(s, n_xm, j_xm);
+        const uint32_t u3 = bond_flag(s, sq[h_yp], bond_expand<RPW>(Jb[(1 * 2 + p) * half + h]));
+        const uint32_t u4 = bond_flag(s, sq[h_ym], bond_expand<RPW>(Jb[(1 * 2 + q) * half + h_ym]));
+        const uint32_t u5 = bond_flag(s, sq[h_zp], bond_expand<RPW>(Jb[(2 * 2 + p) * half + h]));
+        const uint32_t u6 = bond_flag(s, sq[h_zm], bond_expand<RPW>(Jb[(2 * 2 + q) * half + h_zm]));
+        // U = number of unsatisfied bonds, 3 planes (each line one LOP3, sweep.cuh)
+        const uint32_t sa = lop3<kXor3>(u1, u2, u3), ca = lop3<kMaj3>(u1, u2, u3);
+        const uint32_t sb = lop3<kXor3>(u4, u5, u6), cb = lop3<kMaj3>(u4, u5, u6);
         const uint32_t U0 = sa ^ sb, cc = sa & sb;
-        const uint32_t U1 = ca ^ cb ^ cc, U2 = (ca & cb) | (cc & (ca ^ cb));
+        const uint32_t U1 = lop3<kXor3>(ca, cb, cc), U2 = lop3<kMaj3>(ca, cb, cc);
         const uint32_t always = U2 | (U1 & U0);                     // U >= 3: dH <= 0
         const uint32_t need[3] = { ~U2 & U1 & ~U0, ~U2 & ~U1 & U0, ~U2 & ~U1 & ~U0 };   // U = 2, 1, 0: dH = 4, 8, 12
         const uint32_t s_acc = s ^ (always & vm);

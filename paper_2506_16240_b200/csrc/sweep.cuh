@@ -292,20 +292,7 @@ half_sweep_rows_kernel(SweepArgs a, int p)
 // V = m + U + 1 in [1, 10]; accept iff 3 <= m + U <= 6 iff 4 <= V <= 7 iff bit 2
 // of V is set and bit 3 is not -- and bit 3 set implies bit 2 clear here, so
 // accept = V2; new level m + U - 3 = V - 4 = bits 1:0 of V.
-// Every line below is one three-input logic operation, written as the LOP3 it is meant to be: left as C++ the
-// compiler re-associates the XOR chains (it forms neighbour ^ bond first and then needs two or three operations for
-// every sum and carry of the first adder level) and the 20 operations per word become 43.
-template <int LUT>
-__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
-    uint32_t d;
-    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(d) : "r"(a), "r"(b), "r"(c), "n"(LUT));
-    return d;
-}
-constexpr int kXor3 = 0x96, kMaj3 = 0xE8, kSel = 0xCA /* a ? b : c */, kSelNot = 0x3A /* a ? ~b : c */;
-
-// unsatisfied-bond flag of one neighbour: own spin ^ neighbour spin ^ bond
-__device__ __forceinline__ uint32_t bond_flag(uint32_t g, uint32_t n, uint32_t j) { return lop3<kXor3>(g, n, j); }
-
+// Every line below is one three-input logic operation, written as the LOP3 it is meant to be (layout.cuh, lop3).
 __device__ __forceinline__ void creutz_word20(uint32_t u1, uint32_t u2, uint32_t u3,
                                               uint32_t u4, uint32_t u5, uint32_t u6,
                                               uint32_t& sigma, uint32_t& m0, uint32_t& m1) {
