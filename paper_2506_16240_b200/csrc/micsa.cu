@@ -694,14 +694,23 @@ int launch_small_step(micsa_ctx* c, bool do_refresh, double T, uint32_t step, in
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = (unsigned)sh.cs; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    // function attributes are per device and sticky: set them once per context (shape never changes)
+    // Function attributes belong to the (device, kernel), not to the context: another context with a smaller slab
+    // must not lower what this one needs (a launch above the attribute fails with "invalid argument").  So every
+    // context raises them, once, to values no shape exceeds: the device's opt-in shared-memory maximum and the
+    // non-portable cluster size.
     if (!c->small_attr_set) {
+        int dev = 0, optin = 0;
+        CK(c, cudaGetDevice(&dev));
+        CK(c, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        cudaFuncAttributes fa;                     // the kernel's static shared memory counts against the maximum
         if (g.rpw == 2) {
-            if (sh.cs > 8) CK(c, cudaFuncSetAttribute(small_step_kernel<2>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-            CK(c, cudaFuncSetAttribute(small_step_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
+            CK(c, cudaFuncGetAttributes(&fa, small_step_kernel<2>));
+            CK(c, cudaFuncSetAttribute(small_step_kernel<2>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+            CK(c, cudaFuncSetAttribute(small_step_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes));
         } else {
-            if (sh.cs > 8) CK(c, cudaFuncSetAttribute(small_step_kernel<1>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-            CK(c, cudaFuncSetAttribute(small_step_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
+            CK(c, cudaFuncGetAttributes(&fa, small_step_kernel<1>));
+            CK(c, cudaFuncSetAttribute(small_step_kernel<1>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+            CK(c, cudaFuncSetAttribute(small_step_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes));
         }
         c->small_attr_set = true;
     }

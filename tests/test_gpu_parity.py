@@ -461,6 +461,29 @@ def test_prefetched_refresh_covers_every_family(micsa, oracle):
         assert g.counters()["rns_drawn"] == (3 * 3 + 2) * L ** 3 * ns * nr
 
 
+def test_small_lattice_contexts_of_different_shapes_side_by_side(micsa, oracle):
+    """Kernel attributes (dynamic shared memory, cluster size) belong to the device and the kernel, not to a context:
+    a context with a small slab must not lower what a live context with a larger one needs (the second launch of the
+    larger one used to fail with 'invalid argument')."""
+    shapes = [(16, 64, 2, 3), (8, 5, 2, 4), (32, 3, 2, 5)]
+    ctxs = [micsa.MicSA(L, ns, nr, seed) for L, ns, nr, seed in shapes]
+    try:
+        states = []
+        for (L, ns, nr, seed), g in zip(shapes, ctxs):
+            s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+            m = np.zeros_like(s, dtype=np.uint8)
+            g.refresh_demons(1.5, 0); oracle.refresh(L, m, seed, 1.5, 0)
+            states.append((s, m, J))
+        for _ in range(3):
+            for (L, ns, nr, seed), g, (s, m, J) in zip(shapes, ctxs, states):
+                g.sweep(2); oracle.sweep(L, s, m, J, 2)
+        for g, (s, m, J) in zip(ctxs, states):
+            _assert_state(g, s, m, J)
+    finally:
+        for g in ctxs:
+            g.destroy()
+
+
 def test_measure_begin_end(micsa, oracle):
     """The split measurement returns the state at the point of _begin."""
     L, ns, nr = 8, 5, 2
