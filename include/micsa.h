@@ -288,6 +288,35 @@ int micsa_measure_end(micsa_ctx *ctx, int64_t *E, int64_t *E_daemon, int64_t *Q)
 int micsa_measure(micsa_ctx *ctx, double *energy, double *demon_energy,
                   double *q_overlap);
 
+/* micsa_measure_noalloc: micsa_measure_i64 for callers that cannot allocate or
+ * synchronise (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc).  The same kernels as micsa_measure_begin, but their
+ * scratch -- the per-lane 64-bit counters and the ticket word -- lives in a
+ * file-scope `static __device__` array of the library instead of the context's
+ * workspace, and the row goes to a buffer the caller owns:
+ *   ctx    input: the context's state at this point in stream order (created
+ *          and filled beforehand; micsa_create* does allocate).
+ *   d_row  output, DEVICE memory, int64 [2 n_sys + n_pairs]:
+ *          E[n_sys] | E_daemon[n_sys] | Q[n_pairs], the sums and order of
+ *          micsa_measure_i64 (E_daemon over all gamma families).  Anything but
+ *          device / managed memory -> MICSA_ERR_INVALID.
+ * Asynchronous on the context's stream; the call itself performs no cudaMalloc,
+ * cudaFree, host allocation, memcpy or stream synchronisation (two
+ * cudaMemsetAsync of the scratch and the measurement launches, nothing else).
+ * Limit: the array holds MICSA_NOALLOC_MAX_COUNTERS counters (128 KiB + one
+ * 256-byte ticket line, resident on every GPU that loads the library until
+ * exit).  A context needs 64 per word lattice + 32 per (sample group, replica
+ * pair): n_words = ceil(n_samples / (32 / rpw)) * n_replicas / rpw, rpw = 2
+ * for even n_replicas, else 1 -- all five BASELINE configurations fit (96, 384,
+ * 768, 96 and 2 048 counters); more -> MICSA_ERR_INVALID, nothing launched.
+ * The array is shared by every context and stream on a device and keeps the
+ * last call's contents: each call clears what it uses first, and two calls
+ * that OVERLAP on the GPU (different streams, or graphs replayed
+ * concurrently) race on it -- order them.  It does not touch the scratch of the
+ * other measurement calls, which may run concurrently with it. */
+#define MICSA_NOALLOC_MAX_COUNTERS 16384
+int micsa_measure_noalloc(micsa_ctx *ctx, int64_t *d_row);
+
 /* micsa_anneal: for k = 0..n_steps-1: refresh(T_k, step0 + k); n_sweeps_k
  * sweeps with measurement rows as micsa_step says.  The whole schedule is
  * queued without host synchronisation; rows are kept on the device and copied

@@ -32,6 +32,7 @@ EXPORTS = (
     "micsa_measure", "micsa_anneal", "micsa_counters", "micsa_layout_info",
     "micsa_set_tuning",
     "micsa_prefetch_refresh", "micsa_measure_begin", "micsa_measure_end", "micsa_sweep_measure",
+    "micsa_measure_noalloc",
     "micsa_measure_c4", "micsa_xi", "micsa_effective_temperature", "micsa_metropolis_sweep", "micsa_metropolis_half_sweep", "micsa_debug_metropolis_thresholds",
     "micsa_set_gamma", "micsa_select_daemon_set",
     "micsa_wander", "micsa_set_walkers", "micsa_set_time", "micsa_get_time",
@@ -108,6 +109,7 @@ def _bind() -> ctypes.CDLL:
             ("micsa_prefetch_refresh", [vp, f64, u32]),
             ("micsa_debug_thresholds", [f64, vp]), ("micsa_debug_philox", [u64, vp, i32, vp]), ("micsa_effective_temperature", [f64, vp]),
             ("micsa_measure_i64", [vp, vp, vp, vp]),
+            ("micsa_measure_noalloc", [vp, vp]),
             ("micsa_measure_c4", [vp, vp]), ("micsa_xi", [vp, i32, f64, vp, vp, vp]), ("micsa_measure_begin", [vp]), ("micsa_measure_end", [vp, vp, vp, vp]), ("micsa_measure", [vp, vp, vp, vp]),
             ("micsa_anneal", [vp, vp, i32, u32, vp, vp]),
             ("micsa_counters", [vp, vp, vp, vp]), ("micsa_layout_info", [vp, vp]),
@@ -310,6 +312,23 @@ class MicSA:
         Q = np.empty(self.n_pairs, np.int64) if self.n_replicas >= 2 else None
         _check(_lib.micsa_measure_i64(self._h, _ptr(E), _ptr(Ed), _ptr(Q)))
         return E, Ed, (Q if Q is not None else np.empty(0, np.int64))
+
+    @property
+    def row_len(self) -> int:
+        """int64 elements of a measurement row: E[n_sys] | E_daemon[n_sys] | Q[n_pairs]."""
+        return 2 * self.n_sys + self.n_pairs
+
+    def measure_noalloc(self, row):
+        """micsa_measure_noalloc: queue the measurement into `row`, a caller-owned contiguous torch.int64 CUDA tensor
+        of at least row_len elements (or an integer device address).  Nothing is allocated, copied or synchronised;
+        the sums are in row[:n_sys], row[n_sys:2 n_sys], row[2 n_sys:row_len] once the stream gets there."""
+        if isinstance(row, int):
+            ptr = row
+        else:
+            if str(row.dtype) != "torch.int64" or not row.is_cuda or not row.is_contiguous() or row.numel() < self.row_len:
+                raise MicsaError(MICSA_ERR_INVALID, "row must be a contiguous torch.int64 CUDA tensor of >= row_len elements")
+            ptr = row.data_ptr()
+        _check(_lib.micsa_measure_noalloc(self._h, ctypes.c_void_p(ptr)))
 
     def measure_c4(self):
         """S[pair, axis, r] = sum_x q_x q_{x + r e_axis} (exact int64), r = 0..L/2, for every replica pair a < b of

@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstring>
 #include <limits>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -30,6 +31,38 @@ thread_local char g_err[256] = "";
 
 void set_err(const char* fmt, const char* detail = "") {
     snprintf(g_err, sizeof g_err, fmt, detail);
+}
+
+}  // namespace
+
+// ---- scratch of micsa_measure_noalloc (include/micsa.h): counters + ticket of the measurement kernels ----
+// Lives in the module image: every GPU that loads the library holds these 128.25 KiB until exit, and every
+// context on a device shares them.  In HOST code the name below is a host-side stand-in, not a device address;
+// noalloc_scratch() asks the runtime for the address on the current device (cudaGetSymbolAddress) once per
+// device and that pointer is what the kernels get.
+constexpr size_t kNoAllocCounters = MICSA_NOALLOC_MAX_COUNTERS;     // 64-bit lane counters (cntU | cntM | cntX)
+constexpr size_t kNoAllocTicket = 32;                               // one 256-byte line for the ticket word
+static __device__ __align__(256) unsigned long long g_noalloc_scratch[kNoAllocCounters + kNoAllocTicket];
+
+namespace {
+
+// device address of g_noalloc_scratch on the CURRENT device; queried once per device ordinal
+cudaError_t noalloc_scratch(unsigned long long** out) {
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static unsigned long long* cache[kMaxDev] = {};
+    *out = nullptr;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev >= 0 && dev < kMaxDev && cache[dev]) { *out = cache[dev]; return cudaSuccess; }
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < kMaxDev) cache[dev] = (unsigned long long*)p;
+    *out = (unsigned long long*)p;
+    return cudaSuccess;
 }
 
 }  // namespace
@@ -122,6 +155,7 @@ struct micsa_ctx {
     uint32_t* m0s; uint32_t* m1s;             // staging planes (swapped with st.m0/m1 when consumed)
     cudaStream_t side;                        // generates prefetched refreshes under the sweeps
     bool side_below;                          // the context's stream has a higher priority than the side stream
+    unsigned long long* noalloc;              // device address of g_noalloc_scratch on this context's device (or null)
     cudaEvent_t ev_main, ev_side;
     bool pending; double pending_T; uint32_t pending_step;
     bool measure_queued;                      // micsa_measure_begin without its _end yet
@@ -894,6 +928,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->stage_dev = nullptr; c->stage_bytes = 0;
     c->c4_dev = nullptr; c->c4_bytes = 0; c->c4_host = nullptr; c->c4_host_bytes = 0;
     c->host_row = nullptr; c->side = nullptr; c->ev_main = nullptr; c->ev_side = nullptr;
+    c->noalloc = nullptr;
     if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_main, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_side, cudaEventDisableTiming) != cudaSuccess) {
@@ -908,6 +943,9 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
                         cudaStreamGetPriority(c->side, &p_side) == cudaSuccess && p_main < p_side;
         cudaGetLastError();
     }
+    // set-up for micsa_measure_noalloc: the static scratch array's address on this device (no allocation; a failure
+    // is not fatal here, the call itself reports it)
+    if (noalloc_scratch(&c->noalloc) != cudaSuccess) { cudaGetLastError(); c->noalloc = nullptr; }
     if (cudaHostAlloc((void**)&c->host_row, c->plan.row_len * 8, cudaHostAllocDefault) != cudaSuccess) {
         cudaGetLastError(); set_err("out of pinned host memory");
         destroy_side(c); if (c->owns_ws) cudaFree(c->ws); delete c; return nullptr;
@@ -1199,6 +1237,35 @@ int micsa_measure_i64(micsa_ctx* c, int64_t* E, int64_t* Ed, int64_t* Q) {
     if (Q && c->g.n_replicas < 2) { set_err("q_overlap needs n_replicas >= 2"); return MICSA_ERR_INVALID; }
     rc = micsa_measure_begin(c); if (rc) return rc;
     return micsa_measure_end(c, E, Ed, Q);
+}
+
+// The measurement with its counters and ticket in the library's static scratch array instead of the context's
+// workspace, the row written to the caller's DEVICE buffer: no allocation, no host synchronisation, no copy.
+int micsa_measure_noalloc(micsa_ctx* c, int64_t* d_row) {
+    int rc = check_ctx(c); if (rc) return rc;
+    if (!d_row) { set_err("null pointer"); return MICSA_ERR_INVALID; }
+    if (!c->noalloc) { set_err("the address of the static scratch array could not be obtained on this device"); return MICSA_ERR_CUDA; }
+    const size_t need = c->plan.cnt_words;
+    if (need > kNoAllocCounters) {
+        char msg[160];
+        snprintf(msg, sizeof msg, "this context needs %zu lane counters, the static scratch of micsa_measure_noalloc holds %zu "
+                 "(MICSA_NOALLOC_MAX_COUNTERS)", need, kNoAllocCounters);
+        set_err("%s", msg); return MICSA_ERR_INVALID;
+    }
+    cudaPointerAttributes pa;
+    if (cudaPointerGetAttributes(&pa, d_row) != cudaSuccess ||
+        (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged)) {
+        cudaGetLastError(); set_err("d_row must be device (or managed) memory"); return MICSA_ERR_INVALID;
+    }
+    // the array keeps whatever the last call (of any context on this device) left: counters and ticket start at zero
+    CK(c, cudaMemsetAsync(c->noalloc, 0, need * sizeof(unsigned long long), c->stream));
+    CK(c, cudaMemsetAsync(c->noalloc + kNoAllocCounters, 0, kNoAllocTicket * sizeof(unsigned long long), c->stream));
+    // the same launches as micsa_measure_begin, with the scratch pointers exchanged for the duration of the call
+    unsigned long long* const cnt0 = c->cnt; unsigned int* const ticket0 = c->ticket;
+    c->cnt = c->noalloc; c->ticket = reinterpret_cast<unsigned int*>(c->noalloc + kNoAllocCounters);
+    rc = launch_measure(c, reinterpret_cast<long long*>(d_row), false);
+    c->cnt = cnt0; c->ticket = ticket0;
+    return rc;
 }
 
 int micsa_measure_c4(micsa_ctx* c, int64_t* S) {
