@@ -29,11 +29,20 @@ def _per_sweep_parity(micsa, oracle, cfg, T, interval, n_sweeps, blocks, width, 
         J = oracle.init_bonds(L, width, seed, sample_offset=k)
         ref.append((k, s, np.zeros_like(s, dtype=np.uint8), J))
 
-    def compare(g, what):
+    from concurrent.futures import ThreadPoolExecutor
+    pool = ThreadPoolExecutor(1)
+
+    def compare(g, what, oracle_step):
+        # the oracle's step runs on a host thread (its calls release the GIL) while the library's state comes back
+        fut = pool.submit(oracle_step)
         gs, gm, _ = g.get_state(couplings=False)
+        fut.result()
         for k, s, m, _ in ref:
-            np.testing.assert_array_equal(gs[k:k + width], s, err_msg=f"spins, samples {k}.., {what}")
-            np.testing.assert_array_equal(gm[k:k + width], m, err_msg=f"daemons, samples {k}.., {what}")
+            # (np.array_equal first: assert_array_equal is several times slower on 131 MB arrays; it writes the report)
+            if not np.array_equal(gs[k:k + width], s):
+                np.testing.assert_array_equal(gs[k:k + width], s, err_msg=f"spins, samples {k}.., {what}")
+            if not np.array_equal(gm[k:k + width], m):
+                np.testing.assert_array_equal(gm[k:k + width], m, err_msg=f"daemons, samples {k}.., {what}")
 
     with micsa.MicSA(L, cfg.n_samples, nr, seed) as g:
         for key, v in (tune or {}).items():
@@ -47,18 +56,14 @@ def _per_sweep_parity(micsa, oracle, cfg, T, interval, n_sweeps, blocks, width, 
                 g.refresh_demons(T, r)
                 if t + interval < n_sweeps:
                     g.prefetch_refresh(T, r + 1)          # generated under the sweeps, as bench.py does
-                for k, _, m, _ in ref:
-                    oracle.refresh(L, m, seed, T, r, k)
-                compare(g, f"after refresh {r}")
+                compare(g, f"after refresh {r}", lambda: [oracle.refresh(L, m, seed, T, r, k) for k, _, m, _ in ref])
             last_of_group = (t + 1) % interval == 0
             if last_of_group:
                 g.sweep_measure(1)
                 E, Ed, Q = g.measure_end()
             else:
                 g.sweep(1)
-            for _, s, m, J in ref:
-                oracle.sweep(L, s, m, J, 1)
-            compare(g, f"after sweep {t + 1}")
+            compare(g, f"after sweep {t + 1}", lambda: [oracle.sweep(L, s, m, J, 1) for _, s, m, J in ref])
             if last_of_group:
                 for k, s, m, J in ref:
                     oE, oEd, oQ = oracle.measure(L, s, m, J)
@@ -67,6 +72,7 @@ def _per_sweep_parity(micsa, oracle, cfg, T, interval, n_sweeps, blocks, width, 
                     np.testing.assert_array_equal(Ed[sl], oEd)
                     if nr == 2:
                         np.testing.assert_array_equal(Q[k:k + width], oQ)
+    pool.shutdown()
 
 
 def test_config4_every_sample_every_sweep(micsa, oracle):
@@ -307,17 +313,24 @@ def test_table3_shape_sampled(micsa, oracle, l2_groups):
 def test_largest_lattice_offsets_beyond_2_31_bytes(micsa, oracle):
     """Maximum size: L = 1040 (N = 1.125e9 sites, just below the 2^31 limit of the 32-bit site index; a parity array
     holds 2.25 GB, so the kernels' unsigned 32-bit byte offsets go beyond 2^31).  One sample x two replicas: the Philox
-    start, one refresh, one sweep, the separate and the fused measurement against the oracle, every site.  About three
+    start, one refresh, one sweep, the separate and the fused measurement against the oracle, every site.  About two
     minutes, mostly the oracle; 20 GB of host memory."""
+    from concurrent.futures import ThreadPoolExecutor
     L, ns, nr, seed, T = 1040, 1, 2, 3, 0.9
-    s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
-    m = np.zeros_like(s, dtype=np.uint8)
-    with micsa.MicSA(L, ns, nr, seed) as g:
+    # the oracle's start, bonds and refresh do not depend on one another: three host threads (the calls release the
+    # GIL), the library's own start and first sweep meanwhile
+    m = np.zeros((ns, nr, L ** 3), np.uint8)
+    with ThreadPoolExecutor(3) as pool, micsa.MicSA(L, ns, nr, seed) as g:
+        f_s = pool.submit(oracle.init_spins, L, ns, nr, seed)
+        f_J = pool.submit(oracle.init_bonds, L, ns, seed)
+        f_m = pool.submit(oracle.refresh, L, m, seed, T, 7)
         gs, gm, gJ = g.get_state()
-        assert np.array_equal(gs, s) and np.array_equal(gJ, J) and not gm.any()
-        del gJ
         g.refresh_demons(T, 7); g.sweep(1)
-        oracle.refresh(L, m, seed, T, 7); oracle.sweep(L, s, m, J, 1)
+        s, J = f_s.result(), f_J.result()
+        assert np.array_equal(gs, s) and np.array_equal(gJ, J) and not gm.any()
+        del gJ, gs, gm
+        f_m.result()
+        oracle.sweep(L, s, m, J, 1)
         gs, gm, _ = g.get_state(couplings=False)
         assert np.array_equal(gs, s) and np.array_equal(gm, m)
         del gs, gm
