@@ -340,3 +340,40 @@ def test_largest_lattice_offsets_beyond_2_31_bytes(micsa, oracle):
         g.sweep_measure(1); E2, Ed2, _ = g.measure_end()
         np.testing.assert_array_equal(E2 + Ed2, E + Ed)           # PAPER.md:124 at this size too
         assert g.counters()["attempts"] == 2 * L ** 3 * ns * nr
+
+
+@pytest.mark.parametrize("L,ns,nr", [(62, 33, 2), (100, 17, 1), (50, 40, 3), (36, 70, 2)])
+def test_lattices_off_the_fast_path_at_medium_size(micsa, oracle, L, ns, nr):
+    """L not a multiple of 8 (the kernels with 1 or 2 words per thread; L = 36: 4 words but no pipelined kernel), ragged
+    sample counts, 1 / 2 / 3 replicas, at sizes where a plane no longer fits a block: start, two refreshes, sweeps,
+    wandering, Metropolis and both measurement paths against the oracle, every site."""
+    seed, T = 9, 1.1
+    s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+    m = np.zeros_like(s, dtype=np.uint8)
+
+    def same(g, with_J=False):
+        gs, gm, gJ = g.get_state(couplings=with_J)
+        assert np.array_equal(gs, s) and np.array_equal(gm, m) and (not with_J or np.array_equal(gJ, J))
+
+    with micsa.MicSA(L, ns, nr, seed) as g:
+        same(g, True)
+        for r in range(2):
+            g.prefetch_refresh(T - 0.3 * r, r); g.refresh_demons(T - 0.3 * r, r); oracle.refresh(L, m, seed, T - 0.3 * r, r)
+            g.sweep(2); oracle.sweep(L, s, m, J, 2)
+            same(g)
+            g.sweep_measure(1); E, Ed, Q = g.measure_end(); oracle.sweep(L, s, m, J, 1)
+            oE, oEd, oQ = oracle.measure(L, s, m, J)
+            np.testing.assert_array_equal(E, oE); np.testing.assert_array_equal(Ed, oEd)
+            if nr >= 2:
+                np.testing.assert_array_equal(Q, oQ)
+        t0 = g.get_time()
+        g.set_walkers(1); g.sweep(3)
+        for t in range(3):
+            oracle.sweep(L, s, m, J, 1); oracle.wander(L, m, 0, +1, (t0 + t) & 1)
+        same(g)
+        g.set_walkers(0)
+        g.metropolis_sweep(1.3, 5, 2); oracle.metropolis_checkerboard(L, s, J, seed, 1.3, 5, 2)
+        same(g)
+        E, Ed, Q = g.measure_i64()
+        oE, oEd, oQ = oracle.measure(L, s, m, J)
+        np.testing.assert_array_equal(E, oE); np.testing.assert_array_equal(Ed, oEd)
