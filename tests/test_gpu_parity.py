@@ -484,6 +484,31 @@ def test_small_lattice_contexts_of_different_shapes_side_by_side(micsa, oracle):
             g.destroy()
 
 
+@pytest.mark.parametrize("nr", [1, 2])
+def test_largest_sample_offsets(micsa, oracle, nr):
+    """Global sample indices up to 2^31 - 17 (the Philox block word carries sample >> 4 below the chunk bits, the start
+    uses sample >> 7): start, refresh, sweeps, Metropolis against the oracle; a block beyond 2^31 - 1 is refused."""
+    L, ns, seed = 8, 48, 77
+    off = 2 ** 31 - 64                                   # the last three blocks of 16 below the limit
+    s = oracle.init_spins(L, ns, nr, seed, off); J = oracle.init_bonds(L, ns, seed, off)
+    m = np.zeros_like(s, dtype=np.uint8)
+    with micsa.MicSA(L, ns, nr, seed, sample_offset=off) as g:
+        _assert_state(g, s, m, J)
+        for small in (1, 0):
+            g.set_tuning("small_path", small)
+            g.refresh_demons(0.8, 2 ** 32 - 1 - small); oracle.refresh(L, m, seed, 0.8, 2 ** 32 - 1 - small, off)
+            g.sweep(3); oracle.sweep(L, s, m, J, 3)
+            _assert_state(g, s, m)
+        out = g.anneal([(1.4, 2, 1), (1.0, 2, 2)], step0=5)
+        ref = driver.anneal(L, s, m, J, seed, [(1.4, 2, 1), (1.0, 2, 2)], step0=5, sample_offset=off)
+        for k in ("E", "Edem", "Q"):
+            np.testing.assert_array_equal(out[k], ref[k])
+        g.metropolis_sweep(1.7, 3, 2); oracle.metropolis_checkerboard(L, s, J, seed, 1.7, 3, 2, off)
+        _assert_state(g, s, m)
+    with pytest.raises(micsa.MicsaError):
+        micsa.MicSA(L, ns + 16, nr, seed, sample_offset=off)
+
+
 def test_measure_begin_end(micsa, oracle):
     """The split measurement returns the state at the point of _begin."""
     L, ns, nr = 8, 5, 2
