@@ -64,15 +64,28 @@ int gcheck(micsa_gauss_ctx* c) {
     return MICSA_OK;
 }
 
-struct GGeom { int L, Lh; long long half; };
+struct GGeom { int L, Lh; long long half; uint32_t inv_Lh, inv_L; };   // inv_d = ceil(2^32 / d), 0 for d = 1
+
+// n / d and n % d for any n < 2^32 by one multiply and a correction: q' = umulhi(n, ceil(2^32 / d)) overshoots n / d
+// by less than n / 2^32 < 1, so it is the quotient or one more (a 32-bit division costs ~36 instructions, and the
+// refresh and wandering kernels of this file are bound by instruction issue)
+inline uint32_t gdiv_magic(uint32_t d) { return d >= 2 ? (uint32_t)(((1ull << 32) + d - 1) / d) : 0u; }
+__device__ __forceinline__ uint32_t gdivmod(uint32_t n, uint32_t d, uint32_t inv, uint32_t& rem) {
+    if (inv == 0u) { rem = 0u; return n; }
+    uint32_t q = __umulhi(n, inv);
+    uint32_t r = n - q * d;
+    if ((int32_t)r < 0) { q -= 1u; r += d; }
+    rem = r;
+    return q;
+}
 
 // thread -> site of parity p: t = (z L + y) Lh + xh (32-bit arithmetic: half = L^3 / 2 < 2^30)
 __device__ __forceinline__ bool site_of(const GGeom& g, long long t, int p, int& xh, int& y, int& z, int& c) {
     if (t >= g.half) return false;
-    const uint32_t tt = (uint32_t)t, Lh = (uint32_t)g.Lh, L = (uint32_t)g.L;
-    const uint32_t r = tt / Lh;
-    xh = (int)(tt - r * Lh);
-    z = (int)(r / L); y = (int)(r - (uint32_t)z * L);
+    uint32_t rx, ry;
+    const uint32_t r = gdivmod((uint32_t)t, (uint32_t)g.Lh, g.inv_Lh, rx);
+    z = (int)gdivmod(r, (uint32_t)g.L, g.inv_L, ry);
+    xh = (int)rx; y = (int)ry;
     c = (y + z + p) & 1;
     return true;
 }
@@ -341,7 +354,11 @@ gauss_overlap_kernel(const int8_t* __restrict__ spin, long long n, const int* __
     if ((threadIdx.x & 31) == 0 && diff) atomicAdd(&cnt[blockIdx.y], (unsigned long long)diff);
 }
 
-GGeom ggeom(const micsa_gauss_ctx* c) { GGeom g; g.L = c->L; g.Lh = c->Lh; g.half = c->half; return g; }
+GGeom ggeom(const micsa_gauss_ctx* c) {
+    GGeom g; g.L = c->L; g.Lh = c->Lh; g.half = c->half;
+    g.inv_Lh = gdiv_magic((uint32_t)c->Lh); g.inv_L = gdiv_magic((uint32_t)c->L);
+    return g;
+}
 unsigned gblocks(const micsa_gauss_ctx* c) { return (unsigned)((c->half + 255) / 256); }
 
 int greserve(micsa_gauss_ctx* c, size_t bytes) {
