@@ -362,9 +362,11 @@ int micsa_layout_info(micsa_ctx *ctx, uint64_t info[5]);
  *   sweeps runs all of them on one group of word lattices (independent systems) that fits in L2 before
  *   touching the next group, 0 = every half-sweep over all lattices.
  * key MICSA_TUNE_SMALL_PATH: 1 (default) = on small lattices (L a multiple of 8, L*L*L/8 <= 8192 quad rows,
- *   n_replicas <= 2, one daemon per spin) micsa_sweep, micsa_sweep_measure and every schedule step of
- *   micsa_anneal run as ONE launch in which each word lattice is walked by a thread-block cluster (refresh, all
- *   sweeps and the measurement rows; cluster barriers instead of kernel boundaries), 0 = the general path.
+ *   n_replicas <= 2, one daemon per spin) micsa_sweep, micsa_sweep_measure and up to eight consecutive schedule
+ *   steps of micsa_anneal run as ONE launch in which each word lattice is walked by a thread-block cluster (all
+ *   sweeps and the measurement rows; cluster barriers instead of kernel boundaries; the steps' refreshes are
+ *   generated beforehand into staging planes, 2 x 8 plane pairs allocated at the first such micsa_anneal:
+ *   MICSA_ERR_NOMEM if that fails), 0 = the general path.
  * key MICSA_TUNE_SMALL_ITEMS: quad rows per CTA and parity the small-lattice path aims at when it chooses the cluster
  *   size (1 .. 16 CTAs per word lattice): 0 = default, else 1 .. 1024.
  * key MICSA_TUNE_PDL: 1 (default) = kernel 2 is launched with programmatic

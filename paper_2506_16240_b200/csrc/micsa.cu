@@ -156,6 +156,7 @@ struct micsa_ctx {
     cudaStream_t side;                        // generates prefetched refreshes under the sweeps
     bool side_below;                          // the context's stream has a higher priority than the side stream
     unsigned long long* noalloc;              // device address of g_noalloc_scratch on this context's device (or null)
+    char* chain_buf;                          // refreshed planes of chained small-lattice steps (micsa_anneal), or null
     cudaEvent_t ev_main, ev_side;
     bool pending; double pending_T; uint32_t pending_step;
     bool measure_queued;                      // micsa_measure_begin without its _end yet
@@ -694,10 +695,12 @@ bool small_eligible(const micsa_ctx* c) {
     return c->small_path && g.n_replicas <= 2 && c->gamma == 1 && !c->walkers && small_shape(c).ok;
 }
 
-// do_refresh: Eq. (11) at (T, step) first; then n_sweeps sweeps; a measurement row after every measure_every-th
-// sweep (0 = none) into rows[row0 ...] (row index >= rows_cap: into the context's scratch row)
-int launch_small_step(micsa_ctx* c, bool do_refresh, double T, uint32_t step, int n_sweeps, int measure_every,
-                      long long* rows, long long row0, long long rows_cap, bool fold_min) {
+// One link of a chain of schedule steps walked by a single launch (small.cuh): the planes holding the step's
+// refreshed daemon levels (nullptr: the state's own), its sweeps and its measurement interval.
+struct SmallLink { const uint32_t* m0; const uint32_t* m1; int n_sweeps, measure_every; };
+
+int launch_small_chain(micsa_ctx* c, bool do_refresh, double T, uint32_t step, const SmallLink* links, int n_links,
+                       long long* rows, long long row0, long long rows_cap, bool fold_min) {
     const Geom& g = c->g;
     SmallArgs A;
     A.a.spin = c->st.spin; A.a.m0 = c->st.m0; A.a.m1 = c->st.m1; A.a.J = c->st.J;
@@ -711,7 +714,14 @@ int launch_small_step(micsa_ctx* c, bool do_refresh, double T, uint32_t step, in
     A.n_calls = c->calls;
     A.n_words = g.n_words;
     A.do_refresh = do_refresh ? 1 : 0; A.step = step; A.alpha_bits = 0u;
-    A.n_sweeps = n_sweeps; A.measure_every = measure_every;
+    A.n_chain = n_links;
+    long long total_sweeps = 0;
+    for (int j = 0; j < kSmallChain; ++j) {
+        const bool in = j < n_links;
+        A.ch_m0[j] = in ? links[j].m0 : nullptr; A.ch_m1[j] = in ? links[j].m1 : nullptr;
+        A.ch_sweeps[j] = in ? links[j].n_sweeps : 0; A.ch_every[j] = in ? links[j].measure_every : 0;
+        total_sweeps += A.ch_sweeps[j];
+    }
     A.n_samples = g.n_samples; A.n_replicas = g.n_replicas; A.rpw = g.rpw; A.spw = g.spw; A.N = g.N;
     RefreshThr rt = {};
     if (do_refresh) {
@@ -750,9 +760,31 @@ int launch_small_step(micsa_ctx* c, bool do_refresh, double T, uint32_t step, in
     }
     if (g.rpw == 2) CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<2>, A, c->ks, rt));
     else            CK(c, cudaLaunchKernelEx(&cfg, small_step_kernel<1>, A, c->ks, rt));
-    c->attempts += (uint64_t)n_sweeps * (uint64_t)g.N * (uint64_t)g.n_sys;
-    c->t += n_sweeps;
+    c->attempts += (uint64_t)total_sweeps * (uint64_t)g.N * (uint64_t)g.n_sys;
+    c->t += total_sweeps;
     return post_launch(c);
+}
+
+// do_refresh: Eq. (11) at (T, step) first; then n_sweeps sweeps; a measurement row after every measure_every-th
+// sweep (0 = none) into rows[row0 ...] (row index >= rows_cap: into the context's scratch row)
+int launch_small_step(micsa_ctx* c, bool do_refresh, double T, uint32_t step, int n_sweeps, int measure_every,
+                      long long* rows, long long row0, long long rows_cap, bool fold_min) {
+    const SmallLink one = { nullptr, nullptr, n_sweeps, measure_every };
+    return launch_small_chain(c, do_refresh, T, step, &one, 1, rows, row0, rows_cap, fold_min);
+}
+
+// Staging planes of the chained small-lattice steps of micsa_anneal: two sets of kSmallChain plane pairs (one being
+// read by the running launch, one being generated on the side stream), allocated at the first chained call.
+int chain_reserve(micsa_ctx* c) {
+    if (c->chain_buf) return MICSA_OK;
+    const size_t need = (size_t)2 * kSmallChain * 2 * c->plan.plane_bytes;
+    if (cudaMalloc((void**)&c->chain_buf, need) != cudaSuccess) {
+        cudaGetLastError(); c->chain_buf = nullptr; set_err("out of device memory (chained refresh planes)"); return MICSA_ERR_NOMEM;
+    }
+    return MICSA_OK;
+}
+uint32_t* chain_plane(micsa_ctx* c, int set, int j, int which) {
+    return (uint32_t*)(c->chain_buf + ((size_t)(set * kSmallChain + j) * 2 + which) * c->plan.plane_bytes);
 }
 
 // n sweeps, then one measurement into `row`
@@ -928,7 +960,7 @@ micsa_ctx* micsa_create_ex(int L, int n_samples, int n_replicas, uint64_t seed,
     c->stage_dev = nullptr; c->stage_bytes = 0;
     c->c4_dev = nullptr; c->c4_bytes = 0; c->c4_host = nullptr; c->c4_host_bytes = 0;
     c->host_row = nullptr; c->side = nullptr; c->ev_main = nullptr; c->ev_side = nullptr;
-    c->noalloc = nullptr;
+    c->noalloc = nullptr; c->chain_buf = nullptr;
     if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_main, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_side, cudaEventDisableTiming) != cudaSuccess) {
@@ -966,6 +998,7 @@ int micsa_destroy(micsa_ctx* c) {
     destroy_side(c);
     if (c->trace_dev) cudaFree(c->trace_dev);
     if (c->stage_dev) cudaFree(c->stage_dev);
+    if (c->chain_buf) cudaFree(c->chain_buf);
     if (c->c4_dev) cudaFree(c->c4_dev);
     if (c->c4_host) cudaFreeHost(c->c4_host);
     for (uint32_t* p : c->xm0) cudaFree(p);
@@ -1395,18 +1428,66 @@ int micsa_anneal(micsa_ctx* c, const micsa_step* sched, int n_steps, uint32_t st
     std::vector<int64_t> row_sweep;
     std::vector<double> row_T;
     long long r = 0, t = 0;
+    bool chain_ready = false; int chain_first = 0, chain_n = 0, chain_set = 0;   // refreshes generated ahead (small lattices)
     for (int k = 0; k < n_steps; ++k) {
-        if (small_eligible(c) && sched[k].n_sweeps > 0) {     // small lattice: the whole step in one cluster launch
+        if (small_eligible(c) && sched[k].n_sweeps > 0) {     // small lattice: whole steps in one cluster launch
+            // The clusters of a small lattice leave most SMs idle: when that is so, up to kSmallChain steps go into
+            // ONE launch (the lattice stays in shared memory across them) and their refreshes are generated by the
+            // stand-alone kernel into staging planes -- the first batch's on this stream, every later batch's on the
+            // side stream beside the launch before it.
+            auto chain_len = [&](int from) {
+                int n = 0;
+                while (from + n < n_steps && n < kSmallChain && sched[from + n].n_sweeps > 0) ++n;
+                return n;
+            };
+            if (c->g.n_words * small_shape(c).cs * 2 <= c->sms) {
+                rc = chain_reserve(c); if (rc) return rc;
+                const int n = chain_len(k);
+                if (!(chain_ready && chain_first == k && chain_n == n)) {          // nothing generated ahead: do it in line
+                    chain_set = 0;
+                    for (int j = 0; j < n; ++j) {
+                        rc = launch_refresh_into(c, sched[k + j].T, step0 + (uint32_t)(k + j), chain_plane(c, chain_set, j, 0),
+                                                 chain_plane(c, chain_set, j, 1), c->stream);
+                        if (rc) return rc;
+                    }
+                } else {
+                    CK(c, cudaStreamWaitEvent(c->stream, c->ev_side, 0));
+                }
+                chain_ready = false;
+                const int n2 = chain_len(k + n);
+                if (n2 > 0) {                              // the next batch, under this one; the set it overwrites was
+                    CK(c, cudaEventRecord(c->ev_main, c->stream));      // read by the launch before this one
+                    CK(c, cudaStreamWaitEvent(c->side, c->ev_main, 0));
+                    for (int j = 0; j < n2; ++j) {
+                        rc = launch_refresh_into(c, sched[k + n + j].T, step0 + (uint32_t)(k + n + j),
+                                                 chain_plane(c, chain_set ^ 1, j, 0), chain_plane(c, chain_set ^ 1, j, 1), c->side);
+                        if (rc) return rc;
+                    }
+                    CK(c, cudaEventRecord(c->ev_side, c->side));
+                }
+                SmallLink links[kSmallChain];
+                for (int j = 0; j < n; ++j)
+                    links[j] = { chain_plane(c, chain_set, j, 0), chain_plane(c, chain_set, j, 1), sched[k + j].n_sweeps,
+                                 sched[k + j].measure_every };
+                rc = launch_small_chain(c, false, 0.0, 0u, links, n, (long long*)dev_rows.dev, r, keep, true);
+                if (rc) return rc;
+                c->rns += (uint64_t)n * (uint64_t)g.N * (uint64_t)g.n_sys;
+                for (int j = 0; j < n; ++j) {
+                    const int me = sched[k + j].measure_every, n_rows = me > 0 ? sched[k + j].n_sweeps / me : 0;
+                    for (int i = 1; i <= n_rows; ++i)
+                        if (r + i - 1 < keep) { row_sweep.push_back(t + (long long)i * me); row_T.push_back(sched[k + j].T); }
+                    r += n_rows; t += sched[k + j].n_sweeps;
+                }
+                if (n2 > 0) { chain_ready = true; chain_first = k + n; chain_n = n2; chain_set ^= 1; }
+                k += n - 1;
+                continue;
+            }
+            // many lattices (no idle SMs to generate beside): one step per launch, refreshed inside the kernel
             const int me = sched[k].measure_every, n_rows = me > 0 ? sched[k].n_sweeps / me : 0;
             const bool prefetched = c->pending && c->pending_step == step0 + (uint32_t)k &&
                                     memcmp(&c->pending_T, &sched[k].T, sizeof(double)) == 0;
             if (prefetched) { rc = launch_refresh(c, sched[k].T, step0 + (uint32_t)k); if (rc) return rc; }
             else c->rns += (uint64_t)g.N * (uint64_t)g.n_sys;
-            // the clusters of a small lattice leave most SMs idle: the NEXT step's refresh is generated beside them by
-            // the stand-alone kernel on the side stream (into the staging planes) instead of inside the next launch
-            if (k + 1 < n_steps && sched[k + 1].n_sweeps > 0 && c->g.n_words * small_shape(c).cs * 2 <= c->sms) {
-                rc = launch_prefetch(c, sched[k + 1].T, step0 + (uint32_t)k + 1u); if (rc) return rc;
-            }
             rc = launch_small_step(c, !prefetched, sched[k].T, step0 + (uint32_t)k, sched[k].n_sweeps, me,
                                    (long long*)dev_rows.dev, r, keep, true);
             if (rc) return rc;

@@ -22,6 +22,8 @@
 
 namespace micsa {
 
+constexpr int kSmallChain = 8;   // schedule steps one launch can walk through
+
 struct SmallArgs {
     SweepArgs a;                 // state of all word lattices (w0 unused)
     SiteGrid sg;                 // refresh: sample offsets
@@ -33,7 +35,13 @@ struct SmallArgs {
     unsigned long long* n_calls; // Philox calls (device counter)
     int n_words, cs;             // word lattices, CTAs per cluster
     int do_refresh; uint32_t step; uint32_t alpha_bits;
-    int n_sweeps, measure_every; // measure after every measure_every-th sweep (0 = never)
+    // The launch walks through n_chain schedule steps.  Step j first takes its daemon levels from the planes
+    // ch_m0[j] / ch_m1[j] (a refresh generated beforehand by refresh_kernel; nullptr, step 0 only: the levels the
+    // state holds, refreshed here if do_refresh), then does ch_sweeps[j] sweeps and measures after every
+    // ch_every[j]-th of them (0 = never).
+    int n_chain;
+    const uint32_t* ch_m0[kSmallChain]; const uint32_t* ch_m1[kSmallChain];
+    int ch_sweeps[kSmallChain], ch_every[kSmallChain];
     int n_samples, n_replicas, rpw, spw;
     long long N;
 };
@@ -288,12 +296,8 @@ small_step_kernel(SmallArgs A, PhiloxKeys ks, RefreshThr thr)
     for (int p = 0; p < 2; ++p) {
         const long long go = ((long long)w * 2 + p) * half + (long long)z0 * PW;
         const uint4* gs = reinterpret_cast<const uint4*>(A.a.spin + go);
-        const uint4* g0 = reinterpret_cast<const uint4*>(A.a.m0 + go);
-        const uint4* g1 = reinterpret_cast<const uint4*>(A.a.m1 + go);
         uint4* ss = reinterpret_cast<uint4*>(smem + S.spin(p));
-        uint4* s0 = reinterpret_cast<uint4*>(smem + S.m0(p));
-        uint4* s1 = reinterpret_cast<uint4*>(smem + S.m1(p));
-        for (int i = tid; i < slab_words / 4; i += nthr) { ss[i] = gs[i]; s0[i] = g0[i]; s1[i] = g1[i]; }
+        for (int i = tid; i < slab_words / 4; i += nthr) ss[i] = gs[i];
         // bonds: PW * sizeof(JT) bytes per plane, a multiple of 16 (Lh % 4 == 0 and L even)
         const int jq = (int)((size_t)slab_words * sizeof(JT) / 16), pq = (int)((size_t)PW * sizeof(JT) / 16);
         const uint4* gx = reinterpret_cast<const uint4*>(Jb + (0 * 2 + p) * half + (long long)z0 * PW);
@@ -306,46 +310,63 @@ small_step_kernel(SmallArgs A, PhiloxKeys ks, RefreshThr thr)
         for (int i = tid; i < jq; i += nthr) { sx[i] = gx[i]; sy[i] = gy[i]; sz[pq + i] = gz[i]; }
         for (int i = tid; i < pq; i += nthr) sz[i] = gzm[i];
     }
-    __syncthreads();
-
-    if (A.do_refresh) {
-        unsigned calls = 0;
-        for (int u = tid; u < 2 * slab_words; u += nthr) {
-            const int p = (u >= slab_words) ? 1 : 0;
-            calls += slab_refresh_word<RPW>(A, ks, thr, S, smem, w, z0, p, u - p * slab_words);
-        }
-        calls = __reduce_add_sync(0xFFFFFFFFu, calls);
-        if ((threadIdx.x & 31) == 0 && calls) atomicAdd(A.n_calls, (unsigned long long)calls);
-    }
-    cluster_sync_all();                                               // every CTA's slab is in place
     const int items = ZP * L * nq;                                    // quad rows per parity of this CTA
     long long r = A.row0;
-    for (int t = 1; t <= A.n_sweeps; ++t) {
-        for (int p = 0; p < 2; ++p) {
-            for (int it = tid; it < items; it += nthr) slab_update_item<RPW>(S, sm, L, Lh, z0, rank, cs, p, it);
-            cluster_sync_all();
+#pragma unroll 1
+    for (int j = 0; j < A.n_chain; ++j) {
+        // ---- this step's daemon levels: global -> shared.  Nobody reads the CTA's daemon planes any more: the last
+        // half-sweep and the last measurement of the previous step ended with a cluster barrier.
+        {
+            const uint32_t* src0 = A.ch_m0[j] ? A.ch_m0[j] : A.a.m0;
+            const uint32_t* src1 = A.ch_m1[j] ? A.ch_m1[j] : A.a.m1;
+            for (int p = 0; p < 2; ++p) {
+                const long long go = ((long long)w * 2 + p) * half + (long long)z0 * PW;
+                const uint4* g0 = reinterpret_cast<const uint4*>(src0 + go);
+                const uint4* g1 = reinterpret_cast<const uint4*>(src1 + go);
+                uint4* s0 = reinterpret_cast<uint4*>(smem + S.m0(p));
+                uint4* s1 = reinterpret_cast<uint4*>(smem + S.m1(p));
+                for (int i = tid; i < slab_words / 4; i += nthr) { s0[i] = g0[i]; s1[i] = g1[i]; }
+            }
         }
-        if (A.measure_every > 0 && t % A.measure_every == 0) {
-            VCount<kMeasurePlanes> accU, accM, accX; accU.clear(); accM.clear(); accX.clear();
-            for (int u = tid; u < 2 * items; u += nthr) {
-                const int p = (u >= items) ? 1 : 0;
-                ItemSums Sm;
-                if (pair) slab_measure_item<RPW, true>(S, sm, L, Lh, z0, rank, cs, p, u - p * items, Sm);
-                else      slab_measure_item<RPW, false>(S, sm, L, Lh, z0, rank, cs, p, u - p * items, Sm);
-                accU.add(Sm.u); accM.add(Sm.m);
-                if (pair) accX.add(Sm.x);
+        __syncthreads();
+        if (j == 0 && A.do_refresh) {
+            unsigned calls = 0;
+            for (int u = tid; u < 2 * slab_words; u += nthr) {
+                const int p = (u >= slab_words) ? 1 : 0;
+                calls += slab_refresh_word<RPW>(A, ks, thr, S, smem, w, z0, p, u - p * slab_words);
             }
-            block_warp_lane_counts<kMeasurePlanes, 512>(accU.c, s_cnt, A.ma.cntU + (long long)w * 32);
-            block_warp_lane_counts<kMeasurePlanes, 512>(accM.c, s_cnt, A.ma.cntM + (long long)w * 32);
-            if (pair) block_warp_lane_counts<kMeasurePlanes, 512>(accX.c, s_cnt, A.ma.cntX + (long long)(w / A.a.n_rg) * 32);
-            __threadfence();
-            cluster_sync_all();
-            if (rank == 0) {
-                long long* row = (r < A.rows_cap) ? A.rows + r * A.row_len : A.scratch_row;
-                small_finalize_lattice(A, w, row);
+            calls = __reduce_add_sync(0xFFFFFFFFu, calls);
+            if ((threadIdx.x & 31) == 0 && calls) atomicAdd(A.n_calls, (unsigned long long)calls);
+        }
+        cluster_sync_all();                                           // every CTA's slab is in place
+        const int n_sweeps = A.ch_sweeps[j], every = A.ch_every[j];
+        for (int t = 1; t <= n_sweeps; ++t) {
+            for (int p = 0; p < 2; ++p) {
+                for (int it = tid; it < items; it += nthr) slab_update_item<RPW>(S, sm, L, Lh, z0, rank, cs, p, it);
+                cluster_sync_all();
             }
-            ++r;
-            // the counters are zero again before anybody adds to them: two cluster barriers (the next sweep) lie between
+            if (every > 0 && t % every == 0) {
+                VCount<kMeasurePlanes> accU, accM, accX; accU.clear(); accM.clear(); accX.clear();
+                for (int u = tid; u < 2 * items; u += nthr) {
+                    const int p = (u >= items) ? 1 : 0;
+                    ItemSums Sm;
+                    if (pair) slab_measure_item<RPW, true>(S, sm, L, Lh, z0, rank, cs, p, u - p * items, Sm);
+                    else      slab_measure_item<RPW, false>(S, sm, L, Lh, z0, rank, cs, p, u - p * items, Sm);
+                    accU.add(Sm.u); accM.add(Sm.m);
+                    if (pair) accX.add(Sm.x);
+                }
+                block_warp_lane_counts<kMeasurePlanes, 512>(accU.c, s_cnt, A.ma.cntU + (long long)w * 32);
+                block_warp_lane_counts<kMeasurePlanes, 512>(accM.c, s_cnt, A.ma.cntM + (long long)w * 32);
+                if (pair) block_warp_lane_counts<kMeasurePlanes, 512>(accX.c, s_cnt, A.ma.cntX + (long long)(w / A.a.n_rg) * 32);
+                __threadfence();
+                cluster_sync_all();
+                if (rank == 0) {
+                    long long* row = (r < A.rows_cap) ? A.rows + r * A.row_len : A.scratch_row;
+                    small_finalize_lattice(A, w, row);
+                }
+                ++r;
+                // the counters are zero again before anybody adds to them: two cluster barriers (the next sweep) lie between
+            }
         }
     }
     // ---- shared -> global: spins and daemon planes

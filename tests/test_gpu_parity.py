@@ -957,8 +957,8 @@ def test_small_lattice_path_bit_exact(micsa, oracle, L, ns, nr):
             np.testing.assert_allclose(out["min_energy"], ref["min_energy"], rtol=1e-12)
             assert out["sweep"].tolist() == [1, 2, 3, 4, 7, 10, 19]
             if small:
-                # min-energy fill + one cluster launch per step + the next step's refresh on the side stream
-                assert n_launch == 1 + len(sched) + (len(sched) - 1)
+                # min-energy fill + the four refreshes + ONE cluster launch that walks through the four steps
+                assert n_launch == 1 + len(sched) + 1
             c = g.counters()
             assert c["attempts"] == 19 * N * ns * nr and c["rns_drawn"] == 4 * N * ns * nr and c["philox_calls"] > 0
             g.sweep(3); oracle.sweep(L, s, m, J, 3)
@@ -979,6 +979,37 @@ def test_small_lattice_path_bit_exact(micsa, oracle, L, ns, nr):
             for _ in range(4):
                 g.half_sweep(1); g.half_sweep(0)
             _assert_state(g, s0, m0)
+
+
+@pytest.mark.parametrize("L,ns,nr", [(8, 5, 2), (16, 40, 2), (24, 33, 1)])
+def test_small_lattice_chained_steps(micsa, oracle, L, ns, nr):
+    """micsa_anneal on small lattices: up to eight schedule steps per launch, the refreshes of the next batch generated
+    on the side stream.  21 steps with every kind of link -- a step without sweeps in the middle (ends a chain), steps
+    without rows, rows every sweep, a different temperature per step -- on the default and on a high-priority stream,
+    twice in a row on one context (the second call starts from the staging sets the first one left)."""
+    import torch
+    seed = 61
+    sched = [(2.0 - 0.07 * k, 1 + (k * 5) % 4, (0, 1, 2, 3)[k % 4]) for k in range(21)]
+    sched[11] = (1.0, 0, 0)
+    for prio in (None, -1):
+        s = oracle.init_spins(L, ns, nr, seed); J = oracle.init_bonds(L, ns, seed)
+        m = np.zeros_like(s, dtype=np.uint8)
+        stream = torch.cuda.Stream(priority=prio) if prio is not None else None
+        with micsa.MicSA(L, ns, nr, seed, stream=stream) as g:
+            for call in range(2):
+                l0 = g.layout_info()["launches"]
+                out = g.anneal(sched, step0=100 * call)
+                n_launch = g.layout_info()["launches"] - l0
+                ref = driver.anneal(L, s, m, J, seed, sched, step0=100 * call)
+                _assert_state(g, s, m, J)
+                for k in ("sweep", "T", "E", "Edem", "Q"):
+                    np.testing.assert_array_equal(out[k], ref[k])
+                np.testing.assert_allclose(out["min_energy"], ref["min_energy"], rtol=1e-12)
+                # fill + 21 refreshes + chains of 8 + 3 (steps 0-10) and 8 + 1 (steps 12-20)
+                assert n_launch == 1 + 21 + 4
+            c = g.counters()
+            assert c["rns_drawn"] == 2 * 21 * L ** 3 * ns * nr
+            assert c["attempts"] == 2 * sum(n for _, n, _ in sched) * L ** 3 * ns * nr
 
 
 def test_empty_and_rowless_schedules(micsa, oracle):
