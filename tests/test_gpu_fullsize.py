@@ -377,3 +377,38 @@ def test_lattices_off_the_fast_path_at_medium_size(micsa, oracle, L, ns, nr):
         E, Ed, Q = g.measure_i64()
         oE, oEd, oQ = oracle.measure(L, s, m, J)
         np.testing.assert_array_equal(E, oE); np.testing.assert_array_equal(Ed, oEd)
+
+
+def test_full_length_runs_agree_between_the_refresh_modes(micsa):
+    """Beyond what the oracle can follow: the same long schedule with the refreshes generated in line (default
+    stream) and one step ahead on the side stream (high-priority stream) must leave identical bits -- a race between
+    the side stream's writes and the sweeps would show here.  Config 4, 2 000 steps = 20 000 sweeps, rows every 100
+    steps; config 2 at its full 10^4 sweeps on the chained small-lattice path against the general path."""
+    import torch
+    cfg = CONFIGS[4]
+    sched = [(cfg.temperatures[0], 10, 10 if (k + 1) % 100 == 0 else 0) for k in range(2000)]
+    res = []
+    for prio in (None, -1):
+        stream = torch.cuda.Stream(priority=prio) if prio is not None else None
+        with micsa.MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed, stream=stream) as g:
+            out = g.anneal(sched)
+            res.append((out, g.get_state(couplings=False)[:2], g.counters()))
+    (o0, (s0, m0), c0), (o1, (s1, m1), c1) = res
+    assert np.array_equal(s0, s1) and np.array_equal(m0, m1)
+    for k in ("sweep", "E", "Edem", "Q"):
+        np.testing.assert_array_equal(o0[k], o1[k])
+    assert c0 == c1 and o0["E"].shape[0] == 20
+
+    cfg = CONFIGS[2]
+    sched = [(2.0, 10, 10 if (k + 1) % 50 == 0 else 0) for k in range(1000)]
+    res = []
+    for small in (1, 0):
+        with micsa.MicSA(cfg.L, cfg.n_samples, cfg.n_replicas, cfg.seed, stream=torch.cuda.Stream(priority=-1)) as g:
+            g.set_tuning("small_path", small)
+            out = g.anneal(sched)
+            res.append((out, g.get_state(couplings=False)[:2], g.counters()))
+    (o0, (s0, m0), c0), (o1, (s1, m1), c1) = res
+    assert np.array_equal(s0, s1) and np.array_equal(m0, m1)
+    for k in ("sweep", "E", "Edem", "Q"):
+        np.testing.assert_array_equal(o0[k], o1[k])
+    assert c0 == c1 and o0["E"].shape[0] == 20
