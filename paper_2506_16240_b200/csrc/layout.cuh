@@ -120,6 +120,17 @@ __device__ __forceinline__ uint32_t bond_flag(uint32_t g, uint32_t n, uint32_t j
 inline uint32_t fastdiv_magic(uint32_t d) { return d >= 2 ? (uint32_t)(((1ull << 32) + d - 1) / d) : 0u; }
 __device__ __forceinline__ uint32_t fastdiv(uint32_t n, uint32_t m) { return m ? __umulhi(n, m) : n; }
 
+// n / d and n % d for ANY n < 2^32 with the same magic number: umulhi(n, m) overshoots n / d by less than n / 2^32 < 1,
+// so it is the quotient or one more -- one multiply and a correction.
+__device__ __forceinline__ uint32_t fastdivmod(uint32_t n, uint32_t d, uint32_t m, uint32_t& rem) {
+    if (m == 0u) { rem = 0u; return n; }
+    uint32_t q = __umulhi(n, m);
+    uint32_t r = n - q * d;
+    if ((int32_t)r < 0) { q -= 1u; r += d; }
+    rem = r;
+    return q;
+}
+
 // canonical site index i = x + L*(y + L*z) of element xh of row (y,z), parity p
 __device__ __forceinline__ uint32_t canonical_site(int L, int p, int z, int y, int xh) {
     const int x = 2 * xh + ((y + z + p) & 1);

@@ -229,7 +229,7 @@ template <int V, int RPW>
 void launch_half_sweep_t(micsa_ctx* c, int parity) {
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = 0; a.inv_nxv = fastdiv_magic((uint32_t)c->g.Lh / 4u);
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = 0; a.inv_nxv = fastdiv_magic((uint32_t)c->g.Lh / 4u); a.inv_pp = 0u;
     const int per_plane = c->g.L * (c->g.Lh / V);
     dim3 grid((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
     half_sweep_kernel<V, RPW><<<grid, 128, 0, c->stream>>>(a, parity);
@@ -241,7 +241,7 @@ template <int RPW>
 void launch_half_sweep_rows(micsa_ctx* c, int parity) {
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = 0; a.inv_nxv = fastdiv_magic((uint32_t)c->g.Lh / 4u);
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = 0; a.inv_nxv = fastdiv_magic((uint32_t)c->g.Lh / 4u); a.inv_pp = 0u;
     const int per_plane = (c->g.L / kRowsPerThread) * (c->g.Lh / 4);
     dim3 grid((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, (unsigned)c->g.n_words);
     half_sweep_rows_kernel<RPW, kRowsPerThread><<<grid, 128, 0, c->stream>>>(a, parity);
@@ -255,13 +255,15 @@ template <int RPW>
 void launch_half_sweep_pipe(micsa_ctx* c, int parity, int dir = 0, int w0 = 0, int nw = -1) {
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = w0; a.inv_nxv = fastdiv_magic((uint32_t)c->g.Lh / 4u);
+    a.L = c->g.L; a.Lh = c->g.Lh; a.n_rg = c->g.n_rg; a.half = c->g.half; a.w0 = w0; a.inv_nxv = fastdiv_magic((uint32_t)c->g.Lh / 4u); a.inv_pp = 0u;
     const unsigned gz = (unsigned)(nw < 0 ? c->g.n_words : nw);
     const int yc = c->pipe_rows;
     const int per_plane = (c->g.L / yc) * (c->g.Lh / 4);
     const int zw = c->pipe_planes;
+    // zw == 1: the planes of one parity class of z in one index space (sweep.cuh, pipe_item)
     dim3 grid = (zw == 4) ? dim3((unsigned)((per_plane + 31) / 32), (unsigned)(c->g.L / 4), gz)
-                          : dim3((unsigned)((per_plane + 127) / 128), (unsigned)c->g.L, gz);
+                          : dim3((unsigned)(((long long)(c->g.L / 2) * per_plane + 127) / 128), 2u, gz);
+    a.inv_pp = fastdiv_magic((uint32_t)per_plane);
     // programmatic dependent launch (the kernel waits with griddepcontrol.wait before
     // its first load): launch latency and ramp overlap the previous grid's tail
     cudaLaunchConfig_t cfg = {};
@@ -273,7 +275,8 @@ void launch_half_sweep_pipe(micsa_ctx* c, int parity, int dir = 0, int w0 = 0, i
     if (dir != 0) {                                  // 4 rows per thread only (grid was sized for yc; redo it)
         const int pp4 = (c->g.L / 4) * (c->g.Lh / 4);
         cfg.gridDim = (zw == 4) ? dim3((unsigned)((pp4 + 31) / 32), (unsigned)(c->g.L / 4), gz)
-                                : dim3((unsigned)((pp4 + 127) / 128), (unsigned)c->g.L, gz);
+                                : dim3((unsigned)(((long long)(c->g.L / 2) * pp4 + 127) / 128), 2u, gz);
+        a.inv_pp = fastdiv_magic((uint32_t)pp4);
         // dir = +-1: along X; +-2: along Y; +-3: along Z (Y and Z share the DIR = +-2 kernels)
         const int axis = (dir > 0 ? dir : -dir) - 1, walk_z = (axis == 2) ? 1 : 0;
         if (axis == 0) {
@@ -637,13 +640,14 @@ int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min, int dir)
     const Geom& g = c->g;
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
-    a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg; a.half = g.half; a.w0 = 0; a.inv_nxv = fastdiv_magic((uint32_t)g.Lh / 4u);
+    a.L = g.L; a.Lh = g.Lh; a.n_rg = g.n_rg; a.half = g.half; a.w0 = 0; a.inv_nxv = fastdiv_magic((uint32_t)g.Lh / 4u); a.inv_pp = 0u;
     MeasureArgs ma; FinalizeArgs fa;
     make_measure_args(c, row, fold_min, ma, fa);
     const int per_plane = (g.L / 4) * (g.Lh / 4);
     const int zw = c->pipe_planes;
     dim3 grid = (zw == 4) ? dim3((unsigned)((per_plane + 31) / 32), (unsigned)(g.L / 4), (unsigned)g.n_words)
-                          : dim3((unsigned)((per_plane + 127) / 128), (unsigned)g.L, (unsigned)g.n_words);
+                          : dim3((unsigned)(((long long)(g.L / 2) * per_plane + 127) / 128), 2u, (unsigned)g.n_words);
+    a.inv_pp = fastdiv_magic((uint32_t)per_plane);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid; cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
     cudaLaunchAttribute attr[1];
@@ -704,7 +708,7 @@ int launch_small_chain(micsa_ctx* c, bool do_refresh, double T, uint32_t step, c
     const Geom& g = c->g;
     SmallArgs A;
     A.a.spin = c->st.spin; A.a.m0 = c->st.m0; A.a.m1 = c->st.m1; A.a.J = c->st.J;
-    A.a.L = g.L; A.a.Lh = g.Lh; A.a.n_rg = g.n_rg; A.a.half = g.half; A.a.w0 = 0; A.a.inv_nxv = fastdiv_magic((uint32_t)g.Lh / 4u);
+    A.a.L = g.L; A.a.Lh = g.Lh; A.a.n_rg = g.n_rg; A.a.half = g.half; A.a.w0 = 0; A.a.inv_nxv = fastdiv_magic((uint32_t)g.Lh / 4u); A.a.inv_pp = 0u;
     A.sg = site_grid(g);
     MeasureArgs ma; FinalizeArgs fa;
     make_measure_args(c, c->row, fold_min, ma, fa);

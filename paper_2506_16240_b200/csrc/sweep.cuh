@@ -38,6 +38,7 @@ struct SweepArgs {
     long long half;
     int w0;                 // first word lattice of this launch (pipelined kernel: blockIdx.z + w0)
     uint32_t inv_nxv;       // fastdiv_magic(Lh / 4) (pipelined kernels)
+    uint32_t inv_pp;        // fastdiv_magic((L / YC) * (Lh / 4)): items per plane of the launched pipelined kernel
 };
 
 // One thread updates V consecutive words of one row (y,z) of the parity-p
@@ -658,7 +659,26 @@ __device__ __forceinline__ PipeBase pipe_base(const SweepArgs& a, int w, int p)
     return P;
 }
 
-// ZW = 1: grid = (ceil((L/YC)*(Lh/4) / 128), L, n_words), a CTA works inside one plane.
+// thread -> (plane z, item t inside the plane, index idx whose low 5 bits are the lane and in which neighbouring
+// items of a row are neighbours).  ZW = 4: see below.  ZW = 1: the planes of one parity class of z (blockIdx.y) follow
+// each other in one index space, so that the last warp of a plane is filled up from the next plane of the class --
+// a plane of L = 80 has 200 items, 1.56 blocks of 128.  (z + p) & 1, which selects the code path, is the same for
+// every thread of the grid row.
+template <int ZW>
+__device__ __forceinline__ bool pipe_item(const SweepArgs& a, int per_plane, int& z, int& t, int& idx) {
+    if (ZW == 1) {
+        const uint32_t flat = blockIdx.x * blockDim.x + threadIdx.x;
+        uint32_t rem;
+        const uint32_t q = fastdivmod(flat, (uint32_t)per_plane, a.inv_pp, rem);
+        idx = (int)flat; t = (int)rem; z = (int)(2u * q + blockIdx.y);
+        return z < a.L;
+    }
+    t = (int)(blockIdx.x * 32 + (threadIdx.x & 31)); idx = t;
+    z = (int)(blockIdx.y * ZW + (threadIdx.x >> 5));
+    return t < per_plane;
+}
+
+// ZW = 1: grid = (ceil((L/2)*(L/YC)*(Lh/4) / 128), 2, n_words): blockIdx.y = parity class of the planes (pipe_item).
 // ZW = 4: grid = (ceil((L/YC)*(Lh/4) / 32), L/4, n_words), warp k of a CTA works on plane
 //         4*blockIdx.y + k with the same (row chunk, quad) items as its sibling warps: the
 //         +-z neighbour rows of a warp are the own-plane rows of the next / previous warp and
@@ -672,17 +692,14 @@ half_sweep_pipe_kernel(SweepArgs a, int p, int walk_z)
 {
     const int L = a.L, Lh = a.Lh;
     const int nxv = Lh >> 2;
-    // idx: item index inside the plane; a warp always holds 32 consecutive items of one plane
-    const int t = (ZW == 1) ? (int)(blockIdx.x * blockDim.x + threadIdx.x)
-                            : (int)(blockIdx.x * 32 + (threadIdx.x & 31));
-    const int z = (ZW == 1) ? (int)blockIdx.y : (int)(blockIdx.y * ZW + (threadIdx.x >> 5));
-    const bool active = t < (L / YC) * nxv;
+    int z, t, idx;
+    const bool active = pipe_item<ZW>(a, (L / YC) * nxv, z, t, idx);
     const unsigned mask = __ballot_sync(0xFFFFFFFFu, active);
     if (!active) return;
     const int chunk = (int)fastdiv((uint32_t)t, a.inv_nxv), xv = t - chunk * nxv;
     const int w = blockIdx.z + a.w0;
     const PipeBase P = pipe_base<RPW>(a, w, p);
-    XNb nb = x_neighbours(t, xv, nxv, mask, true);                // z is warp-uniform: one code path per warp
+    XNb nb = x_neighbours(idx, xv, nxv, mask, true);              // (z + p) & 1 is warp-uniform: one code path per warp
     nb.walk_z = walk_z;
     // programmatic dependent launch: this grid may have been scheduled while the
     // previous half-sweep was still draining; its results are needed from here on,
@@ -707,10 +724,8 @@ half_sweep_pipe_meas_kernel(SweepArgs a, int p, MeasureArgs ma)
     __shared__ uint32_t s_pl[MeasAcc<YC>::PU + MeasAcc<YC>::PM + MeasAcc<YC>::PX][128];
     const int L = a.L, Lh = a.Lh;
     const int nxv = Lh >> 2;
-    const int t = (ZW == 1) ? (int)(blockIdx.x * blockDim.x + threadIdx.x)
-                            : (int)(blockIdx.x * 32 + (threadIdx.x & 31));
-    const int z = (ZW == 1) ? (int)blockIdx.y : (int)(blockIdx.y * ZW + (threadIdx.x >> 5));
-    const bool active = t < (L / YC) * nxv;
+    int z, t, idx;
+    const bool active = pipe_item<ZW>(a, (L / YC) * nxv, z, t, idx);
     const unsigned mask = __ballot_sync(0xFFFFFFFFu, active);
     const int w = blockIdx.z;
     const bool pair = (RPW == 2) && ma.n_replicas == 2;
@@ -720,7 +735,7 @@ half_sweep_pipe_meas_kernel(SweepArgs a, int p, MeasureArgs ma)
     if (active) {
         const int chunk = (int)fastdiv((uint32_t)t, a.inv_nxv), xv = t - chunk * nxv;
         const PipeBase P = pipe_base<RPW>(a, w, p);
-        const XNb nb = x_neighbours(t, xv, nxv, mask, true);
+        const XNb nb = x_neighbours(idx, xv, nxv, mask, true);
         if ((z + p) & 1) march_rows_pipe<RPW, YC, 1, MEAS, DIR>(P, L, Lh, z, chunk * YC, xv * 4, nb, &acc, pair);
         else             march_rows_pipe<RPW, YC, 0, MEAS, DIR>(P, L, Lh, z, chunk * YC, xv * 4, nb, &acc, pair);
     }
