@@ -509,6 +509,54 @@ def test_largest_sample_offsets(micsa, oracle, nr):
         micsa.MicSA(L, ns + 16, nr, seed, sample_offset=off)
 
 
+@pytest.mark.parametrize("L,ns,nr,gamma,walkers", [(16, 20, 2, 1, 0), (8, 9, 2, 1, 0), (16, 5, 2, 2, 1), (24, 3, 1, 1, 1)])
+def test_checkpoint_and_resume(micsa, L, ns, nr, gamma, walkers):
+    """SURVEY.md (aux subsystems): the state is spins + daemon families + couplings + (seed, next refresh index, time
+    index), and Philox is counter-based, so a run resumed from get_state in a NEW context is bit-identical to the
+    uninterrupted one -- rows, final state, minimum energies of the second leg."""
+    seed = 83
+    sched = [(1.8 - 0.1 * k, 2 + k % 3, 1 + k % 2) for k in range(12)]
+    cut = 5
+
+    def prepare(g):
+        g.set_gamma(gamma); g.set_walkers(walkers)
+
+    with micsa.MicSA(L, ns, nr, seed) as a:
+        prepare(a)
+        full = a.anneal(sched, step0=40)
+        full_state = a.get_state()
+        full_fams = []
+        for alpha in range(gamma):
+            a.select_daemon_set(alpha); full_fams.append(a.get_state(spins=False, couplings=False)[1])
+        t_end = a.get_time()
+    with micsa.MicSA(L, ns, nr, seed) as b:
+        prepare(b)
+        first = b.anneal(sched[:cut], step0=40)
+        spins, _, J = b.get_state()
+        fams = []
+        for alpha in range(gamma):
+            b.select_daemon_set(alpha); fams.append(b.get_state(spins=False, couplings=False)[1])
+        t_cut = b.get_time()
+    with micsa.MicSA(L, ns, nr, seed) as c:                 # a new context: the seed is part of the checkpoint
+        prepare(c)
+        c.set_couplings(J); c.set_spins(spins)
+        for alpha in range(gamma):
+            c.select_daemon_set(alpha); c.set_daemons(fams[alpha])
+        c.set_time(t_cut)
+        second = c.anneal(sched[cut:], step0=40 + cut)
+        assert c.get_time() == t_end
+        n1 = first["E"].shape[0]
+        for k in ("E", "Edem", "Q"):
+            np.testing.assert_array_equal(np.concatenate([first[k], second[k]]), full[k])
+        np.testing.assert_array_equal(second["sweep"] + first["sweep"][-1] if n1 else second["sweep"], full["sweep"][n1:])
+        gs, _, gJ = c.get_state()
+        np.testing.assert_array_equal(gs, full_state[0]); np.testing.assert_array_equal(gJ, full_state[2])
+        for alpha in range(gamma):
+            c.select_daemon_set(alpha)
+            np.testing.assert_array_equal(c.get_state(spins=False, couplings=False)[1], full_fams[alpha])
+        np.testing.assert_allclose(np.minimum(first["min_energy"], second["min_energy"]), full["min_energy"], rtol=0, atol=0)
+
+
 def test_measure_begin_end(micsa, oracle):
     """The split measurement returns the state at the point of _begin."""
     L, ns, nr = 8, 5, 2
