@@ -159,6 +159,34 @@ __device__ __forceinline__ void warp_sum_lane_counts(const uint32_t (*pl)[128], 
     if (mine) atomicAdd(&out[lane], (unsigned long long)mine);
 }
 
+// The warp-level part of the above alone: the count of lane l of the word, summed over the warp's 32 vertical
+// counters, returned to the thread whose lane index is l.
+template <int P>
+__device__ __forceinline__ unsigned int warp_lane_count(const uint32_t (&acc)[P])
+{
+    uint32_t c[P + 5];
+#pragma unroll
+    for (int k = 0; k < P + 5; ++k) c[k] = (k < P) ? acc[k] : 0u;
+#pragma unroll
+    for (int l = 0; l < 5; ++l) {
+        uint32_t carry = 0;
+#pragma unroll
+        for (int k = 0; k < P + 5; ++k) {
+            if (k <= P + l) {
+                const uint32_t x = __shfl_xor_sync(0xFFFFFFFFu, c[k], 1 << l);
+                const uint32_t s = c[k] ^ x ^ carry;
+                carry = maj3(c[k], x, carry);
+                c[k] = s;
+            }
+        }
+    }
+    const int lane = threadIdx.x & 31;
+    unsigned int mine = 0;
+#pragma unroll
+    for (int k = 0; k < P + 5; ++k) mine += ((c[k] >> lane) & 1u) << k;
+    return mine;
+}
+
 struct MeasureArgs {
     const uint32_t* spin; const uint32_t* m0; const uint32_t* m1; const void* J;
     int L, Lh, n_rg, n_replicas, n_samples;

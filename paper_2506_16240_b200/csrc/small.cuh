@@ -245,30 +245,39 @@ __device__ __forceinline__ unsigned slab_refresh_word(const SmallArgs& A, const 
     return calls;
 }
 
-// counts of one lattice -> its entries of a measurement row; the lattice's counters are zeroed for the next one
-__device__ __forceinline__ void small_finalize_lattice(const SmallArgs& A, int w, long long* row)
+__device__ __forceinline__ uint32_t ld_cluster1(uint32_t a) {
+    uint32_t v; asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+
+// Counts of one lattice -> its entries of a measurement row.  The lattice belongs to one cluster, so its counts never
+// leave the chip: every CTA leaves the lane totals of its slab in its shared memory (s_tot[3][32]: unsatisfied bonds,
+// levels, replica differences), and after a cluster barrier the first 32 threads of CTA 0 add them up through
+// distributed shared memory and write the row -- no global atomics, no fence, no counters to read back and re-zero
+// (the first version went through the global counters of the general path: 5.5 us per row instead of 3).
+__device__ __forceinline__ void small_finalize_lattice(const SmallArgs& A, int w, long long* row, const unsigned int* s_tot, int cs)
 {
     const int n_sys = A.n_samples * A.n_replicas;
     const int sg = w / A.a.n_rg, rg = w - sg * A.a.n_rg;
     if (threadIdx.x < 32) {
         const int lane = threadIdx.x;
+        unsigned long long U = 0, M = 0, X = 0;
+        const uint32_t base = smem_u32(s_tot + lane);
+        for (int q = 0; q < cs; ++q) {
+            const uint32_t a = dsmem_addr(base, (uint32_t)q);
+            U += ld_cluster1(a); M += ld_cluster1(a + 32u * 4u); X += ld_cluster1(a + 64u * 4u);
+        }
         const int r_local = lane / A.spw, sl = lane - r_local * A.spw;
         const int sample = sg * A.spw + sl, rep = rg * A.rpw + r_local;
-        unsigned long long* cu = A.ma.cntU + (long long)w * 32 + lane;
-        unsigned long long* cmv = A.ma.cntM + (long long)w * 32 + lane;
         if (sample < A.n_samples && rep < A.n_replicas) {
             const int t = sample * A.n_replicas + rep;
-            const long long E = 2 * (long long)__ldcg(cu) - 3 * A.N;
+            const long long E = 2 * (long long)U - 3 * A.N;
             row[t] = E;
-            row[n_sys + t] = 4 * (long long)__ldcg(cmv);
+            row[n_sys + t] = 4 * (long long)M;
             if (A.min_E && E < A.min_E[t]) A.min_E[t] = E;
         }
-        *cu = 0ull; *cmv = 0ull;
-        if (A.n_replicas == 2) {                    // the pair shares the word (rpw == 2, n_rg == 1)
-            unsigned long long* cx = A.ma.cntX + (long long)sg * 32 + lane;
-            if (lane < A.spw && sample < A.n_samples) row[2 * n_sys + sample] = A.N - 2 * (long long)__ldcg(cx);
-            *cx = 0ull;
-        }
+        if (A.n_replicas == 2 && lane < A.spw && sample < A.n_samples)     // the pair shares the word (rpw == 2, n_rg == 1)
+            row[2 * n_sys + sample] = A.N - 2 * (long long)X;
     }
 }
 
@@ -280,7 +289,7 @@ small_step_kernel(SmallArgs A, PhiloxKeys ks, RefreshThr thr)
 {
     typedef typename BondT<RPW>::type JT;
     extern __shared__ __align__(16) unsigned char smem[];
-    __shared__ unsigned int s_cnt[32];
+    __shared__ unsigned int s_tot[3 * 32];                            // lane totals of this CTA's slab: U | M | X
     const int w = blockIdx.x / A.cs, rank = blockIdx.x - w * A.cs, cs = A.cs;
     const int L = A.a.L, Lh = A.a.Lh, nq = Lh >> 2;
     const int ZP = L / cs, z0 = rank * ZP, PW = L * Lh;
@@ -355,17 +364,20 @@ small_step_kernel(SmallArgs A, PhiloxKeys ks, RefreshThr thr)
                     accU.add(Sm.u); accM.add(Sm.m);
                     if (pair) accX.add(Sm.x);
                 }
-                block_warp_lane_counts<kMeasurePlanes, 512>(accU.c, s_cnt, A.ma.cntU + (long long)w * 32);
-                block_warp_lane_counts<kMeasurePlanes, 512>(accM.c, s_cnt, A.ma.cntM + (long long)w * 32);
-                if (pair) block_warp_lane_counts<kMeasurePlanes, 512>(accX.c, s_cnt, A.ma.cntX + (long long)(w / A.a.n_rg) * 32);
-                __threadfence();
-                cluster_sync_all();
+                const unsigned int mU = warp_lane_count<kMeasurePlanes>(accU.c), mM = warp_lane_count<kMeasurePlanes>(accM.c);
+                const unsigned int mX = pair ? warp_lane_count<kMeasurePlanes>(accX.c) : 0u;
+                if (tid < 96) s_tot[tid] = 0u;                        // nobody reads the previous row's totals any more:
+                __syncthreads();                                      // at least one sweep (two cluster barriers) lies between
+                const int lane = tid & 31;
+                if (mU) atomicAdd(&s_tot[lane], mU);
+                if (mM) atomicAdd(&s_tot[32 + lane], mM);
+                if (mX) atomicAdd(&s_tot[64 + lane], mX);
+                cluster_sync_all();                                   // every CTA's totals are in place and visible
                 if (rank == 0) {
                     long long* row = (r < A.rows_cap) ? A.rows + r * A.row_len : A.scratch_row;
-                    small_finalize_lattice(A, w, row);
+                    small_finalize_lattice(A, w, row, s_tot, cs);
                 }
                 ++r;
-                // the counters are zero again before anybody adds to them: two cluster barriers (the next sweep) lie between
             }
         }
     }
