@@ -255,7 +255,10 @@ __device__ __forceinline__ uint32_t ld_cluster1(uint32_t a) {
 // levels, replica differences), and after a cluster barrier the first 32 threads of CTA 0 add them up through
 // distributed shared memory and write the row -- no global atomics, no fence, no counters to read back and re-zero
 // (the first version went through the global counters of the general path: 5.5 us per row instead of 3).
-__device__ __forceinline__ void small_finalize_lattice(const SmallArgs& A, int w, long long* row, const unsigned int* s_tot, int cs)
+// run_min: the finalising thread's running minimum of E over the rows of this launch (folded into min_E at the end of
+// the launch: a read-modify-write of global memory per row sat on the critical path between two cluster barriers).
+__device__ __forceinline__ void small_finalize_lattice(const SmallArgs& A, int w, long long* row, const unsigned int* s_tot, int cs,
+                                                       long long& run_min)
 {
     const int n_sys = A.n_samples * A.n_replicas;
     const int sg = w / A.a.n_rg, rg = w - sg * A.a.n_rg;
@@ -274,7 +277,7 @@ __device__ __forceinline__ void small_finalize_lattice(const SmallArgs& A, int w
             const long long E = 2 * (long long)U - 3 * A.N;
             row[t] = E;
             row[n_sys + t] = 4 * (long long)M;
-            if (A.min_E && E < A.min_E[t]) A.min_E[t] = E;
+            run_min = E < run_min ? E : run_min;
         }
         if (A.n_replicas == 2 && lane < A.spw && sample < A.n_samples)     // the pair shares the word (rpw == 2, n_rg == 1)
             row[2 * n_sys + sample] = A.N - 2 * (long long)X;
@@ -321,6 +324,8 @@ small_step_kernel(SmallArgs A, PhiloxKeys ks, RefreshThr thr)
     }
     const int items = ZP * L * nq;                                    // quad rows per parity of this CTA
     long long r = A.row0;
+    long long run_min = 0x7FFFFFFFFFFFFFFFll;                         // rank 0, threads 0..31: minimum of E of "their" system
+    const bool few = 2 * items <= 2 * nthr;                           // at most two items per thread: counts < 32, five planes
 #pragma unroll 1
     for (int j = 0; j < A.n_chain; ++j) {
         // ---- this step's daemon levels: global -> shared.  Nobody reads the CTA's daemon planes any more: the last
@@ -364,8 +369,15 @@ small_step_kernel(SmallArgs A, PhiloxKeys ks, RefreshThr thr)
                     accU.add(Sm.u); accM.add(Sm.m);
                     if (pair) accX.add(Sm.x);
                 }
-                const unsigned int mU = warp_lane_count<kMeasurePlanes>(accU.c), mM = warp_lane_count<kMeasurePlanes>(accM.c);
-                const unsigned int mX = pair ? warp_lane_count<kMeasurePlanes>(accX.c) : 0u;
+                unsigned int mU, mM, mX = 0u;
+                if (few) {                                            // block-uniform
+                    typedef const uint32_t (&P5)[5];
+                    mU = warp_lane_count<5>(reinterpret_cast<P5>(accU.c)); mM = warp_lane_count<5>(reinterpret_cast<P5>(accM.c));
+                    if (pair) mX = warp_lane_count<5>(reinterpret_cast<P5>(accX.c));
+                } else {
+                    mU = warp_lane_count<kMeasurePlanes>(accU.c); mM = warp_lane_count<kMeasurePlanes>(accM.c);
+                    if (pair) mX = warp_lane_count<kMeasurePlanes>(accX.c);
+                }
                 if (tid < 96) s_tot[tid] = 0u;                        // nobody reads the previous row's totals any more:
                 __syncthreads();                                      // at least one sweep (two cluster barriers) lies between
                 const int lane = tid & 31;
@@ -375,10 +387,20 @@ small_step_kernel(SmallArgs A, PhiloxKeys ks, RefreshThr thr)
                 cluster_sync_all();                                   // every CTA's totals are in place and visible
                 if (rank == 0) {
                     long long* row = (r < A.rows_cap) ? A.rows + r * A.row_len : A.scratch_row;
-                    small_finalize_lattice(A, w, row, s_tot, cs);
+                    small_finalize_lattice(A, w, row, s_tot, cs, run_min);
                 }
                 ++r;
             }
+        }
+    }
+    // ---- the launch's minimum energies (same thread -> system map as small_finalize_lattice)
+    if (rank == 0 && tid < 32 && A.min_E && run_min != 0x7FFFFFFFFFFFFFFFll) {
+        const int sg = w / A.a.n_rg, rg = w - sg * A.a.n_rg;
+        const int r_local = tid / A.spw, sl = tid - r_local * A.spw;
+        const int sample = sg * A.spw + sl, rep = rg * A.rpw + r_local;
+        if (sample < A.n_samples && rep < A.n_replicas) {
+            const int t = sample * A.n_replicas + rep;
+            if (run_min < A.min_E[t]) A.min_E[t] = run_min;
         }
     }
     // ---- shared -> global: spins and daemon planes
