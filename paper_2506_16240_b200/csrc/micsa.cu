@@ -636,7 +636,7 @@ int launch_measure(micsa_ctx* c, long long* row, bool fold_min) {
 // The last sweep of a measured group with the counting fused into its two launches
 // (sweep.cuh, MeasAcc): the state is not read again for the observables.
 template <int RPW>
-int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min, int dir) {
+int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min) {
     const Geom& g = c->g;
     SweepArgs a;
     a.spin = c->st.spin; a.m0 = c->st.m0; a.m1 = c->st.m1; a.J = c->st.J;
@@ -656,14 +656,10 @@ int launch_measuring_sweep(micsa_ctx* c, long long* row, bool fold_min, int dir)
     cfg.attrs = attr; cfg.numAttrs = 1;
     if (zw == 4) {
         LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 1>, a, 0, ma));
-        if (dir > 0)      LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2, +1>, a, 1, ma));
-        else if (dir < 0) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2, -1>, a, 1, ma));
-        else              LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2>, a, 1, ma));
+        LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 4, 2>, a, 1, ma));
     } else {
         LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 1>, a, 0, ma));
-        if (dir > 0)      LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2, +1>, a, 1, ma));
-        else if (dir < 0) LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2, -1>, a, 1, ma));
-        else              LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2>, a, 1, ma));
+        LK(cudaLaunchKernelEx(&cfg, half_sweep_pipe_meas_kernel<RPW, 1, 2>, a, 1, ma));
     }
     cfg.gridDim = dim3(1);
     LK(cudaLaunchKernelEx(&cfg, finalize_kernel, fa));
@@ -801,11 +797,12 @@ int launch_sweeps_measured(micsa_ctx* c, int n, long long* row, bool fold_min) {
         return launch_measure(c, row, fold_min);
     }
     int rc = launch_sweeps(c, n - 1); if (rc) return rc;
-    // the wandering only permutes the walkers: E, E_daemon and q of the timestep are counted before it
-    const int dir = fused_walk(c) ? ((c->t & 1) ? +1 : -1) : 0;
-    rc = (g.rpw == 2) ? launch_measuring_sweep<2>(c, row, fold_min, dir) : launch_measuring_sweep<1>(c, row, fold_min, dir);
+    // The wandering only permutes the walkers: E, E_daemon and q of the timestep are counted before it, and it follows
+    // as a launch of its own -- counting AND exchanging in the odd launch spilled 700-840 bytes per thread and made a
+    // walker step 1 % slower than this (322 against 319 us at config 4).
+    rc = (g.rpw == 2) ? launch_measuring_sweep<2>(c, row, fold_min) : launch_measuring_sweep<1>(c, row, fold_min);
     if (rc) return rc;
-    if (c->walkers && dir == 0) { rc = launch_wander(c, 0, +1, (int)(c->t & 1)); if (rc) return rc; }
+    if (c->walkers) { rc = launch_wander(c, 0, +1, (int)(c->t & 1)); if (rc) return rc; }
     c->t += 1;
     return MICSA_OK;
 }
